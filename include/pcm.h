@@ -1,0 +1,217 @@
+/*
+ * pcm.h -- C ABI of libpcm_b200: the data-parallel hot path of GPU C-PCM with
+ * switching/Gaussian surface discretization (arxiv 1505.07851; citations are PAPER.md lines).
+ *
+ * What the library computes (all fp64, atomic units: bohr, hartree):
+ *   J_k(r)  = erf(zeta_k |r - r_k|) / |r - r_k|                                  Eq. 6
+ *   v_k     = sum_{mu,nu} P_mu,nu (mu|J_k|nu)      -- pcm_potential               Eq. 5
+ *   F_mu,nu = sum_k q_k (mu|J_k|nu)                -- pcm_fock                    Eq. 10
+ *   (mu|J_k|nu) = sum_ij c_mu,i c_nu,j [chi_i|J_k|chi_j]                          Eq. 11-12
+ *   A_kl    = erf(zeta'_kl r_kl)/r_kl, zeta'_kl = zeta_k zeta_l/sqrt(zeta_k^2+zeta_l^2),
+ *   A_kk    = zeta_k sqrt(2/pi) / S_k              -- pcm_amatvec (y = A q)       Eq. 2, 3, 8
+ *   A x = b by preconditioned CG with the Jacobi or the randomized block-Jacobi
+ *   preconditioner                                  -- pcm_rbj_build, pcm_cg_solve section 4b
+ *
+ * Sign convention: the paper's L^k_mu,nu = -(mu|J_k|nu) carries the electron's charge, so
+ * its c = -v and Delta F^S = -F.  This library returns the unsigned v and F.  Eq. 3 is printed with
+ * zeta/sqrt(2 pi); the Gaussian self-energy is zeta sqrt(2/pi), which is what is used (R1).
+ *
+ * Conventions
+ *   - every call returns int: 0 = PCM_OK, < 0 = error (pcm_last_error gives text), > 0 = a
+ *     documented non-error status (PCM_NOT_CONVERGED).  No exception crosses the ABI.
+ *   - "host" / "device" is stated for every pointer.  Device pointers must be valid on the
+ *     context's device until the given stream has passed the call.
+ *   - the context owns COPIES of everything given to pcm_setup; the caller owns P, q, b, v, F, y, x.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Hot calls
+ *     are asynchronous with respect to the host unless stated otherwise.
+ *   - a context must not be used from two host threads at once (it owns scratch buffers).
+ *   - there is no CPU fallback: every call fails with PCM_ERR_CUDA if the device is unusable.
+ */
+#ifndef PCM_B200_H
+#define PCM_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PCM_OK 0
+#define PCM_NOT_CONVERGED 1    /* pcm_cg_solve hit max_iter; x, iters and resid are still valid */
+#define PCM_ERR_ARG (-1)       /* bad argument (NULL, negative size, l > 2, nprim < 1, ...) */
+#define PCM_ERR_CUDA (-2)      /* a CUDA call failed (text in pcm_last_error) */
+#define PCM_ERR_ALLOC (-3)     /* host or device allocation failed */
+#define PCM_ERR_STATE (-4)     /* call needs something not built (e.g. RBJ before pcm_rbj_build) */
+#define PCM_ERR_NUMERIC (-5)   /* a diagonal block of A was not positive definite */
+
+#define PCM_NCLASS 6           /* shell-pair classes in the paper's order ss, sp, pp, sd, pd, dd */
+#define PCM_NL 5               /* total angular momentum L = l_a + l_b = 0..4 */
+
+typedef struct pcm_ctx pcm_ctx;
+
+typedef struct pcm_options {
+    double screen_eps;     /* primitive-pair Schwarz-like cutoff of Eq. 15; default 1e-12 */
+    int d_pure;            /* 1 (default): 5 real solid harmonics per d shell; 0: 6 Cartesian components */
+    int device;            /* CUDA device ordinal; -1 (default) = the calling thread's current device */
+    int merge_products;    /* 1 (default): primitive pairs with identical (A, alpha, B, beta) -- e.g. the s and p
+                              parts of an sp shell -- share one Hermite Gaussian product in the kernels (exact) */
+    int reserved[4];
+} pcm_options;
+
+typedef struct pcm_info {
+    int64_t nbf;                       /* basis functions */
+    int64_t nshell;
+    int64_t npoint;                    /* M, surface points */
+    int64_t shell_pairs[PCM_NCLASS];   /* unordered shell pairs (I <= J) with at least one surviving primitive pair */
+    int64_t prim_pairs[PCM_NCLASS];    /* surviving primitive pairs per class, counted as the paper does: every
+                                          (i in I, j in J) of an unordered shell pair I <= J, both orders of a
+                                          diagonal shell pair (I == J, i != j) counted once */
+    int64_t prim_pairs_total;
+    int64_t prim_pairs_unscreened;     /* before Eq. 15 */
+    int64_t products[PCM_NL];          /* distinct Hermite Gaussian products per L after merging */
+    int64_t products_total;
+    double prim_pair_points;           /* prim_pairs_total * npoint: the work unit count of one potential or Fock call */
+    double product_points;             /* products_total * npoint: kernel evaluations actually performed */
+    double zeta_min, zeta_max;
+    int64_t rbj_block;                 /* 0 until pcm_rbj_build */
+    int64_t rbj_nblocks;
+    int64_t device_bytes;              /* device memory held by the context */
+} pcm_info;
+
+/* Fills *opt with the defaults listed above. */
+void pcm_options_default(pcm_options *opt);
+
+/*
+ * pcm_setup -- step a1: enumerate shell pairs I <= J, screen primitive pairs with
+ *   |c_i c_j| max_components [chi_a chi_b|chi_a chi_b]^{1/2} >= screen_eps   (Eq. 15),
+ * sort by class and total angular momentum, pack the SoA pair / point arrays and upload them.
+ * All pointers are HOST pointers and are copied.
+ *   nshell, shell_l[nshell] in {0,1,2}, shell_xyz[3*nshell] (bohr), shell_nprim[nshell] >= 1,
+ *   prim_exp / prim_coef[sum nprim]: exponents and contraction coefficients, shell after shell.
+ *     prim_coef multiplies the RAW primitive (x-Ax)^i (y-Ay)^j (z-Az)^k exp(-a |r-A|^2) (normalisation
+ *     folded in by the caller).  An sp shell is passed as an s shell and a p shell with equal exponents.
+ *   basis-function order = shell order; within a shell: s; p = (x,y,z); pure d = (sqrt3 xy, sqrt3 yz,
+ *     zz-(xx+yy)/2, sqrt3 xz, (sqrt3/2)(xx-yy)); Cartesian d = (xx,xy,xz,yy,yz,zz).
+ *   npoint, pt_xyz[3*npoint] (bohr), pt_zeta[npoint] > 0 (Eq. 7), pt_switch[npoint] > 0 (S_k of Eq. 3/9;
+ *     NULL means 1).  npoint == 0 and nshell == 0 are allowed (calls then do nothing / zero-fill).
+ *   opt may be NULL (defaults).
+ * On success *out is a new context.  Errors: PCM_ERR_ARG, PCM_ERR_ALLOC, PCM_ERR_CUDA (*out = NULL;
+ * the text is available from pcm_last_error(NULL)).
+ */
+int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell_xyz, const int *shell_nprim,
+              const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
+              const double *pt_zeta, const double *pt_switch, const pcm_options *opt);
+
+/*
+ * pcm_potential -- v_k = sum over the FULL square of P_mu,nu (mu|J_k|nu), k = 0..M-1  (Eq. 5; the paper's
+ * "build c", c_k = -v_k).  P_dev: DEVICE, row-major nbf x nbf, leading dimension ldp >= nbf;
+ * read only where a shell pair survived screening; (mu,nu) and (nu,mu) are both read, P need not be symmetric.
+ * v_dev: DEVICE, M doubles, overwritten.  Asynchronous on `stream`.
+ */
+int pcm_potential(pcm_ctx *ctx, const double *P_dev, int64_t ldp, double *v_dev, void *stream);
+
+/*
+ * pcm_fock -- F_mu,nu (+)= sum_k q_k (mu|J_k|nu)  (Eq. 10; the paper's "build Delta F^S", PAPER.md:126-143,
+ * Delta F^S = -F).  q_dev: DEVICE, M doubles.  F_dev: DEVICE, row-major nbf x nbf, leading dimension ldf.
+ * accumulate = 0: F is zero-filled first; 1: added to.  Both (mu,nu) and (nu,mu) are written; elements of
+ * screened-out shell pairs are left as they are (or zero).  Deterministic (no atomics).  Asynchronous.
+ */
+int pcm_fock(pcm_ctx *ctx, const double *q_dev, double *F_dev, int64_t ldf, int accumulate, void *stream);
+
+/*
+ * pcm_amatvec -- y = A q with A evaluated on the fly (Eq. 2, 3, 8; never stored, unlike PAPER.md:106).
+ * q_dev, y_dev: DEVICE, M doubles, must not alias.  Coincident points i != j (a caller error) are treated as
+ * r = 0 -> 2 zeta'/sqrt(pi), never NaN.  Deterministic.  Asynchronous.
+ */
+int pcm_amatvec(pcm_ctx *ctx, const double *q_dev, double *y_dev, void *stream);
+
+/*
+ * pcm_pivot_order -- the seeded pivot order used by pcm_rbj_build: indices 0..M-1 sorted by
+ * (splitmix64-finaliser(seed + (i+1)*0x9E3779B97F4A7C15), i).  perm_host: HOST, M int64.  No device work.
+ */
+int pcm_pivot_order(uint64_t seed, int64_t M, int64_t *perm_host);
+
+/*
+ * pcm_rbj_build -- the randomized block-Jacobi preconditioner of PAPER.md:190: take the first still-unassigned
+ * index k of the pivot order, evaluate row k of A over the unassigned indices, the block is k plus the
+ * block-1 unassigned indices with the largest A_kj (ties -> lower index), repeat; the last block takes the
+ * remainder.  Every block of A is then inverted (Cholesky) and the inverses are kept on the device.
+ * pivot_order_host: HOST, a permutation of 0..M-1, or NULL to use pcm_pivot_order(seed, M).
+ * Synchronises the stream before returning.  Errors: PCM_ERR_ARG (block < 1), PCM_ERR_NUMERIC.
+ */
+int pcm_rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, void *stream);
+
+/*
+ * pcm_rbj_get -- copy the block structure back (for inspection and tests).  Any pointer may be NULL.
+ * order_host[M]: indices block after block, pivot first then by descending A_kj; bstart_host[nblocks+1];
+ * inv_host: the inverse blocks, row-major, back to back (sum of n_b^2 doubles).  Synchronous.
+ */
+int pcm_rbj_get(pcm_ctx *ctx, int64_t *order_host, int64_t *bstart_host, double *inv_host);
+
+/*
+ * pcm_cg_solve -- preconditioned conjugate gradient on A x = b:
+ *   r = b - A x0; z = C r; p = z;  repeat { stop if ||r||_2 <= tol;  alpha = (r.z)/(p.Ap); x += alpha p;
+ *   r -= alpha Ap; z = C r; beta = (r.z)'/(r.z); p = z + beta p }.
+ * precond: 0 none, 1 Jacobi (C = diag(A)^-1), 2 RBJ (needs pcm_rbj_build; C = P M^-1 P).
+ * b_dev: DEVICE M doubles.  x_dev: DEVICE M doubles, in: x0 if use_x0 else ignored; out: the solution.
+ * tol is the absolute Euclidean norm of the recurrence residual (the paper's delta).
+ * iters (HOST, may be NULL): matrix-vector products after the initial residual.
+ * resid (HOST, may be NULL): resid[0] = final recurrence ||r||, resid[1] = true ||b - A x|| recomputed at exit.
+ * Synchronous: reads the residual norm back every iteration.  Returns PCM_OK or PCM_NOT_CONVERGED.
+ */
+int pcm_cg_solve(pcm_ctx *ctx, const double *b_dev, double *x_dev, double tol, int max_iter, int precond, int use_x0,
+                 int *iters, double *resid, void *stream);
+
+/*
+ * Host-buffer forms of the four hot calls: same semantics, every array is a HOST pointer; the call
+ * copies inputs to the device, runs the device path on the context's own stream, copies the result back
+ * and synchronises.  These are what bench.py's end-to-end figure times.
+ */
+int pcm_potential_host(pcm_ctx *ctx, const double *P_host, int64_t ldp, double *v_host);
+int pcm_fock_host(pcm_ctx *ctx, const double *q_host, double *F_host, int64_t ldf, int accumulate);
+int pcm_amatvec_host(pcm_ctx *ctx, const double *q_host, double *y_host);
+int pcm_cg_solve_host(pcm_ctx *ctx, const double *b_host, double *x_host, double tol, int max_iter, int precond,
+                      int use_x0, int *iters, double *resid);
+
+/* Counts that define the throughput metric (primitive pair x point per call).  No device work. */
+int pcm_get_info(pcm_ctx *ctx, pcm_info *out);
+
+/*
+ * Kernel timing.  pcm_set_timing(ctx, 1) makes pcm_potential (op 0), pcm_fock (op 1) and pcm_amatvec (op 2) record
+ * CUDA events on the launching stream around their kernels (each op has its own event set).
+ * pcm_last_kernel_ms: for the most recent timed call of `op`, ms[0] = the main integral / matvec kernels,
+ * ms[1] = pre/post transforms and reductions; n_launch (may be NULL) = kernels that call launched.
+ * pcm_last_class_ms: the same call split by total angular momentum, ms[L] = device time of the main kernel of the
+ * products with L = l_a + l_b = 0..4 (op 2: ms[0] is its one kernel).  Both synchronise on the recorded events.
+ */
+int pcm_set_timing(pcm_ctx *ctx, int enable);
+int pcm_last_kernel_ms(pcm_ctx *ctx, int op, double ms[2], int *n_launch);
+int pcm_last_class_ms(pcm_ctx *ctx, int op, double ms[PCM_NL]);
+
+/* pcm_launch_count -- kernels launched by this context since pcm_setup (bench.py's gpu_launches). */
+int pcm_launch_count(pcm_ctx *ctx, int64_t *total);
+
+/*
+ * pcm_fp64_peak -- a register-resident DFMA-chain microbenchmark on the context's device: the measured
+ * FP64 FMA rate in TFLOP/s (2 flop per DFMA), best of `reps`.  The ALU roofline denominator of bench.py.
+ */
+int pcm_fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
+
+/*
+ * pcm_schwarz_bound -- the screening quantity of Eq. 15 for one primitive pair of RAW Cartesian
+ * primitives of angular momenta la, lb in {0,1,2}: max over Cartesian components of
+ * [chi_a chi_b|chi_a chi_b]^{1/2} (a two-electron self-repulsion integral; contraction coefficients NOT
+ * included -- pcm_setup multiplies by |c_i c_j|).  A, B: HOST, 3 doubles.  Host arithmetic only, no device work.
+ */
+int pcm_schwarz_bound(int la, double alpha, const double *A, int lb, double beta, const double *B, double *out);
+
+/* Text of the last error on this context (ctx == NULL: of the last failed pcm_setup on this thread). */
+const char *pcm_last_error(pcm_ctx *ctx);
+
+/* Frees device and host state.  NULL is allowed. */
+int pcm_destroy(pcm_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PCM_B200_H */

@@ -1,0 +1,357 @@
+// pcm_api.cu -- the C ABI of include/pcm.h: argument checks, context life cycle, host-buffer forms.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "pcm_internal.h"
+
+namespace pcm {
+int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *shell_xyz, const int *shell_nprim,
+                  const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
+                  const double *pt_zeta, const double *pt_switch);
+const char *setup_error_text();
+int64_t fock_chunks(const pcm_ctx *ctx, int L);
+int64_t pot_chunks(const pcm_ctx *ctx, int L);
+int64_t amat_chunks(const pcm_ctx *ctx);
+void pivot_order(uint64_t seed, int64_t M, int64_t *perm);
+int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s);
+int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter, int precond, int use_x0, int *iters,
+             double *resid, cudaStream_t s);
+}  // namespace pcm
+
+using namespace pcm;
+
+extern "C" {
+
+void pcm_options_default(pcm_options *opt) {
+    if (!opt) return;
+    std::memset(opt, 0, sizeof(*opt));
+    opt->screen_eps = 1e-12;
+    opt->d_pure = 1;
+    opt->device = -1;
+    opt->merge_products = 1;
+}
+
+static void free_ctx(pcm_ctx *ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    for (void *p : ctx->allocs) cudaFree(p);
+    if (ctx->cg_scal_host) cudaFreeHost(ctx->cg_scal_host);
+    if (ctx->io_a) cudaFree(ctx->io_a);
+    if (ctx->io_b) cudaFree(ctx->io_b);
+    for (auto &e : ctx->ev) if (e) cudaEventDestroy(e);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    delete[] ctx->rbj_bstart_host;
+    delete ctx;
+}
+
+int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell_xyz, const int *shell_nprim,
+              const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
+              const double *pt_zeta, const double *pt_switch, const pcm_options *opt) {
+    if (!out) return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: out is NULL");
+    *out = nullptr;
+    if (nshell < 0 || npoint < 0 || npoint > 0x7fffffff) return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: negative or too large size");
+    if (nshell > 0 && (!shell_l || !shell_xyz || !shell_nprim || !prim_exp || !prim_coef))
+        return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: NULL shell array");
+    if (npoint > 0 && (!pt_xyz || !pt_zeta)) return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: NULL point array");
+    int64_t np = 0;
+    for (int s = 0; s < nshell; ++s) {
+        if (shell_l[s] < 0 || shell_l[s] > 2) return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: shell_l must be 0, 1 or 2");
+        if (shell_nprim[s] < 1) return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: shell_nprim must be >= 1");
+        np += shell_nprim[s];
+    }
+    for (int64_t i = 0; i < np; ++i)
+        if (!(prim_exp[i] > 0.0) || !std::isfinite(prim_exp[i]) || !std::isfinite(prim_coef[i]))
+            return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: exponents must be positive and finite, coefficients finite");
+    for (int64_t k = 0; k < npoint; ++k)
+        if (!(pt_zeta[k] > 0.0) || !std::isfinite(pt_zeta[k]) || (pt_switch && !(pt_switch[k] > 0.0)))
+            return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: pt_zeta and pt_switch must be positive");
+
+    pcm_ctx *ctx = new (std::nothrow) pcm_ctx();
+    if (!ctx) return set_error(nullptr, PCM_ERR_ALLOC, "pcm_setup: out of host memory");
+    if (opt) ctx->opt = *opt; else pcm_options_default(&ctx->opt);
+    if (!(ctx->opt.screen_eps >= 0.0)) { delete ctx; return set_error(nullptr, PCM_ERR_ARG, "pcm_setup: screen_eps < 0"); }
+
+    auto fail = [&](int rc) {
+        set_error(nullptr, rc, ctx->err.empty() ? std::string("pcm_setup failed") : ctx->err);
+        free_ctx(ctx);
+        return rc;
+    };
+    cudaError_t e;
+    int dev = ctx->opt.device;
+    if (dev < 0) {
+        e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) { ctx->err = std::string("cudaGetDevice: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    }
+    e = cudaSetDevice(dev);
+    if (e != cudaSuccess) { ctx->err = std::string("cudaSetDevice: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    ctx->device = dev;
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) { ctx->err = std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    ctx->sm_count = prop.multiProcessorCount;
+    e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { ctx->err = std::string("cudaStreamCreate: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    for (auto &ev : ctx->ev) {
+        e = cudaEventCreate(&ev);
+        if (e != cudaSuccess) { ctx->err = std::string("cudaEventCreate: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    }
+
+    int rc = build_context(ctx, nshell, shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, npoint, pt_xyz, pt_zeta, pt_switch);
+    if (rc) return fail(rc);
+
+    // scratch sized from the fixed work partition
+    const int64_t M = ctx->M;
+    for (int L = 0; L <= MAXL; ++L) {
+        ClassData &c = ctx->cls[L];
+        c.herm_slots = fock_chunks(ctx, L);
+        if ((rc = dev_alloc_t(ctx, &c.herm, (size_t)c.herm_slots * nherm(L) * std::max<int64_t>(c.npad, 1)))) return fail(rc);
+        ctx->vpart_slots += (c.n > 0) ? pot_chunks(ctx, L) : 0;
+    }
+    ctx->ypart_slots = amat_chunks(ctx);
+    if ((rc = dev_alloc_t(ctx, &ctx->vpart, (size_t)std::max<int64_t>(ctx->vpart_slots, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
+    if ((rc = dev_alloc_t(ctx, &ctx->ypart, (size_t)ctx->ypart_slots * std::max<int64_t>(M, 1)))) return fail(rc);
+    if ((rc = dev_alloc_t(ctx, &ctx->cg_vec, (size_t)5 * std::max<int64_t>(M, 1)))) return fail(rc);
+    if ((rc = dev_alloc_t(ctx, &ctx->cg_scal, (size_t)1024))) return fail(rc);
+    e = cudaMemset(ctx->cg_scal, 0, 1024 * 8);
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->cg_scal_host, 64 * sizeof(double));
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { ctx->err = std::string("pcm_setup: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    ctx->info.device_bytes = ctx->device_bytes;
+    *out = ctx;
+    return PCM_OK;
+}
+
+#define PCM_CHECK_CTX(ctx) \
+    if (!(ctx)) return PCM_ERR_ARG
+
+int pcm_potential(pcm_ctx *ctx, const double *P_dev, int64_t ldp, double *v_dev, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->M == 0) return PCM_OK;
+    if (!v_dev || (ctx->nbf > 0 && (!P_dev || ldp < ctx->nbf))) return set_error(ctx, PCM_ERR_ARG, "pcm_potential: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_potential(ctx, P_dev, ldp, v_dev, (cudaStream_t)stream);
+}
+
+int pcm_fock(pcm_ctx *ctx, const double *q_dev, double *F_dev, int64_t ldf, int accumulate, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->nbf == 0) return PCM_OK;
+    if (!F_dev || ldf < ctx->nbf || (ctx->M > 0 && !q_dev)) return set_error(ctx, PCM_ERR_ARG, "pcm_fock: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_fock(ctx, q_dev, F_dev, ldf, accumulate, (cudaStream_t)stream);
+}
+
+int pcm_amatvec(pcm_ctx *ctx, const double *q_dev, double *y_dev, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->M == 0) return PCM_OK;
+    if (!q_dev || !y_dev || q_dev == y_dev) return set_error(ctx, PCM_ERR_ARG, "pcm_amatvec: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_amatvec(ctx, q_dev, y_dev, (cudaStream_t)stream);
+}
+
+int pcm_pivot_order(uint64_t seed, int64_t M, int64_t *perm_host) {
+    if (M < 0 || (M > 0 && !perm_host)) return PCM_ERR_ARG;
+    pivot_order(seed, M, perm_host);
+    return PCM_OK;
+}
+
+int pcm_rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return rbj_build(ctx, block, seed, pivot_order_host, (cudaStream_t)stream);
+}
+
+int pcm_rbj_get(pcm_ctx *ctx, int64_t *order_host, int64_t *bstart_host, double *inv_host) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->rbj_block == 0) return set_error(ctx, PCM_ERR_STATE, "pcm_rbj_get: no RBJ preconditioner built");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const int64_t M = ctx->M, l = ctx->rbj_block, nb = ctx->rbj_nblocks;
+    if (order_host && M > 0) {
+        std::vector<int32_t> o((size_t)M);
+        PCM_CUDA(ctx, cudaMemcpy(o.data(), ctx->rbj_order, (size_t)M * 4, cudaMemcpyDeviceToHost));
+        for (int64_t i = 0; i < M; ++i) order_host[i] = o[i];
+    }
+    if (bstart_host)
+        for (int64_t b = 0; b <= nb; ++b) bstart_host[b] = std::min(b * l, M);
+    if (inv_host) {
+        // device layout: block b at b*l*l with its own leading dimension n_b; host layout: back to back
+        size_t off = 0;
+        for (int64_t b = 0; b < nb; ++b) {
+            const int64_t n = std::min(l, M - b * l);
+            PCM_CUDA(ctx, cudaMemcpy(inv_host + off, ctx->rbj_inv + (size_t)b * l * l, (size_t)n * n * 8, cudaMemcpyDeviceToHost));
+            off += (size_t)n * n;
+        }
+    }
+    return PCM_OK;
+}
+
+int pcm_cg_solve(pcm_ctx *ctx, const double *b_dev, double *x_dev, double tol, int max_iter, int precond, int use_x0,
+                 int *iters, double *resid, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->M > 0 && (!b_dev || !x_dev)) return set_error(ctx, PCM_ERR_ARG, "pcm_cg_solve: NULL vector");
+    if (max_iter < 0 || !(tol >= 0.0)) return set_error(ctx, PCM_ERR_ARG, "pcm_cg_solve: bad tol or max_iter");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return cg_solve(ctx, b_dev, x_dev, tol, max_iter, precond, use_x0, iters, resid, (cudaStream_t)stream);
+}
+
+// ---- host-buffer forms ------------------------------------------------------------------------
+static int ensure_io(pcm_ctx *ctx, double **buf, size_t *have, size_t bytes) {
+    if (*have >= bytes && *buf) return PCM_OK;
+    if (*buf) cudaFree(*buf);
+    *buf = nullptr;
+    *have = 0;
+    cudaError_t e = cudaMalloc((void **)buf, std::max<size_t>(bytes, 8));
+    if (e != cudaSuccess) return set_error(ctx, PCM_ERR_ALLOC, std::string("cudaMalloc (staging): ") + cudaGetErrorString(e));
+    *have = bytes;
+    return PCM_OK;
+}
+
+int pcm_potential_host(pcm_ctx *ctx, const double *P_host, int64_t ldp, double *v_host) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->M == 0) return PCM_OK;
+    if (!v_host || (ctx->nbf > 0 && (!P_host || ldp < ctx->nbf))) return set_error(ctx, PCM_ERR_ARG, "pcm_potential_host: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t nb = (size_t)ctx->nbf;
+    int rc;
+    if ((rc = ensure_io(ctx, &ctx->io_a, &ctx->io_a_bytes, nb * nb * 8))) return rc;
+    if ((rc = ensure_io(ctx, &ctx->io_b, &ctx->io_b_bytes, (size_t)ctx->M * 8))) return rc;
+    cudaStream_t s = ctx->own_stream;
+    if (nb) PCM_CUDA(ctx, cudaMemcpy2DAsync(ctx->io_a, nb * 8, P_host, (size_t)ldp * 8, nb * 8, nb, cudaMemcpyHostToDevice, s));
+    if ((rc = launch_potential(ctx, ctx->io_a, (int64_t)nb, ctx->io_b, s))) return rc;
+    PCM_CUDA(ctx, cudaMemcpyAsync(v_host, ctx->io_b, (size_t)ctx->M * 8, cudaMemcpyDeviceToHost, s));
+    PCM_CUDA(ctx, cudaStreamSynchronize(s));
+    return PCM_OK;
+}
+
+int pcm_fock_host(pcm_ctx *ctx, const double *q_host, double *F_host, int64_t ldf, int accumulate) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->nbf == 0) return PCM_OK;
+    if (!F_host || ldf < ctx->nbf || (ctx->M > 0 && !q_host)) return set_error(ctx, PCM_ERR_ARG, "pcm_fock_host: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t nb = (size_t)ctx->nbf;
+    int rc;
+    if ((rc = ensure_io(ctx, &ctx->io_a, &ctx->io_a_bytes, nb * nb * 8))) return rc;
+    if ((rc = ensure_io(ctx, &ctx->io_b, &ctx->io_b_bytes, (size_t)ctx->M * 8))) return rc;
+    cudaStream_t s = ctx->own_stream;
+    if (ctx->M) PCM_CUDA(ctx, cudaMemcpyAsync(ctx->io_b, q_host, (size_t)ctx->M * 8, cudaMemcpyHostToDevice, s));
+    if (accumulate) PCM_CUDA(ctx, cudaMemcpy2DAsync(ctx->io_a, nb * 8, F_host, (size_t)ldf * 8, nb * 8, nb, cudaMemcpyHostToDevice, s));
+    if ((rc = launch_fock(ctx, ctx->io_b, ctx->io_a, (int64_t)nb, accumulate, s))) return rc;
+    PCM_CUDA(ctx, cudaMemcpy2DAsync(F_host, (size_t)ldf * 8, ctx->io_a, nb * 8, nb * 8, nb, cudaMemcpyDeviceToHost, s));
+    PCM_CUDA(ctx, cudaStreamSynchronize(s));
+    return PCM_OK;
+}
+
+int pcm_amatvec_host(pcm_ctx *ctx, const double *q_host, double *y_host) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->M == 0) return PCM_OK;
+    if (!q_host || !y_host) return set_error(ctx, PCM_ERR_ARG, "pcm_amatvec_host: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    int rc;
+    const size_t bytes = (size_t)ctx->M * 8;
+    if ((rc = ensure_io(ctx, &ctx->io_a, &ctx->io_a_bytes, bytes))) return rc;
+    if ((rc = ensure_io(ctx, &ctx->io_b, &ctx->io_b_bytes, bytes))) return rc;
+    cudaStream_t s = ctx->own_stream;
+    PCM_CUDA(ctx, cudaMemcpyAsync(ctx->io_a, q_host, bytes, cudaMemcpyHostToDevice, s));
+    if ((rc = launch_amatvec(ctx, ctx->io_a, ctx->io_b, s))) return rc;
+    PCM_CUDA(ctx, cudaMemcpyAsync(y_host, ctx->io_b, bytes, cudaMemcpyDeviceToHost, s));
+    PCM_CUDA(ctx, cudaStreamSynchronize(s));
+    return PCM_OK;
+}
+
+int pcm_cg_solve_host(pcm_ctx *ctx, const double *b_host, double *x_host, double tol, int max_iter, int precond,
+                      int use_x0, int *iters, double *resid) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->M > 0 && (!b_host || !x_host)) return set_error(ctx, PCM_ERR_ARG, "pcm_cg_solve_host: NULL vector");
+    if (max_iter < 0 || !(tol >= 0.0)) return set_error(ctx, PCM_ERR_ARG, "pcm_cg_solve_host: bad tol or max_iter");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    int rc;
+    const size_t bytes = (size_t)ctx->M * 8;
+    if ((rc = ensure_io(ctx, &ctx->io_a, &ctx->io_a_bytes, bytes))) return rc;
+    if ((rc = ensure_io(ctx, &ctx->io_b, &ctx->io_b_bytes, bytes))) return rc;
+    cudaStream_t s = ctx->own_stream;
+    if (bytes) PCM_CUDA(ctx, cudaMemcpyAsync(ctx->io_a, b_host, bytes, cudaMemcpyHostToDevice, s));
+    if (bytes && use_x0) PCM_CUDA(ctx, cudaMemcpyAsync(ctx->io_b, x_host, bytes, cudaMemcpyHostToDevice, s));
+    const int status = cg_solve(ctx, ctx->io_a, ctx->io_b, tol, max_iter, precond, use_x0, iters, resid, s);
+    if (status < 0) return status;
+    if (bytes) PCM_CUDA(ctx, cudaMemcpyAsync(x_host, ctx->io_b, bytes, cudaMemcpyDeviceToHost, s));
+    PCM_CUDA(ctx, cudaStreamSynchronize(s));
+    return status;
+}
+
+int pcm_get_info(pcm_ctx *ctx, pcm_info *out) {
+    PCM_CHECK_CTX(ctx);
+    if (!out) return set_error(ctx, PCM_ERR_ARG, "pcm_get_info: out is NULL");
+    ctx->info.device_bytes = ctx->device_bytes;
+    *out = ctx->info;
+    return PCM_OK;
+}
+
+int pcm_set_timing(pcm_ctx *ctx, int enable) {
+    PCM_CHECK_CTX(ctx);
+    ctx->timing = enable ? 1 : 0;
+    return PCM_OK;
+}
+
+int pcm_last_kernel_ms(pcm_ctx *ctx, int op, double ms[2], int *n_launch) {
+    PCM_CHECK_CTX(ctx);
+    if (op < 0 || op > 2) return set_error(ctx, PCM_ERR_ARG, "pcm_last_kernel_ms: op must be 0, 1 or 2");
+    if (n_launch) *n_launch = ctx->launches[op];
+    if (!ms) return PCM_OK;
+    ms[0] = ms[1] = 0.0;
+    if (!ctx->timed[op]) return set_error(ctx, PCM_ERR_STATE, "pcm_last_kernel_ms: the last call of this op was not timed (pcm_set_timing)");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaEvent_t *ev = ctx->ev + 8 * op;
+    PCM_CUDA(ctx, cudaEventSynchronize(ev[7]));
+    float a = 0, b = 0, c = 0;
+    PCM_CUDA(ctx, cudaEventElapsedTime(&a, ev[0], ev[1]));
+    PCM_CUDA(ctx, cudaEventElapsedTime(&b, ev[1], ev[6]));
+    PCM_CUDA(ctx, cudaEventElapsedTime(&c, ev[6], ev[7]));
+    ms[0] = b;
+    ms[1] = (double)a + c;
+    return PCM_OK;
+}
+
+int pcm_last_class_ms(pcm_ctx *ctx, int op, double ms[PCM_NL]) {
+    PCM_CHECK_CTX(ctx);
+    if (op < 0 || op > 2 || !ms) return set_error(ctx, PCM_ERR_ARG, "pcm_last_class_ms: bad argument");
+    if (!ctx->timed[op]) return set_error(ctx, PCM_ERR_STATE, "pcm_last_class_ms: the last call of this op was not timed (pcm_set_timing)");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaEvent_t *ev = ctx->ev + 8 * op;
+    PCM_CUDA(ctx, cudaEventSynchronize(ev[7]));
+    for (int L = 0; L < PCM_NL; ++L) {
+        float t = 0;
+        PCM_CUDA(ctx, cudaEventElapsedTime(&t, ev[1 + L], ev[2 + L]));
+        ms[L] = t;
+    }
+    return PCM_OK;
+}
+
+int pcm_launch_count(pcm_ctx *ctx, int64_t *total) {
+    PCM_CHECK_CTX(ctx);
+    if (!total) return set_error(ctx, PCM_ERR_ARG, "pcm_launch_count: total is NULL");
+    *total = ctx->launch_total;
+    return PCM_OK;
+}
+
+int pcm_fp64_peak(pcm_ctx *ctx, int reps, double *tflops) {
+    PCM_CHECK_CTX(ctx);
+    if (!tflops) return set_error(ctx, PCM_ERR_ARG, "pcm_fp64_peak: tflops is NULL");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return fp64_peak(ctx, reps, tflops);
+}
+
+int pcm_schwarz_bound(int la, double alpha, const double *A, int lb, double beta, const double *B, double *out) {
+    if (la < 0 || la > 2 || lb < 0 || lb > 2 || !A || !B || !out || !(alpha > 0.0) || !(beta > 0.0)) return PCM_ERR_ARG;
+    *out = schwarz_bound(la, alpha, A, lb, beta, B);
+    return PCM_OK;
+}
+
+const char *pcm_last_error(pcm_ctx *ctx) { return ctx ? ctx->err.c_str() : setup_error_text(); }
+
+int pcm_destroy(pcm_ctx *ctx) {
+    free_ctx(ctx);
+    return PCM_OK;
+}
+
+}  // extern "C"

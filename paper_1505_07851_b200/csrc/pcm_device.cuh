@@ -1,0 +1,138 @@
+// pcm_device.cuh -- device arithmetic shared by the three hot kernels: fp64 reciprocal square root,
+// tabulated Boys function, and the Hermite Coulomb recursion R_tuv (McMurchie-Davidson) with the
+// effective exponent rho = p zeta^2/(p + zeta^2) of the smeared-charge operator (Eq. 6).
+#pragma once
+
+#include "pcm_internal.h"
+
+namespace pcm {
+
+__device__ __forceinline__ int hi32(double x) { return __double2hiint(x); }
+
+// 1/sqrt(x), x > 0 normal.  MUFU.RSQ64H seed (2^-22.9 relative) + one third-order step:
+// y <- y (1 + e/2 + 3 e^2/8), e = 1 - x y^2; remaining error 5 e^3/16 ~ 2^-70, i.e. rounding only.
+__device__ __forceinline__ double rsqrt_fast(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double h = x * y;
+    const double e = fma(-h, y, 1.0);
+    const double t = fma(e, 0.375, 0.5);
+    const double ye = y * e;
+    return fma(ye, t, y);
+}
+
+// Far-field Hermite seeds, normalised so that g_n = (-1)^n (2n-1)!! / R^(2n+1)  (derivatives of 1/R):
+// for T >= TFAR(L) the smeared charge is a point charge to fp64 and
+//   (2 pi/p) sqrt(rho/p) (-2 rho)^n F_n(T) = (pi/p)^{3/2} K^-1 ... = [ (2 pi/p) kappa ] g_n,  kappa = sqrt(pi/p)/2.
+template <int L>
+__device__ __forceinline__ void seeds_far(double R2, double (&g)[L + 1]) {
+    const double ri = rsqrt_fast(R2);
+    g[0] = ri;
+    if (L > 0) {
+        const double u = ri * ri;
+#pragma unroll
+        for (int n = 1; n <= L; ++n) g[n] = g[n - 1] * (u * (double)(-(2 * n - 1)));
+    }
+}
+
+// General seeds: g_n = (w/kappa) (-2 rho)^n F_n(rho R2), w = sqrt(rho/p) = 1/sqrt(1 + p/zeta^2).
+// F_L by an 8-term Taylor expansion about the nearest table row, lower orders by downward recursion
+// F_{n-1} = (2T F_n + exp(-T))/(2n-1); beyond the switch the far-field form.
+template <int L>
+__device__ __forceinline__ void seeds_general(double R2, double p, double invk, double iz2,
+                                               const double *__restrict__ boysL, double (&g)[L + 1]) {
+    const double w = rsqrt_fast(fma(p, iz2, 1.0));
+    const double rho = p * w * w;
+    const double T = rho * R2;
+    if (T >= tfar(L)) {
+        seeds_far<L>(R2, g);
+        return;
+    }
+    const int i = __double2int_rn(T * 16.0);
+    const double d = T - (double)i * 0.0625;
+    const double *row = boysL + (size_t)i * BOYS_STRIDE;
+    double f = __ldg(row + BOYS_TERMS - 1);
+#pragma unroll
+    for (int k = BOYS_TERMS - 2; k >= 0; --k) f = fma(f, d, __ldg(row + k));
+    double F[L + 1];
+    F[L] = f;
+    if (L > 0) {
+        // exp(-T) = exp(-T_i) exp(-d), |d| <= 1/32: degree-8 Taylor polynomial (next term 8e-20)
+        double e = 1.0 / 40320.0;
+        e = fma(e, -d, 1.0 / 5040.0);
+        e = fma(e, -d, 1.0 / 720.0);
+        e = fma(e, -d, 1.0 / 120.0);
+        e = fma(e, -d, 1.0 / 24.0);
+        e = fma(e, -d, 1.0 / 6.0);
+        e = fma(e, -d, 0.5);
+        e = fma(e, -d, 1.0);
+        e = fma(e, -d, 1.0);
+        e *= __ldg(row + BOYS_TERMS);
+        const double T2 = T + T;
+#pragma unroll
+        for (int n = L; n >= 1; --n) F[n - 1] = fma(T2, F[n], e) * (1.0 / (double)(2 * n - 1));
+    }
+    double s = w * invk;
+    const double m2r = -2.0 * rho;
+#pragma unroll
+    for (int n = 0; n <= L; ++n) {
+        g[n] = s * F[n];
+        s *= m2r;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Hermite Coulomb integrals from the seeds:  R^n_000 = g_n,
+//   R^n_{t+1,u,v} = t R^{n+1}_{t-1,u,v} + x R^{n+1}_{t,u,v}   (and likewise for u, v), (x,y,z) = P - C.
+// All loops have compile-time bounds: after unrolling every index is a constant and the arrays live in
+// registers.  The direction lowered is the one with the smallest non-zero power (a power of 1 or 2
+// costs one instruction, 3 or 4 costs two).
+// The order-0 integrals are handed to `sink` once per component h = hidx(t,u,v): sink.value(h, R) or, when R
+// is a single product a*b, sink.product(h, a, b) so that the consumer can fuse it into an FMA.
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int pick_dir(int t, int u, int v) {
+    int best = -1, bp = 99;
+    if (t > 0 && t < bp) { best = 0; bp = t; }
+    if (u > 0 && u < bp) { best = 1; bp = u; }
+    if (v > 0 && v < bp) { best = 2; bp = v; }
+    return best;
+}
+
+template <int L, class Sink>
+__device__ __forceinline__ void hermite_R(double x, double y, double z, const double (&g)[L + 1], Sink &sink) {
+    constexpr int NH = nherm(L);
+    double R[L + 1][NH];  // R[n][h] for degree(h) <= L - n; unused entries are never materialised
+#pragma unroll
+    for (int n = 0; n <= L; ++n) R[n][0] = g[n];
+    sink.value(0, R[0][0]);
+#pragma unroll
+    for (int d = 1; d <= L; ++d) {
+#pragma unroll
+        for (int n = L - d; n >= 0; --n) {
+#pragma unroll
+            for (int t = d; t >= 0; --t) {
+#pragma unroll
+                for (int u = d - t; u >= 0; --u) {
+                    const int v = d - t - u;
+                    const int dir = pick_dir(t, u, v);
+                    const int pw = dir == 0 ? t : (dir == 1 ? u : v);          // power being lowered
+                    const double c = dir == 0 ? x : (dir == 1 ? y : z);
+                    const int h1 = dir == 0 ? hidx(t - 1, u, v) : (dir == 1 ? hidx(t, u - 1, v) : hidx(t, u, v - 1));
+                    const int h2 = pw < 2 ? 0 : (dir == 0 ? hidx(t - 2, u, v) : (dir == 1 ? hidx(t, u - 2, v) : hidx(t, u, v - 2)));
+                    const int h = hidx(t, u, v);
+                    if (pw == 1) {
+                        if (n == 0) sink.product(h, c, R[n + 1][h1]);
+                        else R[n][h] = c * R[n + 1][h1];
+                    } else {
+                        const double lower = (pw == 2) ? R[n + 1][h2] : (double)(pw - 1) * R[n + 1][h2];
+                        const double val = fma(c, R[n + 1][h1], lower);
+                        if (n == 0) sink.value(h, val);
+                        else R[n][h] = val;
+                    }
+                }
+            }
+        }
+    }
+}
+
+}  // namespace pcm

@@ -1,0 +1,147 @@
+// pcm_internal.h -- context layout and shared host/device constants of libpcm_b200.
+// Product code: shares nothing with oracle/ (see DESIGN.md "Independence").
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/pcm.h"
+
+namespace pcm {
+
+// ---------------------------------------------------------------------------------------------
+// Hermite index space.  A Hermite Gaussian product of total angular momentum L carries
+// NHERM(L) = (L+1)(L+2)(L+3)/6 components Lambda_tuv, t+u+v <= L, ordered by degree d = t+u+v
+// first so that the components of a lower L are a prefix of those of a higher L:
+//   index(t,u,v) = d(d+1)(d+2)/6 + (d-t)(d-t+1)/2 + (d-t-u)
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int nherm(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
+__host__ __device__ constexpr int hidx(int t, int u, int v) {
+    return (t + u + v) * (t + u + v + 1) * (t + u + v + 2) / 6 + (u + v) * (u + v + 1) / 2 + v;
+}
+
+// Far-field switch: for T = rho |P-C|^2 >= TFAR(L) the Boys functions F_0..F_L equal
+// their asymptotic forms to better than 2e-17 relative (the neglected tail is exp(-T) T^{n-1/2}/Gamma(n+1/2)).
+__host__ __device__ constexpr double tfar(int L) { return 38.0 + 3.0 * L; }
+constexpr double TFAR_AMAT = 38.0;  // erfc(sqrt(38)) = 3e-18
+
+// Boys table: rows T_i = i/16, i = 0..BOYS_ROWS-1 (covers [0, 52]); per L a table of rows
+// {c_0..c_7, exp(-T_i), 0} with c_k = (-1)^k F_{L+k}(T_i)/k!  so that F_L(T_i + d) = sum_k c_k d^k.
+constexpr int BOYS_ROWS = 52 * 16 + 1;
+constexpr int BOYS_STRIDE = 10;
+constexpr int BOYS_TERMS = 8;
+
+constexpr int MAXL = 4;
+
+struct DeviceBuf {  // owning device allocation
+    void *p = nullptr;
+    size_t bytes = 0;
+};
+
+struct ClassData {        // products of one total angular momentum L, padded to a multiple of 128
+    int64_t n = 0;        // products
+    int64_t npad = 0;     // padded count (SoA leading dimension)
+    int64_t first = 0;    // global index of the first product of this class
+    double4 *prodA = nullptr;  // (Px, Py, Pz, thr): hi word of thr is the far-field threshold on |P-C|^2
+    double2 *prodB = nullptr;  // (p, 1/kappa) with kappa = sqrt(pi/p)/2
+    double *herm = nullptr;    // [nchunk_max][nherm(L)][npad] Hermite vectors (density D or potential sums H)
+    int64_t herm_slots = 0;    // chunks the herm buffer can hold
+};
+
+}  // namespace pcm
+
+struct pcm_ctx {
+    int device = 0;
+    int sm_count = 148;
+    pcm_options opt{};
+    pcm_info info{};
+    std::string err;
+
+    // points
+    int64_t M = 0;
+    double4 *pt = nullptr;      // (x, y, z, 1/zeta^2)
+    double *pt_diag = nullptr;  // A_kk = zeta_k sqrt(2/pi)/S_k
+    double zeta_min = 0, zeta_max = 0;
+
+    // basis / pairs
+    int64_t nbf = 0;
+    int64_t nprod = 0;   // all products
+    int64_t nmember = 0; // surviving primitive pairs (diagonal shell pairs: i <= j)
+    int64_t nsp = 0;     // surviving shell pairs
+    int64_t ncomp = 0;   // sum over shell pairs of na*nb
+    pcm::ClassData cls[pcm::MAXL + 1];
+
+    // members (sorted by shell pair)
+    int32_t *m_prod = nullptr;   // global product index
+    int32_t *m_sp = nullptr;     // shell pair of the member
+    int32_t *m_cls = nullptr;    // packed: L_member | (L_product << 8)
+    int64_t *m_goff = nullptr;   // offset of the member's G matrix [na*nb][nherm(L_member)]
+    double *G = nullptr;
+    // product -> members CSR (global product order)
+    int64_t *pm_start = nullptr;
+    int32_t *pm_list = nullptr;
+    // shell pairs
+    int64_t *sp_mstart = nullptr;  // [nsp+1] member range
+    int32_t *sp_i0 = nullptr, *sp_j0 = nullptr;  // basis-function offsets
+    int32_t *sp_dims = nullptr;    // na | nb<<8 | diag<<16
+    // component -> (shell pair, ab)
+    int32_t *c_sp = nullptr;
+    int32_t *c_ab = nullptr;
+
+    double *boys = nullptr;  // [MAXL+1][BOYS_ROWS][BOYS_STRIDE]
+
+    // scratch
+    double *vpart = nullptr;    // potential partial sums [slots][M]
+    int64_t vpart_slots = 0;
+    double *ypart = nullptr;    // amatvec partial sums [slots][M]
+    int64_t ypart_slots = 0;
+    double *cg_vec = nullptr;   // 5 M doubles: r, z, p, Ap, tmp
+    double *cg_scal = nullptr;  // device scalars
+    double *cg_scal_host = nullptr;  // pinned
+    double *io_a = nullptr, *io_b = nullptr;  // staging for the *_host calls
+    size_t io_a_bytes = 0, io_b_bytes = 0;
+
+    // RBJ
+    int64_t rbj_block = 0, rbj_nblocks = 0;
+    int32_t *rbj_order = nullptr;    // [M] point indices block after block
+    int64_t *rbj_bstart_host = nullptr;
+    double *rbj_inv = nullptr;       // inverse blocks back to back (block b at b*l*l)
+
+    cudaStream_t own_stream = nullptr;
+    // events: 0 start, 1 after the pre-transform, 2+L after the class-L main kernel, 7 end, 8 CG residual read-back
+    cudaEvent_t ev[28] = {};   // ev[8*op + i], op = 0 potential, 1 fock, 2 amatvec; 24 CG; 25, 26 peak benchmark
+    int timing = 0;
+    int cur_op = 0;
+    int launches[3] = {0, 0, 0};   // kernels launched by the last call of each op
+    int64_t launch_total = 0;   // kernels launched by this context since pcm_setup
+    bool timed[3] = {false, false, false};
+
+    std::vector<void *> allocs;  // everything cudaMalloc'ed, freed in pcm_destroy
+    int64_t device_bytes = 0;
+};
+
+// ---- internal entry points (pcm_setup.cu, pcm_kernels.cu, pcm_solver.cu) ----
+namespace pcm {
+int set_error(pcm_ctx *ctx, int code, const std::string &msg);
+int dev_alloc(pcm_ctx *ctx, void **p, size_t bytes);
+template <class T>
+inline int dev_alloc_t(pcm_ctx *ctx, T **p, size_t count) {
+    return dev_alloc(ctx, reinterpret_cast<void **>(p), count * sizeof(T));
+}
+int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cudaStream_t s);
+int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accumulate, cudaStream_t s);
+int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s);
+int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
+void build_boys_tables(std::vector<double> &tab);
+double schwarz_bound(int la, double alpha, const double *A, int lb, double beta, const double *B);
+}  // namespace pcm
+
+#define PCM_CUDA(ctx, call)                                                                               \
+    do {                                                                                                  \
+        cudaError_t e__ = (call);                                                                         \
+        if (e__ != cudaSuccess)                                                                           \
+            return pcm::set_error(ctx, PCM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); \
+    } while (0)

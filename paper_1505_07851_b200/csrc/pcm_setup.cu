@@ -1,0 +1,460 @@
+// pcm_setup.cu -- host side of step a1: shell-pair enumeration, Eq. 15 screening,
+// Hermite Gaussian product merging, class sort, SoA packing and upload.  Also the Boys tables.
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <cstring>
+#include <unordered_map>
+
+#include "pcm_internal.h"
+
+namespace pcm {
+
+static thread_local std::string g_setup_error;
+
+int set_error(pcm_ctx *ctx, int code, const std::string &msg) {
+    if (ctx) ctx->err = msg; else g_setup_error = msg;
+    return code;
+}
+const char *setup_error_text() { return g_setup_error.c_str(); }
+
+int dev_alloc(pcm_ctx *ctx, void **p, size_t bytes) {
+    *p = nullptr;
+    if (bytes == 0) bytes = 8;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) return set_error(ctx, PCM_ERR_ALLOC, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    ctx->allocs.push_back(*p);
+    ctx->device_bytes += (int64_t)bytes;
+    return PCM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Boys tables.  F_n(T) = int_0^1 t^2n exp(-T t^2) dt.  Highest order by the all-positive series
+//   F_n(T) = exp(-T) sum_k (2T)^k / ((2n+1)(2n+3)...(2n+2k+1))
+// in long double, lower orders by downward recursion F_{n-1} = (2T F_n + exp(-T))/(2n-1).
+// Row i of table L holds c_k = (-1)^k F_{L+k}(T_i)/k!, k = 0..7 (Taylor coefficients of F_L about T_i:
+// dF_n/dT = -F_{n+1}), then exp(-T_i).
+// ---------------------------------------------------------------------------------------------
+void build_boys_tables(std::vector<double> &tab) {
+    const int nmax = MAXL + BOYS_TERMS - 1;
+    tab.assign((size_t)(MAXL + 1) * BOYS_ROWS * BOYS_STRIDE, 0.0);
+    std::vector<long double> F(nmax + 1);
+    for (int i = 0; i < BOYS_ROWS; ++i) {
+        const long double T = (long double)i / 16.0L;
+        const long double eT = expl(-T);
+        long double term = 1.0L / (2.0L * nmax + 1.0L), sum = term;
+        for (int k = 1; k < 4000; ++k) {
+            term *= 2.0L * T / (2.0L * nmax + 2.0L * k + 1.0L);
+            sum += term;
+            if (term < 1e-22L * sum) break;
+        }
+        F[nmax] = eT * sum;
+        for (int n = nmax; n >= 1; --n) F[n - 1] = (2.0L * T * F[n] + eT) / (2.0L * n - 1.0L);
+        for (int L = 0; L <= MAXL; ++L) {
+            double *row = &tab[((size_t)L * BOYS_ROWS + i) * BOYS_STRIDE];
+            long double fact = 1.0L;
+            for (int k = 0; k < BOYS_TERMS; ++k) {
+                if (k > 0) fact *= k;
+                row[k] = (double)(((k & 1) ? -1.0L : 1.0L) * F[L + k] / fact);
+            }
+            row[BOYS_TERMS] = (double)eT;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// One-dimensional Hermite expansion coefficients E^{ij}_t, i, j <= 2 (McMurchie-Davidson):
+//   E^{00}_0 = exp(-mu X_AB^2),  E^{i+1,j}_t = E^{ij}_{t-1}/2p + X_PA E^{ij}_t + (t+1) E^{ij}_{t+1}
+// ---------------------------------------------------------------------------------------------
+struct E1D {
+    double e[3][3][5];
+};
+static void hermite_E(double a, double b, double Ax, double Bx, int la, int lb, E1D &E) {
+    const double p = a + b, mu = a * b / p;
+    const double Px = (a * Ax + b * Bx) / p;
+    const double XPA = Px - Ax, XPB = Px - Bx, XAB = Ax - Bx, h = 0.5 / p;
+    std::memset(&E, 0, sizeof(E));
+    E.e[0][0][0] = std::exp(-mu * XAB * XAB);
+    for (int i = 0; i < la; ++i)
+        for (int t = 0; t <= i + 1; ++t)
+            E.e[i + 1][0][t] = (t > 0 ? h * E.e[i][0][t - 1] : 0.0) + XPA * E.e[i][0][t] + (t + 1) * (t + 1 <= i ? E.e[i][0][t + 1] : 0.0);
+    for (int i = 0; i <= la; ++i)
+        for (int j = 0; j < lb; ++j)
+            for (int t = 0; t <= i + j + 1; ++t)
+                E.e[i][j + 1][t] = (t > 0 ? h * E.e[i][j][t - 1] : 0.0) + XPB * E.e[i][j][t] + (t + 1) * (t + 1 <= i + j ? E.e[i][j][t + 1] : 0.0);
+}
+
+static const int CARTS[3][6][3] = {{{0, 0, 0}},
+                                   {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}},
+                                   {{2, 0, 0}, {1, 1, 0}, {1, 0, 1}, {0, 2, 0}, {0, 1, 1}, {0, 0, 2}}};
+static const int NCART[3] = {1, 3, 6};
+
+static double dfact_m1(int T) {  // (T-1)!! for even T >= 0
+    double r = 1.0;
+    for (int k = T - 1; k > 1; k -= 2) r *= k;
+    return r;
+}
+
+// max over Cartesian components of [chi_a chi_b|chi_a chi_b]^{1/2} for raw primitives (Eq. 15; closed form
+// SURVEY.md 8(c4)): (ab|ab) = 2 pi^{5/2}/(p^2 sqrt(2p)) sum E_tuv E_t'u'v' (-1)^{t'+u'+v'} R_{t+t',u+u',v+v'}(p/2, 0)
+double schwarz_bound(int la, double alpha, const double *A, int lb, double beta, const double *B) {
+    const double p = alpha + beta;
+    E1D Ex, Ey, Ez;
+    hermite_E(alpha, beta, A[0], B[0], la, lb, Ex);
+    hermite_E(alpha, beta, A[1], B[1], la, lb, Ey);
+    hermite_E(alpha, beta, A[2], B[2], la, lb, Ez);
+    const double pref = 2.0 * std::pow(M_PI, 2.5) / (p * p * std::sqrt(2.0 * p));
+    double best = 0.0;
+    for (int ia = 0; ia < NCART[la]; ++ia)
+        for (int ib = 0; ib < NCART[lb]; ++ib) {
+            const int *a = CARTS[la][ia], *b = CARTS[lb][ib];
+            const int nx = a[0] + b[0], ny = a[1] + b[1], nz = a[2] + b[2];
+            double s = 0.0;
+            for (int t = 0; t <= nx; ++t)
+                for (int u = 0; u <= ny; ++u)
+                    for (int v = 0; v <= nz; ++v) {
+                        const double e1 = Ex.e[a[0]][b[0]][t] * Ey.e[a[1]][b[1]][u] * Ez.e[a[2]][b[2]][v];
+                        if (e1 == 0.0) continue;
+                        for (int t2 = (t & 1); t2 <= nx; t2 += 2)
+                            for (int u2 = (u & 1); u2 <= ny; u2 += 2)
+                                for (int v2 = (v & 1); v2 <= nz; v2 += 2) {
+                                    const double e2 = Ex.e[a[0]][b[0]][t2] * Ey.e[a[1]][b[1]][u2] * Ez.e[a[2]][b[2]][v2];
+                                    const int T = t + t2, U = u + u2, V = v + v2, n = (T + U + V) / 2;
+                                    const double R = std::pow(-p, n) * dfact_m1(T) * dfact_m1(U) * dfact_m1(V) / (2.0 * n + 1.0);
+                                    s += (((t2 + u2 + v2) & 1) ? -1.0 : 1.0) * e1 * e2 * R;
+                                }
+                    }
+            best = std::max(best, pref * s);
+        }
+    return std::sqrt(std::max(best, 0.0));
+}
+
+// rows: pure component, cols: Cartesian d (xx,xy,xz,yy,yz,zz); identity-like for s, p and Cartesian d
+static void component_matrix(int l, int d_pure, double m[6][6], int &ncomp) {
+    std::memset(m, 0, sizeof(double) * 36);
+    if (l < 2 || !d_pure) {
+        ncomp = NCART[l];
+        for (int i = 0; i < ncomp; ++i) m[i][i] = 1.0;
+        return;
+    }
+    const double s3 = std::sqrt(3.0);
+    ncomp = 5;
+    m[0][1] = s3;
+    m[1][4] = s3;
+    m[2][5] = 1.0; m[2][0] = -0.5; m[2][3] = -0.5;
+    m[3][2] = s3;
+    m[4][0] = 0.5 * s3; m[4][3] = -0.5 * s3;
+}
+
+static inline uint64_t spread21(uint64_t x) {
+    x &= 0x1fffff;
+    x = (x | x << 32) & 0x1f00000000ffffULL;
+    x = (x | x << 16) & 0x1f0000ff0000ffULL;
+    x = (x | x << 8) & 0x100f00f00f00f00fULL;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ULL;
+    x = (x | x << 2) & 0x1249249249249249ULL;
+    return x;
+}
+
+struct KeyHash {
+    size_t operator()(const std::array<uint64_t, 4> &k) const {
+        uint64_t h = 0x9E3779B97F4A7C15ULL;
+        for (uint64_t v : k) { h ^= v + 0x9E3779B97F4A7C15ULL + (h << 6) + (h >> 2); h *= 0xBF58476D1CE4E5B9ULL; }
+        return (size_t)h;
+    }
+};
+
+struct HostMember {
+    int32_t sp;       // shell pair (final index)
+    int32_t prod;     // product (temporary index, remapped after the sort)
+    int8_t L;         // la + lb
+    int64_t goff;
+};
+struct HostPair {
+    int I, J, cls;
+    std::vector<std::pair<int, int>> prims;  // surviving (i, j)
+};
+
+template <class T>
+static int upload(pcm_ctx *ctx, T **dst, const std::vector<T> &src) {
+    int rc = dev_alloc_t(ctx, dst, src.size());
+    if (rc) return rc;
+    if (!src.empty()) PCM_CUDA(ctx, cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return PCM_OK;
+}
+
+static int class_of(int la, int lb) {
+    int lo = std::min(la, lb), hi = std::max(la, lb);
+    static const int tab[3][3] = {{0, 1, 3}, {1, 2, 4}, {3, 4, 5}};
+    return tab[lo][hi];
+}
+
+int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *shell_xyz, const int *shell_nprim,
+                  const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
+                  const double *pt_zeta, const double *pt_switch) {
+    const pcm_options &opt = ctx->opt;
+    // ------------------------------------------------------------------ points
+    ctx->M = npoint;
+    {
+        std::vector<double4> pt((size_t)npoint);
+        std::vector<double> diag((size_t)npoint);
+        double zmin = 1e300, zmax = 0.0;
+        for (int64_t k = 0; k < npoint; ++k) {
+            const double z = pt_zeta[k];
+            pt[k] = make_double4(pt_xyz[3 * k], pt_xyz[3 * k + 1], pt_xyz[3 * k + 2], 1.0 / (z * z));
+            diag[k] = z * std::sqrt(2.0 / M_PI) / (pt_switch ? pt_switch[k] : 1.0);
+            zmin = std::min(zmin, z);
+            zmax = std::max(zmax, z);
+        }
+        if (npoint == 0) zmin = zmax = 1.0;
+        ctx->zeta_min = zmin;
+        ctx->zeta_max = zmax;
+        int rc = upload(ctx, &ctx->pt, pt);
+        if (rc) return rc;
+        rc = upload(ctx, &ctx->pt_diag, diag);
+        if (rc) return rc;
+    }
+    {
+        std::vector<double> tab;
+        build_boys_tables(tab);
+        int rc = upload(ctx, &ctx->boys, tab);
+        if (rc) return rc;
+    }
+
+    // ------------------------------------------------------------------ shells
+    std::vector<int64_t> poff(nshell + 1, 0), boff(nshell + 1, 0);
+    std::vector<double> amin(nshell), cmax(nshell);
+    for (int s = 0; s < nshell; ++s) {
+        int nc = shell_l[s] == 0 ? 1 : (shell_l[s] == 1 ? 3 : (opt.d_pure ? 5 : 6));
+        poff[s + 1] = poff[s] + shell_nprim[s];
+        boff[s + 1] = boff[s] + nc;
+        double am = 1e300, cm = 0.0;
+        for (int64_t i = poff[s]; i < poff[s + 1]; ++i) { am = std::min(am, prim_exp[i]); cm = std::max(cm, std::fabs(prim_coef[i])); }
+        amin[s] = am;
+        cmax[s] = cm;
+    }
+    ctx->nbf = boff[nshell];
+    const double eps = opt.screen_eps;
+
+    // ------------------------------------------------------------------ shell pairs + Eq. 15 screening
+    std::vector<std::vector<HostPair>> per_row(nshell);
+    int64_t unscreened = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : unscreened)
+    for (int I = 0; I < nshell; ++I) {
+        const double *A = shell_xyz + 3 * I;
+        for (int J = I; J < nshell; ++J) {
+            const double *B = shell_xyz + 3 * J;
+            const int la = shell_l[I], lb = shell_l[J];
+            const int64_t npp = (I == J) ? (int64_t)shell_nprim[I] * (shell_nprim[I] + 1) / 2 : (int64_t)shell_nprim[I] * shell_nprim[J];
+            unscreened += npp;
+            const double r2 = (A[0] - B[0]) * (A[0] - B[0]) + (A[1] - B[1]) * (A[1] - B[1]) + (A[2] - B[2]) * (A[2] - B[2]);
+            // shell-level upper bound of |c c| [ab|ab]^{1/2}: every factor is an upper bound over the primitive pairs
+            const double mu_min = amin[I] * amin[J] / (amin[I] + amin[J]);
+            if (eps > 0.0) {
+                if (mu_min * r2 > 200.0) continue;
+                const double pmin = amin[I] + amin[J];
+                const double reach = std::sqrt(r2) + std::sqrt(2.0 / pmin);
+                const double ub = cmax[I] * cmax[J] * std::exp(-mu_min * r2) * 50.0 * std::pow(pmin, -1.25) * std::pow(std::max(reach, 1.0), la + lb);
+                if (ub < eps) continue;
+            }
+            HostPair hp;
+            hp.I = I; hp.J = J; hp.cls = class_of(la, lb);
+            for (int i = 0; i < shell_nprim[I]; ++i)
+                for (int j = (I == J ? i : 0); j < shell_nprim[J]; ++j) {
+                    const double a = prim_exp[poff[I] + i], b = prim_exp[poff[J] + j];
+                    const double cc = std::fabs(prim_coef[poff[I] + i] * prim_coef[poff[J] + j]);
+                    if (eps > 0.0) {
+                        const double mu = a * b / (a + b);
+                        if (mu * r2 > 200.0) continue;
+                        if (cc * schwarz_bound(la, a, A, lb, b, B) < eps) continue;
+                    }
+                    hp.prims.emplace_back(i, j);
+                }
+            if (!hp.prims.empty()) per_row[I].push_back(std::move(hp));
+        }
+    }
+    std::vector<HostPair> pairs;
+    for (auto &row : per_row) for (auto &hp : row) pairs.push_back(std::move(hp));
+    per_row.clear();
+    std::stable_sort(pairs.begin(), pairs.end(), [](const HostPair &x, const HostPair &y) { return x.cls < y.cls; });
+    ctx->nsp = (int64_t)pairs.size();
+
+    pcm_info &info = ctx->info;
+    std::memset(&info, 0, sizeof(info));
+    info.nbf = ctx->nbf; info.nshell = nshell; info.npoint = npoint;
+    info.prim_pairs_unscreened = unscreened;
+    info.zeta_min = ctx->zeta_min; info.zeta_max = ctx->zeta_max;
+
+    // ------------------------------------------------------------------ members, products, G matrices
+    std::vector<HostMember> members;
+    std::vector<double> G;
+    std::vector<int64_t> sp_mstart(pairs.size() + 1, 0);
+    std::vector<int32_t> sp_i0(pairs.size()), sp_j0(pairs.size()), sp_dims(pairs.size());
+    std::vector<int32_t> c_sp, c_ab;
+    struct HostProd { double p, x, y, z; int L; };
+    std::vector<HostProd> prods;
+    std::unordered_map<std::array<uint64_t, 4>, int32_t, KeyHash> pmap;
+    auto bits = [](double d) { uint64_t u; std::memcpy(&u, &d, 8); return u; };
+
+    for (size_t sp = 0; sp < pairs.size(); ++sp) {
+        const HostPair &hp = pairs[sp];
+        const int I = hp.I, J = hp.J, la = shell_l[I], lb = shell_l[J], L = la + lb, nh = nherm(L);
+        const double *A = shell_xyz + 3 * I, *B = shell_xyz + 3 * J;
+        double Ta[6][6], Tb[6][6];
+        int na, nb;
+        component_matrix(la, opt.d_pure, Ta, na);
+        component_matrix(lb, opt.d_pure, Tb, nb);
+        sp_i0[sp] = (int32_t)boff[I]; sp_j0[sp] = (int32_t)boff[J];
+        sp_dims[sp] = na | (nb << 8) | ((I == J ? 1 : 0) << 16);
+        for (int ab = 0; ab < na * nb; ++ab) { c_sp.push_back((int32_t)sp); c_ab.push_back(ab); }
+        info.shell_pairs[hp.cls] += 1;
+        info.prim_pairs[hp.cls] += (int64_t)hp.prims.size();
+        sp_mstart[sp] = (int64_t)members.size();
+        for (auto ij : hp.prims) {
+            const double a = prim_exp[poff[I] + ij.first], b = prim_exp[poff[J] + ij.second];
+            const double cc = prim_coef[poff[I] + ij.first] * prim_coef[poff[J] + ij.second] * ((I == J && ij.first != ij.second) ? 2.0 : 1.0);
+            const double p = a + b;
+            const double Px = (a * A[0] + b * B[0]) / p, Py = (a * A[1] + b * B[1]) / p, Pz = (a * A[2] + b * B[2]) / p;
+            int32_t prod;
+            if (opt.merge_products) {
+                std::array<uint64_t, 4> key = {bits(p), bits(Px), bits(Py), bits(Pz)};
+                auto it = pmap.find(key);
+                if (it == pmap.end()) {
+                    prod = (int32_t)prods.size();
+                    pmap.emplace(key, prod);
+                    prods.push_back({p, Px, Py, Pz, L});
+                } else {
+                    prod = it->second;
+                    prods[prod].L = std::max(prods[prod].L, L);
+                }
+            } else {
+                prod = (int32_t)prods.size();
+                prods.push_back({p, Px, Py, Pz, L});
+            }
+            HostMember m;
+            m.sp = (int32_t)sp; m.prod = prod; m.L = (int8_t)L; m.goff = (int64_t)G.size();
+            members.push_back(m);
+            // G[ab][h] = cc (pi/p)^{3/2} sum_cart Ta[a][ca] Tb[b][cb] Ex Ey Ez   (K_AB is inside E^{00}_0)
+            E1D Ex, Ey, Ez;
+            hermite_E(a, b, A[0], B[0], la, lb, Ex);
+            hermite_E(a, b, A[1], B[1], la, lb, Ey);
+            hermite_E(a, b, A[2], B[2], la, lb, Ez);
+            const double pref = cc * std::pow(M_PI / p, 1.5);
+            G.resize(G.size() + (size_t)na * nb * nh, 0.0);
+            double *g = G.data() + m.goff;
+            for (int ca = 0; ca < NCART[la]; ++ca)
+                for (int cb = 0; cb < NCART[lb]; ++cb) {
+                    const int *pa = CARTS[la][ca], *pb = CARTS[lb][cb];
+                    for (int t = 0; t <= pa[0] + pb[0]; ++t)
+                        for (int u = 0; u <= pa[1] + pb[1]; ++u)
+                            for (int v = 0; v <= pa[2] + pb[2]; ++v) {
+                                const double e = pref * Ex.e[pa[0]][pb[0]][t] * Ey.e[pa[1]][pb[1]][u] * Ez.e[pa[2]][pb[2]][v];
+                                const int h = hidx(t, u, v);
+                                for (int x = 0; x < na; ++x) {
+                                    if (Ta[x][ca] == 0.0) continue;
+                                    for (int y = 0; y < nb; ++y)
+                                        if (Tb[y][cb] != 0.0) g[(size_t)(x * nb + y) * nh + h] += Ta[x][ca] * Tb[y][cb] * e;
+                                }
+                            }
+                }
+        }
+    }
+    sp_mstart[pairs.size()] = (int64_t)members.size();
+    ctx->nmember = (int64_t)members.size();
+    ctx->ncomp = (int64_t)c_sp.size();
+    for (int c = 0; c < PCM_NCLASS; ++c) info.prim_pairs_total += info.prim_pairs[c];
+
+    // ------------------------------------------------------------------ sort products by (L, Morton(P), p)
+    const int64_t np = (int64_t)prods.size();
+    ctx->nprod = np;
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (auto &q : prods) {
+        lo[0] = std::min(lo[0], q.x); hi[0] = std::max(hi[0], q.x);
+        lo[1] = std::min(lo[1], q.y); hi[1] = std::max(hi[1], q.y);
+        lo[2] = std::min(lo[2], q.z); hi[2] = std::max(hi[2], q.z);
+    }
+    const double span = std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], 1e-9});
+    // coarse Morton cells (~2 bohr) so that products of one neighbourhood end up sorted by exponent inside a cell
+    const double cell = std::max(span / 2097151.0, 2.0);
+    std::vector<uint64_t> mort(np);
+    for (int64_t i = 0; i < np; ++i)
+        mort[i] = spread21((uint64_t)((prods[i].x - lo[0]) / cell)) | (spread21((uint64_t)((prods[i].y - lo[1]) / cell)) << 1) |
+                  (spread21((uint64_t)((prods[i].z - lo[2]) / cell)) << 2);
+    std::vector<int32_t> order(np);
+    for (int64_t i = 0; i < np; ++i) order[i] = (int32_t)i;
+    std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
+        if (prods[x].L != prods[y].L) return prods[x].L < prods[y].L;
+        if (mort[x] != mort[y]) return mort[x] < mort[y];
+        if (prods[x].p != prods[y].p) return prods[x].p > prods[y].p;
+        return x < y;
+    });
+    std::vector<int32_t> newidx(np);
+    for (int64_t i = 0; i < np; ++i) newidx[order[i]] = (int32_t)i;
+
+    // per class SoA
+    int64_t first = 0;
+    for (int L = 0; L <= MAXL; ++L) {
+        int64_t n = 0;
+        while (first + n < np && prods[order[first + n]].L == L) ++n;
+        ClassData &c = ctx->cls[L];
+        c.n = n; c.first = first; c.npad = (n + 127) / 128 * 128;
+        info.products[L] = n;
+        std::vector<double4> pa((size_t)c.npad);
+        std::vector<double2> pb((size_t)c.npad);
+        const double izmin2 = 1.0 / (ctx->zeta_min * ctx->zeta_min);
+        for (int64_t i = 0; i < c.npad; ++i) {
+            if (i < n) {
+                const HostProd &q = prods[order[first + i]];
+                pa[i] = make_double4(q.x, q.y, q.z, tfar(L) * (1.0 / q.p + izmin2));
+                pb[i] = make_double2(q.p, 2.0 * std::sqrt(q.p / M_PI));
+            } else {  // padding: a product that is far from everything and carries zero density
+                pa[i] = make_double4(1e8, 1e8, 1e8, 1.0);
+                pb[i] = make_double2(1.0, 2.0 * std::sqrt(1.0 / M_PI));
+            }
+        }
+        int rc = upload(ctx, &c.prodA, pa);
+        if (rc) return rc;
+        rc = upload(ctx, &c.prodB, pb);
+        if (rc) return rc;
+        first += n;
+    }
+    info.products_total = np;
+    info.prim_pair_points = (double)info.prim_pairs_total * (double)npoint;
+    info.product_points = (double)np * (double)npoint;
+
+    // members: remap products, CSR product -> members
+    std::vector<int32_t> m_prod(members.size()), m_cls(members.size()), m_sp(members.size());
+    std::vector<int64_t> m_goff(members.size());
+    std::vector<int64_t> pm_start(np + 1, 0);
+    for (size_t m = 0; m < members.size(); ++m) {
+        const int32_t g = newidx[members[m].prod];
+        m_prod[m] = g;
+        m_cls[m] = members[m].L | (prods[members[m].prod].L << 8);
+        m_goff[m] = members[m].goff;
+        m_sp[m] = members[m].sp;
+        pm_start[g + 1] += 1;
+    }
+    for (int64_t i = 0; i < np; ++i) pm_start[i + 1] += pm_start[i];
+    std::vector<int32_t> pm_list(members.size());
+    {
+        std::vector<int64_t> fill(pm_start.begin(), pm_start.end() - 1);
+        for (size_t m = 0; m < members.size(); ++m) pm_list[fill[m_prod[m]]++] = (int32_t)m;
+    }
+    int rc;
+    if ((rc = upload(ctx, &ctx->m_prod, m_prod))) return rc;
+    if ((rc = upload(ctx, &ctx->m_cls, m_cls))) return rc;
+    if ((rc = upload(ctx, &ctx->m_sp, m_sp))) return rc;
+    if ((rc = upload(ctx, &ctx->m_goff, m_goff))) return rc;
+    if ((rc = upload(ctx, &ctx->G, G))) return rc;
+    if ((rc = upload(ctx, &ctx->pm_start, pm_start))) return rc;
+    if ((rc = upload(ctx, &ctx->pm_list, pm_list))) return rc;
+    if ((rc = upload(ctx, &ctx->sp_mstart, sp_mstart))) return rc;
+    if ((rc = upload(ctx, &ctx->sp_i0, sp_i0))) return rc;
+    if ((rc = upload(ctx, &ctx->sp_j0, sp_j0))) return rc;
+    if ((rc = upload(ctx, &ctx->sp_dims, sp_dims))) return rc;
+    if ((rc = upload(ctx, &ctx->c_sp, c_sp))) return rc;
+    if ((rc = upload(ctx, &ctx->c_ab, c_ab))) return rc;
+    return PCM_OK;
+}
+
+}  // namespace pcm

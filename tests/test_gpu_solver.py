@@ -1,0 +1,150 @@
+"""GPU checks of the randomized block-Jacobi build and pcm_cg_solve against the
+oracle.  The 1e-10 parity bar applies to v, F and A q entries; the iterative solve is pinned by its residual, by
+dense LAPACK on small M, by the oracle's iteration count (+-2) and by the paper's qualitative statements
+(block size 1 = Jacobi, block size M = one step, RBJ beats Jacobi for M >~ 1000).
+
+Block selection decides integers from floating point (the l-1 largest A_kj): both sides evaluate A_kj in fp64 but
+not bit-identically (libm erf vs tabulated Boys), so near-ties may legitimately be ordered differently.  The test
+therefore checks what is unique (partition, sizes, pivots) and that every chosen set is valid with respect to the
+oracle's A to a relative 1e-12, and compares the block sets exactly where no near-tie exists.
+"""
+import numpy as np
+import pytest
+
+import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def pcm():
+    import paper_1505_07851_b200 as m
+    m.lib()
+    return m
+
+
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda")
+
+
+def points_ctx(pcm, s):
+    z = np.zeros(0)
+    return pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), z, z, s.xyz, s.zeta, s.switch)
+
+
+@pytest.fixture(scope="module")
+def sys2500(pcm, orc):
+    s, q, q_true = synth.make_solver_points(2500, seed=1004)
+    A = orc.amatrix(s)
+    return s, A, q_true, points_ctx(pcm, s)
+
+
+@pytest.mark.parametrize("l", [1, 7, 64, 100])
+def test_rbj_blocks_valid(pcm, orc, sys2500, l):
+    s, A, _, ctx = sys2500
+    M = s.M
+    piv = pcm.pcm_pivot_order(77, M)
+    pcm.pcm_rbj_build(ctx, l, seed=77)
+    order, bstart, inv = pcm.pcm_rbj_get(ctx)
+    info = pcm.pcm_get_info(ctx)
+    assert info.rbj_block == l and info.rbj_nblocks == (M + l - 1) // l == len(bstart) - 1
+    assert sorted(order.tolist()) == list(range(M))
+    sizes = np.diff(bstart)
+    assert (sizes[:-1] == l).all() and 0 < sizes[-1] <= l
+    o_order, o_bstart, _ = orc.rbj_build(s, l, piv)
+    np.testing.assert_array_equal(bstart, o_bstart)
+    assigned = np.zeros(M, bool)
+    pos = 0
+    same_sets = 0
+    for b in range(len(sizes)):
+        idx = order[bstart[b]:bstart[b + 1]]
+        while assigned[piv[pos]]:
+            pos += 1
+        k = piv[pos]
+        assert idx[0] == k
+        rest = np.flatnonzero(~assigned)
+        rest = rest[rest != k]
+        chosen = idx[1:]
+        assert not assigned[chosen].any()
+        if len(chosen) and len(rest) > len(chosen):
+            excluded = np.setdiff1d(rest, chosen)
+            assert A[k, chosen].min() >= A[k, excluded].max() * (1 - 1e-12)
+        assert (np.diff(A[k, chosen]) <= 1e-12 * A[k, chosen][1:]).all()
+        assigned[idx] = True
+        same_sets += set(idx.tolist()) == set(o_order[bstart[b]:bstart[b + 1]].tolist())
+        n = len(idx)
+        np.testing.assert_allclose(inv[b] @ A[np.ix_(idx, idx)], np.eye(n), atol=1e-9)
+        np.testing.assert_array_equal(inv[b], inv[b].T)
+    assert same_sets == len(sizes)  # no near-ties in this geometry: the partition equals the oracle's
+
+
+def test_rbj_given_pivot_order_and_bad_input(pcm, sys2500):
+    s, _, _, ctx = sys2500
+    perm = np.random.default_rng(1).permutation(s.M)
+    pcm.pcm_rbj_build(ctx, 32, pivot_order=perm)
+    order, bstart, _ = pcm.pcm_rbj_get(ctx)
+    assert order[0] == perm[0]
+    bad = perm.copy()
+    bad[0] = bad[1]
+    with pytest.raises(pcm.PcmError):
+        pcm.pcm_rbj_build(ctx, 32, pivot_order=bad)
+    with pytest.raises(pcm.PcmError):
+        pcm.pcm_rbj_build(ctx, 0)
+
+
+def test_cg_matches_lapack_and_oracle(pcm, orc, sys2500, torch_cuda):
+    s, A, q_true, ctx = sys2500
+    b = A @ q_true
+    x_ref = np.linalg.solve(A, b)
+    piv = pcm.pcm_pivot_order(5, s.M)
+    pcm.pcm_rbj_build(ctx, 64, seed=5)
+    o_rbj = orc.rbj_build(s, 64, piv)
+    iters = {}
+    for name, precond, okw in (("none", 0, {}), ("jacobi", 1, {}), ("rbj", 2, dict(rbj=o_rbj))):
+        x, it, rr, rt, ok = pcm.pcm_cg_solve(ctx, dev(torch_cuda, b), tol=1e-8, max_iter=2000, precond=precond)
+        assert ok and rr <= 1e-8 and rt <= 2e-8
+        np.testing.assert_allclose(x.cpu().numpy(), x_ref, rtol=0, atol=2e-7)
+        _, o_it, _, _ = orc.pcg(s, b, 1e-8, 2000, precond=precond, A=A, **okw)
+        assert abs(it - o_it) <= 2, (name, it, o_it)
+        iters[name] = it
+        xh, ith, _, _, okh = pcm.pcm_cg_solve_host(ctx, b, tol=1e-8, max_iter=2000, precond=precond)
+        assert okh and ith == it
+        np.testing.assert_array_equal(xh, x.cpu().numpy())
+    assert iters["rbj"] < iters["jacobi"]
+
+
+def test_cg_block_one_is_jacobi_and_block_M_is_one_step(pcm, orc, torch_cuda):
+    w = synth.make_workload(1, n_atoms=12, with_density=False, seed=5)
+    s = w.surface
+    ctx = points_ctx(pcm, s)
+    b = np.random.default_rng(0).uniform(-1, 1, s.M)
+    xj, itj, *_ = pcm.pcm_cg_solve(ctx, dev(torch_cuda, b), tol=1e-9, precond=1)
+    pcm.pcm_rbj_build(ctx, 1, seed=3)
+    x1, it1, *_ = pcm.pcm_cg_solve(ctx, dev(torch_cuda, b), tol=1e-9, precond=2)
+    assert abs(it1 - itj) <= 1
+    np.testing.assert_allclose(x1.cpu().numpy(), xj.cpu().numpy(), rtol=0, atol=1e-8)
+    pcm.pcm_rbj_build(ctx, s.M, seed=3)       # block size = dimension of A -> CG converges in 1 step
+    xM, itM, rr, rt, ok = pcm.pcm_cg_solve(ctx, dev(torch_cuda, b), tol=1e-8, precond=2)
+    assert ok and itM == 1 and rt < 1e-8
+
+
+def test_cg_warm_start_max_iter_and_errors(pcm, orc, sys2500, torch_cuda):
+    s, A, q_true, ctx = sys2500
+    b = A @ q_true
+    x, it, rr, rt, ok = pcm.pcm_cg_solve(ctx, dev(torch_cuda, b), tol=1e-8, precond=1)
+    x2, it2, _, _, ok2 = pcm.pcm_cg_solve(ctx, dev(torch_cuda, b), x=x.clone(), tol=1e-8, precond=1, use_x0=True)
+    assert ok2 and it2 == 0
+    x3, it3, rr3, _, ok3 = pcm.pcm_cg_solve(ctx, dev(torch_cuda, b), tol=1e-8, max_iter=3, precond=1)
+    assert not ok3 and it3 == 3 and rr3 > 1e-8
+    fresh = points_ctx(pcm, s)
+    with pytest.raises(pcm.PcmError):
+        pcm.pcm_cg_solve(fresh, dev(torch_cuda, b), precond=2)   # RBJ before pcm_rbj_build
+    with pytest.raises(pcm.PcmError):
+        pcm.pcm_cg_solve(fresh, dev(torch_cuda, b), precond=9)

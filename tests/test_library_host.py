@@ -1,0 +1,119 @@
+"""CPU-side checks of the product library: it builds, loads, exports every symbol include/pcm.h declares,
+and its host-only entry points (no device work) are right.  No compute call is made without a GPU.
+"""
+import ctypes
+import json
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_1505_07851_b200 as pcm
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "survey_checkvalues.json")))
+
+
+@pytest.fixture(scope="module")
+def L():
+    return pcm.lib(build=True)
+
+
+def test_library_exports_every_declared_symbol(L):
+    header = open(os.path.join(ROOT, "include", "pcm.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(pcm_[a-z0-9_]+)\s*\(", header))
+    assert declared, "no declarations found"
+    assert declared == set(pcm.EXPORTS)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_struct_layouts_match_header(L):
+    """ctypes mirrors of pcm_options / pcm_info: sizes as the C compiler lays them out"""
+    import subprocess
+    import tempfile
+    src = '#include <stdio.h>\n#include "pcm.h"\nint main(){printf("%zu %zu\\n", sizeof(pcm_options), sizeof(pcm_info));return 0;}\n'
+    with tempfile.TemporaryDirectory() as d:
+        c = os.path.join(d, "s.c")
+        open(c, "w").write(src)
+        exe = os.path.join(d, "s")
+        subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), c, "-o", exe])
+        so, si = map(int, subprocess.check_output([exe]).split())
+    assert ctypes.sizeof(pcm.pcm_options) == so
+    assert ctypes.sizeof(pcm.pcm_info) == si
+
+
+def test_options_default(L):
+    o = pcm.pcm_options_default()
+    assert o.screen_eps == 1e-12 and o.d_pure == 1 and o.device == -1 and o.merge_products == 1
+
+
+def test_pivot_order_matches_the_documented_generator(L, orc):
+    """include/pcm.h: indices sorted by (splitmix64 finaliser(seed + (i+1) golden), i); the oracle implements the
+    same counter-based generator on its own, so both sides draw the same pivots from a seed"""
+    for seed, M in ((0, 1), (1, 17), (12345, 1000), (2 ** 63 + 5, 4096)):
+        p = pcm.pcm_pivot_order(seed, M)
+        assert sorted(p.tolist()) == list(range(M))
+        np.testing.assert_array_equal(p, orc.pivot_order(seed, M))
+
+
+def test_schwarz_bound_worked_example(L):
+    """SURVEY.md 8(c4) check values for the worked-example pair (survey-derived), and the s-s closed form
+    [ss|ss] = 2 pi^{5/2} K_AB^2 / (p^2 sqrt(2p))."""
+    e = GOLD["worked_example"]
+    g = GOLD["schwarz_worked_example"]
+    A, B, al, be = e["A"], e["B"], e["alpha"], e["beta"]
+    p = al + be
+    K = math.exp(-al * be / p * sum((a - b) ** 2 for a, b in zip(A, B)))
+    ss = pcm.pcm_schwarz_bound(0, al, A, 0, be, B)
+    assert ss ** 2 == pytest.approx(2 * math.pi ** 2.5 * K * K / (p * p * math.sqrt(2 * p)), rel=1e-13)
+    assert ss ** 2 == pytest.approx(g["ss"], rel=1e-11)
+    # the bound is the max over Cartesian components, so it is at least the listed component's value
+    assert pcm.pcm_schwarz_bound(1, al, A, 0, be, B) ** 2 >= g["pxs"] * (1 - 1e-11)
+    assert pcm.pcm_schwarz_bound(1, al, A, 1, be, B) ** 2 >= g["pxpz"] * (1 - 1e-11)
+    assert pcm.pcm_schwarz_bound(2, al, A, 0, be, B) ** 2 >= g["dxxs"] * (1 - 1e-11)
+
+
+def test_schwarz_bound_by_quadrature(L):
+    """[ab|ab] for same-centre primitives has a 1-D closed route: for a = b = s it is the Coulomb self-energy of
+    exp(-p r^2): 2 pi^{5/2}/(p^2 sqrt(2p)); for (p_x s) on one centre the density x exp(-p r^2) has self-repulsion
+    2 pi^{5/2}/(p^2 sqrt(2p)) / (6 p)... checked numerically through the Fourier-space integral
+    (1/2 pi^2) int |rho(k)|^2 / k^2 d^3k."""
+    from scipy import integrate
+    O = [0.0, 0.0, 0.0]
+    al, be = 0.7, 0.5
+    p = al + be
+    # rho(r) = x exp(-p r^2): rho(k) = -i k_x/(2p) (pi/p)^{3/2} exp(-k^2/4p);  angular average of k_x^2 = k^2/3
+    f = lambda k: (1.0 / (2 * math.pi ** 2)) * 4 * math.pi * k * k * ((k * k / 3) / (4 * p * p) * (math.pi / p) ** 3 * math.exp(-k * k / (2 * p))) / (k * k)
+    ref = integrate.quad(f, 0, np.inf, epsabs=0, epsrel=1e-12)[0]
+    got = pcm.pcm_schwarz_bound(1, al, O, 0, be, O) ** 2
+    assert got == pytest.approx(ref, rel=1e-10)
+    # and it is symmetric in the two primitives
+    A, B = [0.1, 0.2, -0.3], [0.5, -0.4, 0.6]
+    for la in range(3):
+        for lb in range(3):
+            assert pcm.pcm_schwarz_bound(la, al, A, lb, be, B) == pytest.approx(pcm.pcm_schwarz_bound(lb, be, B, la, al, A), rel=1e-12)
+
+
+def test_bad_arguments_are_refused(L):
+    out = ctypes.c_double()
+    assert L.pcm_schwarz_bound(3, 1.0, None, 0, 1.0, None, ctypes.byref(out)) < 0
+    assert L.pcm_pivot_order(1, -1, None) < 0
+    h = ctypes.c_void_p()
+    assert L.pcm_setup(ctypes.byref(h), -1, None, None, None, None, None, 0, None, None, None, None) < 0
+    assert b"negative" in L.pcm_last_error(None)
+    assert L.pcm_destroy(None) == 0
+
+
+def test_no_cpu_fallback():
+    """without a CUDA device the product path must fail loudly, not route anywhere else"""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(RuntimeError):
+        pcm.pcm_setup([0], [[0, 0, 0]], [1], [1.0], [1.0], [[1, 0, 0]], [1.0])
+    src = open(os.path.join(ROOT, "paper_1505_07851_b200", "__init__.py")).read()
+    assert "import oracle" not in src and "from oracle" not in src
