@@ -388,6 +388,41 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_kernels(args):
+    """--mode kernels: only the three hot calls (configs[1] potential and Fock, configs[4] A q at M = 50k), W warm-up
+    and K timed rounds, no solver and no oracle.  This is the command the ncu captures under profiles/ are taken with."""
+    import torch
+    import paper_1505_07851_b200 as pcm
+    torch.cuda.set_device(0)
+    pcm.lib()
+    w = synth.make_workload(args.config)
+    ctx = pcm.setup_from_workload(w.basis, w.surface)
+    s4, q4, _ = synth.make_solver_points(args.amat_m)
+    c4 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s4.xyz, s4.zeta, s4.switch)
+    dev = torch.device("cuda", 0)
+    P = torch.as_tensor(w.P, dtype=torch.float64, device=dev)
+    q = torch.as_tensor(w.q, dtype=torch.float64, device=dev)
+    qd = torch.as_tensor(q4, dtype=torch.float64, device=dev)
+    for c in (ctx, c4):
+        pcm.pcm_set_timing(c, True)
+    out = {"potential_ms": [], "fock_ms": [], "amatvec_ms": [], "potential_by_L": None, "fock_by_L": None}
+    for k in range(args.warmup + args.steps):
+        pcm.pcm_potential(ctx, P)
+        pcm.pcm_fock(ctx, q)
+        pcm.pcm_amatvec(c4, qd)
+        torch.cuda.synchronize()
+        if k >= args.warmup:
+            out["potential_ms"].append(sum(pcm.pcm_last_kernel_ms(ctx, pcm.OP_POTENTIAL)[:2]))
+            out["fock_ms"].append(sum(pcm.pcm_last_kernel_ms(ctx, pcm.OP_FOCK)[:2]))
+            out["amatvec_ms"].append(sum(pcm.pcm_last_kernel_ms(c4, pcm.OP_AMATVEC)[:2]))
+            out["potential_by_L"] = pcm.pcm_last_class_ms(ctx, pcm.OP_POTENTIAL)
+            out["fock_by_L"] = pcm.pcm_last_class_ms(ctx, pcm.OP_FOCK)
+    info = pcm.pcm_get_info(ctx)
+    out.update({"mode": "kernels", "config": args.config, "M": ctx.M, "nbf": ctx.nbf, "amat_M": args.amat_m,
+                "products_by_L": list(map(int, info.products)), "prim_pairs": int(info.prim_pairs_total)})
+    print(json.dumps(out), flush=True)
+
+
 def run_reference(args):
     """The oracle, as it stands, on the host cores: K steps, each a bounded sample of the configs[1] step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -431,9 +466,14 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] A q sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing (cpu_baseline)")
+    ap.add_argument("--mode", default="step", choices=["step", "kernels"], help="kernels: only the three hot calls (for ncu)")
+    ap.add_argument("--config", type=int, default=CONFIG_INDEX, help="--mode kernels: BASELINE.json config index 0..3")
+    ap.add_argument("--amat-m", type=int, default=50_000, help="--mode kernels: surface points of the A q call")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.mode == "kernels":
+        run_kernels(args)
     else:
         run_ours(args)
 
