@@ -11,9 +11,6 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
                   const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
                   const double *pt_zeta, const double *pt_switch);
 const char *setup_error_text();
-int64_t fock_chunks(const pcm_ctx *ctx, int L);
-int64_t pot_chunks(const pcm_ctx *ctx, int L);
-int64_t amat_chunks(const pcm_ctx *ctx);
 void pivot_order(uint64_t seed, int64_t M, int64_t *perm);
 int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s);
 int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter, int precond, int use_x0, int *iters,
@@ -103,16 +100,20 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
 
     // scratch sized from the fixed work partition
     const int64_t M = ctx->M;
+    if ((rc = plan_all(ctx))) return fail(rc);
     for (int L = 0; L <= MAXL; ++L) {
         ClassData &c = ctx->cls[L];
-        c.herm_slots = fock_chunks(ctx, L);
+        c.herm_slots = ctx->plan_fock[L].chunks;
+        if ((rc = dev_alloc_t(ctx, &c.near_fock, (size_t)c.fock_map.npiece * nherm(L) * 32))) return fail(rc);
+        if ((rc = dev_alloc_t(ctx, &c.near_pot, (size_t)c.pot_map.npiece * 32))) return fail(rc);
         if ((rc = dev_alloc_t(ctx, &c.herm, (size_t)c.herm_slots * nherm(L) * std::max<int64_t>(c.npad, 1)))) return fail(rc);
-        ctx->vpart_slots += (c.n > 0) ? pot_chunks(ctx, L) : 0;
+        ctx->vpart_slots += (c.n > 0) ? ctx->plan_pot[L].chunks : 0;
     }
-    ctx->ypart_slots = amat_chunks(ctx);
+    ctx->ypart_slots = ctx->plan_amat.chunks;
+    if ((rc = dev_alloc_t(ctx, &ctx->near_amat, (size_t)ctx->amat_map.npiece * 32))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->vpart, (size_t)std::max<int64_t>(ctx->vpart_slots, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->ypart, (size_t)ctx->ypart_slots * std::max<int64_t>(M, 1)))) return fail(rc);
-    if ((rc = dev_alloc_t(ctx, &ctx->cg_vec, (size_t)5 * std::max<int64_t>(M, 1)))) return fail(rc);
+    if ((rc = dev_alloc_t(ctx, &ctx->cg_vec, (size_t)6 * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->cg_scal, (size_t)1024))) return fail(rc);
     e = cudaMemset(ctx->cg_scal, 0, 1024 * 8);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->cg_scal_host, 64 * sizeof(double));
@@ -170,7 +171,7 @@ int pcm_rbj_get(pcm_ctx *ctx, int64_t *order_host, int64_t *bstart_host, double 
     if (order_host && M > 0) {
         std::vector<int32_t> o((size_t)M);
         PCM_CUDA(ctx, cudaMemcpy(o.data(), ctx->rbj_order, (size_t)M * 4, cudaMemcpyDeviceToHost));
-        for (int64_t i = 0; i < M; ++i) order_host[i] = o[i];
+        for (int64_t i = 0; i < M; ++i) order_host[i] = ctx->s2c_host[(size_t)o[i]];  // sorted -> caller numbering
     }
     if (bstart_host)
         for (int64_t b = 0; b <= nb; ++b) bstart_host[b] = std::min(b * l, M);

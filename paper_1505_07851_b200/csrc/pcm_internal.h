@@ -41,14 +41,44 @@ struct DeviceBuf {  // owning device allocation
     size_t bytes = 0;
 };
 
+// Far/near classification of the (32 rows) x (32 columns) patches of a hot kernel's sweep, fixed at setup from the
+// bounding boxes of the groups: a patch is "far" when its boxes are further apart than the far-field radius of every
+// evaluation in it.  The main kernels run the far patches branch-free and skip the others, which the near kernels
+// pick up from the per-row-group lists.
+struct PatchMap {
+    int64_t nrg = 0;            // row groups
+    int64_t ncg = 0;            // column groups
+    int64_t nbyte = 0;          // bytes per row of `far` = ceil(ncg / 8)
+    uint8_t *far = nullptr;     // [nrg][nbyte]: bit s of byte b = patch (row group, column group 8 b + s) is far
+    int64_t *start = nullptr;   // [nrg + 1] CSR into list
+    int32_t *list = nullptr;    // column groups of the patches that are not far, row group after row group
+    int64_t nnear = 0;          // entries of list
+    // near-kernel work items ("pieces"): piece q belongs to row group piece_rg[q] and covers entries
+    // start[rg] + NEAR_PIECE (q - pstart[rg]) ... of that group's list; pieces of one group are consecutive.
+    int64_t npiece = 0;
+    int64_t *pstart = nullptr;  // [nrg + 1] CSR: pieces of each row group
+    int32_t *piece_rg = nullptr;  // [npiece]
+};
+constexpr int NEAR_PIECE = 8;
+
 struct ClassData {        // products of one total angular momentum L, padded to a multiple of 128
     int64_t n = 0;        // products
-    int64_t npad = 0;     // padded count (SoA leading dimension)
+    int64_t npad = 0;     // padded count (SoA leading dimension); the padding repeats the last product
     int64_t first = 0;    // global index of the first product of this class
     double4 *prodA = nullptr;  // (Px, Py, Pz, thr): hi word of thr is the far-field threshold on |P-C|^2
     double2 *prodB = nullptr;  // (p, 1/kappa) with kappa = sqrt(pi/p)/2
-    double *herm = nullptr;    // [nchunk_max][nherm(L)][npad] Hermite vectors (density D or potential sums H)
-    int64_t herm_slots = 0;    // chunks the herm buffer can hold
+    PatchMap pot_map;          // rows = groups of 32 points, columns = groups of 32 products of this class
+    PatchMap fock_map;         // rows = groups of 32 products of this class, columns = groups of 32 points
+    double *herm = nullptr;    // [chunks][nherm(L)][npad] Hermite vectors (density D or potential sums H)
+    int64_t herm_slots = 0;    // chunks the herm buffer holds
+    double *near_fock = nullptr;  // [fock_map.npiece][nherm(L)][32] sums of the near pieces
+    double *near_pot = nullptr;   // [pot_map.npiece][32]
+};
+
+struct Plan {             // work partition of one hot kernel launch: grid = (xb, chunks)
+    int64_t xb = 0;        // blocks along the register-resident ("row") dimension
+    int64_t chunks = 1;    // pieces the streamed ("column") dimension is cut into; each writes its own partial-sum slot
+    int64_t chunk_len = 0; // columns per chunk (a multiple of the tile)
 };
 
 }  // namespace pcm
@@ -62,8 +92,13 @@ struct pcm_ctx {
 
     // points
     int64_t M = 0;
+    // points, stored in Morton order ("sorted index" s); the caller's index of sorted point s is s2c[s].
+    // Vectors crossing the C ABI (v, q, y, b, x) are in the caller's order; the kernels gather/scatter through s2c.
     double4 *pt = nullptr;      // (x, y, z, 1/zeta^2)
     double *pt_diag = nullptr;  // A_kk = zeta_k sqrt(2/pi)/S_k
+    pcm::PatchMap amat_map;     // rows and columns = groups of 32 sorted points
+    int32_t *s2c = nullptr;     // [M] device
+    std::vector<int32_t> s2c_host, c2s_host;
     double zeta_min = 0, zeta_max = 0;
 
     // basis / pairs
@@ -93,12 +128,16 @@ struct pcm_ctx {
 
     double *boys = nullptr;  // [MAXL+1][BOYS_ROWS][BOYS_STRIDE]
 
+    // fixed work partitions (sizes and SM count only; set once in pcm_setup by plan_all)
+    pcm::Plan plan_pot[pcm::MAXL + 1], plan_fock[pcm::MAXL + 1], plan_amat;
+
     // scratch
     double *vpart = nullptr;    // potential partial sums [slots][M]
     int64_t vpart_slots = 0;
+    double *near_amat = nullptr;  // [amat_map.npiece][32] sums of the near pieces
     double *ypart = nullptr;    // amatvec partial sums [slots][M]
     int64_t ypart_slots = 0;
-    double *cg_vec = nullptr;   // 5 M doubles: r, z, p, Ap, tmp
+    double *cg_vec = nullptr;   // 6 M doubles: r, z, p, Ap, x, b (sorted point order)
     double *cg_scal = nullptr;  // device scalars
     double *cg_scal_host = nullptr;  // pinned
     double *io_a = nullptr, *io_b = nullptr;  // staging for the *_host calls
@@ -134,6 +173,8 @@ inline int dev_alloc_t(pcm_ctx *ctx, T **p, size_t count) {
 int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cudaStream_t s);
 int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accumulate, cudaStream_t s);
 int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s);
+int launch_amatvec_sorted(pcm_ctx *ctx, const double *q_sorted, double *y_sorted, cudaStream_t s);  // both in sorted order
+int plan_all(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
 void build_boys_tables(std::vector<double> &tab);
 double schwarz_bound(int la, double alpha, const double *A, int lb, double beta, const double *B);

@@ -16,46 +16,57 @@
 
 namespace pcm {
 
-constexpr int TPB = 128;        // threads per block of the hot kernels ("1 x 128", still a good size)
-constexpr int FOCK_TILE = 256;  // points staged per shared-memory tile
-constexpr int POT_TILE = 64;    // products staged per shared-memory tile
-constexpr int AMAT_TILE = 256;
+constexpr int TPB = 128;   // threads per block of the hot kernels ("1 x 128", still a good size)
+constexpr int SUB = 32;    // rows / columns per classified group
+constexpr int PT_TILE = 256;  // surface points staged per shared-memory tile (Fock, A q): 8 groups = one byte of the far map
 
 // ---------------------------------------------------------------------------------------------
-// work partition: how many chunks the reduction dimension is split into (fixed by sizes only)
+// Blocking.  Every hot kernel is a "rows x columns" sweep: a thread keeps R row objects in registers (points for
+// A q and the potential, Hermite products for Fock) and the column objects stream through shared memory, C per
+// inner step, so that R*C independent evaluations are in flight per thread (instruction-level parallelism is what
+// keeps the FP64 pipe busy; profiles/).  Rows and columns are sorted in space and cut into groups of 32; pcm_setup
+// classified every (row group, column group) patch from the groups' bounding boxes (PatchMap).  The *main* kernels
+// below run the far patches only, branch-free (derivatives of 1/R, no table, no exp); the *near* kernels further
+// down run the remaining patches with the per-evaluation far/near switch.  Lane = row inside a group, so a warp
+// holds R whole row groups and every skip/run decision is warp-uniform.
 // ---------------------------------------------------------------------------------------------
-static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+struct Blocking { int R, C; };
+__host__ __device__ constexpr Blocking amat_blocking() { return {4, 2}; }
+__host__ __device__ constexpr Blocking fock_blocking(int L) {
+    return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{2, 2} : L == 2 ? Blocking{1, 4} : Blocking{1, 2};
+}
+__host__ __device__ constexpr Blocking pot_blocking(int L) {
+    return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{4, 1} : L == 2 ? Blocking{2, 2} : L == 3 ? Blocking{1, 2} : Blocking{1, 1};
+}
+__host__ __device__ constexpr int pot_tile(int L) { return L <= 2 ? 256 : 64; }  // products staged per tile (8 or 2 groups)
 
-int64_t fock_chunks(const pcm_ctx *ctx, int L) {
-    const int64_t xb = ceil_div(ctx->cls[L].n, TPB);
-    if (xb == 0 || ctx->M == 0) return 1;
-    const int64_t target = (int64_t)ctx->sm_count * 8;
-    int64_t c = ceil_div(target, xb);
-    c = std::min<int64_t>(c, ceil_div(ctx->M, FOCK_TILE));
-    return std::max<int64_t>(c, 1);
+// far bits of the R row groups of this warp for the NS column groups starting at column group cg0 (cg0 % NS == 0,
+// NS = 8 or 2): bit (r * 8 + s) = patch (row group rg0 + r, column group cg0 + s) is far.  Warp-uniform result.
+template <int R, int NS>
+__device__ __forceinline__ unsigned far_bits(const uint8_t *__restrict__ farmap, int64_t nbyte, int64_t rg0, int64_t nrg,
+                                             int64_t cg0, int lane) {
+    unsigned mine = 0;
+    if (lane < R && rg0 + lane < nrg) mine = farmap[(rg0 + lane) * nbyte + (cg0 >> 3)];
+    mine = (mine >> (cg0 & 7)) & ((1u << NS) - 1u);
+    unsigned bits = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) bits |= __shfl_sync(0xffffffffu, mine, r) << (8 * r);
+    return bits;
 }
-int pot_ppt(int L) { return L <= 2 ? 2 : 1; }
-int64_t pot_chunks(const pcm_ctx *ctx, int L) {
-    const int64_t xb = ceil_div(ctx->M, (int64_t)TPB * pot_ppt(L));
-    if (xb == 0 || ctx->cls[L].n == 0) return 1;
-    const int64_t target = (int64_t)ctx->sm_count * 8;
-    int64_t c = ceil_div(target, xb);
-    c = std::min<int64_t>(c, ceil_div(ctx->cls[L].n, POT_TILE));
-    return std::max<int64_t>(c, 1);
-}
-int64_t amat_chunks(const pcm_ctx *ctx) {
-    const int64_t xb = ceil_div(ctx->M, (int64_t)TPB * 2);
-    if (xb == 0) return 1;
-    const int64_t target = (int64_t)ctx->sm_count * 8;
-    int64_t c = ceil_div(target, xb);
-    c = std::min<int64_t>(c, ceil_div(ctx->M, AMAT_TILE));
-    return std::max<int64_t>(c, 1);
+// rows of the warp that are far from column group s: bit r
+template <int R>
+__device__ __forceinline__ unsigned row_mask(unsigned bits, int s) {
+    unsigned m = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) m |= ((bits >> (8 * r + s)) & 1u) << r;
+    return m;
 }
 
 // ---------------------------------------------------------------------------------------------
-// a4: y = A q on the fly (Eq. 2, 3, 8).  Thread = 2 rows, the column points stream through shared memory.
+// a4: y = A q on the fly (Eq. 2, 3, 8).  Rows = points i (registers), columns = points j (shared memory).
 //   far (zeta'^2 r^2 >= 38, erf = 1 to fp64):  A_ij = 1/r                       -- 12 FP64 instructions + MUFU
 //   general:  A_ij = (2 zeta'/sqrt pi) F_0(zeta'^2 r^2), zeta'^2 = 1/(1/zeta_i^2 + 1/zeta_j^2); A_ii from pt_diag
+// q is read through qidx (sorted -> caller index) when qidx != nullptr; the partial sums are in sorted order.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double amat_general(double r2, double izi, double izj, const double *__restrict__ boys0) {
     const double zp = rsqrt_fast(izi + izj);
@@ -70,67 +81,156 @@ __device__ __forceinline__ double amat_general(double r2, double izi, double izj
     return 1.1283791670955125739 * zp * f;  // 2/sqrt(pi)
 }
 
-__global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ diag,
-                                                      const double *__restrict__ q, int M, int chunk_len,
-                                                      double *__restrict__ out, const double *__restrict__ boys0,
-                                                      int thr_hi) {
-    __shared__ double4 s_pt[AMAT_TILE];   // x, y, z, q
-    __shared__ double s_iz[AMAT_TILE];
-    const int i0 = blockIdx.x * (2 * TPB) + threadIdx.x, i1 = i0 + TPB;
-    const double4 a0 = pt[min(i0, M - 1)], a1 = pt[min(i1, M - 1)];
-    double y0 = 0.0, y1 = 0.0;
-    const int jbeg = blockIdx.y * chunk_len, jend = min(M, jbeg + chunk_len);
-    for (int base = jbeg; base < jend; base += AMAT_TILE) {
-        __syncthreads();
-        for (int t = threadIdx.x; t < AMAT_TILE; t += TPB) {
-            const int j = base + t;
-            if (j < jend) {
-                const double4 b = pt[j];
-                s_pt[t] = make_double4(b.x, b.y, b.z, q[j]);
-                s_iz[t] = b.w;
-            } else {  // padding: far away, zero charge
-                s_pt[t] = make_double4(3e8, 3e8, 3e8, 0.0);
-                s_iz[t] = 1.0;
-            }
+// stages the points [base, base + nst*32) of the chunk ending at jend as (x, y, z, charge)
+__device__ __forceinline__ void stage_points(const double4 *__restrict__ pt, const double *__restrict__ q,
+                                             const int32_t *__restrict__ qidx, int base, int jend, int nst, double4 *s_pt) {
+    for (int t = threadIdx.x; t < nst * SUB; t += TPB) {
+        const int j = base + t;
+        if (j < jend) {
+            const double4 b = pt[j];
+            s_pt[t] = make_double4(b.x, b.y, b.z, q[qidx ? qidx[j] : j]);
+        } else {  // padding: far from everything, zero charge (its patch bit is never set anyway)
+            s_pt[t] = make_double4(3e8, 3e8, 3e8, 0.0);
         }
+    }
+}
+
+template <int R, int C>
+__global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ q,
+                                                      const int32_t *__restrict__ qidx, int M, int chunk_len,
+                                                      double *__restrict__ out, const uint8_t *__restrict__ farmap,
+                                                      int64_t nbyte, int64_t nrg) {
+    constexpr int NS = PT_TILE / SUB;
+    __shared__ double4 s_pt[PT_TILE];   // x, y, z, q
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
+    double4 a[R];
+    int ii[R];
+    double y[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        ii[r] = (int)(rg0 + r) * SUB + lane;
+        a[r] = pt[min(ii[r], M - 1)];
+        y[r] = 0.0;
+    }
+    const int jbeg = blockIdx.y * chunk_len, jend = min(M, jbeg + chunk_len);
+    for (int base = jbeg; base < jend; base += PT_TILE) {
+        const int nst = (min(PT_TILE, jend - base) + SUB - 1) / SUB;
+        const unsigned bits = far_bits<R, NS>(farmap, nbyte, rg0, nrg, base / SUB, lane);
         __syncthreads();
-        const int cnt = min(AMAT_TILE, jend - base);
-#pragma unroll 2
-        for (int t = 0; t < cnt; ++t) {
-            const double4 b = s_pt[t];
-            const double dx0 = a0.x - b.x, dy0 = a0.y - b.y, dz0 = a0.z - b.z;
-            const double dx1 = a1.x - b.x, dy1 = a1.y - b.y, dz1 = a1.z - b.z;
-            const double r20 = fma(dz0, dz0, fma(dy0, dy0, dx0 * dx0));
-            const double r21 = fma(dz1, dz1, fma(dy1, dy1, dx1 * dx1));
-            if (min(hi32(r20), hi32(r21)) > thr_hi) {
-                y0 = fma(b.w, rsqrt_fast(r20), y0);
-                y1 = fma(b.w, rsqrt_fast(r21), y1);
-            } else {
-                const int j = base + t;
-                const double izj = s_iz[t];
-                const double e0 = (j == i0) ? diag[j] : amat_general(r20, a0.w, izj, boys0);
-                const double e1 = (j == i1) ? diag[j] : amat_general(r21, a1.w, izj, boys0);
-                y0 = fma(b.w, e0, y0);
-                y1 = fma(b.w, e1, y1);
+        stage_points(pt, q, qidx, base, jend, nst, s_pt);
+        __syncthreads();
+        for (int st = 0; st < nst; ++st) {
+            const double4 *sp = s_pt + st * SUB;
+            const unsigned m = row_mask<R>(bits, st);
+            if (m == (1u << R) - 1u) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; t += C) {
+                    double4 b[C];
+                    double r2[C][R];
+#pragma unroll
+                    for (int c = 0; c < C; ++c) b[c] = sp[t + c];
+#pragma unroll
+                    for (int c = 0; c < C; ++c)
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const double dx = a[r].x - b[c].x, dy = a[r].y - b[c].y, dz = a[r].z - b[c].z;
+                            r2[c][r] = fma(dz, dz, fma(dy, dy, dx * dx));
+                        }
+#pragma unroll
+                    for (int c = 0; c < C; ++c)
+#pragma unroll
+                        for (int r = 0; r < R; ++r) y[r] = fma(b[c].w, rsqrt_fast(r2[c][r]), y[r]);
+                }
+            } else if (m) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; ++t) {
+                    const double4 b = sp[t];
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+                        if ((m >> r) & 1u) {
+                            const double dx = a[r].x - b.x, dy = a[r].y - b.y, dz = a[r].z - b.z;
+                            y[r] = fma(b.w, rsqrt_fast(fma(dz, dz, fma(dy, dy, dx * dx))), y[r]);
+                        }
+                }
             }
         }
     }
-    if (i0 < M) out[(size_t)blockIdx.y * M + i0] = y0;
-    if (i1 < M) out[(size_t)blockIdx.y * M + i1] = y1;
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        if (ii[r] < M) out[(size_t)blockIdx.y * M + ii[r]] = y[r];
 }
 
-// out[k] = sum_slots part[slot][k]  (fixed order)
-__global__ void reduce_slots_kernel(const double *__restrict__ part, int64_t n, int slots, double *__restrict__ out) {
+// near patches of A q: one warp per piece (<= NEAR_PIECE listed patches of one row group); lane = row; the 32 columns
+// of a listed group are staged in the warp's own shared memory.  Writes near[piece][lane].
+__global__ void __launch_bounds__(TPB) amat_near_kernel(const double4 *__restrict__ pt, const double *__restrict__ diag,
+                                                        const double *__restrict__ q, const int32_t *__restrict__ qidx, int M,
+                                                        const int64_t *__restrict__ start, const int32_t *__restrict__ list,
+                                                        const int64_t *__restrict__ pstart, const int32_t *__restrict__ piece_rg,
+                                                        int64_t npiece, double *__restrict__ near,
+                                                        const double *__restrict__ boys0, double thr) {
+    __shared__ double4 s_pt[TPB / 32][SUB];
+    __shared__ double s_iz[TPB / 32][SUB];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
+    if (piece >= npiece) return;
+    const int64_t rg = piece_rg[piece];
+    const int i = (int)rg * SUB + lane;
+    const double4 a = pt[min(i, M - 1)];
+    const int thr_hi = hi32(thr);
+    const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
+    double y = 0.0;
+    for (int64_t e = ebeg; e < eend; ++e) {
+        const int j0 = list[e] * SUB, j = j0 + lane;
+        __syncwarp();
+        if (j < M) {
+            const double4 b = pt[j];
+            s_pt[warp][lane] = make_double4(b.x, b.y, b.z, q[qidx ? qidx[j] : j]);
+            s_iz[warp][lane] = b.w;
+        } else {
+            s_pt[warp][lane] = make_double4(3e8, 3e8, 3e8, 0.0);
+            s_iz[warp][lane] = 1.0;
+        }
+        __syncwarp();
+#pragma unroll 2
+        for (int t = 0; t < SUB; ++t) {
+            const double4 b = s_pt[warp][t];
+            const double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            double ev;
+            if (hi32(r2) > thr_hi) ev = rsqrt_fast(r2);
+            else ev = (j0 + t == i) ? diag[i] : amat_general(r2, a.w, s_iz[warp][t], boys0);
+            y = fma(b.w, ev, y);
+        }
+    }
+    near[piece * SUB + lane] = y;
+}
+
+// sums of the near pieces, per class: near[c][piece][lane], pieces of row group rg = pstart[c][rg] .. pstart[c][rg+1]
+struct NearRefs {
+    const double *near[MAXL + 1];
+    const int64_t *pstart[MAXL + 1];
+    int count;
+};
+// out[idx ? idx[k] : k] = sum_slots part[slot][k] + sum of the near pieces of row k  (fixed order)
+__global__ void reduce_slots_kernel(const double *__restrict__ part, int64_t n, int slots, double *__restrict__ out,
+                                    const int32_t *__restrict__ idx, NearRefs nr) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
     double s = 0.0;
     for (int c = 0; c < slots; ++c) s += part[(size_t)c * n + k];
-    out[k] = s;
+    const int64_t rg = k / SUB, lane = k % SUB;
+    for (int c = 0; c < nr.count; ++c) {
+        double t = 0.0;
+        for (int64_t q = nr.pstart[c][rg]; q < nr.pstart[c][rg + 1]; ++q) t += nr.near[c][q * SUB + lane];
+        s += t;
+    }
+    out[idx ? idx[k] : k] = s;
 }
 
 // ---------------------------------------------------------------------------------------------
-// a3 main kernel: H_h(product) = sum_k q_k Rt_h(P - C_k).  Thread = product (NHERM(L) register accumulators),
-// the points stream through shared memory, two points per step for instruction-level parallelism.
+// a3 main kernel: H_h(product) = sum_k q_k Rt_h(P - C_k).  Rows = R products per thread (R NHERM(L) register
+// accumulators), columns = surface points (shared memory), C points per step.
 // ---------------------------------------------------------------------------------------------
 template <int L>
 struct FockSink {
@@ -140,38 +240,114 @@ struct FockSink {
 };
 
 template <int L>
-__global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ prodA, const double2 *__restrict__ prodB,
-                                                   int64_t npad, const double4 *__restrict__ pt, const double *__restrict__ q,
-                                                   int M, int chunk_len, double *__restrict__ herm,
-                                                   const double *__restrict__ boysL) {
+__device__ __forceinline__ void fock_far_unit(const double4 &A, const double4 &pc, FockSink<L> &sink) {
+    const double x = A.x - pc.x, y = A.y - pc.y, z = A.z - pc.z;
+    double g[L + 1];
+    seeds_far<L>(fma(z, z, fma(y, y, x * x)), g);
+#pragma unroll
+    for (int n = 0; n <= L; ++n) g[n] *= pc.w;
+    hermite_R<L>(x, y, z, g, sink);
+}
+
+template <int L, int R, int C>
+__global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ prodA, int64_t npad,
+                                                   const double4 *__restrict__ pt, const double *__restrict__ q,
+                                                   const int32_t *__restrict__ qidx, int M, int chunk_len,
+                                                   double *__restrict__ herm, const uint8_t *__restrict__ farmap,
+                                                   int64_t nbyte, int64_t nrg) {
     constexpr int NH = nherm(L);
-    __shared__ double4 s_pt[FOCK_TILE];  // x, y, z, q
-    __shared__ double s_iz[FOCK_TILE];
-    const int64_t ip = (int64_t)blockIdx.x * TPB + threadIdx.x;  // < npad by construction
+    constexpr int NS = PT_TILE / SUB;
+    __shared__ double4 s_pt[PT_TILE];  // x, y, z, q
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
+    double4 A[R];
+    FockSink<L> sink[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        A[r] = prodA[min((rg0 + r) * SUB + lane, npad - 1)];
+#pragma unroll
+        for (int h = 0; h < NH; ++h) sink[r].acc[h] = 0.0;
+    }
+    const int kbeg = blockIdx.y * chunk_len, kend = min(M, kbeg + chunk_len);
+    for (int base = kbeg; base < kend; base += PT_TILE) {
+        const int nst = (min(PT_TILE, kend - base) + SUB - 1) / SUB;
+        const unsigned bits = far_bits<R, NS>(farmap, nbyte, rg0, nrg, base / SUB, lane);
+        __syncthreads();
+        stage_points(pt, q, qidx, base, kend, nst, s_pt);
+        __syncthreads();
+        for (int st = 0; st < nst; ++st) {
+            const double4 *sp = s_pt + st * SUB;
+            const unsigned m = row_mask<R>(bits, st);
+            if (m == (1u << R) - 1u) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; t += C) {
+#pragma unroll
+                    for (int c = 0; c < C; ++c) {
+                        const double4 pc = sp[t + c];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) fock_far_unit<L>(A[r], pc, sink[r]);
+                    }
+                }
+            } else if (R > 1 && m) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; ++t) {
+                    const double4 pc = sp[t];
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+                        if ((m >> r) & 1u) fock_far_unit<L>(A[r], pc, sink[r]);
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t ip = (rg0 + r) * SUB + lane;
+        if (ip < npad) {
+            double *out = herm + (size_t)blockIdx.y * NH * npad + ip;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) out[(size_t)h * npad] = sink[r].acc[h];
+        }
+    }
+}
+
+// near patches of the Fock sweep: one warp per piece; lane = product.  Writes near[piece][h][lane].
+template <int L>
+__global__ void __launch_bounds__(TPB) fock_near_kernel(const double4 *__restrict__ prodA, const double2 *__restrict__ prodB,
+                                                        int64_t npad, const double4 *__restrict__ pt, const double *__restrict__ q,
+                                                        const int32_t *__restrict__ qidx, int M, const int64_t *__restrict__ start,
+                                                        const int32_t *__restrict__ list, const int64_t *__restrict__ pstart,
+                                                        const int32_t *__restrict__ piece_rg, int64_t npiece,
+                                                        double *__restrict__ near, const double *__restrict__ boysL) {
+    constexpr int NH = nherm(L);
+    __shared__ double4 s_pt[TPB / 32][SUB];
+    __shared__ double s_iz[TPB / 32][SUB];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
+    if (piece >= npiece) return;
+    const int64_t rg = piece_rg[piece];
+    const int64_t ip = rg * SUB + lane;  // < npad (npad is a multiple of 32)
     const double4 A = prodA[ip];
     const double2 B = prodB[ip];
     const int thr_hi = hi32(A.w);
     FockSink<L> sink;
 #pragma unroll
     for (int h = 0; h < NH; ++h) sink.acc[h] = 0.0;
-    const int kbeg = blockIdx.y * chunk_len, kend = min(M, kbeg + chunk_len);
-    for (int base = kbeg; base < kend; base += FOCK_TILE) {
-        __syncthreads();
-        for (int t = threadIdx.x; t < FOCK_TILE; t += TPB) {
-            const int k = base + t;
-            if (k < kend) {
-                const double4 c = pt[k];
-                s_pt[t] = make_double4(c.x, c.y, c.z, q[k]);
-                s_iz[t] = c.w;
-            } else {
-                s_pt[t] = make_double4(-3e8, -3e8, -3e8, 0.0);
-                s_iz[t] = 1.0;
-            }
+    const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
+    for (int64_t e = ebeg; e < eend; ++e) {
+        const int k = list[e] * SUB + lane;
+        __syncwarp();
+        if (k < M) {
+            const double4 c = pt[k];
+            s_pt[warp][lane] = make_double4(c.x, c.y, c.z, q[qidx ? qidx[k] : k]);
+            s_iz[warp][lane] = c.w;
+        } else {
+            s_pt[warp][lane] = make_double4(-3e8, -3e8, -3e8, 0.0);
+            s_iz[warp][lane] = 1.0;
         }
-        __syncthreads();
-        const int cnt = min(FOCK_TILE, kend - base);  // an odd count runs one padding point (zero charge)
-        for (int t = 0; t < cnt; t += 2) {
-            const double4 c0 = s_pt[t], c1 = s_pt[t + 1];
+        __syncwarp();
+#pragma unroll 1
+        for (int t = 0; t < SUB; t += 2) {
+            const double4 c0 = s_pt[warp][t], c1 = s_pt[warp][t + 1];
             const double x0 = A.x - c0.x, y0 = A.y - c0.y, z0 = A.z - c0.z;
             const double x1 = A.x - c1.x, y1 = A.y - c1.y, z1 = A.z - c1.z;
             const double r20 = fma(z0, z0, fma(y0, y0, x0 * x0));
@@ -181,32 +357,36 @@ __global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ p
                 seeds_far<L>(r20, g0);
                 seeds_far<L>(r21, g1);
             } else {
-                seeds_general<L>(r20, B.x, B.y, s_iz[t], boysL, g0);
-                seeds_general<L>(r21, B.x, B.y, s_iz[t + 1], boysL, g1);
+                seeds_general<L>(r20, B.x, B.y, s_iz[warp][t], boysL, g0);
+                seeds_general<L>(r21, B.x, B.y, s_iz[warp][t + 1], boysL, g1);
             }
 #pragma unroll
-            for (int n = 0; n <= L; ++n) { g0[n] *= c0.w; g1[n] *= c1.w; }
+            for (int n2 = 0; n2 <= L; ++n2) { g0[n2] *= c0.w; g1[n2] *= c1.w; }
             hermite_R<L>(x0, y0, z0, g0, sink);
             hermite_R<L>(x1, y1, z1, g1, sink);
         }
     }
-    double *out = herm + (size_t)blockIdx.y * NH * npad + ip;
+    double *out = near + (size_t)piece * NH * SUB + lane;
 #pragma unroll
-    for (int h = 0; h < NH; ++h) out[(size_t)h * npad] = sink.acc[h];
+    for (int h = 0; h < NH; ++h) out[h * SUB] = sink.acc[h];
 }
 
-// herm[0][h][i] += sum_{c>=1} herm[c][h][i]
-__global__ void reduce_herm_kernel(double *__restrict__ herm, int64_t plane, int chunks) {
+// herm[0][h][i] = sum_c herm[c][h][i] + sum of the near pieces of product i  (fixed order); plane = nh * npad
+__global__ void reduce_herm_kernel(double *__restrict__ herm, int64_t plane, int chunks, int64_t npad, int nh,
+                                   const double *__restrict__ near, const int64_t *__restrict__ pstart) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= plane) return;
     double s = herm[k];
     for (int c = 1; c < chunks; ++c) s += herm[(size_t)c * plane + k];
-    herm[k] = s;
+    const int64_t h = k / npad, i = k - h * npad, rg = i / SUB, lane = i % SUB;
+    double t = 0.0;
+    for (int64_t q = pstart[rg]; q < pstart[rg + 1]; ++q) t += near[((size_t)q * nh + h) * SUB + lane];
+    herm[k] = s + t;
 }
 
 // ---------------------------------------------------------------------------------------------
-// a2 main kernel: v_k = sum_products sum_h D_h Rt_h(P - C_k).  Thread = PPT points (register accumulators),
-// the products (centre, threshold, Hermite density) stream through shared memory.
+// a2 main kernel: v_k = sum_products sum_h D_h Rt_h(P - C_k).  Rows = R points per thread (register accumulators),
+// columns = products (centre, Hermite density) staged in shared memory, C per step.
 // ---------------------------------------------------------------------------------------------
 template <int L>
 struct PotSink {
@@ -217,75 +397,134 @@ struct PotSink {
 };
 
 template <int L>
-__host__ __device__ constexpr int pot_rec() { return (4 + nherm(L) + 2 + 1) / 2 * 2; }  // doubles per staged product
+__host__ __device__ constexpr int pot_rec() { return (4 + nherm(L) + 1) / 2 * 2; }      // main kernel: centre, pad, D_h
+template <int L>
+__host__ __device__ constexpr int pot_rec_near() { return (4 + nherm(L) + 2 + 1) / 2 * 2; }  // + (p, 1/kappa)
 
-template <int L, int PPT>
-__global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restrict__ prodA, const double2 *__restrict__ prodB,
-                                                        const double *__restrict__ herm, int64_t npad, int64_t nprod,
-                                                        int chunk_len, const double4 *__restrict__ pt, int M,
-                                                        double *__restrict__ vpart, const double *__restrict__ boysL) {
+template <int L>
+__device__ __forceinline__ void pot_far_unit(const double *rec, const double4 &c, double &v) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+    const double x = h01.x - c.x, y = h01.y - c.y, z = rec[2] - c.z;
+    double g[L + 1];
+    seeds_far<L>(fma(z, z, fma(y, y, x * x)), g);
+    PotSink<L> sink{rec + 4, v};
+    hermite_R<L>(x, y, z, g, sink);
+    v = sink.v;
+}
+
+template <int L, int R, int C>
+__global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restrict__ prodA, const double *__restrict__ herm,
+                                                        int64_t npad, int chunk_len, const double4 *__restrict__ pt, int M,
+                                                        double *__restrict__ vpart, const uint8_t *__restrict__ farmap,
+                                                        int64_t nbyte, int64_t nrg) {
     constexpr int NH = nherm(L);
     constexpr int REC = pot_rec<L>();
-    __shared__ __align__(16) double s_rec[POT_TILE * REC];
-    double4 c[PPT];
-    int kk[PPT];
-    double v[PPT];
+    constexpr int TILE = pot_tile(L), NS = TILE / SUB;
+    __shared__ __align__(16) double s_rec[TILE * REC];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
+    double4 c[R];
+    int kk[R];
+    double v[R];
 #pragma unroll
-    for (int r = 0; r < PPT; ++r) {
-        kk[r] = blockIdx.x * (TPB * PPT) + r * TPB + threadIdx.x;
+    for (int r = 0; r < R; ++r) {
+        kk[r] = (int)(rg0 + r) * SUB + lane;
         c[r] = pt[min(kk[r], M - 1)];
         v[r] = 0.0;
     }
-    const int64_t pbeg = (int64_t)blockIdx.y * chunk_len, pend = min(nprod, pbeg + (int64_t)chunk_len);
-    for (int64_t base = pbeg; base < pend; base += POT_TILE) {
-        const int cnt = (int)min((int64_t)POT_TILE, pend - base);
+    // products [pbeg, pend): pend <= npad, both multiples of 32 (the padding carries zero density)
+    const int64_t pbeg = (int64_t)blockIdx.y * chunk_len, pend = min(npad, pbeg + (int64_t)chunk_len);
+    for (int64_t base = pbeg; base < pend; base += TILE) {
+        const int cnt = (int)min((int64_t)TILE, pend - base), nst = cnt / SUB;
+        const unsigned bits = far_bits<R, NS>(farmap, nbyte, rg0, nrg, base / SUB, lane);
         __syncthreads();
-        // stage: header (Px,Py,Pz,thr), D_0..D_{NH-1}, (p, 1/kappa)
         for (int t = threadIdx.x; t < cnt; t += TPB) {
             const double4 a = prodA[base + t];
-            const double2 b = prodB[base + t];
             double *r = s_rec + t * REC;
-            r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = a.w;
-            r[4 + NH] = b.x; r[5 + NH] = b.y;
+            r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = 0.0;
         }
         for (int t = threadIdx.x; t < cnt * NH; t += TPB) {
             const int h = t / cnt, i = t - h * cnt;  // consecutive threads read consecutive products of one component
             s_rec[i * REC + 4 + h] = herm[(size_t)h * npad + base + i];
         }
         __syncthreads();
-        for (int t = 0; t < cnt; ++t) {
-            const double *r = s_rec + t * REC;
-            const double2 h01 = *reinterpret_cast<const double2 *>(r);
-            const double2 h23 = *reinterpret_cast<const double2 *>(r + 2);
-            const int thr_hi = hi32(h23.y);
-            double x[PPT], y[PPT], z[PPT], r2[PPT];
-            int mn = 0x7fffffff;
+        for (int st = 0; st < nst; ++st) {
+            const double *sr = s_rec + st * SUB * REC;
+            const unsigned m = row_mask<R>(bits, st);
+            if (m == (1u << R) - 1u) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; t += C) {
 #pragma unroll
-            for (int s = 0; s < PPT; ++s) {
-                x[s] = h01.x - c[s].x; y[s] = h01.y - c[s].y; z[s] = h23.x - c[s].z;
-                r2[s] = fma(z[s], z[s], fma(y[s], y[s], x[s] * x[s]));
-                mn = min(mn, hi32(r2[s]));
-            }
-            double g[PPT][L + 1];
-            if (mn > thr_hi) {
+                    for (int cc = 0; cc < C; ++cc)
 #pragma unroll
-                for (int s = 0; s < PPT; ++s) seeds_far<L>(r2[s], g[s]);
-            } else {
-                const double p = r[4 + NH], invk = r[5 + NH];
+                        for (int r = 0; r < R; ++r) pot_far_unit<L>(sr + (t + cc) * REC, c[r], v[r]);
+                }
+            } else if (R > 1 && m) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; ++t) {
 #pragma unroll
-                for (int s = 0; s < PPT; ++s) seeds_general<L>(r2[s], p, invk, c[s].w, boysL, g[s]);
-            }
-#pragma unroll
-            for (int s = 0; s < PPT; ++s) {
-                PotSink<L> sink{r + 4, v[s]};
-                hermite_R<L>(x[s], y[s], z[s], g[s], sink);
-                v[s] = sink.v;
+                    for (int r = 0; r < R; ++r)
+                        if ((m >> r) & 1u) pot_far_unit<L>(sr + t * REC, c[r], v[r]);
+                }
             }
         }
     }
 #pragma unroll
-    for (int s = 0; s < PPT; ++s)
-        if (kk[s] < M) vpart[(size_t)blockIdx.y * M + kk[s]] = v[s];
+    for (int r = 0; r < R; ++r)
+        if (kk[r] < M) vpart[(size_t)blockIdx.y * M + kk[r]] = v[r];
+}
+
+// near patches of the potential sweep: one warp per piece; lane = point; the 32 products of a listed group are
+// staged in the warp's own shared memory.  Writes near[piece][lane].
+template <int L>
+__global__ void __launch_bounds__(TPB) potential_near_kernel(const double4 *__restrict__ prodA, const double2 *__restrict__ prodB,
+                                                             const double *__restrict__ herm, int64_t npad,
+                                                             const double4 *__restrict__ pt, int M,
+                                                             const int64_t *__restrict__ start, const int32_t *__restrict__ list,
+                                                             const int64_t *__restrict__ pstart, const int32_t *__restrict__ piece_rg,
+                                                             int64_t npiece, double *__restrict__ near,
+                                                             const double *__restrict__ boysL) {
+    constexpr int NH = nherm(L);
+    constexpr int REC = pot_rec_near<L>();
+    __shared__ __align__(16) double s_rec[TPB / 32][SUB * REC];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
+    if (piece >= npiece) return;
+    const int64_t rg = piece_rg[piece];
+    const int k = (int)rg * SUB + lane;
+    const double4 c = pt[min(k, M - 1)];
+    double v = 0.0;
+    const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
+    double *mine = s_rec[warp];
+    for (int64_t e = ebeg; e < eend; ++e) {
+        const int64_t i0 = (int64_t)list[e] * SUB;
+        __syncwarp();
+        {
+            const double4 a = prodA[i0 + lane];
+            const double2 b = prodB[i0 + lane];
+            double *r = mine + lane * REC;
+            r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = a.w;
+            r[4 + NH] = b.x; r[5 + NH] = b.y;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) r[4 + h] = herm[(size_t)h * npad + i0 + lane];
+        }
+        __syncwarp();
+#pragma unroll 1
+        for (int t = 0; t < SUB; ++t) {
+            const double *rec = mine + t * REC;
+            const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+            const double2 h23 = *reinterpret_cast<const double2 *>(rec + 2);
+            const double x = h01.x - c.x, y = h01.y - c.y, z = h23.x - c.z;
+            const double r2 = fma(z, z, fma(y, y, x * x));
+            double g[L + 1];
+            if (hi32(r2) > hi32(h23.y)) seeds_far<L>(r2, g);
+            else seeds_general<L>(r2, rec[4 + NH], rec[5 + NH], c.w, boysL, g);
+            PotSink<L> sink{rec + 4, v};
+            hermite_R<L>(x, y, z, g, sink);
+            v = sink.v;
+        }
+    }
+    near[piece * SUB + lane] = v;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -374,6 +613,61 @@ __global__ void hermite_to_fock_kernel(int64_t ncomp, const int32_t *__restrict_
 }
 
 // ---------------------------------------------------------------------------------------------
+// work partition (fixed by the sizes, the SM count and the kernels' occupancy only -> results are reproducible)
+// ---------------------------------------------------------------------------------------------
+static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// rows: register-resident objects, rows_per_block of them per block; cols: streamed objects, cut into chunks of whole
+// tiles.  The grid (xb x chunks) is cut into about four waves of `wave` co-resident blocks when the sizes allow (the
+// hardware block scheduler then evens out what the skipped near patches unbalance): the smallest chunk count >= 4
+// waves whose last wave is at least 90 % full, or the best available.
+static Plan make_plan(int64_t rows, int rows_per_block, int64_t cols, int tile, int64_t wave) {
+    Plan p;
+    p.xb = ceil_div(std::max<int64_t>(rows, 1), rows_per_block);
+    const int64_t tiles = ceil_div(std::max<int64_t>(cols, 1), tile);
+    const int64_t maxc = std::min<int64_t>(tiles, 512);
+    int64_t best = 1;
+    double best_score = 0.0;
+    for (int64_t c = 1; c <= maxc; ++c) {
+        const int64_t len = ceil_div(tiles, c);            // tiles per chunk
+        const int64_t cc = ceil_div(tiles, len);           // chunks actually needed
+        const double t = (double)p.xb * (double)cc;
+        const double eff = t / ((double)ceil_div((int64_t)t, wave) * (double)wave);
+        const double score = eff * std::min(1.0, 0.55 + 0.45 * t / (4.0 * (double)wave));  // prefer >= 4 waves
+        if (score > best_score + 1e-9) { best_score = score; best = cc; }
+        if (t >= 4.0 * (double)wave && eff >= 0.9) break;
+    }
+    const int64_t len = ceil_div(tiles, best);
+    p.chunk_len = len * tile;
+    p.chunks = ceil_div(tiles, len);
+    return p;
+}
+
+template <class K>
+static int64_t wave_of(const pcm_ctx *ctx, K kernel) {
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, TPB, 0) != cudaSuccess || nb < 1) nb = 1;
+    return (int64_t)nb * ctx->sm_count;
+}
+
+template <int L>
+static void plan_class(pcm_ctx *ctx) {
+    constexpr Blocking fb = fock_blocking(L), pb = pot_blocking(L);
+    const ClassData &c = ctx->cls[L];
+    ctx->plan_fock[L] = make_plan(c.npad, TPB * fb.R, ctx->M, PT_TILE, wave_of(ctx, fock_kernel<L, fb.R, fb.C>));
+    ctx->plan_pot[L] = make_plan(ctx->M, TPB * pb.R, c.npad, pot_tile(L), wave_of(ctx, potential_kernel<L, pb.R, pb.C>));
+}
+
+int plan_all(pcm_ctx *ctx) {
+    constexpr Blocking ab = amat_blocking();
+    ctx->plan_amat = make_plan(ctx->M, TPB * ab.R, ctx->M, PT_TILE, wave_of(ctx, amatvec_kernel<ab.R, ab.C>));
+    plan_class<0>(ctx); plan_class<1>(ctx); plan_class<2>(ctx); plan_class<3>(ctx); plan_class<4>(ctx);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_error(ctx, PCM_ERR_CUDA, std::string("plan_all: ") + cudaGetErrorString(e));
+    return PCM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
 #define PCM_LAUNCH_CHECK(ctx)                                                                      \
@@ -387,56 +681,74 @@ static int mark(pcm_ctx *ctx, int i, cudaStream_t s) {
     return PCM_OK;
 }
 
-int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s) {
+// y = A q.  caller_order: q and y are indexed by the caller's point order (gather/scatter through s2c);
+// otherwise both are in the library's sorted order (the CG solver's internal vectors).
+static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool caller_order, cudaStream_t s) {
+    constexpr Blocking ab = amat_blocking();
     ctx->cur_op = 2;
     ctx->launches[2] = 0;
     ctx->timed[2] = ctx->timing != 0;
     const int M = (int)ctx->M;
     if (M == 0) return PCM_OK;
-    const int64_t chunks = amat_chunks(ctx);
-    const int chunk_len = (int)(ceil_div(ceil_div(M, chunks), 2) * 2);
+    const Plan &pl = ctx->plan_amat;
+    const PatchMap &pm = ctx->amat_map;
     const double thr = TFAR_AMAT * 2.0 / (ctx->zeta_min * ctx->zeta_min);
-    int64_t thr_bits;
-    memcpy(&thr_bits, &thr, 8);
-    const int thr_hi = (int)(thr_bits >> 32);
-    dim3 grid((unsigned)ceil_div(M, 2 * TPB), (unsigned)chunks);
+    const int32_t *idx = caller_order ? ctx->s2c : nullptr;
+    dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
     int rc;
     if ((rc = mark(ctx, 0, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
-    amatvec_kernel<<<grid, TPB, 0, s>>>(ctx->pt, ctx->pt_diag, q, M, chunk_len, chunks > 1 ? ctx->ypart : y, ctx->boys, thr_hi);
+    amatvec_kernel<ab.R, ab.C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);
-    { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
-    for (int i = 2; i <= 6; ++i)
-        if ((rc = mark(ctx, i, s))) return rc;
-    if (chunks > 1) {
-        reduce_slots_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(ctx->ypart, M, (int)chunks, y);
+    if (pm.npiece > 0) {
+        amat_near_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+            ctx->pt, ctx->pt_diag, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, ctx->boys, thr);
         PCM_LAUNCH_CHECK(ctx);
         { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     }
+    { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+    for (int i = 2; i <= 6; ++i)
+        if ((rc = mark(ctx, i, s))) return rc;
+    NearRefs nr;
+    nr.count = 1; nr.near[0] = ctx->near_amat; nr.pstart[0] = pm.pstart;
+    reduce_slots_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(ctx->ypart, M, (int)pl.chunks, y, idx, nr);
+    PCM_LAUNCH_CHECK(ctx);
+    { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return mark(ctx, 7, s);
 }
+int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s) { return launch_amatvec_impl(ctx, q, y, true, s); }
+int launch_amatvec_sorted(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s) { return launch_amatvec_impl(ctx, q, y, false, s); }
 
 template <int L>
 static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s) {
+    constexpr Blocking fb = fock_blocking(L);
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
-    const int64_t chunks = fock_chunks(ctx, L);
-    const int chunk_len = (int)(ceil_div(ceil_div(ctx->M, chunks), 2) * 2);
-    dim3 grid((unsigned)(c.npad / TPB), (unsigned)chunks);
-    fock_kernel<L><<<grid, TPB, 0, s>>>(c.prodA, c.prodB, c.npad, ctx->pt, q, (int)ctx->M, chunk_len, c.herm,
-                                        ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
+    const Plan &pl = ctx->plan_fock[L];
+    const PatchMap &pm = c.fock_map;
+    dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
+    fock_kernel<L, fb.R, fb.C><<<grid, TPB, 0, s>>>(c.prodA, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, (int)pl.chunk_len, c.herm,
+                                                    pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+    if (pm.npiece > 0) {
+        fock_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+            c.prodA, c.prodB, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
+            c.near_fock, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
+        PCM_LAUNCH_CHECK(ctx);
+        { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+    }
     return PCM_OK;
 }
 
 template <int L>
 static int reduce_fock_class(pcm_ctx *ctx, cudaStream_t s) {
     ClassData &c = ctx->cls[L];
-    const int64_t chunks = fock_chunks(ctx, L);
-    if (c.n == 0 || chunks <= 1) return PCM_OK;
+    const int64_t chunks = ctx->plan_fock[L].chunks;
+    if (c.n == 0) return PCM_OK;
     const int64_t plane = (int64_t)nherm(L) * c.npad;
-    reduce_herm_kernel<<<(unsigned)ceil_div(plane, 256), 256, 0, s>>>(c.herm, plane, (int)chunks);
+    reduce_herm_kernel<<<(unsigned)ceil_div(plane, 256), 256, 0, s>>>(c.herm, plane, (int)chunks, c.npad, nherm(L), c.near_fock,
+                                                                      c.fock_map.pstart);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
@@ -490,19 +802,26 @@ static int launch_density_class(pcm_ctx *ctx, const double *P, int64_t ldp, cuda
     return PCM_OK;
 }
 
-template <int L, int PPT>
+template <int L>
 static int launch_potential_class(pcm_ctx *ctx, int64_t &slot, cudaStream_t s) {
+    constexpr Blocking pb = pot_blocking(L);
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
-    const int64_t chunks = pot_chunks(ctx, L);
-    const int chunk_len = (int)ceil_div(c.n, chunks);
-    dim3 grid((unsigned)ceil_div(ctx->M, (int64_t)TPB * PPT), (unsigned)chunks);
-    potential_kernel<L, PPT><<<grid, TPB, 0, s>>>(c.prodA, c.prodB, c.herm, c.npad, c.n, chunk_len, ctx->pt, (int)ctx->M,
-                                                  ctx->vpart + (size_t)slot * ctx->M,
-                                                  ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
+    const Plan &pl = ctx->plan_pot[L];
+    const PatchMap &pm = c.pot_map;
+    dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
+    potential_kernel<L, pb.R, pb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
+                                                         ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);
+    slot += pl.chunks;
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
-    slot += chunks;
+    if (pm.npiece > 0) {
+        potential_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+            c.prodA, c.prodB, c.herm, c.npad, ctx->pt, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
+            c.near_pot, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
+        PCM_LAUNCH_CHECK(ctx);
+        { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+    }
     return PCM_OK;
 }
 
@@ -520,15 +839,19 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
     if ((rc = launch_density_class<4>(ctx, P, ldp, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
     int64_t slot = 0;
-    if ((rc = launch_potential_class<0, 2>(ctx, slot, s)) || (rc = mark(ctx, 2, s))) return rc;
-    if ((rc = launch_potential_class<1, 2>(ctx, slot, s)) || (rc = mark(ctx, 3, s))) return rc;
-    if ((rc = launch_potential_class<2, 2>(ctx, slot, s)) || (rc = mark(ctx, 4, s))) return rc;
-    if ((rc = launch_potential_class<3, 1>(ctx, slot, s)) || (rc = mark(ctx, 5, s))) return rc;
-    if ((rc = launch_potential_class<4, 1>(ctx, slot, s)) || (rc = mark(ctx, 6, s))) return rc;
+    if ((rc = launch_potential_class<0>(ctx, slot, s)) || (rc = mark(ctx, 2, s))) return rc;
+    if ((rc = launch_potential_class<1>(ctx, slot, s)) || (rc = mark(ctx, 3, s))) return rc;
+    if ((rc = launch_potential_class<2>(ctx, slot, s)) || (rc = mark(ctx, 4, s))) return rc;
+    if ((rc = launch_potential_class<3>(ctx, slot, s)) || (rc = mark(ctx, 5, s))) return rc;
+    if ((rc = launch_potential_class<4>(ctx, slot, s)) || (rc = mark(ctx, 6, s))) return rc;
     if (slot == 0) {
         PCM_CUDA(ctx, cudaMemsetAsync(v, 0, (size_t)ctx->M * 8, s));
     } else {
-        reduce_slots_kernel<<<(unsigned)ceil_div(ctx->M, 256), 256, 0, s>>>(ctx->vpart, ctx->M, (int)slot, v);
+        NearRefs nr;
+        nr.count = 0;
+        for (int L = 0; L <= MAXL; ++L)
+            if (ctx->cls[L].n > 0) { nr.near[nr.count] = ctx->cls[L].near_pot; nr.pstart[nr.count] = ctx->cls[L].pot_map.pstart; nr.count++; }
+        reduce_slots_kernel<<<(unsigned)ceil_div(ctx->M, 256), 256, 0, s>>>(ctx->vpart, ctx->M, (int)slot, v, ctx->s2c, nr);
         PCM_LAUNCH_CHECK(ctx);
         { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     }

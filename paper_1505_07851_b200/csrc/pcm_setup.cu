@@ -3,6 +3,8 @@
 #include <algorithm>
 #include <array>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <unordered_map>
 
@@ -156,6 +158,27 @@ static inline uint64_t spread21(uint64_t x) {
     return x;
 }
 
+// Hilbert-curve key of a cell (x, y, z), 21 bits per axis (Skilling's transpose algorithm): unlike the Morton order,
+// consecutive keys are always adjacent cells, so 32 consecutive objects of the sorted order stay compact in space.
+static inline uint64_t hilbert_key(uint64_t x, uint64_t y, uint64_t z) {
+    uint64_t X[3] = {x & 0x1fffff, y & 0x1fffff, z & 0x1fffff};
+    const uint64_t Mb = 1ULL << 20;
+    for (uint64_t Q = Mb; Q > 1; Q >>= 1) {
+        const uint64_t P = Q - 1;
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) X[0] ^= P;
+            else { const uint64_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    X[1] ^= X[0];
+    X[2] ^= X[1];
+    uint64_t t = 0;
+    for (uint64_t Q = Mb; Q > 1; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1;
+    for (int i = 0; i < 3; ++i) X[i] ^= t;
+    return (spread21(X[0]) << 2) | (spread21(X[1]) << 1) | spread21(X[2]);
+}
+
 struct KeyHash {
     size_t operator()(const std::array<uint64_t, 4> &k) const {
         uint64_t h = 0x9E3779B97F4A7C15ULL;
@@ -183,6 +206,66 @@ static int upload(pcm_ctx *ctx, T **dst, const std::vector<T> &src) {
     return PCM_OK;
 }
 
+// Group boxes: 7 doubles per group of 32 sorted objects -- lo xyz, hi xyz, largest far-field radius^2 in the group.
+struct GroupBoxes {
+    std::vector<double> b;
+    int64_t n() const { return (int64_t)b.size() / 7; }
+};
+static double box_gap2(const double *a, const double *b) {
+    double s = 0.0;
+    for (int d = 0; d < 3; ++d) {
+        const double g = std::max(std::max(a[d] - b[3 + d], b[d] - a[3 + d]), 0.0);
+        s += g * g;
+    }
+    return s;
+}
+// patch (rg, cg) is far when the boxes are further apart than both groups' far-field radii (1 % margin)
+static int build_patch_map(pcm_ctx *ctx, const GroupBoxes &rows, const GroupBoxes &cols, PatchMap &pm) {
+    const int64_t nrg = rows.n(), ncg = cols.n(), nbyte = (ncg + 7) / 8;
+    pm.nrg = nrg; pm.ncg = ncg; pm.nbyte = nbyte;
+    std::vector<uint8_t> far((size_t)std::max<int64_t>(nrg * nbyte, 1), 0);
+    std::vector<int64_t> start((size_t)nrg + 1, 0);
+#pragma omp parallel for schedule(static)
+    for (int64_t rg = 0; rg < nrg; ++rg) {
+        const double *a = &rows.b[(size_t)rg * 7];
+        int64_t cnt = 0;
+        for (int64_t cg = 0; cg < ncg; ++cg) {
+            const double *c = &cols.b[(size_t)cg * 7];
+            if (box_gap2(a, c) > 1.01 * std::max(a[6], c[6])) far[(size_t)rg * nbyte + cg / 8] |= (uint8_t)(1u << (cg & 7));
+            else ++cnt;
+        }
+        start[rg + 1] = cnt;
+    }
+    for (int64_t rg = 0; rg < nrg; ++rg) start[rg + 1] += start[rg];
+    std::vector<int32_t> list((size_t)std::max<int64_t>(start[nrg], 1), 0);
+#pragma omp parallel for schedule(static)
+    for (int64_t rg = 0; rg < nrg; ++rg) {
+        int64_t o = start[rg];
+        for (int64_t cg = 0; cg < ncg; ++cg)
+            if (!((far[(size_t)rg * nbyte + cg / 8] >> (cg & 7)) & 1)) list[o++] = (int32_t)cg;
+    }
+    pm.nnear = start[nrg];
+    // near-kernel work items: each row group's list is cut into pieces of at most NEAR_PIECE patches
+    std::vector<int64_t> pstart((size_t)nrg + 1, 0);
+    for (int64_t rg = 0; rg < nrg; ++rg) pstart[rg + 1] = pstart[rg] + (start[rg + 1] - start[rg] + NEAR_PIECE - 1) / NEAR_PIECE;
+    pm.npiece = pstart[nrg];
+    std::vector<int32_t> piece_rg((size_t)std::max<int64_t>(pm.npiece, 1), 0);
+    for (int64_t rg = 0; rg < nrg; ++rg)
+        for (int64_t q = pstart[rg]; q < pstart[rg + 1]; ++q) piece_rg[q] = (int32_t)rg;
+    if (getenv("PCM_VERBOSE")) {
+        int64_t mx = 0;
+        for (int64_t rg = 0; rg < nrg; ++rg) mx = std::max(mx, start[rg + 1] - start[rg]);
+        fprintf(stderr, "[pcm] patch map %lld x %lld: near %lld (%.2f %%), longest list %lld\n", (long long)nrg, (long long)ncg,
+                (long long)pm.nnear, 100.0 * (double)pm.nnear / std::max<double>(1.0, (double)nrg * (double)ncg), (long long)mx);
+    }
+    int rc;
+    if ((rc = upload(ctx, &pm.far, far))) return rc;
+    if ((rc = upload(ctx, &pm.start, start))) return rc;
+    if ((rc = upload(ctx, &pm.pstart, pstart))) return rc;
+    if ((rc = upload(ctx, &pm.piece_rg, piece_rg))) return rc;
+    return upload(ctx, &pm.list, list);
+}
+
 static int class_of(int la, int lb) {
     int lo = std::min(la, lb), hi = std::max(la, lb);
     static const int tab[3][3] = {{0, 1, 3}, {1, 2, 4}, {3, 4, 5}};
@@ -193,26 +276,54 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
                   const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
                   const double *pt_zeta, const double *pt_switch) {
     const pcm_options &opt = ctx->opt;
-    // ------------------------------------------------------------------ points
+    // ------------------------------------------------------------------ points (Hilbert order, boxes of 32)
     ctx->M = npoint;
+    GroupBoxes ptboxes;  // radius^2 entry 0: the product groups carry the far-field radius of a (product, point) pair
     {
-        std::vector<double4> pt((size_t)npoint);
-        std::vector<double> diag((size_t)npoint);
         double zmin = 1e300, zmax = 0.0;
+        double plo[3] = {1e300, 1e300, 1e300}, phi[3] = {-1e300, -1e300, -1e300};
         for (int64_t k = 0; k < npoint; ++k) {
-            const double z = pt_zeta[k];
-            pt[k] = make_double4(pt_xyz[3 * k], pt_xyz[3 * k + 1], pt_xyz[3 * k + 2], 1.0 / (z * z));
-            diag[k] = z * std::sqrt(2.0 / M_PI) / (pt_switch ? pt_switch[k] : 1.0);
-            zmin = std::min(zmin, z);
-            zmax = std::max(zmax, z);
+            zmin = std::min(zmin, pt_zeta[k]);
+            zmax = std::max(zmax, pt_zeta[k]);
+            for (int d = 0; d < 3; ++d) { plo[d] = std::min(plo[d], pt_xyz[3 * k + d]); phi[d] = std::max(phi[d], pt_xyz[3 * k + d]); }
         }
         if (npoint == 0) zmin = zmax = 1.0;
         ctx->zeta_min = zmin;
         ctx->zeta_max = zmax;
+        const double pspan = npoint ? std::max({phi[0] - plo[0], phi[1] - plo[1], phi[2] - plo[2], 1e-9}) : 1.0;
+        const double pcell = std::max(pspan / 2097151.0, 0.25);
+        std::vector<uint64_t> key((size_t)npoint);
+        for (int64_t k = 0; k < npoint; ++k)
+            key[k] = hilbert_key((uint64_t)((pt_xyz[3 * k] - plo[0]) / pcell), (uint64_t)((pt_xyz[3 * k + 1] - plo[1]) / pcell),
+                                 (uint64_t)((pt_xyz[3 * k + 2] - plo[2]) / pcell));
+        std::vector<int32_t> &s2c = ctx->s2c_host, &c2s = ctx->c2s_host;
+        s2c.resize((size_t)npoint);
+        c2s.resize((size_t)npoint);
+        for (int64_t k = 0; k < npoint; ++k) s2c[k] = (int32_t)k;
+        std::sort(s2c.begin(), s2c.end(), [&](int32_t a, int32_t b) { return key[a] != key[b] ? key[a] < key[b] : a < b; });
+        for (int64_t s = 0; s < npoint; ++s) c2s[s2c[s]] = (int32_t)s;
+        std::vector<double4> pt((size_t)npoint);
+        std::vector<double> diag((size_t)npoint);
+        const int64_t ng = (npoint + 31) / 32;
+        ptboxes.b.assign((size_t)ng * 7, 0.0);
+        std::vector<double> &box = ptboxes.b;
+        for (int64_t s = 0; s < npoint; ++s) {
+            const int64_t k = s2c[s];
+            const double z = pt_zeta[k];
+            pt[s] = make_double4(pt_xyz[3 * k], pt_xyz[3 * k + 1], pt_xyz[3 * k + 2], 1.0 / (z * z));
+            diag[s] = z * std::sqrt(2.0 / M_PI) / (pt_switch ? pt_switch[k] : 1.0);
+            double *bx = &box[(size_t)(s / 32) * 7];
+            if (s % 32 == 0) { for (int d = 0; d < 3; ++d) { bx[d] = 1e300; bx[3 + d] = -1e300; } }
+            for (int d = 0; d < 3; ++d) { bx[d] = std::min(bx[d], pt_xyz[3 * k + d]); bx[3 + d] = std::max(bx[3 + d], pt_xyz[3 * k + d]); }
+        }
         int rc = upload(ctx, &ctx->pt, pt);
         if (rc) return rc;
-        rc = upload(ctx, &ctx->pt_diag, diag);
-        if (rc) return rc;
+        if ((rc = upload(ctx, &ctx->pt_diag, diag))) return rc;
+        if ((rc = upload(ctx, &ctx->s2c, s2c))) return rc;
+        // A q patches: far-field radius^2 of a pair of points is at most TFAR_AMAT (1/zeta_i^2 + 1/zeta_j^2)
+        GroupBoxes amat_boxes = ptboxes;
+        for (int64_t g = 0; g < ng; ++g) amat_boxes.b[(size_t)g * 7 + 6] = TFAR_AMAT * 2.0 / (zmin * zmin);
+        if ((rc = build_patch_map(ctx, amat_boxes, amat_boxes, ctx->amat_map))) return rc;
     }
     {
         std::vector<double> tab;
@@ -364,7 +475,10 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
     ctx->ncomp = (int64_t)c_sp.size();
     for (int c = 0; c < PCM_NCLASS; ++c) info.prim_pairs_total += info.prim_pairs[c];
 
-    // ------------------------------------------------------------------ sort products by (L, Morton(P), p)
+    // ------------------------------------------------------------------ sort products by (L, reach, Hilbert(P), p)
+    // "reach" = binary order of magnitude of 1/p + 1/zeta_min^2, which the far-field radius^2 is proportional to:
+    // tight products (far from every surface point) and diffuse ones end up in different groups of 32, so that the
+    // box test of the hot kernels classifies whole groups.
     const int64_t np = (int64_t)prods.size();
     ctx->nprod = np;
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
@@ -374,16 +488,20 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         lo[2] = std::min(lo[2], q.z); hi[2] = std::max(hi[2], q.z);
     }
     const double span = std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], 1e-9});
-    // coarse Morton cells (~2 bohr) so that products of one neighbourhood end up sorted by exponent inside a cell
-    const double cell = std::max(span / 2097151.0, 2.0);
+    const double cell = std::max(span / 2097151.0, 0.25);
+    const double izmin2 = 1.0 / (ctx->zeta_min * ctx->zeta_min);
     std::vector<uint64_t> mort(np);
-    for (int64_t i = 0; i < np; ++i)
-        mort[i] = spread21((uint64_t)((prods[i].x - lo[0]) / cell)) | (spread21((uint64_t)((prods[i].y - lo[1]) / cell)) << 1) |
-                  (spread21((uint64_t)((prods[i].z - lo[2]) / cell)) << 2);
+    std::vector<int> reach(np);
+    for (int64_t i = 0; i < np; ++i) {
+        mort[i] = hilbert_key((uint64_t)((prods[i].x - lo[0]) / cell), (uint64_t)((prods[i].y - lo[1]) / cell),
+                              (uint64_t)((prods[i].z - lo[2]) / cell));
+        reach[i] = std::min(std::max(std::ilogb(1.0 / prods[i].p + izmin2), -6), 4);
+    }
     std::vector<int32_t> order(np);
     for (int64_t i = 0; i < np; ++i) order[i] = (int32_t)i;
     std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
         if (prods[x].L != prods[y].L) return prods[x].L < prods[y].L;
+        if (reach[x] != reach[y]) return reach[x] < reach[y];
         if (mort[x] != mort[y]) return mort[x] < mort[y];
         if (prods[x].p != prods[y].p) return prods[x].p > prods[y].p;
         return x < y;
@@ -401,21 +519,26 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         info.products[L] = n;
         std::vector<double4> pa((size_t)c.npad);
         std::vector<double2> pb((size_t)c.npad);
-        const double izmin2 = 1.0 / (ctx->zeta_min * ctx->zeta_min);
+        GroupBoxes pboxes;
+        pboxes.b.assign((size_t)(c.npad / 32) * 7, 0.0);
+        std::vector<double> &box = pboxes.b;
         for (int64_t i = 0; i < c.npad; ++i) {
-            if (i < n) {
-                const HostProd &q = prods[order[first + i]];
-                pa[i] = make_double4(q.x, q.y, q.z, tfar(L) * (1.0 / q.p + izmin2));
-                pb[i] = make_double2(q.p, 2.0 * std::sqrt(q.p / M_PI));
-            } else {  // padding: a product that is far from everything and carries zero density
-                pa[i] = make_double4(1e8, 1e8, 1e8, 1.0);
-                pb[i] = make_double2(1.0, 2.0 * std::sqrt(1.0 / M_PI));
-            }
+            // padding repeats the last product: it never carries density (D = 0) and its sums are never read
+            const HostProd &q = prods[order[first + std::min(i, n - 1)]];
+            pa[i] = make_double4(q.x, q.y, q.z, tfar(L) * (1.0 / q.p + izmin2));
+            pb[i] = make_double2(q.p, 2.0 * std::sqrt(q.p / M_PI));
+            double *bx = &box[(size_t)(i / 32) * 7];
+            if (i % 32 == 0) { for (int d = 0; d < 3; ++d) { bx[d] = 1e300; bx[3 + d] = -1e300; } bx[6] = 0.0; }
+            bx[0] = std::min(bx[0], q.x); bx[1] = std::min(bx[1], q.y); bx[2] = std::min(bx[2], q.z);
+            bx[3] = std::max(bx[3], q.x); bx[4] = std::max(bx[4], q.y); bx[5] = std::max(bx[5], q.z);
+            bx[6] = std::max(bx[6], pa[i].w);
         }
         int rc = upload(ctx, &c.prodA, pa);
         if (rc) return rc;
         rc = upload(ctx, &c.prodB, pb);
         if (rc) return rc;
+        if ((rc = build_patch_map(ctx, ptboxes, pboxes, c.pot_map))) return rc;
+        if ((rc = build_patch_map(ctx, pboxes, ptboxes, c.fock_map))) return rc;
         first += n;
     }
     info.products_total = np;

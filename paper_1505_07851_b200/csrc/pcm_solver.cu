@@ -130,7 +130,8 @@ __global__ void rbj_collect_kernel(int M, int block, const long long *__restrict
 // single block: rank the candidates by (key descending, index ascending), keep the first `take`
 __global__ void rbj_select_kernel(int M, int block, long long *__restrict__ state, int *__restrict__ cand_count,
                                   const int2 *__restrict__ cand_meta, const double *__restrict__ cand_key,
-                                  int *__restrict__ hist, unsigned char *__restrict__ assigned, int32_t *__restrict__ order) {
+                                  int *__restrict__ hist, unsigned char *__restrict__ assigned, int32_t *__restrict__ order,
+                                  const int32_t *__restrict__ s2c) {
     const long long filled = state[1];
     const int k = (int)state[2];
     const long long remaining = M - filled - 1;
@@ -138,12 +139,11 @@ __global__ void rbj_select_kernel(int M, int block, long long *__restrict__ stat
     const int n = *cand_count;
     for (int c = threadIdx.x; c < n; c += blockDim.x) {
         const double key = cand_key[c];
-        const int idx = cand_meta[c].x;
+        const int idx = cand_meta[c].x, cidx = s2c[idx];  // ties -> lower index in the caller's numbering
         int rank = 0;
         for (int o = 0; o < n; ++o) {
             const double ko = cand_key[o];
-            const int io = cand_meta[o].x;
-            rank += (ko > key) || (ko == key && io < idx);
+            rank += (ko > key) || (ko == key && s2c[cand_meta[o].x] < cidx);
         }
         if (rank < take) {
             order[filled + 1 + rank] = idx;
@@ -314,6 +314,16 @@ __global__ void residual_kernel(int M, const double *__restrict__ b, const doubl
     if (i < M) r[i] = b[i] - Ax[i];
 }
 
+// caller order <-> sorted order
+__global__ void gather_kernel(int M, const int32_t *__restrict__ s2c, const double *__restrict__ src, double *__restrict__ dst) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < M) dst[i] = src[s2c[i]];
+}
+__global__ void scatter_kernel(int M, const int32_t *__restrict__ s2c, const double *__restrict__ src, double *__restrict__ dst) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < M) dst[s2c[i]] = src[i];
+}
+
 // ---------------------------------------------------------------------------------------------
 // host drivers
 // ---------------------------------------------------------------------------------------------
@@ -334,8 +344,8 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     } else {
         pivot_order(seed, M, perm64.data());
     }
-    std::vector<int32_t> perm((size_t)M);
-    for (int64_t i = 0; i < M; ++i) perm[i] = (int32_t)perm64[i];
+    std::vector<int32_t> perm((size_t)M);  // pivot order in the library's sorted point numbering
+    for (int64_t i = 0; i < M; ++i) perm[i] = ctx->c2s_host[(size_t)perm64[i]];
 
     const int64_t nb = cdiv(M, block);
     // (re)allocate RBJ storage; earlier builds are released
@@ -385,7 +395,7 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     for (int64_t b = 0; b < nb; ++b) {
         rbj_keys_kernel<<<grid, threads, 0, s>>>(ctx->pt, ctx->pt_diag, (int)M, d_perm, d_assigned, d_state, d_keys, d_hist, ctx->boys);
         rbj_collect_kernel<<<grid, threads, 0, s>>>((int)M, block, d_state, d_keys, d_hist, d_count, d_meta, d_ckey);
-        rbj_select_kernel<<<1, 1024, 0, s>>>((int)M, block, d_state, d_count, d_meta, d_ckey, d_hist, d_assigned, ctx->rbj_order);
+        rbj_select_kernel<<<1, 1024, 0, s>>>((int)M, block, d_state, d_count, d_meta, d_ckey, d_hist, d_assigned, ctx->rbj_order, ctx->s2c);
         ctx->launch_total += 3;
     }
     ctx->launch_total += 1;
@@ -435,25 +445,30 @@ static int dot2(pcm_ctx *ctx, const double *a, const double *b, const double *c,
     return PCM_OK;
 }
 
-int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter, int precond, int use_x0, int *iters,
-             double *resid, cudaStream_t s) {
+int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol, int max_iter, int precond, int use_x0,
+             int *iters, double *resid, cudaStream_t s) {
     const int M = (int)ctx->M;
     if (precond < 0 || precond > 2) return set_error(ctx, PCM_ERR_ARG, "pcm_cg_solve: precond must be 0, 1 or 2");
     if (precond == 2 && ctx->rbj_block == 0) return set_error(ctx, PCM_ERR_STATE, "pcm_cg_solve: RBJ requested before pcm_rbj_build");
     if (M == 0) { if (iters) *iters = 0; if (resid) resid[0] = resid[1] = 0.0; return PCM_OK; }
-    double *r = ctx->cg_vec, *z = r + M, *p = z + M, *Ap = p + M;
+    // all solver vectors live in the library's sorted point order; b is gathered on entry, x scattered on exit
+    double *r = ctx->cg_vec, *z = r + M, *p = z + M, *Ap = p + M, *x = Ap + M, *b = x + M;
     double *scal = ctx->cg_scal, *partial = scal + 16;
     double *h = ctx->cg_scal_host;
     int rc;
     const int saved_timing = ctx->timing;
     ctx->timing = 0;
+    const unsigned gb = (unsigned)cdiv(M, 256);
 #define CG_TRY(expr) do { rc = (expr); if (rc) { ctx->timing = saved_timing; return rc; } } while (0)
 #define CG_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { ctx->timing = saved_timing; \
         return set_error(ctx, PCM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); } } while (0)
+    gather_kernel<<<gb, 256, 0, s>>>(M, ctx->s2c, b_caller, b);
+    ctx->launch_total += 1;
     if (use_x0) {
-        CG_TRY(launch_amatvec(ctx, x, Ap, s));
-        residual_kernel<<<(unsigned)cdiv(M, 256), 256, 0, s>>>(M, b, Ap, r);
-        ctx->launch_total += 1;
+        gather_kernel<<<gb, 256, 0, s>>>(M, ctx->s2c, x_caller, x);
+        CG_TRY(launch_amatvec_sorted(ctx, x, Ap, s));
+        residual_kernel<<<gb, 256, 0, s>>>(M, b, Ap, r);
+        ctx->launch_total += 2;
     } else {
         CG_CUDA(cudaMemsetAsync(x, 0, (size_t)M * 8, s));
         CG_CUDA(cudaMemcpyAsync(r, b, (size_t)M * 8, cudaMemcpyDeviceToDevice, s));
@@ -466,7 +481,7 @@ int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter,
     double rn = std::sqrt(h[2]);
     int it = 0;
     while (rn > tol && it < max_iter) {
-        CG_TRY(launch_amatvec(ctx, p, Ap, s));
+        CG_TRY(launch_amatvec_sorted(ctx, p, Ap, s));
         CG_TRY(dot2(ctx, p, Ap, nullptr, nullptr, 1, -1, s));  // pAp
         cg_update_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, scal, p, Ap, x, r, partial);
         dot_final_kernel<<<1, DOT_THREADS, 0, s>>>(partial, scal, 2, -1);  // rr
@@ -475,7 +490,7 @@ int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter,
         // queue the rest of the iteration before looking at the residual
         CG_TRY(apply_precond(ctx, precond, r, z, s));
         CG_TRY(dot2(ctx, r, z, nullptr, nullptr, 3, -1, s));  // rz_new
-        cg_direction_kernel<<<(unsigned)cdiv(M, 256), 256, 0, s>>>(M, scal, z, p);
+        cg_direction_kernel<<<gb, 256, 0, s>>>(M, scal, z, p);
         cg_shift_kernel<<<1, 1, 0, s>>>(scal);
         ctx->launch_total += 4;  // update, rr reduction, direction, shift
         CG_CUDA(cudaGetLastError());
@@ -484,10 +499,11 @@ int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter,
         rn = std::sqrt(h[2]);
     }
     // true residual
-    CG_TRY(launch_amatvec(ctx, x, Ap, s));
-    residual_kernel<<<(unsigned)cdiv(M, 256), 256, 0, s>>>(M, b, Ap, z);
-    ctx->launch_total += 1;
+    CG_TRY(launch_amatvec_sorted(ctx, x, Ap, s));
+    residual_kernel<<<gb, 256, 0, s>>>(M, b, Ap, z);
     CG_TRY(dot2(ctx, z, z, nullptr, nullptr, 4, -1, s));
+    scatter_kernel<<<gb, 256, 0, s>>>(M, ctx->s2c, x, x_caller);
+    ctx->launch_total += 2;
     CG_CUDA(cudaMemcpyAsync(h, scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, s));
     CG_CUDA(cudaStreamSynchronize(s));
 #undef CG_TRY
