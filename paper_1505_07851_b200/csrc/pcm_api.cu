@@ -39,6 +39,9 @@ static void free_ctx(pcm_ctx *ctx) {
     if (ctx->io_b) cudaFree(ctx->io_b);
     for (auto &e : ctx->ev) if (e) cudaEventDestroy(e);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    if (ctx->near_stream) cudaStreamDestroy(ctx->near_stream);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     delete[] ctx->rbj_bstart_host;
     delete ctx;
 }
@@ -89,6 +92,13 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     if (e != cudaSuccess) { ctx->err = std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
     ctx->sm_count = prop.multiProcessorCount;
     e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) {
+        int prio_lo = 0, prio_hi = 0;
+        cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+        e = cudaStreamCreateWithPriority(&ctx->near_stream, cudaStreamNonBlocking, prio_hi);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
     if (e != cudaSuccess) { ctx->err = std::string("cudaStreamCreate: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
     for (auto &ev : ctx->ev) {
         e = cudaEventCreate(&ev);

@@ -59,7 +59,7 @@ struct PatchMap {
     int64_t *pstart = nullptr;  // [nrg + 1] CSR: pieces of each row group
     int32_t *piece_rg = nullptr;  // [npiece]
 };
-constexpr int NEAR_PIECE = 8;
+constexpr int NEAR_PIECE = 4;
 
 struct ClassData {        // products of one total angular momentum L, padded to a multiple of 128
     int64_t n = 0;        // products
@@ -148,8 +148,15 @@ struct pcm_ctx {
     int32_t *rbj_order = nullptr;    // [M] point indices block after block
     int64_t *rbj_bstart_host = nullptr;
     double *rbj_inv = nullptr;       // inverse blocks back to back (block b at b*l*l)
+    double *rbj_partial = nullptr;   // [2][rbj_nblocks] per-block r.r and r.z of the CG update kernel
+    char *rbj_arena = nullptr;       // grow-only allocation holding the three arrays above and the build scratch
+    size_t rbj_arena_bytes = 0;
 
     cudaStream_t own_stream = nullptr;
+    // the near kernels run on near_stream, forked from and joined back into the caller's stream around the main
+    // kernels of the same call, so that their latency-bound work fills what the FP64-bound main kernels leave idle
+    cudaStream_t near_stream = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     // events: 0 start, 1 after the pre-transform, 2+L after the class-L main kernel, 7 end, 8 CG residual read-back
     cudaEvent_t ev[28] = {};   // ev[8*op + i], op = 0 potential, 1 fock, 2 amatvec; 24 CG; 25, 26 peak benchmark
     int timing = 0;
@@ -174,6 +181,7 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
 int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accumulate, cudaStream_t s);
 int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s);
 int launch_amatvec_sorted(pcm_ctx *ctx, const double *q_sorted, double *y_sorted, cudaStream_t s);  // both in sorted order
+int launch_amatvec_partials(pcm_ctx *ctx, const double *q_sorted, const int *stop, cudaStream_t s);  // ypart slots + near_amat only
 int plan_all(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
 void build_boys_tables(std::vector<double> &tab);

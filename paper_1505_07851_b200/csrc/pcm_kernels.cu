@@ -99,9 +99,10 @@ template <int R, int C>
 __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ q,
                                                       const int32_t *__restrict__ qidx, int M, int chunk_len,
                                                       double *__restrict__ out, const uint8_t *__restrict__ farmap,
-                                                      int64_t nbyte, int64_t nrg) {
+                                                      int64_t nbyte, int64_t nrg, const int *__restrict__ stop) {
     constexpr int NS = PT_TILE / SUB;
     __shared__ double4 s_pt[PT_TILE];   // x, y, z, q
+    if (stop && *stop) return;  // a converged CG solve: the iterations queued behind it are no-ops
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
     double4 a[R];
@@ -168,9 +169,11 @@ __global__ void __launch_bounds__(TPB) amat_near_kernel(const double4 *__restric
                                                         const int64_t *__restrict__ start, const int32_t *__restrict__ list,
                                                         const int64_t *__restrict__ pstart, const int32_t *__restrict__ piece_rg,
                                                         int64_t npiece, double *__restrict__ near,
-                                                        const double *__restrict__ boys0, double thr) {
+                                                        const double *__restrict__ boys0, double thr,
+                                                        const int *__restrict__ stop) {
     __shared__ double4 s_pt[TPB / 32][SUB];
     __shared__ double s_iz[TPB / 32][SUB];
+    if (stop && *stop) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
     if (piece >= npiece) return;
@@ -681,10 +684,37 @@ static int mark(pcm_ctx *ctx, int i, cudaStream_t s) {
     return PCM_OK;
 }
 
+// Partial sums of y = A q: near pieces into near_amat (near stream, forked from and joined back into s), main kernel
+// slots into ypart.  idx: sorted -> caller index of q (nullptr: q is in sorted order).  stop: see cg_solve.
+static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *idx, const int *stop, cudaStream_t s) {
+    constexpr Blocking ab = amat_blocking();
+    const int M = (int)ctx->M;
+    const Plan &pl = ctx->plan_amat;
+    const PatchMap &pm = ctx->amat_map;
+    const double thr = TFAR_AMAT * 2.0 / (ctx->zeta_min * ctx->zeta_min);
+    dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
+    if (pm.npiece > 0) {
+        PCM_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
+        PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->near_stream, ctx->ev_fork, 0));
+        amat_near_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, ctx->near_stream>>>(
+            ctx->pt, ctx->pt_diag, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, ctx->boys, thr, stop);
+        PCM_LAUNCH_CHECK(ctx);
+        PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
+        { ctx->launches[2]++; ctx->launch_total++; }
+    }
+    amatvec_kernel<ab.R, ab.C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, pm.far, pm.nbyte, pm.nrg, stop);
+    PCM_LAUNCH_CHECK(ctx);
+    { ctx->launches[2]++; ctx->launch_total++; }
+    if (pm.npiece > 0) PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
+    return PCM_OK;
+}
+int launch_amatvec_partials(pcm_ctx *ctx, const double *q_sorted, const int *stop, cudaStream_t s) {
+    return launch_amatvec_kernels(ctx, q_sorted, nullptr, stop, s);
+}
+
 // y = A q.  caller_order: q and y are indexed by the caller's point order (gather/scatter through s2c);
 // otherwise both are in the library's sorted order (the CG solver's internal vectors).
 static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool caller_order, cudaStream_t s) {
-    constexpr Blocking ab = amat_blocking();
     ctx->cur_op = 2;
     ctx->launches[2] = 0;
     ctx->timed[2] = ctx->timing != 0;
@@ -692,21 +722,11 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
     if (M == 0) return PCM_OK;
     const Plan &pl = ctx->plan_amat;
     const PatchMap &pm = ctx->amat_map;
-    const double thr = TFAR_AMAT * 2.0 / (ctx->zeta_min * ctx->zeta_min);
     const int32_t *idx = caller_order ? ctx->s2c : nullptr;
-    dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
     int rc;
     if ((rc = mark(ctx, 0, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
-    amatvec_kernel<ab.R, ab.C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, pm.far, pm.nbyte, pm.nrg);
-    PCM_LAUNCH_CHECK(ctx);
-    if (pm.npiece > 0) {
-        amat_near_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
-            ctx->pt, ctx->pt_diag, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, ctx->boys, thr);
-        PCM_LAUNCH_CHECK(ctx);
-        { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
-    }
-    { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+    if ((rc = launch_amatvec_kernels(ctx, q, idx, nullptr, s))) return rc;
     for (int i = 2; i <= 6; ++i)
         if ((rc = mark(ctx, i, s))) return rc;
     NearRefs nr;
@@ -720,6 +740,19 @@ int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s) { r
 int launch_amatvec_sorted(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s) { return launch_amatvec_impl(ctx, q, y, false, s); }
 
 template <int L>
+static int launch_fock_near(pcm_ctx *ctx, const double *q, cudaStream_t s) {
+    ClassData &c = ctx->cls[L];
+    const PatchMap &pm = c.fock_map;
+    if (c.n == 0 || pm.npiece == 0) return PCM_OK;
+    fock_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+        c.prodA, c.prodB, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
+        c.near_fock, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
+    PCM_LAUNCH_CHECK(ctx);
+    { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+    return PCM_OK;
+}
+
+template <int L>
 static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s) {
     constexpr Blocking fb = fock_blocking(L);
     ClassData &c = ctx->cls[L];
@@ -731,13 +764,6 @@ static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s) {
                                                     pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
-    if (pm.npiece > 0) {
-        fock_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
-            c.prodA, c.prodB, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
-            c.near_fock, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
-        PCM_LAUNCH_CHECK(ctx);
-        { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
-    }
     return PCM_OK;
 }
 
@@ -762,11 +788,21 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
     if ((rc = mark(ctx, 0, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
     if (ctx->M > 0) {
+        // near kernels of all classes on the near stream, concurrently with the main kernels on s
+        PCM_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
+        PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->near_stream, ctx->ev_fork, 0));
+        if ((rc = launch_fock_near<0>(ctx, q, ctx->near_stream))) return rc;
+        if ((rc = launch_fock_near<1>(ctx, q, ctx->near_stream))) return rc;
+        if ((rc = launch_fock_near<2>(ctx, q, ctx->near_stream))) return rc;
+        if ((rc = launch_fock_near<3>(ctx, q, ctx->near_stream))) return rc;
+        if ((rc = launch_fock_near<4>(ctx, q, ctx->near_stream))) return rc;
+        PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
         if ((rc = launch_fock_class<0>(ctx, q, s)) || (rc = mark(ctx, 2, s))) return rc;
         if ((rc = launch_fock_class<1>(ctx, q, s)) || (rc = mark(ctx, 3, s))) return rc;
         if ((rc = launch_fock_class<2>(ctx, q, s)) || (rc = mark(ctx, 4, s))) return rc;
         if ((rc = launch_fock_class<3>(ctx, q, s)) || (rc = mark(ctx, 5, s))) return rc;
         if ((rc = launch_fock_class<4>(ctx, q, s)) || (rc = mark(ctx, 6, s))) return rc;
+        PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
     } else {
         for (int i = 2; i <= 6; ++i)
             if ((rc = mark(ctx, i, s))) return rc;
@@ -803,6 +839,19 @@ static int launch_density_class(pcm_ctx *ctx, const double *P, int64_t ldp, cuda
 }
 
 template <int L>
+static int launch_potential_near(pcm_ctx *ctx, cudaStream_t s) {
+    ClassData &c = ctx->cls[L];
+    const PatchMap &pm = c.pot_map;
+    if (c.n == 0 || pm.npiece == 0) return PCM_OK;
+    potential_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+        c.prodA, c.prodB, c.herm, c.npad, ctx->pt, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
+        c.near_pot, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
+    PCM_LAUNCH_CHECK(ctx);
+    { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+    return PCM_OK;
+}
+
+template <int L>
 static int launch_potential_class(pcm_ctx *ctx, int64_t &slot, cudaStream_t s) {
     constexpr Blocking pb = pot_blocking(L);
     ClassData &c = ctx->cls[L];
@@ -815,13 +864,6 @@ static int launch_potential_class(pcm_ctx *ctx, int64_t &slot, cudaStream_t s) {
     PCM_LAUNCH_CHECK(ctx);
     slot += pl.chunks;
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
-    if (pm.npiece > 0) {
-        potential_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
-            c.prodA, c.prodB, c.herm, c.npad, ctx->pt, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
-            c.near_pot, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
-        PCM_LAUNCH_CHECK(ctx);
-        { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
-    }
     return PCM_OK;
 }
 
@@ -838,12 +880,22 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
     if ((rc = launch_density_class<3>(ctx, P, ldp, s))) return rc;
     if ((rc = launch_density_class<4>(ctx, P, ldp, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
+    // near kernels of all classes on the near stream (they need the Hermite densities), concurrently with the main kernels on s
+    PCM_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
+    PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->near_stream, ctx->ev_fork, 0));
+    if ((rc = launch_potential_near<0>(ctx, ctx->near_stream))) return rc;
+    if ((rc = launch_potential_near<1>(ctx, ctx->near_stream))) return rc;
+    if ((rc = launch_potential_near<2>(ctx, ctx->near_stream))) return rc;
+    if ((rc = launch_potential_near<3>(ctx, ctx->near_stream))) return rc;
+    if ((rc = launch_potential_near<4>(ctx, ctx->near_stream))) return rc;
+    PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
     int64_t slot = 0;
     if ((rc = launch_potential_class<0>(ctx, slot, s)) || (rc = mark(ctx, 2, s))) return rc;
     if ((rc = launch_potential_class<1>(ctx, slot, s)) || (rc = mark(ctx, 3, s))) return rc;
     if ((rc = launch_potential_class<2>(ctx, slot, s)) || (rc = mark(ctx, 4, s))) return rc;
     if ((rc = launch_potential_class<3>(ctx, slot, s)) || (rc = mark(ctx, 5, s))) return rc;
     if ((rc = launch_potential_class<4>(ctx, slot, s)) || (rc = mark(ctx, 6, s))) return rc;
+    PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
     if (slot == 0) {
         PCM_CUDA(ctx, cudaMemsetAsync(v, 0, (size_t)ctx->M * 8, s));
     } else {

@@ -1,6 +1,9 @@
 // pcm_solver.cu -- steps a5 (randomized block-Jacobi build) and a6 (preconditioned CG,
 // PAPER.md:164-170) of SURVEY.md 8(a).  The matrix-vector product is pcm_kernels.cu's on-the-fly A q.
 #include <algorithm>
+#include <chrono>
+#include <cstdio>
+#include <cstdlib>
 #include <cmath>
 #include <cstring>
 #include <numeric>
@@ -26,22 +29,17 @@ static inline uint64_t mix64(uint64_t z) {
     return z ^ (z >> 31);
 }
 void pivot_order(uint64_t seed, int64_t M, int64_t *perm) {
-    std::vector<uint64_t> key((size_t)M);
-    for (int64_t i = 0; i < M; ++i) key[i] = mix64(seed + (uint64_t)(i + 1) * 0x9E3779B97F4A7C15ULL);
-    std::iota(perm, perm + M, (int64_t)0);
-    std::sort(perm, perm + M, [&](int64_t a, int64_t b) { return key[a] != key[b] ? key[a] < key[b] : a < b; });
+    std::vector<std::pair<uint64_t, int64_t>> key((size_t)M);
+    for (int64_t i = 0; i < M; ++i) key[i] = {mix64(seed + (uint64_t)(i + 1) * 0x9E3779B97F4A7C15ULL), i};
+    std::sort(key.begin(), key.end());  // by key, ties by index
+    for (int64_t i = 0; i < M; ++i) perm[i] = key[i].second;
 }
 
 // ---------------------------------------------------------------------------------------------
 // A_ij for arbitrary i, j (Eq. 2, 3, 8)
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double a_entry(const double4 *__restrict__ pt, const double *__restrict__ diag, int i, int j,
-                                          const double *__restrict__ boys0) {
-    if (i == j) return diag[i];
-    const double4 a = pt[i], b = pt[j];
-    const double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
-    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-    const double zp = rsqrt_fast(a.w + b.w);
+__device__ __forceinline__ double amat_entry(double r2, double izi, double izj, const double *__restrict__ boys0) {
+    const double zp = rsqrt_fast(izi + izj);
     const double T = r2 * zp * zp;
     if (T >= TFAR_AMAT) return rsqrt_fast(r2);
     const int t = __double2int_rn(T * 16.0);
@@ -52,113 +50,194 @@ __device__ __forceinline__ double a_entry(const double4 *__restrict__ pt, const 
     for (int k = BOYS_TERMS - 2; k >= 0; --k) f = fma(f, d, __ldg(row + k));
     return 1.1283791670955125739 * zp * f;
 }
+__device__ __forceinline__ double a_entry(const double4 *__restrict__ pt, const double *__restrict__ diag, int i, int j,
+                                          const double *__restrict__ boys0) {
+    if (i == j) return diag[i];
+    const double4 a = pt[i], b = pt[j];
+    const double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
+    return amat_entry(fma(dz, dz, fma(dy, dy, dx * dx)), a.w, b.w, boys0);
+}
 
 // ---------------------------------------------------------------------------------------------
-// RBJ block selection.  One step = one block: three small kernels over device-resident state.
-//   state[0] = pos (next position in the pivot order), [1] = filled, [2] = pivot, [3] = candidate count,
-//   [4] = error flag, [5] = take (block size - 1 for this step)
-// Keys are A_kj > 0, compared as 64-bit integers.  Buckets = the top 16 bits of the key (sign, exponent,
-// 4 mantissa bits) shifted into [0, 1023]: a monotone map, so "bucket >= b*" is a superset of the top `take`.
+// RBJ block selection: ONE persistent cooperative kernel for the whole sequence of blocks.  The blocks
+// are inherently sequential (the next pivot depends on what the previous blocks took), a step's work -- one row of A
+// over the unassigned points, then the l-1 largest -- is tiny, so the cost is synchronisation: two grid barriers per
+// step instead of three kernel launches.
+//   phase A  every CTA finds the step's pivot (first unassigned index of the pivot order; same answer everywhere),
+//            evaluates A_kj for its own unassigned j, keeps the keys, histograms them (1024 buckets of the top 16
+//            key bits, a monotone map)                                                     -- grid barrier 1
+//   phase B  every CTA reads the histogram, finds the cut bucket b* (the top `take` keys all have bucket >= b*) and
+//            appends its own candidates (bucket >= b*) to the step's candidate list        -- grid barrier 2
+//   phase C  every CTA ranks the (few) candidates by (key descending, caller index ascending) and marks the first
+//            `take` as assigned: all CTAs compute the same set and write the same flags, so no third barrier is
+//            needed; CTA 0 also writes the block to `order`.
+// Histograms are triple-buffered, candidate lists double-buffered; CTA 0 clears a buffer two phases after its last
+// reader.  Keys are A_kj > 0 compared as doubles.
 // ---------------------------------------------------------------------------------------------
 constexpr int RBJ_BINS = 1024;
 constexpr int RBJ_BIN_BASE = 0x3e00;  // bucket of 2^-31
+constexpr int RBJ_THREADS = 512;
+constexpr int RBJ_CAP = 1536;         // candidates ranked from shared memory; more (many near-ties) take the global path
 
 __device__ __forceinline__ int rbj_bucket(double a) {
     const int b = (int)((unsigned long long)__double_as_longlong(a) >> 48) - RBJ_BIN_BASE;
     return min(max(b, 0), RBJ_BINS - 1);
 }
 
-__global__ void rbj_keys_kernel(const double4 *__restrict__ pt, const double *__restrict__ diag, int M,
-                                const int32_t *__restrict__ perm, const unsigned char *__restrict__ assigned,
-                                long long *__restrict__ state, double *__restrict__ keys, int *__restrict__ hist,
-                                const double *__restrict__ boys0) {
+struct RbjWork {
+    int *hist;                 // [3][RBJ_BINS]
+    int *cand_count;           // [2]
+    double *cand_key;          // [2][M]
+    int *cand_idx;             // [2][M]
+    double *keys;              // [M]
+    unsigned char *assigned;   // [M]
+    unsigned long long *bar;   // grid barrier counter
+    int *err;
+};
+
+__device__ __forceinline__ void grid_barrier(unsigned long long *bar, unsigned long long &target, unsigned nblocks) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += nblocks;
+        __threadfence();
+        atomicAdd(bar, 1ULL);
+        while (*((volatile unsigned long long *)bar) < target) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(RBJ_THREADS) rbj_select_kernel(const double4 *__restrict__ pt, const double *__restrict__ diag,
+                                                                 int M, int block, const int32_t *__restrict__ perm,
+                                                                 const int32_t *__restrict__ s2c, int32_t *__restrict__ order,
+                                                                 RbjWork w, const double *__restrict__ boys0) {
     __shared__ int s_hist[RBJ_BINS];
-    __shared__ int s_pivot;
-    // every block finds the same pivot: the first unassigned index of the pivot order at or after pos
-    if (threadIdx.x == 0) s_pivot = M;
-    for (int t = threadIdx.x; t < RBJ_BINS; t += blockDim.x) s_hist[t] = 0;
-    __syncthreads();
-    long long pos = state[0];
-    while (true) {
-        const long long p = pos + threadIdx.x;
-        if (p < M && !assigned[perm[p]]) atomicMin(&s_pivot, (int)p);
+    __shared__ int s_scan[RBJ_THREADS];
+    __shared__ double s_key[RBJ_CAP];
+    __shared__ int s_idx[RBJ_CAP];
+    __shared__ int s_cidx[RBJ_CAP];
+    __shared__ int s_pivot, s_bstar;
+    const unsigned nblocks = gridDim.x;
+    const int tid = threadIdx.x, gtid = blockIdx.x * RBJ_THREADS + tid, gstride = nblocks * RBJ_THREADS;
+    unsigned long long target = 0;
+    long long pos = 0, filled = 0;
+    for (long long step = 0; filled < M; ++step) {
+        int *hist = w.hist + (step % 3) * RBJ_BINS;
+        int *cnt = w.cand_count + (step & 1);
+        double *ckey = w.cand_key + (size_t)(step & 1) * M;
+        int *cidx = w.cand_idx + (size_t)(step & 1) * M;
+        // ---- phase A: pivot, keys, histogram
+        if (tid == 0) s_pivot = M;
+        for (int t = tid; t < RBJ_BINS; t += RBJ_THREADS) s_hist[t] = 0;
         __syncthreads();
-        if (s_pivot < M || pos + blockDim.x >= M) break;
-        pos += blockDim.x;
+        while (true) {
+            const long long p = pos + tid;
+            if (p < M && !w.assigned[perm[p]]) atomicMin(&s_pivot, (int)p);
+            __syncthreads();
+            if (s_pivot < M || pos + RBJ_THREADS >= M) break;
+            pos += RBJ_THREADS;
+            __syncthreads();
+        }
+        const int ppos = s_pivot;
+        if (ppos >= M) { if (gtid == 0) *w.err = 2; return; }  // cannot happen while filled < M (uniform exit)
+        pos = ppos;
+        const int k = perm[ppos];
+        const long long remaining = M - filled - 1;
+        const int take = (int)min((long long)block - 1, remaining);
+        const double4 pk = pt[k];
+        for (int j = gtid; j < M; j += gstride) {
+            double a = 0.0;
+            if (!w.assigned[j] && j != k) {
+                const double4 b = pt[j];
+                const double dx = pk.x - b.x, dy = pk.y - b.y, dz = pk.z - b.z;
+                a = amat_entry(fma(dz, dz, fma(dy, dy, dx * dx)), pk.w, b.w, boys0);
+                atomicAdd(&s_hist[rbj_bucket(a)], 1);
+            }
+            w.keys[j] = a;
+        }
         __syncthreads();
-    }
-    const int ppos = s_pivot;
-    if (ppos >= M) return;  // nothing left (not reached in a correct schedule)
-    const int k = perm[ppos];
-    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
-        double a = 0.0;
-        if (!assigned[j] && j != k) {
-            a = a_entry(pt, diag, k, j, boys0);
-            atomicAdd(&s_hist[rbj_bucket(a)], 1);
+        if (take > 0)
+            for (int t = tid; t < RBJ_BINS; t += RBJ_THREADS)
+                if (s_hist[t]) atomicAdd(&hist[t], s_hist[t]);
+        if (blockIdx.x == 0) {  // clear what step + 1 will accumulate into (last read in phase B of step - 2)
+            int *nh = w.hist + ((step + 1) % 3) * RBJ_BINS;
+            for (int t = tid; t < RBJ_BINS; t += RBJ_THREADS) nh[t] = 0;
         }
-        keys[j] = a;
-    }
-    __syncthreads();
-    for (int t = threadIdx.x; t < RBJ_BINS; t += blockDim.x)
-        if (s_hist[t]) atomicAdd(&hist[t], s_hist[t]);
-    if (blockIdx.x == 0 && threadIdx.x == 0) { state[0] = ppos; state[2] = k; }
-}
-
-__global__ void rbj_collect_kernel(int M, int block, const long long *__restrict__ state, const double *__restrict__ keys,
-                                   const int *__restrict__ hist, int *__restrict__ cand_count, int2 *__restrict__ cand_meta,
-                                   double *__restrict__ cand_key) {
-    __shared__ int s_bstar;
-    if (threadIdx.x == 0) {
-        const long long remaining = M - state[1] - 1;  // unassigned other than the pivot
-        const long long take = min((long long)block - 1, remaining);
-        int b = RBJ_BINS, cum = 0;
-        while (b > 0 && cum < take) { --b; cum += hist[b]; }
-        s_bstar = (take > 0) ? b : RBJ_BINS;
-    }
-    __syncthreads();
-    const int bstar = s_bstar;
-    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
-        const double a = keys[j];
-        if (a > 0.0 && rbj_bucket(a) >= bstar) {
-            const int slot = atomicAdd(cand_count, 1);
-            cand_meta[slot] = make_int2(j, 0);
-            cand_key[slot] = a;
+        grid_barrier(w.bar, target, nblocks);
+        // ---- phase B: cut bucket, candidates
+        if (take > 0) {
+            // suffix counts: s_scan[t] = keys in buckets >= 2t (two buckets per thread)
+            const int h0 = __ldcg(hist + 2 * tid), h1 = __ldcg(hist + 2 * tid + 1);
+            s_scan[tid] = h0 + h1;
+            __syncthreads();
+            for (int o = 1; o < RBJ_THREADS; o <<= 1) {
+                const int v = (tid + o < RBJ_THREADS) ? s_scan[tid + o] : 0;
+                __syncthreads();
+                s_scan[tid] += v;
+                __syncthreads();
+            }
+            // b* = the largest bucket b with count(bucket >= b) >= take
+            const int above = (tid + 1 < RBJ_THREADS) ? s_scan[tid + 1] : 0;  // buckets >= 2 tid + 2
+            if (above < take && above + h1 >= take) s_bstar = 2 * tid + 1;
+            else if (above + h1 < take && above + h1 + h0 >= take) s_bstar = 2 * tid;
+            __syncthreads();
+            const int bstar = s_bstar;
+            for (int j = gtid; j < M; j += gstride) {
+                const double a = w.keys[j];
+                if (a > 0.0 && rbj_bucket(a) >= bstar) {
+                    const int slot = atomicAdd(cnt, 1);
+                    ckey[slot] = a;
+                    cidx[slot] = j;
+                }
+            }
         }
-    }
-}
-
-// single block: rank the candidates by (key descending, index ascending), keep the first `take`
-__global__ void rbj_select_kernel(int M, int block, long long *__restrict__ state, int *__restrict__ cand_count,
-                                  const int2 *__restrict__ cand_meta, const double *__restrict__ cand_key,
-                                  int *__restrict__ hist, unsigned char *__restrict__ assigned, int32_t *__restrict__ order,
-                                  const int32_t *__restrict__ s2c) {
-    const long long filled = state[1];
-    const int k = (int)state[2];
-    const long long remaining = M - filled - 1;
-    const int take = (int)min((long long)block - 1, remaining);
-    const int n = *cand_count;
-    for (int c = threadIdx.x; c < n; c += blockDim.x) {
-        const double key = cand_key[c];
-        const int idx = cand_meta[c].x, cidx = s2c[idx];  // ties -> lower index in the caller's numbering
-        int rank = 0;
-        for (int o = 0; o < n; ++o) {
-            const double ko = cand_key[o];
-            rank += (ko > key) || (ko == key && s2c[cand_meta[o].x] < cidx);
+        if (blockIdx.x == 0 && tid == 0) w.cand_count[(step + 1) & 1] = 0;  // last read in phase C of step - 1
+        grid_barrier(w.bar, target, nblocks);
+        // ---- phase C: rank, mark, record (every CTA computes the same selection)
+        if (take > 0) {
+            const int n = *((volatile int *)cnt);
+            if (n < take) { if (gtid == 0) *w.err = 1; return; }  // cannot happen: the cut keeps at least `take`
+            if (n <= RBJ_CAP) {
+                for (int c = tid; c < n; c += RBJ_THREADS) {
+                    const int j = __ldcg(cidx + c);
+                    s_key[c] = __ldcg(ckey + c);
+                    s_idx[c] = j;
+                    s_cidx[c] = s2c[j];
+                }
+                __syncthreads();
+                for (int c = tid; c < n; c += RBJ_THREADS) {
+                    const double key = s_key[c];
+                    const int ci = s_cidx[c];  // ties -> lower index in the caller's numbering
+                    int rank = 0;
+                    for (int o = 0; o < n; ++o) rank += (s_key[o] > key) || (s_key[o] == key && s_cidx[o] < ci);
+                    if (rank < take) {
+                        w.assigned[s_idx[c]] = 1;
+                        if (blockIdx.x == 0) order[filled + 1 + rank] = s_idx[c];
+                    }
+                }
+            } else {
+                for (int c = tid; c < n; c += RBJ_THREADS) {
+                    const double key = __ldcg(ckey + c);
+                    const int j = __ldcg(cidx + c), ci = s2c[j];
+                    int rank = 0;
+                    for (int o = 0; o < n; ++o) {
+                        const double ko = __ldcg(ckey + o);
+                        rank += (ko > key) || (ko == key && s2c[__ldcg(cidx + o)] < ci);
+                    }
+                    if (rank < take) {
+                        w.assigned[j] = 1;
+                        if (blockIdx.x == 0) order[filled + 1 + rank] = j;
+                    }
+                }
+            }
         }
-        if (rank < take) {
-            order[filled + 1 + rank] = idx;
-            assigned[idx] = 1;
+        if (tid == 0) {
+            w.assigned[k] = 1;
+            if (blockIdx.x == 0) order[filled] = k;
         }
-    }
-    for (int t = threadIdx.x; t < RBJ_BINS; t += blockDim.x) hist[t] = 0;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        order[filled] = k;
-        assigned[k] = 1;
-        state[0] = state[0] + 1;
-        state[1] = filled + 1 + take;
-        *cand_count = 0;
-        if (n < take) state[4] = 1;  // cannot happen: the bucket cut keeps at least `take`
+        filled += 1 + take;
+        pos += 1;
+        __syncthreads();  // this CTA's own flag writes are visible to its own threads in the next phase A
     }
 }
 
@@ -183,7 +262,7 @@ __global__ void rbj_invert_kernel(const double4 *__restrict__ pt, const double *
     for (int j = 0; j < n; ++j) {
         const double d = a[(size_t)j * n + j];
         if (!(d > 0.0)) {
-            if (threadIdx.x == 0) *err = 1;
+            if (threadIdx.x == 0) *err = 3;
             return;
         }
         const double s = sqrt(d), is = 1.0 / s;
@@ -221,29 +300,19 @@ __global__ void rbj_invert_kernel(const double4 *__restrict__ pt, const double *
     }
 }
 
-// z = C r = scatter( blockdiag(M_b^-1) gather(r) ); one thread block per diagonal block
-__global__ void rbj_apply_kernel(int M, int block, const int32_t *__restrict__ order, const double *__restrict__ inv,
-                                 const double *__restrict__ r, double *__restrict__ z) {
-    extern __shared__ double s_r[];
-    const long long start = (long long)blockIdx.x * block;
-    const int n = (int)min((long long)block, (long long)M - start);
-    const double *a = inv + (size_t)blockIdx.x * block * block;
-    const int32_t *idx = order + start;
-    for (int j = threadIdx.x; j < n; j += blockDim.x) s_r[j] = r[idx[j]];
-    __syncthreads();
-    for (int i = threadIdx.x; i < n; i += blockDim.x) {
-        double s = 0.0;
-        for (int j = 0; j < n; ++j) s = fma(a[(size_t)j * n + i], s_r[j], s);  // inv is symmetric: column read is coalesced
-        z[idx[i]] = s;
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
-// CG vector kernels.  Dot products: fixed-shape two-stage reduction (DOT_BLOCKS partials, then one block).
-// scal[]: 0 rz, 1 pAp, 2 rr, 3 rz_new, 4 bAx2
+// PCG (textbook recurrences).  One iteration is five kernels on device-resident scalars:
+//   A q main + near (pcm_kernels.cu)  ->  cg_matvec_reduce (Ap = sum of the partial-sum slots, p.Ap)
+//   ->  cg_update_* (x += alpha p, r -= alpha Ap, z = C r, r.r, r.z, beta, convergence test)  ->  cg_direction.
+// Dot products are two-stage and fixed-order: per-CTA partials, then the last CTA to finish (atomic ticket) sums
+// them in index order.  The convergence test runs on the device: when ||r|| <= tol (or max_iter is reached) it raises
+// ctl[STOP] and every later kernel of the solve returns at once, so the host can queue iterations in batches without
+// changing what is computed.
+// scal: 0 rz, 1 pAp, 2 rr, 4 |b - Ax|^2, 5 beta.   ctl: 0 stop, 1 iterations, 2 ticket
 // ---------------------------------------------------------------------------------------------
 constexpr int DOT_BLOCKS = 296;
 constexpr int DOT_THREADS = 256;
+enum { CTL_STOP = 0, CTL_ITERS = 1, CTL_TICKET = 2 };
 
 __device__ __forceinline__ double block_sum(double v) {
     __shared__ double s_w[DOT_THREADS / 32];
@@ -261,57 +330,162 @@ __device__ __forceinline__ double block_sum(double v) {
     return t;  // valid in thread 0
 }
 
-// partial[blockIdx] = sum a.b over this block's grid-stride slice;  partial2 likewise for c.d when c != nullptr
-__global__ void __launch_bounds__(DOT_THREADS) dot_partial_kernel(int M, const double *__restrict__ a, const double *__restrict__ b,
-                                                                  const double *__restrict__ c, const double *__restrict__ d,
-                                                                  double *__restrict__ partial) {
-    double s1 = 0.0, s2 = 0.0;
-    for (int i = blockIdx.x * DOT_THREADS + threadIdx.x; i < M; i += DOT_BLOCKS * DOT_THREADS) {
-        s1 = fma(a[i], b[i], s1);
-        if (c) s2 = fma(c[i], d[i], s2);
-    }
-    s1 = block_sum(s1);
-    s2 = block_sum(s2);
-    if (threadIdx.x == 0) { partial[blockIdx.x] = s1; partial[DOT_BLOCKS + blockIdx.x] = s2; }
+// true for the last CTA of the grid to get here; its threads then see every other CTA's partials
+__device__ __forceinline__ bool last_block(int *ctl) {
+    __shared__ int s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(&ctl[CTL_TICKET], 1) == (int)gridDim.x - 1);
+    __syncthreads();
+    if (s_last) __threadfence();
+    return s_last != 0;
 }
-// scal[o1] = sum partial[0..), scal[o2] = sum partial[DOT_BLOCKS..)
-__global__ void __launch_bounds__(DOT_THREADS) dot_final_kernel(const double *__restrict__ partial, double *__restrict__ scal,
-                                                                int o1, int o2) {
-    double s1 = 0.0, s2 = 0.0;
-    for (int i = threadIdx.x; i < DOT_BLOCKS; i += DOT_THREADS) { s1 += partial[i]; s2 += partial[DOT_BLOCKS + i]; }
-    s1 = block_sum(s1);
-    s2 = block_sum(s2);
-    if (threadIdx.x == 0) { scal[o1] = s1; if (o2 >= 0) scal[o2] = s2; }
-}
-// x += alpha p; r -= alpha Ap with alpha = rz/pAp; partial sums of r.r
-__global__ void __launch_bounds__(DOT_THREADS) cg_update_kernel(int M, const double *__restrict__ scal, const double *__restrict__ p,
-                                                                const double *__restrict__ Ap, double *__restrict__ x,
-                                                                double *__restrict__ r, double *__restrict__ partial) {
-    const double alpha = scal[0] / scal[1];
+// sum of partial[0..n) in a fixed order (valid in thread 0); blockDim.x == DOT_THREADS
+__device__ __forceinline__ double ordered_sum(const double *partial, int n) {
     double s = 0.0;
-    for (int i = blockIdx.x * DOT_THREADS + threadIdx.x; i < M; i += DOT_BLOCKS * DOT_THREADS) {
-        x[i] = fma(alpha, p[i], x[i]);
-        const double ri = fma(-alpha, Ap[i], r[i]);
-        r[i] = ri;
-        s = fma(ri, ri, s);
+    for (int i = threadIdx.x; i < n; i += DOT_THREADS) s += __ldcg(partial + i);
+    return block_sum(s);
+}
+
+// Ap = sum of the A q partial-sum slots + near pieces (sorted order), pAp = p.Ap
+__global__ void __launch_bounds__(DOT_THREADS) cg_matvec_reduce_kernel(int M, const double *__restrict__ part, int slots,
+                                                                       const double *__restrict__ near,
+                                                                       const int64_t *__restrict__ pstart,
+                                                                       const double *__restrict__ p, double *__restrict__ Ap,
+                                                                       double *__restrict__ scal, double *__restrict__ partial,
+                                                                       int *__restrict__ ctl) {
+    if (*((volatile int *)&ctl[CTL_STOP])) return;
+    double dot = 0.0;
+    for (int k = blockIdx.x * DOT_THREADS + threadIdx.x; k < M; k += DOT_BLOCKS * DOT_THREADS) {
+        double s = 0.0;
+        for (int c = 0; c < slots; ++c) s += part[(size_t)c * M + k];
+        const int64_t rg = k / 32;
+        double t = 0.0;
+        for (int64_t q = pstart[rg]; q < pstart[rg + 1]; ++q) t += near[q * 32 + (k & 31)];
+        s += t;
+        Ap[k] = s;
+        dot = fma(p[k], s, dot);
     }
-    s = block_sum(s);
-    if (threadIdx.x == 0) { partial[blockIdx.x] = s; partial[DOT_BLOCKS + blockIdx.x] = 0.0; }
+    dot = block_sum(dot);
+    if (threadIdx.x == 0) partial[blockIdx.x] = dot;
+    if (last_block(ctl)) {
+        const double pAp = ordered_sum(partial, DOT_BLOCKS);
+        if (threadIdx.x == 0) { scal[1] = pAp; ctl[CTL_TICKET] = 0; }
+    }
 }
-// p = z + beta p, beta = rz_new/rz; then rz <- rz_new (done by the last step of the single-thread tail kernel)
-__global__ void cg_direction_kernel(int M, const double *__restrict__ scal, const double *__restrict__ z, double *__restrict__ p) {
-    const double beta = scal[3] / scal[0];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < M) p[i] = fma(beta, p[i], z[i]);
+
+// what the last CTA of an update kernel does with the two fixed-order sums
+__device__ __forceinline__ void cg_finish(double rr, double rz_new, double *scal, int *ctl, double tol, int max_iter, int init) {
+    if (threadIdx.x != 0) return;
+    if (!init) {
+        scal[5] = rz_new / scal[0];
+        ctl[CTL_ITERS] += 1;
+    }
+    scal[0] = rz_new;
+    scal[2] = rr;
+    if (!(sqrt(rr) > tol) || ctl[CTL_ITERS] >= max_iter) ctl[CTL_STOP] = 1;
+    ctl[CTL_TICKET] = 0;
 }
-__global__ void cg_shift_kernel(double *scal) { scal[0] = scal[3]; }
-__global__ void jacobi_kernel(int M, const double *__restrict__ diag, const double *__restrict__ r, double *__restrict__ z) {
+
+// RBJ: one CTA per diagonal block b (a partition of the points): x += alpha p, r -= alpha Ap on the block's points,
+// z = M_b^-1 r (C = scatter o blockdiag(M_b^-1) o gather), partial r.r and r.z.  init: r is given, no update.
+__global__ void __launch_bounds__(DOT_THREADS) cg_update_rbj_kernel(int M, int block, const int32_t *__restrict__ order,
+                                                                    const double *__restrict__ inv, const double *__restrict__ p,
+                                                                    const double *__restrict__ Ap, double *__restrict__ x,
+                                                                    double *__restrict__ r, double *__restrict__ z,
+                                                                    double *__restrict__ scal, double *__restrict__ partial,
+                                                                    int *__restrict__ ctl, double tol, int max_iter, int init) {
+    extern __shared__ double s_r[];
+    if (*((volatile int *)&ctl[CTL_STOP])) return;
+    const long long start = (long long)blockIdx.x * block;
+    const int n = (int)min((long long)block, (long long)M - start);
+    const double *a = inv + (size_t)blockIdx.x * block * block;
+    const int32_t *idx = order + start;
+    const double alpha = init ? 0.0 : scal[0] / scal[1];
+    double rr = 0.0, rz = 0.0;
+    for (int j = threadIdx.x; j < n; j += DOT_THREADS) {
+        const int i = idx[j];
+        double ri = r[i];
+        if (!init) {
+            x[i] = fma(alpha, p[i], x[i]);
+            ri = fma(-alpha, Ap[i], ri);
+            r[i] = ri;
+        }
+        s_r[j] = ri;
+        rr = fma(ri, ri, rr);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += DOT_THREADS) {
+        double s = 0.0;
+        for (int j = 0; j < n; ++j) s = fma(a[(size_t)j * n + i], s_r[j], s);  // inv is symmetric: column read is coalesced
+        z[idx[i]] = s;
+        rz = fma(s_r[i], s, rz);
+    }
+    rr = block_sum(rr);
+    rz = block_sum(rz);
+    if (threadIdx.x == 0) { partial[blockIdx.x] = rr; partial[gridDim.x + blockIdx.x] = rz; }
+    if (last_block(ctl)) {
+        const double srr = ordered_sum(partial, gridDim.x);
+        const double srz = ordered_sum(partial + gridDim.x, gridDim.x);
+        cg_finish(srr, srz, scal, ctl, tol, max_iter, init);
+    }
+}
+
+// Jacobi (C = diag(A)^-1) or no preconditioner (diag == nullptr)
+__global__ void __launch_bounds__(DOT_THREADS) cg_update_diag_kernel(int M, const double *__restrict__ diag,
+                                                                     const double *__restrict__ p, const double *__restrict__ Ap,
+                                                                     double *__restrict__ x, double *__restrict__ r,
+                                                                     double *__restrict__ z, double *__restrict__ scal,
+                                                                     double *__restrict__ partial, int *__restrict__ ctl,
+                                                                     double tol, int max_iter, int init) {
+    if (*((volatile int *)&ctl[CTL_STOP])) return;
+    const double alpha = init ? 0.0 : scal[0] / scal[1];
+    double rr = 0.0, rz = 0.0;
+    for (int i = blockIdx.x * DOT_THREADS + threadIdx.x; i < M; i += DOT_BLOCKS * DOT_THREADS) {
+        double ri = r[i];
+        if (!init) {
+            x[i] = fma(alpha, p[i], x[i]);
+            ri = fma(-alpha, Ap[i], ri);
+            r[i] = ri;
+        }
+        const double zi = diag ? ri / diag[i] : ri;
+        z[i] = zi;
+        rr = fma(ri, ri, rr);
+        rz = fma(ri, zi, rz);
+    }
+    rr = block_sum(rr);
+    rz = block_sum(rz);
+    if (threadIdx.x == 0) { partial[blockIdx.x] = rr; partial[DOT_BLOCKS + blockIdx.x] = rz; }
+    if (last_block(ctl)) {
+        const double srr = ordered_sum(partial, DOT_BLOCKS);
+        const double srz = ordered_sum(partial + DOT_BLOCKS, DOT_BLOCKS);
+        cg_finish(srr, srz, scal, ctl, tol, max_iter, init);
+    }
+}
+
+// p = z + beta p  (init: p = z)
+__global__ void cg_direction_kernel(int M, const double *__restrict__ scal, const double *__restrict__ z, double *__restrict__ p,
+                                    const int *__restrict__ ctl, int init) {
+    if (!init && *((volatile const int *)&ctl[CTL_STOP])) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < M) z[i] = r[i] / diag[i];
+    if (i >= M) return;
+    p[i] = init ? z[i] : fma(scal[5], p[i], z[i]);
 }
 __global__ void residual_kernel(int M, const double *__restrict__ b, const double *__restrict__ Ax, double *__restrict__ r) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < M) r[i] = b[i] - Ax[i];
+}
+// scal[o] = a.a  (single CTA per DOT_BLOCKS slice, then last-CTA sum)
+__global__ void __launch_bounds__(DOT_THREADS) norm2_kernel(int M, const double *__restrict__ a, double *__restrict__ scal, int o,
+                                                            double *__restrict__ partial, int *__restrict__ ctl) {
+    double s = 0.0;
+    for (int i = blockIdx.x * DOT_THREADS + threadIdx.x; i < M; i += DOT_BLOCKS * DOT_THREADS) s = fma(a[i], a[i], s);
+    s = block_sum(s);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+    if (last_block(ctl)) {
+        const double t = ordered_sum(partial, DOT_BLOCKS);
+        if (threadIdx.x == 0) { scal[o] = t; ctl[CTL_TICKET] = 0; }
+    }
 }
 
 // caller order <-> sorted order
@@ -331,6 +505,9 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     const int64_t M = ctx->M;
     if (block < 1) return set_error(ctx, PCM_ERR_ARG, "pcm_rbj_build: block < 1");
     if (M == 0) { ctx->rbj_block = block; ctx->rbj_nblocks = 0; return PCM_OK; }
+    const bool verbose = getenv("PCM_VERBOSE") != nullptr;
+    auto now = []() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); };
+    const double t0 = now();
     if ((int64_t)block > M) block = (int)M;
     std::vector<int64_t> perm64((size_t)M);
     if (pivot_order_host) {
@@ -348,100 +525,87 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     for (int64_t i = 0; i < M; ++i) perm[i] = ctx->c2s_host[(size_t)perm64[i]];
 
     const int64_t nb = cdiv(M, block);
-    // (re)allocate RBJ storage; earlier builds are released
-    auto release = [&](void *p) {
-        if (!p) return;
-        auto it = std::find(ctx->allocs.begin(), ctx->allocs.end(), p);
-        if (it != ctx->allocs.end()) ctx->allocs.erase(it);
-        cudaFree(p);
-    };
-    release(ctx->rbj_order); release(ctx->rbj_inv);
-    ctx->rbj_order = nullptr; ctx->rbj_inv = nullptr; ctx->rbj_block = 0; ctx->rbj_nblocks = 0;
+    // RBJ storage and build scratch live in one grow-only device arena (no allocation when a build is repeated)
+    auto al = [](size_t b) { return (b + 255) / 256 * 256; };
+    const size_t blk2 = (size_t)nb * block * block * 8;
+    const size_t need = al((size_t)M * 4) + al(blk2) + al((size_t)2 * nb * 8) + al(blk2) + al((size_t)M * 4) + al((size_t)M) +
+                        al((size_t)M * 8) + al((size_t)2 * M * 8) + al((size_t)2 * M * 4) + al(3 * RBJ_BINS * 4) + al(64);
     int rc;
-    if ((rc = dev_alloc_t(ctx, &ctx->rbj_order, (size_t)M))) return rc;
-    if ((rc = dev_alloc_t(ctx, &ctx->rbj_inv, (size_t)nb * block * block))) return rc;
-
-    // scratch for the build
-    int32_t *d_perm = nullptr; unsigned char *d_assigned = nullptr; long long *d_state = nullptr; double *d_keys = nullptr;
-    int *d_hist = nullptr, *d_count = nullptr, *d_err = nullptr; int2 *d_meta = nullptr; double *d_ckey = nullptr, *d_work = nullptr;
-    auto cleanup = [&]() {
-        cudaFree(d_perm); cudaFree(d_assigned); cudaFree(d_state); cudaFree(d_keys); cudaFree(d_hist);
-        cudaFree(d_count); cudaFree(d_err); cudaFree(d_meta); cudaFree(d_ckey); cudaFree(d_work);
-    };
+    ctx->rbj_block = 0; ctx->rbj_nblocks = 0;
+    if (need > ctx->rbj_arena_bytes) {
+        if (ctx->rbj_arena) {
+            auto it = std::find(ctx->allocs.begin(), ctx->allocs.end(), (void *)ctx->rbj_arena);
+            if (it != ctx->allocs.end()) ctx->allocs.erase(it);
+            cudaFree(ctx->rbj_arena);
+            ctx->device_bytes -= (int64_t)ctx->rbj_arena_bytes;
+            ctx->rbj_arena = nullptr; ctx->rbj_arena_bytes = 0;
+        }
+        if ((rc = dev_alloc(ctx, (void **)&ctx->rbj_arena, need))) return rc;
+        ctx->rbj_arena_bytes = need;
+    }
+    char *cur = ctx->rbj_arena;
+    auto take = [&](size_t b) { char *p = cur; cur += al(b); return (void *)p; };
+    ctx->rbj_order = (int32_t *)take((size_t)M * 4);
+    ctx->rbj_inv = (double *)take(blk2);
+    ctx->rbj_partial = (double *)take((size_t)2 * nb * 8);
+    double *d_work = (double *)take(blk2);
+    int32_t *d_perm = (int32_t *)take((size_t)M * 4);
+    RbjWork w{};
+    w.assigned = (unsigned char *)take((size_t)M);
+    w.keys = (double *)take((size_t)M * 8);
+    w.cand_key = (double *)take((size_t)2 * M * 8);
+    w.cand_idx = (int *)take((size_t)2 * M * 4);
+    w.hist = (int *)take(3 * RBJ_BINS * 4);
+    char *small = (char *)take(64);
+    w.cand_count = (int *)small;
+    w.err = (int *)(small + 16);
+    w.bar = (unsigned long long *)(small + 32);
+    auto cleanup = [&]() {};
 #define RBJ_TRY(call)                                                                                     \
     do {                                                                                                  \
         cudaError_t e__ = (call);                                                                         \
         if (e__ != cudaSuccess) { cleanup(); return set_error(ctx, PCM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); } \
     } while (0)
-    RBJ_TRY(cudaMalloc(&d_perm, (size_t)M * 4));
-    RBJ_TRY(cudaMalloc(&d_assigned, (size_t)M));
-    RBJ_TRY(cudaMalloc(&d_state, 8 * sizeof(long long)));
-    RBJ_TRY(cudaMalloc(&d_keys, (size_t)M * 8));
-    RBJ_TRY(cudaMalloc(&d_hist, RBJ_BINS * 4));
-    RBJ_TRY(cudaMalloc(&d_count, 4));
-    RBJ_TRY(cudaMalloc(&d_err, 4));
-    RBJ_TRY(cudaMalloc(&d_meta, (size_t)M * sizeof(int2)));
-    RBJ_TRY(cudaMalloc(&d_ckey, (size_t)M * 8));
-    RBJ_TRY(cudaMalloc(&d_work, (size_t)nb * block * block * 8));
     RBJ_TRY(cudaMemcpyAsync(d_perm, perm.data(), (size_t)M * 4, cudaMemcpyHostToDevice, s));
-    RBJ_TRY(cudaMemsetAsync(d_assigned, 0, (size_t)M, s));
-    RBJ_TRY(cudaMemsetAsync(d_state, 0, 8 * sizeof(long long), s));
-    RBJ_TRY(cudaMemsetAsync(d_hist, 0, RBJ_BINS * 4, s));
-    RBJ_TRY(cudaMemsetAsync(d_count, 0, 4, s));
-    RBJ_TRY(cudaMemsetAsync(d_err, 0, 4, s));
+    RBJ_TRY(cudaMemsetAsync(w.assigned, 0, (size_t)M, s));
+    RBJ_TRY(cudaMemsetAsync(w.hist, 0, 3 * RBJ_BINS * 4, s));
+    RBJ_TRY(cudaMemsetAsync(small, 0, 64, s));
+    int *d_err = w.err;
 
-    const int threads = 256;
-    const int grid = (int)std::min<int64_t>(cdiv(M, threads), (int64_t)ctx->sm_count * 4);
-    for (int64_t b = 0; b < nb; ++b) {
-        rbj_keys_kernel<<<grid, threads, 0, s>>>(ctx->pt, ctx->pt_diag, (int)M, d_perm, d_assigned, d_state, d_keys, d_hist, ctx->boys);
-        rbj_collect_kernel<<<grid, threads, 0, s>>>((int)M, block, d_state, d_keys, d_hist, d_count, d_meta, d_ckey);
-        rbj_select_kernel<<<1, 1024, 0, s>>>((int)M, block, d_state, d_count, d_meta, d_ckey, d_hist, d_assigned, ctx->rbj_order, ctx->s2c);
-        ctx->launch_total += 3;
+    double t1 = 0, t2 = 0;
+    if (verbose) { cudaStreamSynchronize(s); t1 = now(); }
+    // one cooperative launch: all CTAs must be co-resident for the grid barrier
+    {
+        int per_sm = 0;
+        RBJ_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rbj_select_kernel, RBJ_THREADS, 0));
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(cdiv(M, RBJ_THREADS), (int64_t)std::max(per_sm, 1) * ctx->sm_count));
+        int Mi = (int)M;
+        const double4 *pt = ctx->pt;
+        const double *diag = ctx->pt_diag, *boys = ctx->boys;
+        const int32_t *permc = d_perm, *s2c = ctx->s2c;
+        int32_t *order = ctx->rbj_order;
+        void *args[] = {&pt, &diag, &Mi, &block, &permc, &s2c, &order, &w, &boys};
+        RBJ_TRY(cudaLaunchCooperativeKernel((const void *)rbj_select_kernel, dim3(grid), dim3(RBJ_THREADS), args, 0, s));
+        ctx->launch_total += 1;
     }
     ctx->launch_total += 1;
     RBJ_TRY(cudaGetLastError());
+    if (verbose) { cudaStreamSynchronize(s); t2 = now(); }
     rbj_invert_kernel<<<(unsigned)nb, 256, 0, s>>>(ctx->pt, ctx->pt_diag, (int)M, block, ctx->rbj_order, ctx->rbj_inv, d_work, d_err, ctx->boys);
     RBJ_TRY(cudaGetLastError());
-    long long h_state[8];
     int h_err = 0;
-    RBJ_TRY(cudaMemcpyAsync(h_state, d_state, sizeof(h_state), cudaMemcpyDeviceToHost, s));
     RBJ_TRY(cudaMemcpyAsync(&h_err, d_err, 4, cudaMemcpyDeviceToHost, s));
     RBJ_TRY(cudaStreamSynchronize(s));
+    if (verbose) fprintf(stderr, "[pcm] rbj_build M=%lld l=%d: host prep %.3f ms, select %.3f ms, invert %.3f ms\n", (long long)M, block,
+                         t1 - t0, t2 - t1, now() - t2);
     cleanup();
 #undef RBJ_TRY
-    if (h_state[1] != M || h_state[4] != 0) return set_error(ctx, PCM_ERR_STATE, "pcm_rbj_build: block selection did not cover all points");
+    if (h_err == 1 || h_err == 2) return set_error(ctx, PCM_ERR_STATE, "pcm_rbj_build: block selection did not cover all points");
     if (h_err) return set_error(ctx, PCM_ERR_NUMERIC, "pcm_rbj_build: a diagonal block of A is not positive definite");
     ctx->rbj_block = block;
     ctx->rbj_nblocks = nb;
     ctx->info.rbj_block = block;
     ctx->info.rbj_nblocks = nb;
-    return PCM_OK;
-}
-
-static int apply_precond(pcm_ctx *ctx, int precond, const double *r, double *z, cudaStream_t s) {
-    const int M = (int)ctx->M;
-    if (precond == 0) {
-        PCM_CUDA(ctx, cudaMemcpyAsync(z, r, (size_t)M * 8, cudaMemcpyDeviceToDevice, s));
-    } else if (precond == 1) {
-        jacobi_kernel<<<(unsigned)cdiv(M, 256), 256, 0, s>>>(M, ctx->pt_diag, r, z);
-        PCM_LAUNCH_CHECK(ctx);
-        ctx->launch_total += 1;
-    } else {
-        const int block = (int)ctx->rbj_block;
-        const int threads = std::min(256, std::max(32, (block + 31) / 32 * 32));
-        rbj_apply_kernel<<<(unsigned)ctx->rbj_nblocks, threads, (size_t)block * 8, s>>>(M, block, ctx->rbj_order, ctx->rbj_inv, r, z);
-        PCM_LAUNCH_CHECK(ctx);
-        ctx->launch_total += 1;
-    }
-    return PCM_OK;
-}
-
-static int dot2(pcm_ctx *ctx, const double *a, const double *b, const double *c, const double *d, int o1, int o2, cudaStream_t s) {
-    double *partial = ctx->cg_scal + 16;
-    dot_partial_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>((int)ctx->M, a, b, c, d, partial);
-    dot_final_kernel<<<1, DOT_THREADS, 0, s>>>(partial, ctx->cg_scal, o1, o2);
-    PCM_LAUNCH_CHECK(ctx);
-    ctx->launch_total += 2;
     return PCM_OK;
 }
 
@@ -453,15 +617,34 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     if (M == 0) { if (iters) *iters = 0; if (resid) resid[0] = resid[1] = 0.0; return PCM_OK; }
     // all solver vectors live in the library's sorted point order; b is gathered on entry, x scattered on exit
     double *r = ctx->cg_vec, *z = r + M, *p = z + M, *Ap = p + M, *x = Ap + M, *b = x + M;
-    double *scal = ctx->cg_scal, *partial = scal + 16;
-    double *h = ctx->cg_scal_host;
+    double *scal = ctx->cg_scal, *partial = precond == 2 ? ctx->rbj_partial : scal + 16;
+    int *ctl = reinterpret_cast<int *>(scal + 8);
+    double *h = ctx->cg_scal_host;   // pinned: scal[0..8) then ctl
     int rc;
     const int saved_timing = ctx->timing;
     ctx->timing = 0;
     const unsigned gb = (unsigned)cdiv(M, 256);
+    const Plan &pl = ctx->plan_amat;
+    const PatchMap &pm = ctx->amat_map;
 #define CG_TRY(expr) do { rc = (expr); if (rc) { ctx->timing = saved_timing; return rc; } } while (0)
 #define CG_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { ctx->timing = saved_timing; \
         return set_error(ctx, PCM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); } } while (0)
+    auto update = [&](int init) -> int {
+        if (precond == 2) {
+            const int block = (int)ctx->rbj_block;
+            cg_update_rbj_kernel<<<(unsigned)ctx->rbj_nblocks, DOT_THREADS, (size_t)block * 8, s>>>(
+                M, block, ctx->rbj_order, ctx->rbj_inv, p, Ap, x, r, z, scal, partial, ctl, tol, max_iter, init);
+        } else {
+            cg_update_diag_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, precond == 1 ? ctx->pt_diag : nullptr, p, Ap, x, r, z, scal,
+                                                                      scal + 16, ctl, tol, max_iter, init);
+        }
+        cg_direction_kernel<<<gb, 256, 0, s>>>(M, scal, z, p, ctl, init);
+        ctx->launch_total += 2;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return set_error(ctx, PCM_ERR_CUDA, std::string("CG kernel launch: ") + cudaGetErrorString(e));
+        return PCM_OK;
+    };
+    CG_CUDA(cudaMemsetAsync(scal, 0, 16 * sizeof(double), s));
     gather_kernel<<<gb, 256, 0, s>>>(M, ctx->s2c, b_caller, b);
     ctx->launch_total += 1;
     if (use_x0) {
@@ -473,38 +656,34 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         CG_CUDA(cudaMemsetAsync(x, 0, (size_t)M * 8, s));
         CG_CUDA(cudaMemcpyAsync(r, b, (size_t)M * 8, cudaMemcpyDeviceToDevice, s));
     }
-    CG_TRY(apply_precond(ctx, precond, r, z, s));
-    CG_CUDA(cudaMemcpyAsync(p, z, (size_t)M * 8, cudaMemcpyDeviceToDevice, s));
-    CG_TRY(dot2(ctx, r, z, r, r, 0, 2, s));  // rz, rr
-    CG_CUDA(cudaMemcpyAsync(h, scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, s));
-    CG_CUDA(cudaStreamSynchronize(s));
-    double rn = std::sqrt(h[2]);
+    CG_TRY(update(1));  // z = C r, p = z, rz, rr; raises STOP if already converged (or max_iter == 0)
+    const int batch = 4;
     int it = 0;
-    while (rn > tol && it < max_iter) {
-        CG_TRY(launch_amatvec_sorted(ctx, p, Ap, s));
-        CG_TRY(dot2(ctx, p, Ap, nullptr, nullptr, 1, -1, s));  // pAp
-        cg_update_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, scal, p, Ap, x, r, partial);
-        dot_final_kernel<<<1, DOT_THREADS, 0, s>>>(partial, scal, 2, -1);  // rr
-        CG_CUDA(cudaMemcpyAsync(h, scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, s));
-        CG_CUDA(cudaEventRecord(ctx->ev[24], s));
-        // queue the rest of the iteration before looking at the residual
-        CG_TRY(apply_precond(ctx, precond, r, z, s));
-        CG_TRY(dot2(ctx, r, z, nullptr, nullptr, 3, -1, s));  // rz_new
-        cg_direction_kernel<<<gb, 256, 0, s>>>(M, scal, z, p);
-        cg_shift_kernel<<<1, 1, 0, s>>>(scal);
-        ctx->launch_total += 4;  // update, rr reduction, direction, shift
-        CG_CUDA(cudaGetLastError());
-        CG_CUDA(cudaEventSynchronize(ctx->ev[24]));
-        ++it;
-        rn = std::sqrt(h[2]);
+    double rr = 0.0;
+    while (true) {
+        CG_CUDA(cudaMemcpyAsync(h, scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CG_CUDA(cudaStreamSynchronize(s));
+        const int *hc = reinterpret_cast<const int *>(h + 8);
+        it = hc[CTL_ITERS];
+        rr = h[2];
+        if (hc[CTL_STOP]) break;
+        for (int k = 0; k < batch; ++k) {
+            CG_TRY(launch_amatvec_partials(ctx, p, ctl, s));
+            cg_matvec_reduce_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, ctx->ypart, (int)pl.chunks, ctx->near_amat, pm.pstart, p, Ap,
+                                                                        scal, scal + 16, ctl);
+            ctx->launch_total += 1;
+            CG_TRY(update(0));
+        }
     }
+    const double rn = std::sqrt(rr);
     // true residual
     CG_TRY(launch_amatvec_sorted(ctx, x, Ap, s));
     residual_kernel<<<gb, 256, 0, s>>>(M, b, Ap, z);
-    CG_TRY(dot2(ctx, z, z, nullptr, nullptr, 4, -1, s));
+    norm2_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, z, scal, 4, scal + 16, ctl);
     scatter_kernel<<<gb, 256, 0, s>>>(M, ctx->s2c, x, x_caller);
-    ctx->launch_total += 2;
-    CG_CUDA(cudaMemcpyAsync(h, scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    ctx->launch_total += 3;
+    CG_CUDA(cudaGetLastError());
+    CG_CUDA(cudaMemcpyAsync(h, scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
     CG_CUDA(cudaStreamSynchronize(s));
 #undef CG_TRY
 #undef CG_CUDA
