@@ -123,6 +123,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     if ((rc = dev_alloc_t(ctx, &ctx->near_amat, (size_t)ctx->amat_map.npiece * 32))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->vpart, (size_t)std::max<int64_t>(ctx->vpart_slots, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->ypart, (size_t)ctx->ypart_slots * std::max<int64_t>(M, 1)))) return fail(rc);
+    if ((rc = dev_alloc_t(ctx, &ctx->colpart, (size_t)std::max<int64_t>(ctx->plan_amat.xb, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->cg_vec, (size_t)6 * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->cg_scal, (size_t)1024))) return fail(rc);
     e = cudaMemset(ctx->cg_scal, 0, 1024 * 8);

@@ -21,6 +21,30 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
     return fma(ye, t, y);
 }
 
+// Partial sums of y = A q as the symmetric sweep leaves them (pcm_kernels.cu, amatvec_kernel): row slots
+// ypart[chunk][k] for the chunks that reach the row block of k, column sums colpart[rb][k] of the row blocks lying
+// wholly before the tile of k, and the near pieces of k's row group.  Summed in this fixed order.
+struct AmatParts {
+    const double *ypart, *colpart, *near;
+    const int64_t *pstart;
+    int slots, chunk_len, RB, tile;
+};
+__device__ __forceinline__ double amat_row_sum(const AmatParts &a, int M, int k) {
+    const int r0 = k / a.RB * a.RB;
+    double s = 0.0;
+    for (int c = r0 / a.chunk_len; c < a.slots; ++c) s += a.ypart[(size_t)c * M + k];
+    const int nsym = (k / a.tile * a.tile) / a.RB;
+    double u = 0.0;
+    for (int rb = 0; rb < nsym; ++rb) u += a.colpart[(size_t)rb * M + k];
+    s += u;
+    const int64_t rg = k / 32;
+    double t = 0.0;
+    for (int64_t e = a.pstart[rg]; e < a.pstart[rg + 1]; ++e) t += a.near[e * 32 + (k & 31)];
+    return s + t;
+}
+
+AmatParts amat_parts(const pcm_ctx *ctx);  // pcm_kernels.cu
+
 // Far-field Hermite seeds, normalised so that g_n = (-1)^n (2n-1)!! / R^(2n+1)  (derivatives of 1/R):
 // for T >= TFAR(L) the smeared charge is a point charge to fp64 and
 //   (2 pi/p) sqrt(rho/p) (-2 rho)^n F_n(T) = (pi/p)^{3/2} K^-1 ... = [ (2 pi/p) kappa ] g_n,  kappa = sqrt(pi/p)/2.

@@ -135,8 +135,10 @@ struct pcm_ctx {
     double *vpart = nullptr;    // potential partial sums [slots][M]
     int64_t vpart_slots = 0;
     double *near_amat = nullptr;  // [amat_map.npiece][32] sums of the near pieces
-    double *ypart = nullptr;    // amatvec partial sums [slots][M]
+    double *ypart = nullptr;    // amatvec row partial sums [slots][M]
     int64_t ypart_slots = 0;
+    double *colpart = nullptr;  // amatvec column partial sums of the symmetric sweep [plan_amat.xb][M]
+    int amat_R = 4;             // row groups per warp of the A q kernel (row block = 128 amat_R points)
     double *cg_vec = nullptr;   // 6 M doubles: r, z, p, Ap, x, b (sorted point order)
     double *cg_scal = nullptr;  // device scalars
     double *cg_scal_host = nullptr;  // pinned

@@ -11,6 +11,7 @@
 //   Fock:       H_h(product) = sum_k q_k Rt_h(P - C_k)          ;  F_ab = sum_members sum_h G[ab][h] H_h
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 
 #include "pcm_device.cuh"
 
@@ -31,7 +32,9 @@ constexpr int PT_TILE = 256;  // surface points staged per shared-memory tile (F
 // holds R whole row groups and every skip/run decision is warp-uniform.
 // ---------------------------------------------------------------------------------------------
 struct Blocking { int R, C; };
-__host__ __device__ constexpr Blocking amat_blocking() { return {4, 2}; }
+// A q: R = 4 (row blocks of 512) for large M, R = 2 (row blocks of 256, four times the blocks) below AMAT_R4_MIN points
+constexpr int AMAT_C = 2;
+constexpr int64_t AMAT_R4_MIN = 60000;
 __host__ __device__ constexpr Blocking fock_blocking(int L) {
     return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{2, 2} : L == 2 ? Blocking{1, 4} : Blocking{1, 2};
 }
@@ -95,28 +98,52 @@ __device__ __forceinline__ void stage_points(const double4 *__restrict__ pt, con
     }
 }
 
+// Symmetric sweep: A_ij = A_ji, so an evaluation 1/r_ij serves row i (y_i += q_j/r) and column j (y_j += q_i/r).
+// Block (rb, chunk) owns the rows [rb RB, (rb+1) RB), RB = TPB R, and the column tiles of its chunk that do not lie
+// before its rows:  tiles inside the row range (the diagonal band) are swept the plain way, rows only; tiles beyond it
+// are swept once for both triangles.  Row sums go to out[chunk][i] (only chunks that reach the row's block are written,
+// amat_first_slot), column sums to colpart[rb][j] (only rb < amat_sym_blocks(j) are written); amat_row_sum adds them
+// in a fixed order.  Per evaluation 13 FP64 instructions + 1/R DADD for two entries of A instead of 12 per entry.
+// Column sums: a lane adds its R rows in registers, the 32 lanes are then summed through a [16][33] shared-memory
+// transpose per warp (one DADD per column and lane), the 4 warps at the end of the tile.
 template <int R, int C>
 __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ q,
                                                       const int32_t *__restrict__ qidx, int M, int chunk_len,
-                                                      double *__restrict__ out, const uint8_t *__restrict__ farmap,
-                                                      int64_t nbyte, int64_t nrg, const int *__restrict__ stop) {
+                                                      double *__restrict__ out, double *__restrict__ colpart,
+                                                      const uint8_t *__restrict__ farmap, int64_t nbyte, int64_t nrg,
+                                                      const int *__restrict__ stop) {
     constexpr int NS = PT_TILE / SUB;
-    __shared__ double4 s_pt[PT_TILE];   // x, y, z, q
+    constexpr int RB = TPB * R;
+    constexpr int NW = TPB / 32;
+    static_assert(RB % PT_TILE == 0, "row blocks must be whole column tiles");
+    __shared__ double4 s_pt[PT_TILE];       // x, y, z, q
+    __shared__ double s_c[NW][16 * 33];     // per warp: [column of the half group][lane]
+    __shared__ double s_cs[NW][PT_TILE];    // per warp: column sums of the tile
     if (stop && *stop) return;  // a converged CG solve: the iterations queued behind it are no-ops
+    const int r0 = blockIdx.x * RB;
+    const int jbeg = blockIdx.y * chunk_len, jend = min(M, jbeg + chunk_len);
+    if (jend <= r0) return;     // the chunk lies before the rows: the blocks of those rows cover it (amat_first_slot)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
-    double4 a[R];
+    const int64_t rg0 = ((int64_t)blockIdx.x * NW + warp) * R;
+    double ax[R], ay[R], az[R], qa[R], y[R];
     int ii[R];
-    double y[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         ii[r] = (int)(rg0 + r) * SUB + lane;
-        a[r] = pt[min(ii[r], M - 1)];
+        if (ii[r] < M) {
+            const double4 a = pt[ii[r]];
+            ax[r] = a.x; ay[r] = a.y; az[r] = a.z;
+            qa[r] = q[qidx ? qidx[ii[r]] : ii[r]];
+        } else {  // padding: far from everything (and from the column padding), zero charge
+            ax[r] = ay[r] = az[r] = -3e8;
+            qa[r] = 0.0;
+        }
         y[r] = 0.0;
     }
-    const int jbeg = blockIdx.y * chunk_len, jend = min(M, jbeg + chunk_len);
-    for (int base = jbeg; base < jend; base += PT_TILE) {
+    double *sc = s_c[warp];
+    for (int base = max(jbeg, r0); base < jend; base += PT_TILE) {
         const int nst = (min(PT_TILE, jend - base) + SUB - 1) / SUB;
+        const bool sym = base >= r0 + RB;
         const unsigned bits = far_bits<R, NS>(farmap, nbyte, rg0, nrg, base / SUB, lane);
         __syncthreads();
         stage_points(pt, q, qidx, base, jend, nst, s_pt);
@@ -124,36 +151,107 @@ __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict_
         for (int st = 0; st < nst; ++st) {
             const double4 *sp = s_pt + st * SUB;
             const unsigned m = row_mask<R>(bits, st);
-            if (m == (1u << R) - 1u) {
+            if (!sym) {
+                if (m == (1u << R) - 1u) {
 #pragma unroll 1
-                for (int t = 0; t < SUB; t += C) {
-                    double4 b[C];
-                    double r2[C][R];
+                    for (int t = 0; t < SUB; t += C) {
+                        double4 b[C];
+                        double r2[C][R];
 #pragma unroll
-                    for (int c = 0; c < C; ++c) b[c] = sp[t + c];
+                        for (int c = 0; c < C; ++c) b[c] = sp[t + c];
 #pragma unroll
-                    for (int c = 0; c < C; ++c)
+                        for (int c = 0; c < C; ++c)
 #pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const double dx = a[r].x - b[c].x, dy = a[r].y - b[c].y, dz = a[r].z - b[c].z;
-                            r2[c][r] = fma(dz, dz, fma(dy, dy, dx * dx));
-                        }
+                            for (int r = 0; r < R; ++r) {
+                                const double dx = ax[r] - b[c].x, dy = ay[r] - b[c].y, dz = az[r] - b[c].z;
+                                r2[c][r] = fma(dz, dz, fma(dy, dy, dx * dx));
+                            }
 #pragma unroll
-                    for (int c = 0; c < C; ++c)
+                        for (int c = 0; c < C; ++c)
 #pragma unroll
-                        for (int r = 0; r < R; ++r) y[r] = fma(b[c].w, rsqrt_fast(r2[c][r]), y[r]);
-                }
-            } else if (m) {
+                            for (int r = 0; r < R; ++r) y[r] = fma(b[c].w, rsqrt_fast(r2[c][r]), y[r]);
+                    }
+                } else if (m) {
 #pragma unroll 1
-                for (int t = 0; t < SUB; ++t) {
-                    const double4 b = sp[t];
+                    for (int t = 0; t < SUB; ++t) {
+                        const double4 b = sp[t];
 #pragma unroll
-                    for (int r = 0; r < R; ++r)
-                        if ((m >> r) & 1u) {
-                            const double dx = a[r].x - b.x, dy = a[r].y - b.y, dz = a[r].z - b.z;
-                            y[r] = fma(b.w, rsqrt_fast(fma(dz, dz, fma(dy, dy, dx * dx))), y[r]);
-                        }
+                        for (int r = 0; r < R; ++r)
+                            if ((m >> r) & 1u) {
+                                const double dx = ax[r] - b.x, dy = ay[r] - b.y, dz = az[r] - b.z;
+                                y[r] = fma(b.w, rsqrt_fast(fma(dz, dz, fma(dy, dy, dx * dx))), y[r]);
+                            }
+                    }
                 }
+                continue;
+            }
+            if (m == 0) {
+                s_cs[warp][st * SUB + lane] = 0.0;
+                continue;
+            }
+#pragma unroll 1
+            for (int half = 0; half < 2; ++half) {
+                if (m == (1u << R) - 1u) {
+#pragma unroll 1
+                    for (int t = 0; t < 16; t += C) {
+                        double4 b[C];
+                        double r2[C][R], cc[C];
+#pragma unroll
+                        for (int c = 0; c < C; ++c) b[c] = sp[half * 16 + t + c];
+#pragma unroll
+                        for (int c = 0; c < C; ++c)
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double dx = ax[r] - b[c].x, dy = ay[r] - b[c].y, dz = az[r] - b[c].z;
+                                r2[c][r] = fma(dz, dz, fma(dy, dy, dx * dx));
+                            }
+#pragma unroll
+                        for (int c = 0; c < C; ++c) {
+                            cc[c] = 0.0;
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double rs = rsqrt_fast(r2[c][r]);
+                                y[r] = fma(b[c].w, rs, y[r]);
+                                cc[c] = fma(qa[r], rs, cc[c]);
+                            }
+                            sc[(t + c) * 33 + lane] = cc[c];
+                        }
+                    }
+                } else {
+#pragma unroll 1
+                    for (int t = 0; t < 16; ++t) {
+                        const double4 b = sp[half * 16 + t];
+                        double cc = 0.0;
+#pragma unroll
+                        for (int r = 0; r < R; ++r)
+                            if ((m >> r) & 1u) {
+                                const double dx = ax[r] - b.x, dy = ay[r] - b.y, dz = az[r] - b.z;
+                                const double rs = rsqrt_fast(fma(dz, dz, fma(dy, dy, dx * dx)));
+                                y[r] = fma(b.w, rs, y[r]);
+                                cc = fma(qa[r], rs, cc);
+                            }
+                        sc[t * 33 + lane] = cc;
+                    }
+                }
+                __syncwarp();
+                // lane l sums column (l & 15) over the lanes [16 (l >> 4), 16 (l >> 4) + 16), fixed order
+                const double *col = sc + (lane & 15) * 33 + (lane >> 4) * 16;
+                double s = col[0];
+#pragma unroll
+                for (int k = 1; k < 16; ++k) s += col[k];
+                const double o = __shfl_xor_sync(0xffffffffu, s, 16);
+                if (lane < 16) s_cs[warp][st * SUB + half * 16 + lane] = s + o;
+                __syncwarp();
+            }
+        }
+        if (sym) {
+            __syncthreads();
+            for (int t = threadIdx.x; t < nst * SUB; t += TPB) {
+                const int j = base + t;
+                double s = s_cs[0][t];
+#pragma unroll
+                for (int w2 = 1; w2 < NW; ++w2) s += s_cs[w2][t];
+                if (j < M) colpart[(size_t)blockIdx.x * M + j] = s;
             }
         }
     }
@@ -229,6 +327,19 @@ __global__ void reduce_slots_kernel(const double *__restrict__ part, int64_t n, 
         s += t;
     }
     out[idx ? idx[k] : k] = s;
+}
+
+// y[idx ? idx[k] : k] = the partial sums of row k of the symmetric A q sweep, in amat_row_sum's fixed order
+__global__ void amat_reduce_kernel(AmatParts parts, int M, double *__restrict__ out, const int32_t *__restrict__ idx) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= M) return;
+    out[idx ? idx[k] : k] = amat_row_sum(parts, M, k);
+}
+AmatParts amat_parts(const pcm_ctx *ctx) {
+    AmatParts a;
+    a.ypart = ctx->ypart; a.colpart = ctx->colpart; a.near = ctx->near_amat; a.pstart = ctx->amat_map.pstart;
+    a.slots = (int)ctx->plan_amat.chunks; a.chunk_len = (int)ctx->plan_amat.chunk_len; a.RB = TPB * ctx->amat_R; a.tile = PT_TILE;
+    return a;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -624,7 +735,7 @@ static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 // tiles.  The grid (xb x chunks) is cut into about four waves of `wave` co-resident blocks when the sizes allow (the
 // hardware block scheduler then evens out what the skipped near patches unbalance): the smallest chunk count >= 4
 // waves whose last wave is at least 90 % full, or the best available.
-static Plan make_plan(int64_t rows, int rows_per_block, int64_t cols, int tile, int64_t wave) {
+static Plan make_plan(int64_t rows, int rows_per_block, int64_t cols, int tile, int64_t wave, double fill = 1.0, double waves = 4.0) {
     Plan p;
     p.xb = ceil_div(std::max<int64_t>(rows, 1), rows_per_block);
     const int64_t tiles = ceil_div(std::max<int64_t>(cols, 1), tile);
@@ -634,11 +745,11 @@ static Plan make_plan(int64_t rows, int rows_per_block, int64_t cols, int tile, 
     for (int64_t c = 1; c <= maxc; ++c) {
         const int64_t len = ceil_div(tiles, c);            // tiles per chunk
         const int64_t cc = ceil_div(tiles, len);           // chunks actually needed
-        const double t = (double)p.xb * (double)cc;
+        const double t = std::max(1.0, (double)p.xb * (double)cc * fill);   // blocks that have work (fill < 1: triangular sweep)
         const double eff = t / ((double)ceil_div((int64_t)t, wave) * (double)wave);
-        const double score = eff * std::min(1.0, 0.55 + 0.45 * t / (4.0 * (double)wave));  // prefer >= 4 waves
+        const double score = eff * std::min(1.0, 0.55 + 0.45 * t / (waves * (double)wave));  // prefer >= `waves` waves
         if (score > best_score + 1e-9) { best_score = score; best = cc; }
-        if (t >= 4.0 * (double)wave && eff >= 0.9) break;
+        if (t >= waves * (double)wave && eff >= 0.9) break;
     }
     const int64_t len = ceil_div(tiles, best);
     p.chunk_len = len * tile;
@@ -662,8 +773,16 @@ static void plan_class(pcm_ctx *ctx) {
 }
 
 int plan_all(pcm_ctx *ctx) {
-    constexpr Blocking ab = amat_blocking();
-    ctx->plan_amat = make_plan(ctx->M, TPB * ab.R, ctx->M, PT_TILE, wave_of(ctx, amatvec_kernel<ab.R, ab.C>));
+    // symmetric sweep: about half of the (row block, chunk) grid has work
+    ctx->amat_R = ctx->M >= AMAT_R4_MIN ? 4 : 2;
+    if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 2 || r == 4) ctx->amat_R = r; }
+    double aw = 8.0;
+    if (const char *e = getenv("PCM_AMAT_WAVES")) aw = atof(e);
+    ctx->plan_amat = ctx->amat_R == 4
+        ? make_plan(ctx->M, TPB * 4, ctx->M, PT_TILE, wave_of(ctx, amatvec_kernel<4, AMAT_C>), 0.5, aw)
+        : make_plan(ctx->M, TPB * 2, ctx->M, PT_TILE, wave_of(ctx, amatvec_kernel<2, AMAT_C>), 0.5, aw);
+    if (getenv("PCM_VERBOSE")) fprintf(stderr, "[pcm] amat plan: R %d xb %lld chunks %lld chunk_len %lld\n", ctx->amat_R,
+                                       (long long)ctx->plan_amat.xb, (long long)ctx->plan_amat.chunks, (long long)ctx->plan_amat.chunk_len);
     plan_class<0>(ctx); plan_class<1>(ctx); plan_class<2>(ctx); plan_class<3>(ctx); plan_class<4>(ctx);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_error(ctx, PCM_ERR_CUDA, std::string("plan_all: ") + cudaGetErrorString(e));
@@ -687,7 +806,6 @@ static int mark(pcm_ctx *ctx, int i, cudaStream_t s) {
 // Partial sums of y = A q: near pieces into near_amat (near stream, forked from and joined back into s), main kernel
 // slots into ypart.  idx: sorted -> caller index of q (nullptr: q is in sorted order).  stop: see cg_solve.
 static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *idx, const int *stop, cudaStream_t s) {
-    constexpr Blocking ab = amat_blocking();
     const int M = (int)ctx->M;
     const Plan &pl = ctx->plan_amat;
     const PatchMap &pm = ctx->amat_map;
@@ -702,7 +820,10 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
         { ctx->launches[2]++; ctx->launch_total++; }
     }
-    amatvec_kernel<ab.R, ab.C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, pm.far, pm.nbyte, pm.nrg, stop);
+    if (ctx->amat_R == 4)
+        amatvec_kernel<4, AMAT_C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+    else
+        amatvec_kernel<2, AMAT_C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[2]++; ctx->launch_total++; }
     if (pm.npiece > 0) PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
@@ -720,8 +841,6 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
     ctx->timed[2] = ctx->timing != 0;
     const int M = (int)ctx->M;
     if (M == 0) return PCM_OK;
-    const Plan &pl = ctx->plan_amat;
-    const PatchMap &pm = ctx->amat_map;
     const int32_t *idx = caller_order ? ctx->s2c : nullptr;
     int rc;
     if ((rc = mark(ctx, 0, s))) return rc;
@@ -729,9 +848,7 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
     if ((rc = launch_amatvec_kernels(ctx, q, idx, nullptr, s))) return rc;
     for (int i = 2; i <= 6; ++i)
         if ((rc = mark(ctx, i, s))) return rc;
-    NearRefs nr;
-    nr.count = 1; nr.near[0] = ctx->near_amat; nr.pstart[0] = pm.pstart;
-    reduce_slots_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(ctx->ypart, M, (int)pl.chunks, y, idx, nr);
+    amat_reduce_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(amat_parts(ctx), M, y, idx);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return mark(ctx, 7, s);

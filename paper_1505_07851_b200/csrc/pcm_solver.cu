@@ -348,21 +348,14 @@ __device__ __forceinline__ double ordered_sum(const double *partial, int n) {
 }
 
 // Ap = sum of the A q partial-sum slots + near pieces (sorted order), pAp = p.Ap
-__global__ void __launch_bounds__(DOT_THREADS) cg_matvec_reduce_kernel(int M, const double *__restrict__ part, int slots,
-                                                                       const double *__restrict__ near,
-                                                                       const int64_t *__restrict__ pstart,
+__global__ void __launch_bounds__(DOT_THREADS) cg_matvec_reduce_kernel(int M, AmatParts parts,
                                                                        const double *__restrict__ p, double *__restrict__ Ap,
                                                                        double *__restrict__ scal, double *__restrict__ partial,
                                                                        int *__restrict__ ctl) {
     if (*((volatile int *)&ctl[CTL_STOP])) return;
     double dot = 0.0;
     for (int k = blockIdx.x * DOT_THREADS + threadIdx.x; k < M; k += DOT_BLOCKS * DOT_THREADS) {
-        double s = 0.0;
-        for (int c = 0; c < slots; ++c) s += part[(size_t)c * M + k];
-        const int64_t rg = k / 32;
-        double t = 0.0;
-        for (int64_t q = pstart[rg]; q < pstart[rg + 1]; ++q) t += near[q * 32 + (k & 31)];
-        s += t;
+        const double s = amat_row_sum(parts, M, k);
         Ap[k] = s;
         dot = fma(p[k], s, dot);
     }
@@ -624,8 +617,6 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     const int saved_timing = ctx->timing;
     ctx->timing = 0;
     const unsigned gb = (unsigned)cdiv(M, 256);
-    const Plan &pl = ctx->plan_amat;
-    const PatchMap &pm = ctx->amat_map;
 #define CG_TRY(expr) do { rc = (expr); if (rc) { ctx->timing = saved_timing; return rc; } } while (0)
 #define CG_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { ctx->timing = saved_timing; \
         return set_error(ctx, PCM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); } } while (0)
@@ -669,8 +660,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         if (hc[CTL_STOP]) break;
         for (int k = 0; k < batch; ++k) {
             CG_TRY(launch_amatvec_partials(ctx, p, ctl, s));
-            cg_matvec_reduce_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, ctx->ypart, (int)pl.chunks, ctx->near_amat, pm.pstart, p, Ap,
-                                                                        scal, scal + 16, ctl);
+            cg_matvec_reduce_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, amat_parts(ctx), p, Ap, scal, scal + 16, ctl);
             ctx->launch_total += 1;
             CG_TRY(update(0));
         }
