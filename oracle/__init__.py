@@ -57,6 +57,11 @@ def lib():
         L.orc_pcg.restype = C.c_long
         L.orc_pcg.argtypes = [C.c_long, C.c_void_p, _dp, _dp, C.c_void_p, _dp, _dp, C.c_int, C.c_double, C.c_long,
                               C.c_int, C.c_long, C.c_void_p, C.c_void_p, C.c_void_p, _dp, C.c_void_p]
+        L.orc_bz.argtypes = [C.c_long, _dp, _dp, C.c_long, _dp, _dp, _dp]
+        L.orc_rhs.argtypes = [C.c_long, _dp, _dp, C.c_double, _dp]
+        L.orc_energy.argtypes = [C.c_long, _dp, _dp, _dp, _dp, C.c_double, _dp]
+        L.orc_cg_threshold.restype = C.c_double
+        L.orc_cg_threshold.argtypes = [C.c_double, C.c_double]
         _lib = L
     return _lib
 
@@ -219,3 +224,31 @@ def pcg(surface, b, tol, max_iter=1000, precond=0, rbj=None, x0=None, A=None, hi
     if history:
         out = out + (hist[:it + 1].copy(),)
     return out
+
+
+# ------------------------------------------------------------------ the rest of a C-PCM step (Eq. 1, 4, 13, 21)
+def nuclear_potential(surface, atom_xyz, z) -> np.ndarray:
+    """u = B z (Eq. 4)."""
+    u = np.zeros(surface.M)
+    a = _f(atom_xyz).reshape(-1)
+    lib().orc_bz(surface.M, _f(surface.xyz).reshape(-1), _f(surface.zeta), len(a) // 3, a, _f(z), u)
+    return u
+
+
+def rhs(u, v, f: float) -> np.ndarray:
+    """b = -f (B z - v): the right-hand side of Eq. 1 with c = -v."""
+    b = np.zeros(len(u))
+    lib().orc_rhs(len(u), _f(u), _f(v), float(f), b)
+    return b
+
+
+def energy(u, v, q, Aq, f: float) -> np.ndarray:
+    """Eq. 13: [(B z).q, c.q, q.A q/(2 f), total] with c = -v."""
+    out = np.zeros(4)
+    lib().orc_energy(len(u), _f(u), _f(v), _f(q), _f(Aq), float(f), out)
+    return out
+
+
+def cg_threshold(diis_prev: float, delta_min: float = 1e-6) -> float:
+    """Eq. 21: the dynamic CG threshold for the next SCF iteration (diis_prev <= 0: first iteration, delta = 1)."""
+    return float(lib().orc_cg_threshold(float(diis_prev), float(delta_min)))

@@ -620,3 +620,53 @@ long orc_pcg(long M, const double *Adense, const double *pt_xyz, const double *p
     free(r); free(z); free(p); free(Ap); free(dg);
     return it;
 }
+
+/* ------------------------------------------------------------------------------------
+ * The rest of one C-PCM step around the hot path.
+ *   B z  (Eq. 4):  u_k = sum_J z_J erf(zeta_k |r_k - R_J|)/|r_k - R_J|; a nucleus is a point
+ *        charge, so the exponent is the surface point's own zeta_k.  r = 0 -> 2 zeta_k/sqrt(pi) (the limit).
+ *   right-hand side of Eq. 1 with the library's sign (reading R2: c = -v):  b = -f (B z - v),  f = (eps-1)/(eps+k)
+ *   Delta G_els (Eq. 13):  (B z).q + c.q + (1/2f) q.A q  with c = -v; out[0..2] the three terms, out[3] the sum
+ *   dynamic CG threshold (Eq. 21; reading R10 in DESIGN.md): the delta for which
+ *        Err(delta) = 0.01 delta^1.07 equals 1e-3 x the previous SCF step's DIIS error; delta = 1 on the first SCF
+ *        iteration (no previous error: diis_prev <= 0); never tighter than delta_min, never looser than 1.
+ * ---------------------------------------------------------------------------------- */
+void orc_bz(long M, const double *pt_xyz, const double *pt_zeta, long N, const double *atom_xyz, const double *z, double *u) {
+#pragma omp parallel for schedule(static)
+    for (long k = 0; k < M; ++k) {
+        double sum = 0.0, comp = 0.0;
+        for (long J = 0; J < N; ++J) {
+            double dx = pt_xyz[3 * k] - atom_xyz[3 * J], dy = pt_xyz[3 * k + 1] - atom_xyz[3 * J + 1],
+                   dz = pt_xyz[3 * k + 2] - atom_xyz[3 * J + 2];
+            double r = sqrt(dx * dx + dy * dy + dz * dz);
+            double B = r == 0.0 ? 2.0 * pt_zeta[k] / sqrt(ORC_PI) : erf(pt_zeta[k] * r) / r;
+            nsum(&sum, &comp, z[J] * B);
+        }
+        u[k] = sum + comp;
+    }
+}
+
+void orc_rhs(long M, const double *u, const double *v, double f, double *b) {
+    for (long k = 0; k < M; ++k) b[k] = -f * (u[k] - v[k]);
+}
+
+void orc_energy(long M, const double *u, const double *v, const double *q, const double *Aq, double f, double *out) {
+    double s0 = 0, c0 = 0, s1 = 0, c1 = 0, s2 = 0, c2 = 0;
+    for (long k = 0; k < M; ++k) {
+        nsum(&s0, &c0, u[k] * q[k]);
+        nsum(&s1, &c1, -v[k] * q[k]);
+        nsum(&s2, &c2, q[k] * Aq[k]);
+    }
+    out[0] = s0 + c0;
+    out[1] = s1 + c1;
+    out[2] = (s2 + c2) / (2.0 * f);
+    out[3] = out[0] + out[1] + out[2];
+}
+
+double orc_cg_threshold(double diis_prev, double delta_min) {
+    if (!(diis_prev > 0.0)) return 1.0;
+    double delta = pow(1e-3 * diis_prev / 0.01, 1.0 / 1.07);
+    if (delta > 1.0) delta = 1.0;
+    if (delta < delta_min) delta = delta_min;
+    return delta;
+}

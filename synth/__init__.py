@@ -19,5 +19,6 @@ from .generators import (  # noqa: F401
     make_charges,
     make_workload,
     make_solver_points,
+    nuclear_charges,
     CONFIG_ATOMS,
 )

@@ -22,6 +22,12 @@ ANGSTROM = 1.8897261246  # bohr per Angstrom
 
 # van der Waals (Bondi) radii in Angstrom, as listed in BASELINE.json configs[0]
 _VDW = {"H": 1.20, "C": 1.70, "N": 1.55, "O": 1.52}
+_Z = {"H": 1.0, "C": 6.0, "N": 7.0, "O": 8.0}
+
+
+def nuclear_charges(elements) -> np.ndarray:
+    """The vector z of Eq. 1 (nuclear charges of the solute's atoms)."""
+    return np.array([_Z[e] for e in elements], dtype=np.float64)
 _CAVITY_SCALE = 1.2          # PAPER.md:106 "20% larger than the Bondi radii"
 _ZETA_TABLE_STANDIN = 4.9    # stands in for the tabulated zeta of Eq. 7 (PAPER.md:48)
 
