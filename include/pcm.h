@@ -163,6 +163,35 @@ int pcm_cg_solve(pcm_ctx *ctx, const double *b_dev, double *x_dev, double tol, i
                  int *iters, double *resid, void *stream);
 
 /*
+ * The rest of one C-PCM step around the hot path (Eq. 1, 4, 13, 21).
+ *
+ * pcm_set_nuclei -- the solute's nuclei for B z.  atom_xyz_host: HOST, 3*natom doubles (bohr); z_host: HOST,
+ * natom doubles (nuclear charges).  The context keeps a copy; a later call replaces it.  natom = 0 is allowed.
+ *
+ * pcm_nuclear_potential -- u = B z, u_k = sum_J z_J erf(zeta_k |r_k - R_J|)/|r_k - R_J| (Eq. 4): a
+ * nucleus is a point charge, so the exponent is the surface point's own zeta_k; r = 0 -> 2 zeta_k/sqrt(pi).
+ * u_dev: DEVICE, M doubles, overwritten.  Asynchronous.  PCM_ERR_STATE before pcm_set_nuclei.
+ *
+ * pcm_rhs -- b = -f (u - v): the right-hand side of Eq. 1, A q = -f (B z + c), with this library's unsigned
+ * v (c = -v, see "Sign convention" above); f = (eps - 1)/(eps + k).  u_dev, v_dev, b_dev: DEVICE,
+ * M doubles (b may alias u or v).  Asynchronous.
+ *
+ * pcm_energy -- Delta G_els = (B z).q + c.q + (1/2f) q.A q (Eq. 13) with c = -v; A q by one
+ * pcm_amatvec.  u_dev, v_dev, q_dev: DEVICE, M doubles.  terms_host: HOST, 4 doubles: the three terms and their
+ * sum.  Fixed-order sums (bit-reproducible).  Synchronises the stream.
+ *
+ * pcm_cg_threshold -- the dynamic CG threshold of PAPER.md:182-184: the delta at which Err(delta) = 0.01 delta^1.07
+ * (Eq. 21) equals 1e-3 x the DIIS error of the previous SCF iteration, clamped to [delta_min, 1];
+ * diis_prev <= 0 means "first SCF iteration" -> delta = 1.  Host arithmetic only.
+ */
+int pcm_set_nuclei(pcm_ctx *ctx, int natom, const double *atom_xyz_host, const double *z_host);
+int pcm_nuclear_potential(pcm_ctx *ctx, double *u_dev, void *stream);
+int pcm_rhs(pcm_ctx *ctx, const double *u_dev, const double *v_dev, double f, double *b_dev, void *stream);
+int pcm_energy(pcm_ctx *ctx, const double *u_dev, const double *v_dev, const double *q_dev, double f, double *terms_host,
+               void *stream);
+int pcm_cg_threshold(double diis_prev, double delta_min, double *delta_out);
+
+/*
  * Host-buffer forms of the four hot calls: same semantics, every array is a HOST pointer; the call
  * copies inputs to the device, runs the device path on the context's own stream, copies the result back
  * and synchronises.  These are what bench.py's end-to-end figure times.

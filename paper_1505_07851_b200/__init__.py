@@ -29,7 +29,8 @@ EXPORTS = (
     "pcm_options_default", "pcm_setup", "pcm_potential", "pcm_fock", "pcm_amatvec", "pcm_pivot_order",
     "pcm_rbj_build", "pcm_rbj_get", "pcm_cg_solve", "pcm_potential_host", "pcm_fock_host", "pcm_amatvec_host",
     "pcm_cg_solve_host", "pcm_get_info", "pcm_set_timing", "pcm_last_kernel_ms", "pcm_last_class_ms",
-    "pcm_launch_count", "pcm_fp64_peak",
+    "pcm_launch_count", "pcm_fp64_peak", "pcm_set_nuclei", "pcm_nuclear_potential", "pcm_rhs", "pcm_energy",
+    "pcm_cg_threshold",
     "pcm_schwarz_bound", "pcm_last_error", "pcm_destroy",
 )
 
@@ -92,6 +93,11 @@ def lib(build: bool = False):
         L.pcm_last_class_ms.argtypes = [vp, C.c_int, _dp]
         L.pcm_launch_count.argtypes = [vp, _lp]
         L.pcm_fp64_peak.argtypes = [vp, C.c_int, _dp]
+        L.pcm_set_nuclei.argtypes = [vp, C.c_int, vp, vp]
+        L.pcm_nuclear_potential.argtypes = [vp, vp, vp]
+        L.pcm_rhs.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.pcm_energy.argtypes = [vp, vp, vp, vp, C.c_double, _dp, vp]
+        L.pcm_cg_threshold.argtypes = [C.c_double, C.c_double, _dp]
         L.pcm_schwarz_bound.argtypes = [C.c_int, C.c_double, vp, C.c_int, C.c_double, vp, _dp]
         L.pcm_last_error.argtypes = [vp]
         L.pcm_last_error.restype = C.c_char_p
@@ -222,6 +228,44 @@ def pcm_amatvec(ctx: Context, q, y=None, stream=None):
         y = torch.empty(ctx.M, dtype=torch.float64, device=q.device)
     _check(lib().pcm_amatvec(ctx.handle, _dev(q, ctx.M), _dev(y, ctx.M), _stream(stream)), ctx.handle)
     return y
+
+
+def pcm_set_nuclei(ctx: Context, atom_xyz, z) -> None:
+    xyz = _np(atom_xyz, np.float64).reshape(-1)
+    zz = _np(z, np.float64)
+    if len(xyz) != 3 * len(zz):
+        raise ValueError("atom_xyz must hold 3 doubles per nuclear charge")
+    _check(lib().pcm_set_nuclei(ctx.handle, len(zz), _hp(xyz), _hp(zz)), ctx.handle)
+
+
+def pcm_nuclear_potential(ctx: Context, u=None, stream=None):
+    import torch
+    if u is None:
+        u = torch.empty(ctx.M, dtype=torch.float64, device=torch.device("cuda", torch.cuda.current_device()))
+    _check(lib().pcm_nuclear_potential(ctx.handle, _dev(u, ctx.M), _stream(stream)), ctx.handle)
+    return u
+
+
+def pcm_rhs(ctx: Context, u, v, f: float, b=None, stream=None):
+    import torch
+    if b is None:
+        b = torch.empty(ctx.M, dtype=torch.float64, device=u.device)
+    _check(lib().pcm_rhs(ctx.handle, _dev(u, ctx.M), _dev(v, ctx.M), float(f), _dev(b, ctx.M), _stream(stream)), ctx.handle)
+    return b
+
+
+def pcm_energy(ctx: Context, u, v, q, f: float, stream=None) -> np.ndarray:
+    """[(B z).q, c.q, q.A q/(2 f), total] (Eq. 13, c = -v)."""
+    terms = np.zeros(4)
+    _check(lib().pcm_energy(ctx.handle, _dev(u, ctx.M), _dev(v, ctx.M), _dev(q, ctx.M), float(f),
+                            terms.ctypes.data_as(_dp), _stream(stream)), ctx.handle)
+    return terms
+
+
+def pcm_cg_threshold(diis_prev: float, delta_min: float = 1e-6) -> float:
+    out = C.c_double(0.0)
+    _check(lib().pcm_cg_threshold(float(diis_prev), float(delta_min), C.byref(out)))
+    return out.value
 
 
 def pcm_pivot_order(seed: int, M: int) -> np.ndarray:

@@ -162,6 +162,55 @@ int pcm_amatvec(pcm_ctx *ctx, const double *q_dev, double *y_dev, void *stream) 
     return launch_amatvec(ctx, q_dev, y_dev, (cudaStream_t)stream);
 }
 
+int pcm_set_nuclei(pcm_ctx *ctx, int natom, const double *atom_xyz_host, const double *z_host) {
+    PCM_CHECK_CTX(ctx);
+    if (natom < 0 || (natom > 0 && (!atom_xyz_host || !z_host))) return set_error(ctx, PCM_ERR_ARG, "pcm_set_nuclei: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    std::vector<double4> at((size_t)std::max(natom, 1));
+    for (int j = 0; j < natom; ++j) at[j] = make_double4(atom_xyz_host[3 * j], atom_xyz_host[3 * j + 1], atom_xyz_host[3 * j + 2], z_host[j]);
+    if (ctx->atoms == nullptr || natom > ctx->natom) {   // grow-only; the old buffer stays on the context's free list
+        int rc = dev_alloc_t(ctx, &ctx->atoms, at.size());
+        if (rc) return rc;
+    }
+    PCM_CUDA(ctx, cudaMemcpy(ctx->atoms, at.data(), at.size() * sizeof(double4), cudaMemcpyHostToDevice));
+    ctx->natom = natom;
+    return PCM_OK;
+}
+
+int pcm_nuclear_potential(pcm_ctx *ctx, double *u_dev, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->natom < 0) return set_error(ctx, PCM_ERR_STATE, "pcm_nuclear_potential: call pcm_set_nuclei first");
+    if (ctx->M == 0) return PCM_OK;
+    if (!u_dev) return set_error(ctx, PCM_ERR_ARG, "pcm_nuclear_potential: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_nuclear_potential(ctx, u_dev, (cudaStream_t)stream);
+}
+
+int pcm_rhs(pcm_ctx *ctx, const double *u_dev, const double *v_dev, double f, double *b_dev, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->M == 0) return PCM_OK;
+    if (!u_dev || !v_dev || !b_dev) return set_error(ctx, PCM_ERR_ARG, "pcm_rhs: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_rhs(ctx, u_dev, v_dev, f, b_dev, (cudaStream_t)stream);
+}
+
+int pcm_energy(pcm_ctx *ctx, const double *u_dev, const double *v_dev, const double *q_dev, double f, double *terms_host,
+               void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (!terms_host || !(f != 0.0) || (ctx->M > 0 && (!u_dev || !v_dev || !q_dev)))
+        return set_error(ctx, PCM_ERR_ARG, "pcm_energy: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return energy_terms(ctx, u_dev, v_dev, q_dev, f, terms_host, (cudaStream_t)stream);
+}
+
+int pcm_cg_threshold(double diis_prev, double delta_min, double *delta_out) {
+    if (!delta_out) return PCM_ERR_ARG;
+    double delta = 1.0;   // first SCF iteration: no previous DIIS error
+    if (diis_prev > 0.0) delta = std::exp(std::log(0.1 * diis_prev) / 1.07);   // 0.01 delta^1.07 = 1e-3 diis_prev
+    *delta_out = std::min(1.0, std::max(delta_min, delta));
+    return PCM_OK;
+}
+
 int pcm_pivot_order(uint64_t seed, int64_t M, int64_t *perm_host) {
     if (M < 0 || (M > 0 && !perm_host)) return PCM_ERR_ARG;
     pivot_order(seed, M, perm_host);

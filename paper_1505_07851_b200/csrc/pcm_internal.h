@@ -126,6 +126,10 @@ struct pcm_ctx {
     int32_t *c_sp = nullptr;
     int32_t *c_ab = nullptr;
 
+    // nuclei (pcm_set_nuclei): (x, y, z, charge)
+    int64_t natom = -1;
+    double4 *atoms = nullptr;
+
     double *boys = nullptr;  // [MAXL+1][BOYS_ROWS][BOYS_STRIDE]
 
     // fixed work partitions (sizes and SM count only; set once in pcm_setup by plan_all)
@@ -184,6 +188,9 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
 int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s);
 int launch_amatvec_sorted(pcm_ctx *ctx, const double *q_sorted, double *y_sorted, cudaStream_t s);  // both in sorted order
 int launch_amatvec_partials(pcm_ctx *ctx, const double *q_sorted, const int *stop, cudaStream_t s);  // ypart slots + near_amat only
+int launch_nuclear_potential(pcm_ctx *ctx, double *u, cudaStream_t s);
+int launch_rhs(pcm_ctx *ctx, const double *u, const double *v, double f, double *b, cudaStream_t s);
+int energy_terms(pcm_ctx *ctx, const double *u, const double *v, const double *q, double f, double *terms_host, cudaStream_t s);
 int plan_all(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
 void build_boys_tables(std::vector<double> &tab);

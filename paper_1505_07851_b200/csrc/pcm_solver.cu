@@ -492,6 +492,125 @@ __global__ void scatter_kernel(int M, const int32_t *__restrict__ s2c, const dou
 }
 
 // ---------------------------------------------------------------------------------------------
+// The rest of a C-PCM step (Eq. 1, 4, 13): u = B z, b = -f (u - v), Delta G_els.
+// ---------------------------------------------------------------------------------------------
+// u_k = sum_J z_J erf(zeta_k r_kJ)/r_kJ (Eq. 4): thread = point (sorted order), nuclei staged in shared memory and
+// summed in the caller's order; far field (zeta_k^2 r^2 >= 38: erf = 1) is z/r, otherwise (2 zeta/sqrt pi) F_0(zeta^2 r^2).
+__global__ void __launch_bounds__(128) nuclear_potential_kernel(const double4 *__restrict__ pt, int M, const double4 *__restrict__ atoms,
+                                                                int natom, const int32_t *__restrict__ s2c,
+                                                                const double *__restrict__ boys0, double *__restrict__ u) {
+    __shared__ double4 s_at[256];
+    const int k = blockIdx.x * 128 + threadIdx.x;
+    const double4 a = pt[min(k, M - 1)];
+    const double thr = TFAR_AMAT * a.w;   // zeta_k^2 r^2 >= 38  <=>  r^2 >= 38/zeta_k^2
+    const double zk = rsqrt_fast(a.w);
+    double sum = 0.0;
+    for (int base = 0; base < natom; base += 256) {
+        const int cnt = min(256, natom - base);
+        __syncthreads();
+        for (int t = threadIdx.x; t < cnt; t += 128) s_at[t] = atoms[base + t];
+        __syncthreads();
+        for (int t = 0; t < cnt; ++t) {
+            const double4 b = s_at[t];
+            const double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            double ev;
+            if (r2 >= thr) {
+                ev = rsqrt_fast(r2);
+            } else {
+                const double T = r2 * zk * zk;
+                const int i = __double2int_rn(T * 16.0);
+                const double d = T - (double)i * 0.0625;
+                const double *row = boys0 + (size_t)i * BOYS_STRIDE;
+                double f = __ldg(row + BOYS_TERMS - 1);
+#pragma unroll
+                for (int n = BOYS_TERMS - 2; n >= 0; --n) f = fma(f, d, __ldg(row + n));
+                ev = 1.1283791670955125739 * zk * f;  // 2/sqrt(pi)
+            }
+            sum = fma(b.w, ev, sum);
+        }
+    }
+    if (k < M) u[s2c[k]] = sum;
+}
+
+__global__ void rhs_kernel(int M, const double *__restrict__ u, const double *__restrict__ v, double f, double *__restrict__ b) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < M) b[i] = -f * (u[i] - v[i]);
+}
+
+// scal[12..14] = u.q, -v.q, q.Aq  (per-CTA partials, then the last CTA sums them in index order)
+constexpr int ENERGY_BLOCKS = 128;
+__global__ void __launch_bounds__(DOT_THREADS) energy_kernel(int M, const double *__restrict__ u, const double *__restrict__ v,
+                                                             const double *__restrict__ q, const double *__restrict__ Aq,
+                                                             double *__restrict__ scal, double *__restrict__ partial,
+                                                             int *__restrict__ ctl) {
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int i = blockIdx.x * DOT_THREADS + threadIdx.x; i < M; i += ENERGY_BLOCKS * DOT_THREADS) {
+        const double qi = q[i];
+        s0 = fma(u[i], qi, s0);
+        s1 = fma(-v[i], qi, s1);
+        s2 = fma(qi, Aq[i], s2);
+    }
+    s0 = block_sum(s0);
+    s1 = block_sum(s1);
+    s2 = block_sum(s2);
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x] = s0;
+        partial[ENERGY_BLOCKS + blockIdx.x] = s1;
+        partial[2 * ENERGY_BLOCKS + blockIdx.x] = s2;
+    }
+    if (last_block(ctl)) {
+        const double t0 = ordered_sum(partial, ENERGY_BLOCKS);
+        const double t1 = ordered_sum(partial + ENERGY_BLOCKS, ENERGY_BLOCKS);
+        const double t2 = ordered_sum(partial + 2 * ENERGY_BLOCKS, ENERGY_BLOCKS);
+        if (threadIdx.x == 0) { scal[12] = t0; scal[13] = t1; scal[14] = t2; ctl[CTL_TICKET] = 0; }
+    }
+}
+
+int launch_nuclear_potential(pcm_ctx *ctx, double *u, cudaStream_t s) {
+    const int M = (int)ctx->M;
+    if (M == 0) return PCM_OK;
+    nuclear_potential_kernel<<<(unsigned)cdiv(M, 128), 128, 0, s>>>(ctx->pt, M, ctx->atoms, (int)ctx->natom, ctx->s2c, ctx->boys, u);
+    ctx->launch_total += 1;
+    PCM_CUDA(ctx, cudaGetLastError());
+    return PCM_OK;
+}
+
+int launch_rhs(pcm_ctx *ctx, const double *u, const double *v, double f, double *b, cudaStream_t s) {
+    const int M = (int)ctx->M;
+    if (M == 0) return PCM_OK;
+    rhs_kernel<<<(unsigned)cdiv(M, 256), 256, 0, s>>>(M, u, v, f, b);
+    ctx->launch_total += 1;
+    PCM_CUDA(ctx, cudaGetLastError());
+    return PCM_OK;
+}
+
+int energy_terms(pcm_ctx *ctx, const double *u, const double *v, const double *q, double f, double *terms, cudaStream_t s) {
+    const int M = (int)ctx->M;
+    terms[0] = terms[1] = terms[2] = terms[3] = 0.0;
+    if (M == 0) return PCM_OK;
+    double *Aq = ctx->cg_vec;   // scratch (caller order)
+    double *scal = ctx->cg_scal;
+    int *ctl = reinterpret_cast<int *>(scal + 8);
+    const int saved_timing = ctx->timing;
+    ctx->timing = 0;
+    int rc = launch_amatvec(ctx, q, Aq, s);
+    ctx->timing = saved_timing;
+    if (rc) return rc;
+    energy_kernel<<<ENERGY_BLOCKS, DOT_THREADS, 0, s>>>(M, u, v, q, Aq, scal, scal + 16, ctl);
+    ctx->launch_total += 1;
+    PCM_CUDA(ctx, cudaGetLastError());
+    double *h = ctx->cg_scal_host;
+    PCM_CUDA(ctx, cudaMemcpyAsync(h, scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    PCM_CUDA(ctx, cudaStreamSynchronize(s));
+    terms[0] = h[12];
+    terms[1] = h[13];
+    terms[2] = h[14] / (2.0 * f);
+    terms[3] = terms[0] + terms[1] + terms[2];
+    return PCM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // host drivers
 // ---------------------------------------------------------------------------------------------
 int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s) {

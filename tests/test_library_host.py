@@ -117,3 +117,12 @@ def test_no_cpu_fallback():
         pcm.pcm_setup([0], [[0, 0, 0]], [1], [1.0], [1.0], [[1, 0, 0]], [1.0])
     src = open(os.path.join(ROOT, "paper_1505_07851_b200", "__init__.py")).read()
     assert "import oracle" not in src and "from oracle" not in src
+
+
+def test_cg_threshold_matches_oracle_and_eq21(L, orc):
+    """pcm_cg_threshold (host arithmetic only) against the oracle and against Eq. 21 inverted."""
+    for d in (0.0, -1.0, 1e-8, 3e-5, 1e-3, 0.2, 50.0):
+        for dmin in (1e-12, 1e-6):
+            assert pcm.pcm_cg_threshold(d, dmin) == pytest.approx(orc.cg_threshold(d, dmin), rel=1e-14)
+    delta = pcm.pcm_cg_threshold(1e-3, 1e-12)
+    assert 0.01 * delta ** 1.07 == pytest.approx(1e-6, rel=1e-12)
