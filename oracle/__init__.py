@@ -57,6 +57,9 @@ def lib():
         L.orc_pcg.restype = C.c_long
         L.orc_pcg.argtypes = [C.c_long, C.c_void_p, _dp, _dp, C.c_void_p, _dp, _dp, C.c_int, C.c_double, C.c_long,
                               C.c_int, C.c_long, C.c_void_p, C.c_void_p, C.c_void_p, _dp, C.c_void_p]
+        L.orc_prim_deriv.argtypes = [C.c_int, C.c_double, _dp, C.c_int, C.c_double, _dp, C.c_double, _dp, _dp, _dp]
+        L.orc_gradient.argtypes = basis + [C.c_long, _dp, _dp, _dp, _dp, C.c_long, C.c_double, C.c_long, C.c_void_p,
+                                           C.c_long, C.c_void_p, _dp, _dp]
         L.orc_bz.argtypes = [C.c_long, _dp, _dp, C.c_long, _dp, _dp, _dp]
         L.orc_rhs.argtypes = [C.c_long, _dp, _dp, C.c_double, _dp]
         L.orc_energy.argtypes = [C.c_long, _dp, _dp, _dp, _dp, C.c_double, _dp]
@@ -252,3 +255,30 @@ def energy(u, v, q, Aq, f: float) -> np.ndarray:
 def cg_threshold(diis_prev: float, delta_min: float = 1e-6) -> float:
     """Eq. 21: the dynamic CG threshold for the next SCF iteration (diis_prev <= 0: first iteration, delta = 1)."""
     return float(lib().orc_cg_threshold(float(diis_prev), float(delta_min)))
+
+
+# ------------------------------------------------------------------ gradient of E = v.q (Eq. 14 / 22, one-electron term)
+
+def prim_deriv(la, alpha, A, lb, beta, B, zeta, Cpt):
+    """Cartesian blocks d/dA_x and d/dB_x of [chi_a|J|chi_b]: two arrays [3, NCART[la], NCART[lb]]."""
+    n = _NCART[la] * _NCART[lb]
+    dA, dB = np.zeros(3 * n), np.zeros(3 * n)
+    lib().orc_prim_deriv(int(la), float(alpha), _f(A), int(lb), float(beta), _f(B), float(zeta), _f(Cpt), dA, dB)
+    return dA.reshape(3, _NCART[la], _NCART[lb]), dB.reshape(3, _NCART[la], _NCART[lb])
+
+
+def gradient(basis, surface, P, q, shells=None, points=None, cutoff: float = 1e-20):
+    """dE/d(shell centre) [nsel, 3] and dE/d(point position) [nsel, 3] for E = v.q at fixed P and q (the paper's
+    (grad* c^T) q is the negative).  shells / points: index lists (None: all)."""
+    def sel(x, n):
+        if x is None:
+            return n, None
+        a = np.ascontiguousarray(x, np.int64)
+        return len(a), a
+    nS, sS = sel(shells, basis.nshell)
+    nK, sK = sel(points, surface.M)
+    gs, gp = np.zeros((nS, 3)), np.zeros((nK, 3))
+    Pm = _f(P)
+    lib().orc_gradient(*_basis_args(basis), surface.M, _f(surface.xyz).reshape(-1), _f(surface.zeta), _f(q), Pm.reshape(-1),
+                       Pm.shape[1], float(cutoff), nS, _ptr(sS), nK, _ptr(sK), gs.reshape(-1), gp.reshape(-1))
+    return gs, gp

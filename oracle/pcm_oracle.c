@@ -44,8 +44,9 @@
 
 #define ORC_PI 3.14159265358979323846264338327950288
 #define LMAX_SHELL 2          /* s, p, d */
-#define LSUM (2 * LMAX_SHELL) /* l_a + l_b <= 4 */
-#define NA (LSUM + 1)         /* 0..4 per Cartesian power in the recursion tables */
+#define LTAB (LMAX_SHELL + 1) /* the recursion tables go one power further: derivative integrals raise one side */
+#define LSUM (2 * LMAX_SHELL + 1) /* l_a + l_b <= 4, + 1 for a raised side */
+#define NA (LSUM + 1)         /* 0..5 per Cartesian power in the recursion tables */
 
 int orc_num_threads(void) {
 #ifdef _OPENMP
@@ -113,7 +114,7 @@ void orc_boys(int nmax, double T, double *F) {
  * reads |a| = la, |b| = lb.
  * ---------------------------------------------------------------------------------- */
 #define AIDX(x, y, z) (((x) * NA + (y)) * NA + (z))
-#define NB (LMAX_SHELL + 1)
+#define NB (LTAB + 1)
 #define BIDX(x, y, z) (((x) * NB + (y)) * NB + (z))
 
 static void os_tables(int la, double alpha, const double *A, int lb, double beta, const double *B,
@@ -196,7 +197,7 @@ static const int CART[3][6][3] = {
 };
 static const int NCART[3] = {1, 3, 6};
 
-/* one primitive integral with explicit powers (any |a|,|b| <= 2) */
+/* one primitive integral with explicit powers (any |a|,|b| <= 3, |a| + |b| <= 5) */
 double orc_prim_integral(const int *a, double alpha, const double *A, const int *b, double beta, const double *B,
                          double zeta, const double *C, int path) {
     int la = a[0] + a[1] + a[2], lb = b[0] + b[1] + b[2];
@@ -669,4 +670,159 @@ double orc_cg_threshold(double diis_prev, double delta_min) {
     if (delta > 1.0) delta = 1.0;
     if (delta < delta_min) delta = delta_min;
     return delta;
+}
+
+/* ------------------------------------------------------------------------------------
+ * Gradient of E = v.q = sum_k q_k sum_{mu,nu} P_mu,nu (mu|J_k|nu) with respect to the shell centres and the
+ * surface points at fixed P and q: the one-electron part (grad* c^T) q of Eq. 14, PAPER.md:202-218 (Eq. 22:
+ * ga, gb per primitive pair, gc per point).  Library sign (reading R2): the paper's c = -v, so its term is -E.
+ *   [d/dA_x chi_a | J | chi_b] = 2 alpha [a+1_x|J|b] - a_x [a-1_x|J|b]      (derivative of a Cartesian Gaussian)
+ *   [chi_a | J | d/dB_x chi_b] = 2 beta  [a|J|b+1_x] - b_x [a|J|b-1_x]
+ *   [chi_a | d/dC_x J | chi_b] = -(d/dA_x + d/dB_x)[a|J|b]                  (the integral depends on A-C, B-C only)
+ * each bracket on the right by the Obara-Saika tables above.  zeta_k does not move with the point (Eq. 7).
+ *   g_shell[S] = sum_J sum_k q_k ( P_{S,J} . d/dA (S J|J_k)  +  P_{J,S} . d/dB (J S|J_k) )     (S as bra and as ket)
+ *   g_point[k] = q_k sum_{I,J} P_{I,J} . d/dC (I J|J_k)
+ * ---------------------------------------------------------------------------------- */
+typedef double hrr_table[NB * NB * NB][NA * NA * NA];
+
+/* Cartesian derivative blocks of one primitive pair at one point: dA[x][ia*NCART[lb]+ib], dB likewise */
+static void prim_deriv_blocks(int la, double alpha, const double *A, int lb, double beta, const double *B, double zeta,
+                              const double *C, double dA[3][36], double dB[3][36]) {
+    static _Thread_local hrr_table up, dn;
+    /* bra raised / lowered */
+    os_tables(la + 1, alpha, A, lb, beta, B, zeta, C, 0, up);
+    if (la > 0) os_tables(la - 1, alpha, A, lb, beta, B, zeta, C, 0, dn);
+    for (int ia = 0; ia < NCART[la]; ++ia)
+        for (int ib = 0; ib < NCART[lb]; ++ib) {
+            const int *a = CART[la][ia], *b = CART[lb][ib];
+            for (int x = 0; x < 3; ++x) {
+                int ap[3] = {a[0], a[1], a[2]}, am[3] = {a[0], a[1], a[2]};
+                ap[x] += 1; am[x] -= 1;
+                double v = 2.0 * alpha * up[BIDX(b[0], b[1], b[2])][AIDX(ap[0], ap[1], ap[2])];
+                if (a[x] > 0) v -= a[x] * dn[BIDX(b[0], b[1], b[2])][AIDX(am[0], am[1], am[2])];
+                dA[x][ia * NCART[lb] + ib] = v;
+            }
+        }
+    /* ket raised / lowered */
+    os_tables(la, alpha, A, lb + 1, beta, B, zeta, C, 0, up);
+    if (lb > 0) os_tables(la, alpha, A, lb - 1, beta, B, zeta, C, 0, dn);
+    for (int ia = 0; ia < NCART[la]; ++ia)
+        for (int ib = 0; ib < NCART[lb]; ++ib) {
+            const int *a = CART[la][ia], *b = CART[lb][ib];
+            for (int x = 0; x < 3; ++x) {
+                int bp[3] = {b[0], b[1], b[2]}, bm[3] = {b[0], b[1], b[2]};
+                bp[x] += 1; bm[x] -= 1;
+                double v = 2.0 * beta * up[BIDX(bp[0], bp[1], bp[2])][AIDX(a[0], a[1], a[2])];
+                if (b[x] > 0) v -= b[x] * dn[BIDX(bm[0], bm[1], bm[2])][AIDX(a[0], a[1], a[2])];
+                dB[x][ia * NCART[lb] + ib] = v;
+            }
+        }
+}
+
+/* public: the derivative blocks of one primitive pair (for the pins) */
+void orc_prim_deriv(int la, double alpha, const double *A, int lb, double beta, const double *B, double zeta, const double *C,
+                    double *dA_out, double *dB_out) {
+    double dA[3][36], dB[3][36];
+    prim_deriv_blocks(la, alpha, A, lb, beta, B, zeta, C, dA, dB);
+    int n = NCART[la] * NCART[lb];
+    for (int x = 0; x < 3; ++x)
+        for (int c = 0; c < n; ++c) { dA_out[x * n + c] = dA[x][c]; dB_out[x * n + c] = dB[x][c]; }
+}
+
+/* contracted component blocks of d/dA and d/dB of (mu in I, nu in J | J_k): outA[x][ncompI*ncompJ], outB likewise */
+static void shell_deriv_block(const orc_basis *bs, const long *po, int I, int J, const unsigned char *keep, double zeta,
+                              const double *C, double outA[3][36], double outB[3][36]) {
+    int la = bs->l[I], lb = bs->l[J];
+    double cA[3][36], cB[3][36], pA[3][36], pB[3][36];
+    int n = NCART[la] * NCART[lb];
+    for (int x = 0; x < 3; ++x)
+        for (int c = 0; c < n; ++c) { cA[x][c] = 0.0; cB[x][c] = 0.0; }
+    for (int i = 0; i < bs->nprim[I]; ++i)
+        for (int j = 0; j < bs->nprim[J]; ++j) {
+            if (keep && !keep[i * bs->nprim[J] + j]) continue;
+            prim_deriv_blocks(la, bs->ex[po[I] + i], bs->xyz + 3 * I, lb, bs->ex[po[J] + j], bs->xyz + 3 * J, zeta, C, pA, pB);
+            double cc = bs->co[po[I] + i] * bs->co[po[J] + j];
+            for (int x = 0; x < 3; ++x)
+                for (int c = 0; c < n; ++c) { cA[x][c] += cc * pA[x][c]; cB[x][c] += cc * pB[x][c]; }
+        }
+    for (int x = 0; x < 3; ++x) {
+        to_components(la, lb, bs->d_pure, cA[x], outA[x]);
+        to_components(la, lb, bs->d_pure, cB[x], outB[x]);
+    }
+}
+
+/* g_shell_out[3*nselS]: gradient with respect to the centres of the shells selS[0..nselS) (NULL: shells 0..nselS-1);
+ * g_point_out[3*nselK]: gradient with respect to the positions of the points selK[0..nselK) (NULL: 0..nselK-1).
+ * Every sum runs over the full square of shell pairs and over all npt points. */
+void orc_gradient(int nshell, const int *l, const double *xyz, const int *nprim, const double *ex, const double *co,
+                  int d_pure, long npt, const double *pt_xyz, const double *pt_zeta, const double *q, const double *P,
+                  long ldp, double cutoff, long nselS, const long *selS, long nselK, const long *selK,
+                  double *g_shell_out, double *g_point_out) {
+    orc_basis bs = {nshell, l, xyz, nprim, ex, co, d_pure};
+    long *po = malloc(sizeof(long) * (nshell + 1)), *bo = malloc(sizeof(long) * (nshell + 1));
+    offsets(&bs, po, bo);
+    long *moff = malloc(sizeof(long) * (size_t)nshell * nshell);
+    long tot = 0;
+    for (int I = 0; I < nshell; ++I)
+        for (int J = 0; J < nshell; ++J) { moff[(long)I * nshell + J] = tot; tot += nprim[I] * nprim[J]; }
+    unsigned char *mask = malloc((size_t)tot + 1);
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int I = 0; I < nshell; ++I)
+        for (int J = 0; J < nshell; ++J) {
+            long o = moff[(long)I * nshell + J];
+            if (!keep_mask(&bs, po, I, J, cutoff, mask + o)) moff[(long)I * nshell + J] = -1;
+        }
+    /* shells: one (selected shell, partner shell) pair per task, partner sums added in order afterwards */
+    double *part = calloc((size_t)(nselS > 0 ? nselS : 1) * nshell * 3, sizeof(double));
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+    for (long s = 0; s < nselS; ++s)
+        for (int J = 0; J < nshell; ++J) {
+            int S = (int)(selS ? selS[s] : s);
+            int nS = ncomp_of(l[S], d_pure), nJ = ncomp_of(l[J], d_pure);
+            long o_sj = moff[(long)S * nshell + J], o_js = moff[(long)J * nshell + S];
+            double sum[3] = {0, 0, 0}, comp[3] = {0, 0, 0}, dA[3][36], dB[3][36];
+            for (long k = 0; k < npt; ++k) {
+                if (o_sj >= 0) {   /* S as the bra */
+                    shell_deriv_block(&bs, po, S, J, mask + o_sj, pt_zeta[k], pt_xyz + 3 * k, dA, dB);
+                    for (int x = 0; x < 3; ++x)
+                        for (int i = 0; i < nS; ++i)
+                            for (int j = 0; j < nJ; ++j)
+                                nsum(&sum[x], &comp[x], q[k] * P[(bo[S] + i) * ldp + bo[J] + j] * dA[x][i * nJ + j]);
+                }
+                if (o_js >= 0) {   /* S as the ket */
+                    shell_deriv_block(&bs, po, J, S, mask + o_js, pt_zeta[k], pt_xyz + 3 * k, dA, dB);
+                    for (int x = 0; x < 3; ++x)
+                        for (int j = 0; j < nJ; ++j)
+                            for (int i = 0; i < nS; ++i)
+                                nsum(&sum[x], &comp[x], q[k] * P[(bo[J] + j) * ldp + bo[S] + i] * dB[x][j * nS + i]);
+                }
+            }
+            for (int x = 0; x < 3; ++x) part[((size_t)s * nshell + J) * 3 + x] = sum[x] + comp[x];
+        }
+    for (long s = 0; s < nselS; ++s)
+        for (int x = 0; x < 3; ++x) {
+            double sum = 0.0, comp = 0.0;
+            for (int J = 0; J < nshell; ++J) nsum(&sum, &comp, part[((size_t)s * nshell + J) * 3 + x]);
+            g_shell_out[3 * s + x] = sum + comp;
+        }
+    free(part);
+    /* points */
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long s = 0; s < nselK; ++s) {
+        long k = selK ? selK[s] : s;
+        double sum[3] = {0, 0, 0}, comp[3] = {0, 0, 0}, dA[3][36], dB[3][36];
+        for (int I = 0; I < nshell; ++I)
+            for (int J = 0; J < nshell; ++J) {
+                long o = moff[(long)I * nshell + J];
+                if (o < 0) continue;
+                shell_deriv_block(&bs, po, I, J, mask + o, pt_zeta[k], pt_xyz + 3 * k, dA, dB);
+                int na = ncomp_of(l[I], d_pure), nb = ncomp_of(l[J], d_pure);
+                for (int x = 0; x < 3; ++x)
+                    for (int i = 0; i < na; ++i)
+                        for (int j = 0; j < nb; ++j)
+                            nsum(&sum[x], &comp[x], -P[(bo[I] + i) * ldp + bo[J] + j] * (dA[x][i * nb + j] + dB[x][i * nb + j]));
+            }
+        for (int x = 0; x < 3; ++x) g_point_out[3 * s + x] = q[k] * (sum[x] + comp[x]);
+    }
+    free(mask); free(moff); free(po); free(bo);
 }
