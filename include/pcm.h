@@ -55,7 +55,8 @@ typedef struct pcm_options {
     int device;            /* CUDA device ordinal; -1 (default) = the calling thread's current device */
     int merge_products;    /* 1 (default): primitive pairs with identical (A, alpha, B, beta) -- e.g. the s and p
                               parts of an sp shell -- share one Hermite Gaussian product in the kernels (exact) */
-    int reserved[4];
+    int gradient;          /* 1: also build what pcm_gradient needs (derivative tables, 3x the G matrices); default 0 */
+    int reserved[3];
 } pcm_options;
 
 typedef struct pcm_info {
@@ -190,6 +191,20 @@ int pcm_rhs(pcm_ctx *ctx, const double *u_dev, const double *v_dev, double f, do
 int pcm_energy(pcm_ctx *ctx, const double *u_dev, const double *v_dev, const double *q_dev, double f, double *terms_host,
                void *stream);
 int pcm_cg_threshold(double diis_prev, double delta_min, double *delta_out);
+
+/*
+ * pcm_gradient -- the one-electron PCM gradient term (grad* c^T) q of Eq. 14 (Eq. 22: ga, gb per
+ * primitive pair, gc per point), in this library's sign: the gradient of E = v.q = sum_k q_k sum_{mu,nu} P_mu,nu (mu|J_k|nu)
+ * at fixed P and q (the paper's c = -v, so its term is -E).
+ *   g_shell[3*S + x] = dE/d(x coordinate of the centre of shell S)   (bra and ket derivatives of every pair with S, summed)
+ *   g_point[3*k + x] = dE/d(x coordinate of surface point k)         (zeta_k does not move with the point, Eq. 7)
+ * The caller adds shell and point rows to the atoms they sit on.  Needs pcm_options.gradient = 1 at pcm_setup.
+ * P_dev: DEVICE nbf x nbf (symmetric, as pcm_potential); q_dev: DEVICE M; g_shell_dev: DEVICE 3*nshell doubles;
+ * g_point_dev: DEVICE 3*M doubles (either may be NULL).  Overwrites.  Deterministic.  Asynchronous (the first call
+ * allocates its scratch and synchronises).
+ */
+int pcm_gradient(pcm_ctx *ctx, const double *P_dev, int64_t ldp, const double *q_dev, double *g_shell_dev, double *g_point_dev,
+                 void *stream);
 
 /*
  * Host-buffer forms of the four hot calls: same semantics, every array is a HOST pointer; the call

@@ -30,14 +30,14 @@ EXPORTS = (
     "pcm_rbj_build", "pcm_rbj_get", "pcm_cg_solve", "pcm_potential_host", "pcm_fock_host", "pcm_amatvec_host",
     "pcm_cg_solve_host", "pcm_get_info", "pcm_set_timing", "pcm_last_kernel_ms", "pcm_last_class_ms",
     "pcm_launch_count", "pcm_fp64_peak", "pcm_set_nuclei", "pcm_nuclear_potential", "pcm_rhs", "pcm_energy",
-    "pcm_cg_threshold",
+    "pcm_cg_threshold", "pcm_gradient",
     "pcm_schwarz_bound", "pcm_last_error", "pcm_destroy",
 )
 
 
 class pcm_options(C.Structure):
     _fields_ = [("screen_eps", C.c_double), ("d_pure", C.c_int), ("device", C.c_int), ("merge_products", C.c_int),
-                ("reserved", C.c_int * 4)]
+                ("gradient", C.c_int), ("reserved", C.c_int * 3)]
 
 
 class pcm_info(C.Structure):
@@ -98,6 +98,7 @@ def lib(build: bool = False):
         L.pcm_rhs.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.pcm_energy.argtypes = [vp, vp, vp, vp, C.c_double, _dp, vp]
         L.pcm_cg_threshold.argtypes = [C.c_double, C.c_double, _dp]
+        L.pcm_gradient.argtypes = [vp, vp, C.c_int64, vp, vp, vp, vp]
         L.pcm_schwarz_bound.argtypes = [C.c_int, C.c_double, vp, C.c_int, C.c_double, vp, _dp]
         L.pcm_last_error.argtypes = [vp]
         L.pcm_last_error.restype = C.c_char_p
@@ -164,7 +165,8 @@ def pcm_options_default() -> pcm_options:
 
 
 def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_zeta, pt_switch=None, *,
-              screen_eps: float = 1e-12, d_pure: bool = True, device: int = -1, merge_products: bool = True) -> Context:
+              screen_eps: float = 1e-12, d_pure: bool = True, device: int = -1, merge_products: bool = True,
+              gradient: bool = False) -> Context:
     """Host numpy arrays in, context out (include/pcm.h: pcm_setup)."""
     import torch
     if not torch.cuda.is_available():
@@ -185,12 +187,14 @@ def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_z
     opt.d_pure = 1 if d_pure else 0
     opt.device = int(device)
     opt.merge_products = 1 if merge_products else 0
+    opt.gradient = 1 if gradient else 0
     h = C.c_void_p()
     rc = lib().pcm_setup(C.byref(h), len(sl), _hp(sl), _hp(sx), _hp(sn), _hp(pe), _hp(pc), len(pz), _hp(px), _hp(pz),
                          _hp(ps), C.byref(opt))
     _check(rc, None)
     ctx = Context(h, 0, len(pz), device)
     ctx.nbf = int(pcm_get_info(ctx).nbf)
+    ctx.nshell = len(sl)
     return ctx
 
 
@@ -260,6 +264,19 @@ def pcm_energy(ctx: Context, u, v, q, f: float, stream=None) -> np.ndarray:
     _check(lib().pcm_energy(ctx.handle, _dev(u, ctx.M), _dev(v, ctx.M), _dev(q, ctx.M), float(f),
                             terms.ctypes.data_as(_dp), _stream(stream)), ctx.handle)
     return terms
+
+
+def pcm_gradient(ctx: Context, P, q, stream=None):
+    """(g_shell [nshell, 3], g_point [M, 3]) of E = v.q at fixed P and q (Eq. 14/22; needs pcm_setup(gradient=True))."""
+    import torch
+    if P.dim() != 2 or P.shape[0] != ctx.nbf or P.shape[1] != ctx.nbf or P.stride(1) != 1:
+        raise ValueError("P must be nbf x nbf, row-major")
+    gs = torch.empty((ctx.nshell, 3), dtype=torch.float64, device=P.device)
+    gp = torch.empty((ctx.M, 3), dtype=torch.float64, device=P.device)
+    _dev(P)
+    _check(lib().pcm_gradient(ctx.handle, C.c_void_p(P.data_ptr()), P.stride(0), _dev(q, ctx.M), C.c_void_p(gs.data_ptr()),
+                              C.c_void_p(gp.data_ptr()), _stream(stream)), ctx.handle)
+    return gs, gp
 
 
 def pcm_cg_threshold(diis_prev: float, delta_min: float = 1e-6) -> float:

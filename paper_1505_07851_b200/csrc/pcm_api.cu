@@ -28,6 +28,7 @@ void pcm_options_default(pcm_options *opt) {
     opt->d_pure = 1;
     opt->device = -1;
     opt->merge_products = 1;
+    opt->gradient = 0;
 }
 
 static void free_ctx(pcm_ctx *ctx) {
@@ -201,6 +202,15 @@ int pcm_energy(pcm_ctx *ctx, const double *u_dev, const double *v_dev, const dou
         return set_error(ctx, PCM_ERR_ARG, "pcm_energy: bad argument");
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
     return energy_terms(ctx, u_dev, v_dev, q_dev, f, terms_host, (cudaStream_t)stream);
+}
+
+int pcm_gradient(pcm_ctx *ctx, const double *P_dev, int64_t ldp, const double *q_dev, double *g_shell_dev, double *g_point_dev,
+                 void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (!ctx->opt.gradient) return set_error(ctx, PCM_ERR_STATE, "pcm_gradient: pcm_setup was called without pcm_options.gradient");
+    if ((ctx->nbf > 0 && !P_dev) || (ctx->M > 0 && !q_dev) || ldp < ctx->nbf) return set_error(ctx, PCM_ERR_ARG, "pcm_gradient: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_gradient(ctx, P_dev, ldp, q_dev, g_shell_dev, g_point_dev, (cudaStream_t)stream);
 }
 
 int pcm_cg_threshold(double diis_prev, double delta_min, double *delta_out) {

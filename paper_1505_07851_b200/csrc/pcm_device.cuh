@@ -111,8 +111,8 @@ __device__ __forceinline__ void seeds_general(double R2, double p, double invk, 
 // All loops have compile-time bounds: after unrolling every index is a constant and the arrays live in
 // registers.  The direction lowered is the one with the smallest non-zero power (a power of 1 or 2
 // costs one instruction, 3 or 4 costs two).
-// The order-0 integrals are handed to `sink` once per component h = hidx(t,u,v): sink.value(h, R) or, when R
-// is a single product a*b, sink.product(h, a, b) so that the consumer can fuse it into an FMA.
+// The order-0 integrals are handed to `sink` once per component h = hidx(t,u,v): sink.value(h, t, u, v, R) or, when R
+// is a single product a*b, sink.product(h, t, u, v, a, b) so that the consumer can fuse it into an FMA.
 // ---------------------------------------------------------------------------------------------
 __host__ __device__ constexpr int pick_dir(int t, int u, int v) {
     int best = -1, bp = 99;
@@ -128,7 +128,7 @@ __device__ __forceinline__ void hermite_R(double x, double y, double z, const do
     double R[L + 1][NH];  // R[n][h] for degree(h) <= L - n; unused entries are never materialised
 #pragma unroll
     for (int n = 0; n <= L; ++n) R[n][0] = g[n];
-    sink.value(0, R[0][0]);
+    sink.value(0, 0, 0, 0, R[0][0]);
 #pragma unroll
     for (int d = 1; d <= L; ++d) {
 #pragma unroll
@@ -145,12 +145,12 @@ __device__ __forceinline__ void hermite_R(double x, double y, double z, const do
                     const int h2 = pw < 2 ? 0 : (dir == 0 ? hidx(t - 2, u, v) : (dir == 1 ? hidx(t, u - 2, v) : hidx(t, u, v - 2)));
                     const int h = hidx(t, u, v);
                     if (pw == 1) {
-                        if (n == 0) sink.product(h, c, R[n + 1][h1]);
+                        if (n == 0) sink.product(h, t, u, v, c, R[n + 1][h1]);
                         else R[n][h] = c * R[n + 1][h1];
                     } else {
                         const double lower = (pw == 2) ? R[n + 1][h2] : (double)(pw - 1) * R[n + 1][h2];
                         const double val = fma(c, R[n + 1][h1], lower);
-                        if (n == 0) sink.value(h, val);
+                        if (n == 0) sink.value(h, t, u, v, val);
                         else R[n][h] = val;
                     }
                 }

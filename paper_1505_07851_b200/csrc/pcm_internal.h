@@ -28,13 +28,14 @@ __host__ __device__ constexpr int hidx(int t, int u, int v) {
 __host__ __device__ constexpr double tfar(int L) { return 38.0 + 3.0 * L; }
 constexpr double TFAR_AMAT = 38.0;  // erfc(sqrt(38)) = 3e-18
 
-// Boys table: rows T_i = i/16, i = 0..BOYS_ROWS-1 (covers [0, 52]); per L a table of rows
+// Boys table: rows T_i = i/16, i = 0..BOYS_ROWS-1 (covers [0, 54] >= tfar(MAXLG)); per L a table of rows
 // {c_0..c_7, exp(-T_i), 0} with c_k = (-1)^k F_{L+k}(T_i)/k!  so that F_L(T_i + d) = sum_k c_k d^k.
-constexpr int BOYS_ROWS = 52 * 16 + 1;
+constexpr int BOYS_ROWS = 54 * 16 + 1;
 constexpr int BOYS_STRIDE = 10;
 constexpr int BOYS_TERMS = 8;
 
 constexpr int MAXL = 4;
+constexpr int MAXLG = MAXL + 1;  // the gradient kernels evaluate Hermite integrals one order higher (Boys tables 0..MAXLG)
 
 struct DeviceBuf {  // owning device allocation
     void *p = nullptr;
@@ -73,6 +74,10 @@ struct ClassData {        // products of one total angular momentum L, padded to
     int64_t herm_slots = 0;    // chunks the herm buffer holds
     double *near_fock = nullptr;  // [fock_map.npiece][nherm(L)][32] sums of the near pieces
     double *near_pot = nullptr;   // [pot_map.npiece][32]
+    // pcm_gradient scratch (allocated by its first call): Hermite potential sums one order higher
+    double *gherm = nullptr;       // [plan_gfock.chunks][nherm(L+1)][npad]
+    double *near_gfock = nullptr;  // [fock_map.npiece][nherm(L+1)][32]
+    double *near_gpoint = nullptr; // [pot_map.npiece][3][32]
 };
 
 struct Plan {             // work partition of one hot kernel launch: grid = (xb, chunks)
@@ -130,7 +135,23 @@ struct pcm_ctx {
     int64_t natom = -1;
     double4 *atoms = nullptr;
 
-    double *boys = nullptr;  // [MAXL+1][BOYS_ROWS][BOYS_STRIDE]
+    // pcm_gradient (pcm_options.gradient): derivative tables and the shell bookkeeping of the pair transform
+    int64_t nshell = 0;
+    double *dG = nullptr;        // per member [na*nb][3][nherm(L_member)] = dG/dX_AB at fixed P, at 3 * m_goff[m]
+    double *m_ap = nullptr;      // per member alpha/p (weight of the bra centre in P)
+    int32_t *sp_shI = nullptr, *sp_shJ = nullptr;  // shells of a shell pair
+    int64_t *sp_cstart = nullptr;  // [nsp+1] first component of a shell pair (components are grouped by shell pair)
+    int64_t *sh_start = nullptr;   // [nshell+1] CSR: shell -> entries 2 * sp + side (0: bra, 1: ket)
+    int32_t *sh_list = nullptr;
+    int32_t *hshift = nullptr;     // [3][nherm(MAXL)]: index of (t,u,v) + 1_x
+    double *gcomp = nullptr;       // [ncomp][6] per component: dE/dA xyz, dE/dB xyz
+    double *gsp = nullptr;         // [nsp][6]
+    double *gpart = nullptr;       // [slots][3][M] partial sums of the point gradient
+    int64_t gpart_slots = 0;
+    bool grad_ready = false;
+    pcm::Plan plan_gfock[pcm::MAXL + 1], plan_gpoint[pcm::MAXL + 1];
+
+    double *boys = nullptr;  // [MAXLG+1][BOYS_ROWS][BOYS_STRIDE]
 
     // fixed work partitions (sizes and SM count only; set once in pcm_setup by plan_all)
     pcm::Plan plan_pot[pcm::MAXL + 1], plan_fock[pcm::MAXL + 1], plan_amat;
@@ -191,6 +212,7 @@ int launch_amatvec_partials(pcm_ctx *ctx, const double *q_sorted, const int *sto
 int launch_nuclear_potential(pcm_ctx *ctx, double *u, cudaStream_t s);
 int launch_rhs(pcm_ctx *ctx, const double *u, const double *v, double f, double *b, cudaStream_t s);
 int energy_terms(pcm_ctx *ctx, const double *u, const double *v, const double *q, double f, double *terms_host, cudaStream_t s);
+int launch_gradient(pcm_ctx *ctx, const double *P, int64_t ldp, const double *q, double *g_shell, double *g_point, cudaStream_t s);
 int plan_all(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
 void build_boys_tables(std::vector<double> &tab);

@@ -349,8 +349,8 @@ AmatParts amat_parts(const pcm_ctx *ctx) {
 template <int L>
 struct FockSink {
     double acc[nherm(L)];
-    __device__ __forceinline__ void value(int h, double v) { acc[h] += v; }
-    __device__ __forceinline__ void product(int h, double a, double b) { acc[h] = fma(a, b, acc[h]); }
+    __device__ __forceinline__ void value(int h, int, int, int, double v) { acc[h] += v; }
+    __device__ __forceinline__ void product(int h, int, int, int, double a, double b) { acc[h] = fma(a, b, acc[h]); }
 };
 
 template <int L>
@@ -506,8 +506,8 @@ template <int L>
 struct PotSink {
     const double *D;
     double v;
-    __device__ __forceinline__ void value(int h, double x) { v = fma(D[h], x, v); }
-    __device__ __forceinline__ void product(int h, double a, double b) { v = fma(D[h], a * b, v); }
+    __device__ __forceinline__ void value(int h, int, int, int, double x) { v = fma(D[h], x, v); }
+    __device__ __forceinline__ void product(int h, int, int, int, double a, double b) { v = fma(D[h], a * b, v); }
 };
 
 template <int L>
@@ -1063,5 +1063,7 @@ int fp64_peak(pcm_ctx *ctx, int reps, double *tflops) {
     *tflops = flops / (best_ms * 1e-3) * 1e-12;
     return PCM_OK;
 }
+
+#include "pcm_gradient.inl"
 
 }  // namespace pcm

@@ -38,8 +38,8 @@ int dev_alloc(pcm_ctx *ctx, void **p, size_t bytes) {
 // dF_n/dT = -F_{n+1}), then exp(-T_i).
 // ---------------------------------------------------------------------------------------------
 void build_boys_tables(std::vector<double> &tab) {
-    const int nmax = MAXL + BOYS_TERMS - 1;
-    tab.assign((size_t)(MAXL + 1) * BOYS_ROWS * BOYS_STRIDE, 0.0);
+    const int nmax = MAXLG + BOYS_TERMS - 1;
+    tab.assign((size_t)(MAXLG + 1) * BOYS_ROWS * BOYS_STRIDE, 0.0);
     std::vector<long double> F(nmax + 1);
     for (int i = 0; i < BOYS_ROWS; ++i) {
         const long double T = (long double)i / 16.0L;
@@ -52,7 +52,7 @@ void build_boys_tables(std::vector<double> &tab) {
         }
         F[nmax] = eT * sum;
         for (int n = nmax; n >= 1; --n) F[n - 1] = (2.0L * T * F[n] + eT) / (2.0L * n - 1.0L);
-        for (int L = 0; L <= MAXL; ++L) {
+        for (int L = 0; L <= MAXLG; ++L) {
             double *row = &tab[((size_t)L * BOYS_ROWS + i) * BOYS_STRIDE];
             long double fact = 1.0L;
             for (int k = 0; k < BOYS_TERMS; ++k) {
@@ -84,6 +84,25 @@ static void hermite_E(double a, double b, double Ax, double Bx, int la, int lb, 
         for (int j = 0; j < lb; ++j)
             for (int t = 0; t <= i + j + 1; ++t)
                 E.e[i][j + 1][t] = (t > 0 ? h * E.e[i][j][t - 1] : 0.0) + XPB * E.e[i][j][t] + (t + 1) * (t + 1 <= i + j ? E.e[i][j][t + 1] : 0.0);
+}
+
+// dE^{ij}_t/dX_AB at fixed P (X_PA = -(b/p) X_AB, X_PB = (a/p) X_AB, E^{00}_0 = exp(-mu X_AB^2)): the recursion differentiated
+static void hermite_dE(double a, double b, double Ax, double Bx, int la, int lb, const E1D &E, E1D &D) {
+    const double p = a + b, mu = a * b / p;
+    const double Px = (a * Ax + b * Bx) / p;
+    const double XPA = Px - Ax, XPB = Px - Bx, XAB = Ax - Bx, h = 0.5 / p;
+    const double dXPA = -b / p, dXPB = a / p;
+    std::memset(&D, 0, sizeof(D));
+    D.e[0][0][0] = -2.0 * mu * XAB * E.e[0][0][0];
+    for (int i = 0; i < la; ++i)
+        for (int t = 0; t <= i + 1; ++t)
+            D.e[i + 1][0][t] = (t > 0 ? h * D.e[i][0][t - 1] : 0.0) + dXPA * E.e[i][0][t] + XPA * D.e[i][0][t] +
+                               (t + 1) * (t + 1 <= i ? D.e[i][0][t + 1] : 0.0);
+    for (int i = 0; i <= la; ++i)
+        for (int j = 0; j < lb; ++j)
+            for (int t = 0; t <= i + j + 1; ++t)
+                D.e[i][j + 1][t] = (t > 0 ? h * D.e[i][j][t - 1] : 0.0) + dXPB * E.e[i][j][t] + XPB * D.e[i][j][t] +
+                                   (t + 1) * (t + 1 <= i + j ? D.e[i][j][t + 1] : 0.0);
 }
 
 static const int CARTS[3][6][3] = {{{0, 0, 0}},
@@ -398,7 +417,8 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
 
     // ------------------------------------------------------------------ members, products, G matrices
     std::vector<HostMember> members;
-    std::vector<double> G;
+    std::vector<double> G, dG, m_ap;
+    const bool want_grad = opt.gradient != 0;
     std::vector<int64_t> sp_mstart(pairs.size() + 1, 0);
     std::vector<int32_t> sp_i0(pairs.size()), sp_j0(pairs.size()), sp_dims(pairs.size());
     std::vector<int32_t> c_sp, c_ab;
@@ -453,6 +473,16 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
             const double pref = cc * std::pow(M_PI / p, 1.5);
             G.resize(G.size() + (size_t)na * nb * nh, 0.0);
             double *g = G.data() + m.goff;
+            E1D Dx, Dy, Dz;
+            double *dg = nullptr;
+            if (want_grad) {
+                hermite_dE(a, b, A[0], B[0], la, lb, Ex, Dx);
+                hermite_dE(a, b, A[1], B[1], la, lb, Ey, Dy);
+                hermite_dE(a, b, A[2], B[2], la, lb, Ez, Dz);
+                dG.resize(3 * G.size(), 0.0);
+                dg = dG.data() + 3 * m.goff;
+                m_ap.push_back(a / p);
+            }
             for (int ca = 0; ca < NCART[la]; ++ca)
                 for (int cb = 0; cb < NCART[lb]; ++cb) {
                     const int *pa = CARTS[la][ca], *pb = CARTS[lb][cb];
@@ -461,10 +491,21 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
                             for (int v = 0; v <= pa[2] + pb[2]; ++v) {
                                 const double e = pref * Ex.e[pa[0]][pb[0]][t] * Ey.e[pa[1]][pb[1]][u] * Ez.e[pa[2]][pb[2]][v];
                                 const int h = hidx(t, u, v);
+                                double de[3] = {0.0, 0.0, 0.0};
+                                if (want_grad) {
+                                    de[0] = pref * Dx.e[pa[0]][pb[0]][t] * Ey.e[pa[1]][pb[1]][u] * Ez.e[pa[2]][pb[2]][v];
+                                    de[1] = pref * Ex.e[pa[0]][pb[0]][t] * Dy.e[pa[1]][pb[1]][u] * Ez.e[pa[2]][pb[2]][v];
+                                    de[2] = pref * Ex.e[pa[0]][pb[0]][t] * Ey.e[pa[1]][pb[1]][u] * Dz.e[pa[2]][pb[2]][v];
+                                }
                                 for (int x = 0; x < na; ++x) {
                                     if (Ta[x][ca] == 0.0) continue;
                                     for (int y = 0; y < nb; ++y)
-                                        if (Tb[y][cb] != 0.0) g[(size_t)(x * nb + y) * nh + h] += Ta[x][ca] * Tb[y][cb] * e;
+                                        if (Tb[y][cb] != 0.0) {
+                                            const double w = Ta[x][ca] * Tb[y][cb];
+                                            g[(size_t)(x * nb + y) * nh + h] += w * e;
+                                            if (want_grad)
+                                                for (int d = 0; d < 3; ++d) dg[((size_t)(x * nb + y) * 3 + d) * nh + h] += w * de[d];
+                                        }
                                 }
                             }
                 }
@@ -525,7 +566,8 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         for (int64_t i = 0; i < c.npad; ++i) {
             // padding repeats the last product: it never carries density (D = 0) and its sums are never read
             const HostProd &q = prods[order[first + std::min(i, n - 1)]];
-            pa[i] = make_double4(q.x, q.y, q.z, tfar(L) * (1.0 / q.p + izmin2));
+            // far-field radius for one order more than L, so that pcm_gradient (orders 0..L+1) can share the patch maps
+            pa[i] = make_double4(q.x, q.y, q.z, tfar(L + 1) * (1.0 / q.p + izmin2));
             pb[i] = make_double2(q.p, 2.0 * std::sqrt(q.p / M_PI));
             double *bx = &box[(size_t)(i / 32) * 7];
             if (i % 32 == 0) { for (int d = 0; d < 3; ++d) { bx[d] = 1e300; bx[3 + d] = -1e300; } bx[6] = 0.0; }
@@ -577,6 +619,42 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
     if ((rc = upload(ctx, &ctx->sp_dims, sp_dims))) return rc;
     if ((rc = upload(ctx, &ctx->c_sp, c_sp))) return rc;
     if ((rc = upload(ctx, &ctx->c_ab, c_ab))) return rc;
+    ctx->nshell = nshell;
+    if (want_grad) {
+        std::vector<int32_t> shI(pairs.size()), shJ(pairs.size());
+        std::vector<int64_t> cstart(pairs.size() + 1, 0), sh_start((size_t)nshell + 1, 0);
+        for (size_t sp = 0; sp < pairs.size(); ++sp) {
+            shI[sp] = pairs[sp].I; shJ[sp] = pairs[sp].J;
+            cstart[sp + 1] = cstart[sp] + (sp_dims[sp] & 0xff) * ((sp_dims[sp] >> 8) & 0xff);
+            sh_start[pairs[sp].I + 1] += 1;
+            sh_start[pairs[sp].J + 1] += 1;   // a diagonal shell pair is listed as bra and as ket of its shell
+        }
+        for (int sidx = 0; sidx < nshell; ++sidx) sh_start[sidx + 1] += sh_start[sidx];
+        std::vector<int32_t> sh_list((size_t)std::max<int64_t>(sh_start[nshell], 1), 0);
+        {
+            std::vector<int64_t> fill(sh_start.begin(), sh_start.end() - 1);
+            for (size_t sp = 0; sp < pairs.size(); ++sp) {
+                sh_list[fill[pairs[sp].I]++] = (int32_t)(2 * sp);
+                sh_list[fill[pairs[sp].J]++] = (int32_t)(2 * sp + 1);
+            }
+        }
+        std::vector<int32_t> hshift((size_t)3 * nherm(MAXL), 0);
+        for (int t = 0; t <= MAXL; ++t)
+            for (int u = 0; t + u <= MAXL; ++u)
+                for (int v = 0; t + u + v <= MAXL; ++v) {
+                    hshift[0 * nherm(MAXL) + hidx(t, u, v)] = hidx(t + 1, u, v);
+                    hshift[1 * nherm(MAXL) + hidx(t, u, v)] = hidx(t, u + 1, v);
+                    hshift[2 * nherm(MAXL) + hidx(t, u, v)] = hidx(t, u, v + 1);
+                }
+        if ((rc = upload(ctx, &ctx->dG, dG))) return rc;
+        if ((rc = upload(ctx, &ctx->m_ap, m_ap))) return rc;
+        if ((rc = upload(ctx, &ctx->sp_shI, shI))) return rc;
+        if ((rc = upload(ctx, &ctx->sp_shJ, shJ))) return rc;
+        if ((rc = upload(ctx, &ctx->sp_cstart, cstart))) return rc;
+        if ((rc = upload(ctx, &ctx->sh_start, sh_start))) return rc;
+        if ((rc = upload(ctx, &ctx->sh_list, sh_list))) return rc;
+        if ((rc = upload(ctx, &ctx->hshift, hshift))) return rc;
+    }
     return PCM_OK;
 }
 
