@@ -221,7 +221,7 @@ def run_ours(args):
     w = synth.make_workload(CONFIG_INDEX)
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
-    ctx = pcm.setup_from_workload(w.basis, w.surface)
+    ctx = pcm.setup_from_workload(w.basis, w.surface, gradient=True)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t0
     info = pcm.pcm_get_info(ctx)
@@ -248,7 +248,7 @@ def run_ours(args):
     peak_tflops = pcm.pcm_fp64_peak(ctx, 10)
 
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
-    cls_pot, cls_fock, main_ms = [], [], []
+    cls_pot, cls_fock, main_ms, cg_mv = [], [], [], []
     sampler = ClockSampler(local)
     if dist is not None:
         dist.barrier()
@@ -271,6 +271,7 @@ def run_ours(args):
         cls_pot.append(pcm.pcm_last_class_ms(ctx, pcm.OP_POTENTIAL))
         cls_fock.append(pcm.pcm_last_class_ms(ctx, pcm.OP_FOCK))
         main_ms.append((pcm.pcm_last_kernel_ms(ctx, pcm.OP_POTENTIAL), pcm.pcm_last_kernel_ms(ctx, pcm.OP_FOCK)))
+        cg_mv.append(pcm.pcm_last_cg_matvec_ms(ctx)[0])
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
     launches = pcm.pcm_launch_count(ctx) - launches0
@@ -297,13 +298,23 @@ def run_ours(args):
     mean = lambda xs: float(sum(xs) / len(xs))
     cp = [mean([c[L] for c in cls_pot]) for L in range(5)]
     cf = [mean([c[L] for c in cls_fock]) for L in range(5)]
-    # dominant kernel = the (op, L) launch with the largest average device time
-    cands = [("potential", L, cp[L]) for L in range(5)] + [("fock", L, cf[L]) for L in range(5)]
-    op, Ld, ms_dom = max(cands, key=lambda c: c[2])
-    n_units = float(info.products[Ld]) * M
+    # dominant kernel = the kernel with the largest share of the step's device time (launch time x launches per step):
+    # the A q sweep of the CG iterations (timed per launch inside pcm_cg_solve, main + concurrent near kernel) or one
+    # of the integral kernels (one launch per step each)
+    mv_ms = mean(cg_mv)
+    cands = [("potential", L, cp[L], 1) for L in range(5)] + [("fock", L, cf[L], 1) for L in range(5)]
+    cands.append(("amatvec", 0, mv_ms, int(iters) + 1))
+    op, Ld, ms_dom, per_step = max(cands, key=lambda c: c[2] * c[3])
+    n_units = 0.5 * float(M) * M if op == "amatvec" else float(info.products[Ld]) * M
     instr, flop = WORK[op][Ld]
     achieved = n_units * flop / (ms_dom * 1e-3) * 1e-12
-    roofline = {"bound": "alu", "kernel": f"{op}_kernel<L={Ld}>", "achieved": achieved, "peak": peak_tflops,
+    kernels = {f"{o}_L{L}": {"ms_per_launch": ms, "launches_per_step": n,
+                             "frac": (0.5 * float(M) * M if o == "amatvec" else float(info.products[L]) * M) * WORK[o][L][1] / (ms * 1e-3) * 1e-12 / peak_tflops}
+               for (o, L, ms, n) in cands if ms > 0.01}
+    roofline = {"bound": "alu", "kernel": ("amatvec_kernel (CG iteration, M = %d; unit = pair evaluation of the symmetric sweep)" % M)
+                if op == "amatvec" else f"{op}_kernel<L={Ld}>", "launches_per_step": per_step,
+                "share_of_step": ms_dom * per_step / ms_per_step, "all_hot_kernels": kernels,
+                "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
                 "fp64_pipe_frac": n_units * instr * 2.0 / (ms_dom * 1e-3) * 1e-12 / peak_tflops,
                 "units_per_launch": n_units, "flop_per_unit": flop, "fp64_instr_per_unit": instr, "ms_per_launch": ms_dom,
@@ -348,6 +359,30 @@ def run_ours(args):
     line["e2e"] = {"value": world * units_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
                    "h2d_bytes_per_step": int(nbf * nbf * 8 + 2 * M * 8), "d2h_bytes_per_step": int(nbf * nbf * 8 + 2 * M * 8),
                    "api": "pcm_potential_host + pcm_rbj_build + pcm_cg_solve_host + pcm_fock_host"}
+
+    # ---- SURVEY 8(f) rows built so far, timed outside the step: the PCM gradient term (Eq. 14/22) and the glue of Eq. 1/4/13
+    ge = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    pcm.pcm_set_nuclei(ctx, w.atom_xyz, synth.nuclear_charges(w.elements))
+    f_eps = (78.39 - 1.0) / 78.39
+    gms, glue_ms = [], []
+    for k in range(3 + 5):
+        flush.zero_()
+        ge[0].record(stream)
+        pcm.pcm_gradient(ctx, P, q, stream=stream)
+        ge[1].record(stream)
+        u = pcm.pcm_nuclear_potential(ctx, stream=stream)
+        b = pcm.pcm_rhs(ctx, u, v, f_eps, stream=stream)
+        ge[2].record(stream)
+        en = pcm.pcm_energy(ctx, u, v, q, f_eps, stream=stream)
+        ge[3].record(stream)
+        torch.cuda.synchronize()
+        if k >= 3:
+            gms.append(ge[0].elapsed_time(ge[1]))
+            glue_ms.append((ge[1].elapsed_time(ge[2]), ge[2].elapsed_time(ge[3])))
+    line["gradient"] = {"ms": min(gms), "ms_median": statistics.median(gms), "prim_pair_point_per_s": info.prim_pair_points / (min(gms) * 1e-3),
+                        "note": "pcm_gradient: Fock sweep at Hermite order L+1 and a three-accumulator point sweep; not part of the step"}
+    line["glue"] = {"bz_plus_rhs_ms": min(g[0] for g in glue_ms), "energy_ms": min(g[1] for g in glue_ms),
+                    "energy_hartree": float(en[3])}
 
     # ---- A q sweep of configs[4] (BASELINE metric: A q FP64 fraction; HBM GB/s reported as asked)
     if not args.no_sweep:
@@ -400,7 +435,7 @@ def run_kernels(args):
     torch.cuda.set_device(0)
     pcm.lib()
     w = synth.make_workload(args.config)
-    ctx = pcm.setup_from_workload(w.basis, w.surface)
+    ctx = pcm.setup_from_workload(w.basis, w.surface, gradient=True)
     s4, q4, _ = synth.make_solver_points(args.amat_m)
     c4 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s4.xyz, s4.zeta, s4.switch)
     dev = torch.device("cuda", 0)
@@ -409,13 +444,18 @@ def run_kernels(args):
     qd = torch.as_tensor(q4, dtype=torch.float64, device=dev)
     for c in (ctx, c4):
         pcm.pcm_set_timing(c, True)
-    out = {"potential_ms": [], "fock_ms": [], "amatvec_ms": [], "potential_by_L": None, "fock_by_L": None}
+    out = {"potential_ms": [], "fock_ms": [], "amatvec_ms": [], "gradient_ms": [], "potential_by_L": None, "fock_by_L": None}
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for k in range(args.warmup + args.steps):
         pcm.pcm_potential(ctx, P)
         pcm.pcm_fock(ctx, q)
         pcm.pcm_amatvec(c4, qd)
+        e0.record()
+        pcm.pcm_gradient(ctx, P, q)
+        e1.record()
         torch.cuda.synchronize()
         if k >= args.warmup:
+            out["gradient_ms"].append(e0.elapsed_time(e1))
             out["potential_ms"].append(sum(pcm.pcm_last_kernel_ms(ctx, pcm.OP_POTENTIAL)[:2]))
             out["fock_ms"].append(sum(pcm.pcm_last_kernel_ms(ctx, pcm.OP_FOCK)[:2]))
             out["amatvec_ms"].append(sum(pcm.pcm_last_kernel_ms(c4, pcm.OP_AMATVEC)[:2]))

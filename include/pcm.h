@@ -56,7 +56,10 @@ typedef struct pcm_options {
     int merge_products;    /* 1 (default): primitive pairs with identical (A, alpha, B, beta) -- e.g. the s and p
                               parts of an sp shell -- share one Hermite Gaussian product in the kernels (exact) */
     int gradient;          /* 1: also build what pcm_gradient needs (derivative tables, 3x the G matrices); default 0 */
-    int reserved[3];
+    int store_near;        /* 1 (default): the patches of A that are not in the far field (the entries that need erf) are
+                              evaluated once at pcm_setup and kept on the device (8 KB per 32 x 32 patch, up to 16 GB; beyond
+                              that, or with 0, they are re-evaluated in every pcm_amatvec).  Same values either way. */
+    int reserved[2];
 } pcm_options;
 
 typedef struct pcm_info {
@@ -231,6 +234,11 @@ int pcm_get_info(pcm_ctx *ctx, pcm_info *out);
 int pcm_set_timing(pcm_ctx *ctx, int enable);
 int pcm_last_kernel_ms(pcm_ctx *ctx, int op, double ms[2], int *n_launch);
 int pcm_last_class_ms(pcm_ctx *ctx, int op, double ms[PCM_NL]);
+
+/* pcm_last_cg_matvec_ms -- with timing on: mean device time of the A q launches (main + near kernels) of the first
+ * 16 iterations of the most recent pcm_cg_solve, and how many were timed (n may be NULL).  Note that queued iterations
+ * after convergence are no-ops; only solves of >= 16 iterations give the figure of a working iteration. */
+int pcm_last_cg_matvec_ms(pcm_ctx *ctx, double *avg_ms, int *n);
 
 /* pcm_launch_count -- kernels launched by this context since pcm_setup (bench.py's gpu_launches). */
 int pcm_launch_count(pcm_ctx *ctx, int64_t *total);

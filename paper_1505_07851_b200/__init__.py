@@ -30,14 +30,14 @@ EXPORTS = (
     "pcm_rbj_build", "pcm_rbj_get", "pcm_cg_solve", "pcm_potential_host", "pcm_fock_host", "pcm_amatvec_host",
     "pcm_cg_solve_host", "pcm_get_info", "pcm_set_timing", "pcm_last_kernel_ms", "pcm_last_class_ms",
     "pcm_launch_count", "pcm_fp64_peak", "pcm_set_nuclei", "pcm_nuclear_potential", "pcm_rhs", "pcm_energy",
-    "pcm_cg_threshold", "pcm_gradient",
+    "pcm_cg_threshold", "pcm_gradient", "pcm_last_cg_matvec_ms",
     "pcm_schwarz_bound", "pcm_last_error", "pcm_destroy",
 )
 
 
 class pcm_options(C.Structure):
     _fields_ = [("screen_eps", C.c_double), ("d_pure", C.c_int), ("device", C.c_int), ("merge_products", C.c_int),
-                ("gradient", C.c_int), ("reserved", C.c_int * 3)]
+                ("gradient", C.c_int), ("store_near", C.c_int), ("reserved", C.c_int * 2)]
 
 
 class pcm_info(C.Structure):
@@ -92,6 +92,7 @@ def lib(build: bool = False):
         L.pcm_last_kernel_ms.argtypes = [vp, C.c_int, _dp, _ip]
         L.pcm_last_class_ms.argtypes = [vp, C.c_int, _dp]
         L.pcm_launch_count.argtypes = [vp, _lp]
+        L.pcm_last_cg_matvec_ms.argtypes = [vp, _dp, _ip]
         L.pcm_fp64_peak.argtypes = [vp, C.c_int, _dp]
         L.pcm_set_nuclei.argtypes = [vp, C.c_int, vp, vp]
         L.pcm_nuclear_potential.argtypes = [vp, vp, vp]
@@ -166,7 +167,7 @@ def pcm_options_default() -> pcm_options:
 
 def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_zeta, pt_switch=None, *,
               screen_eps: float = 1e-12, d_pure: bool = True, device: int = -1, merge_products: bool = True,
-              gradient: bool = False) -> Context:
+              gradient: bool = False, store_near: bool = True) -> Context:
     """Host numpy arrays in, context out (include/pcm.h: pcm_setup)."""
     import torch
     if not torch.cuda.is_available():
@@ -188,6 +189,7 @@ def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_z
     opt.device = int(device)
     opt.merge_products = 1 if merge_products else 0
     opt.gradient = 1 if gradient else 0
+    opt.store_near = 1 if store_near else 0
     h = C.c_void_p()
     rc = lib().pcm_setup(C.byref(h), len(sl), _hp(sl), _hp(sx), _hp(sn), _hp(pe), _hp(pc), len(pz), _hp(px), _hp(pz),
                          _hp(ps), C.byref(opt))
@@ -384,6 +386,13 @@ def pcm_last_class_ms(ctx: Context, op: int):
     ms = (C.c_double * PCM_NL)()
     _check(lib().pcm_last_class_ms(ctx.handle, int(op), ms), ctx.handle)
     return [float(x) for x in ms]
+
+
+def pcm_last_cg_matvec_ms(ctx: Context):
+    """(mean ms of the first <= 16 A q launches of the last timed pcm_cg_solve, how many)"""
+    ms, n = C.c_double(0.0), C.c_int(0)
+    _check(lib().pcm_last_cg_matvec_ms(ctx.handle, C.byref(ms), C.byref(n)), ctx.handle)
+    return ms.value, n.value
 
 
 def pcm_launch_count(ctx: Context) -> int:

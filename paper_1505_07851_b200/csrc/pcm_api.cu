@@ -29,6 +29,7 @@ void pcm_options_default(pcm_options *opt) {
     opt->device = -1;
     opt->merge_products = 1;
     opt->gradient = 0;
+    opt->store_near = 1;
 }
 
 static void free_ctx(pcm_ctx *ctx) {
@@ -39,6 +40,7 @@ static void free_ctx(pcm_ctx *ctx) {
     if (ctx->io_a) cudaFree(ctx->io_a);
     if (ctx->io_b) cudaFree(ctx->io_b);
     for (auto &e : ctx->ev) if (e) cudaEventDestroy(e);
+    for (auto &e : ctx->cg_ev) if (e) cudaEventDestroy(e);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->near_stream) cudaStreamDestroy(ctx->near_stream);
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -106,6 +108,11 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
         if (e != cudaSuccess) { ctx->err = std::string("cudaEventCreate: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
     }
 
+    for (auto &ev : ctx->cg_ev) {
+        e = cudaEventCreate(&ev);
+        if (e != cudaSuccess) { ctx->err = std::string("cudaEventCreate: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    }
+
     int rc = build_context(ctx, nshell, shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, npoint, pt_xyz, pt_zeta, pt_switch);
     if (rc) return fail(rc);
 
@@ -122,6 +129,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     }
     ctx->ypart_slots = ctx->plan_amat.chunks;
     if ((rc = dev_alloc_t(ctx, &ctx->near_amat, (size_t)ctx->amat_map.npiece * 32))) return fail(rc);
+    if ((rc = fill_amat_blocks(ctx))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->vpart, (size_t)std::max<int64_t>(ctx->vpart_slots, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->ypart, (size_t)ctx->ypart_slots * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->colpart, (size_t)std::max<int64_t>(ctx->plan_amat.xb, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
@@ -395,6 +403,22 @@ int pcm_last_class_ms(pcm_ctx *ctx, int op, double ms[PCM_NL]) {
         PCM_CUDA(ctx, cudaEventElapsedTime(&t, ev[1 + L], ev[2 + L]));
         ms[L] = t;
     }
+    return PCM_OK;
+}
+
+int pcm_last_cg_matvec_ms(pcm_ctx *ctx, double *avg_ms, int *n) {
+    PCM_CHECK_CTX(ctx);
+    if (!avg_ms) return set_error(ctx, PCM_ERR_ARG, "pcm_last_cg_matvec_ms: avg_ms is NULL");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    double sum = 0.0;
+    for (int i = 0; i < ctx->cg_ev_n; ++i) {
+        float t = 0;
+        PCM_CUDA(ctx, cudaEventSynchronize(ctx->cg_ev[2 * i + 1]));
+        PCM_CUDA(ctx, cudaEventElapsedTime(&t, ctx->cg_ev[2 * i], ctx->cg_ev[2 * i + 1]));
+        sum += t;
+    }
+    *avg_ms = ctx->cg_ev_n ? sum / ctx->cg_ev_n : 0.0;
+    if (n) *n = ctx->cg_ev_n;
     return PCM_OK;
 }
 

@@ -160,6 +160,7 @@ struct pcm_ctx {
     double *vpart = nullptr;    // potential partial sums [slots][M]
     int64_t vpart_slots = 0;
     double *near_amat = nullptr;  // [amat_map.npiece][32] sums of the near pieces
+    double *amat_blocks = nullptr;  // [amat_map.nnear][32][32] stored near patches of A (nullptr: evaluated on the fly)
     double *ypart = nullptr;    // amatvec row partial sums [slots][M]
     int64_t ypart_slots = 0;
     double *colpart = nullptr;  // amatvec column partial sums of the symmetric sweep [plan_amat.xb][M]
@@ -186,6 +187,10 @@ struct pcm_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     // events: 0 start, 1 after the pre-transform, 2+L after the class-L main kernel, 7 end, 8 CG residual read-back
     cudaEvent_t ev[28] = {};   // ev[8*op + i], op = 0 potential, 1 fock, 2 amatvec; 24 CG; 25, 26 peak benchmark
+    // CG: events around the A q launches (main + near kernels) of the first CG_EV iterations of the last timed solve
+    static constexpr int CG_EV = 16;
+    cudaEvent_t cg_ev[2 * CG_EV] = {};
+    int cg_ev_n = 0;
     int timing = 0;
     int cur_op = 0;
     int launches[3] = {0, 0, 0};   // kernels launched by the last call of each op
@@ -214,6 +219,7 @@ int launch_rhs(pcm_ctx *ctx, const double *u, const double *v, double f, double 
 int energy_terms(pcm_ctx *ctx, const double *u, const double *v, const double *q, double f, double *terms_host, cudaStream_t s);
 int launch_gradient(pcm_ctx *ctx, const double *P, int64_t ldp, const double *q, double *g_shell, double *g_point, cudaStream_t s);
 int plan_all(pcm_ctx *ctx);
+int fill_amat_blocks(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
 void build_boys_tables(std::vector<double> &tab);
 double schwarz_bound(int la, double alpha, const double *A, int lb, double beta, const double *B);

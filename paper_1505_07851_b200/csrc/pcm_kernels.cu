@@ -307,6 +307,70 @@ __global__ void __launch_bounds__(TPB) amat_near_kernel(const double4 *__restric
     near[piece * SUB + lane] = y;
 }
 
+// Stored near field (the paper stores all of A; here only the patches that are not far are kept, which is
+// what fits and what pays: they are the entries that need erf).  A depends on the geometry only, so pcm_setup evaluates
+// every listed patch once -- with the same arithmetic as amat_near_kernel -- into blocks[e][t][lane] = A(row lane of the
+// row group, column t of column group list[e]); entries of rows or columns beyond M are 0.
+__global__ void __launch_bounds__(TPB) amat_near_fill_kernel(const double4 *__restrict__ pt, const double *__restrict__ diag, int M,
+                                                             const int64_t *__restrict__ start, const int32_t *__restrict__ list,
+                                                             const int64_t *__restrict__ pstart, const int32_t *__restrict__ piece_rg,
+                                                             int64_t npiece, double *__restrict__ blocks,
+                                                             const double *__restrict__ boys0, double thr) {
+    __shared__ double4 s_pt[TPB / 32][SUB];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
+    if (piece >= npiece) return;
+    const int64_t rg = piece_rg[piece];
+    const int i = (int)rg * SUB + lane;
+    const double4 a = pt[min(i, M - 1)];
+    const int thr_hi = hi32(thr);
+    const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
+    for (int64_t e = ebeg; e < eend; ++e) {
+        const int j0 = list[e] * SUB, j = j0 + lane;
+        __syncwarp();
+        s_pt[warp][lane] = pt[min(j, M - 1)];
+        __syncwarp();
+        double *blk = blocks + (size_t)e * (SUB * SUB);
+        for (int t = 0; t < SUB; ++t) {
+            const double4 b = s_pt[warp][t];
+            const double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            double ev;
+            if (i >= M || j0 + t >= M) ev = 0.0;
+            else if (hi32(r2) > thr_hi) ev = rsqrt_fast(r2);
+            else ev = (j0 + t == i) ? diag[i] : amat_general(r2, a.w, b.w, boys0);
+            blk[t * SUB + lane] = ev;
+        }
+    }
+}
+
+// near pieces of A q from the stored blocks: one warp per piece, lane = row; near[piece][lane] = sum over the piece's
+// patches (in list order) of sum_t A(lane, t) q_t (t ascending) -- the order amat_near_kernel uses
+__global__ void __launch_bounds__(TPB) amat_near_stored_kernel(const double *__restrict__ blocks, const double *__restrict__ q,
+                                                               const int32_t *__restrict__ qidx, int M,
+                                                               const int64_t *__restrict__ start, const int32_t *__restrict__ list,
+                                                               const int64_t *__restrict__ pstart, const int32_t *__restrict__ piece_rg,
+                                                               int64_t npiece, double *__restrict__ near, const int *__restrict__ stop) {
+    if (stop && *stop) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
+    if (piece >= npiece) return;
+    const int64_t rg = piece_rg[piece];
+    const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
+    double y = 0.0;
+    for (int64_t e = ebeg; e < eend; ++e) {
+        const int j = list[e] * SUB + lane;
+        const double qj = j < M ? q[qidx ? qidx[j] : j] : 0.0;
+        const double *blk = blocks + (size_t)e * (SUB * SUB) + lane;
+        double a[SUB];
+#pragma unroll
+        for (int t = 0; t < SUB; ++t) a[t] = __ldg(blk + t * SUB);
+#pragma unroll
+        for (int t = 0; t < SUB; ++t) y = fma(__shfl_sync(0xffffffffu, qj, t), a[t], y);
+    }
+    near[piece * SUB + lane] = y;
+}
+
 // sums of the near pieces, per class: near[c][piece][lane], pieces of row group rg = pstart[c][rg] .. pstart[c][rg+1]
 struct NearRefs {
     const double *near[MAXL + 1];
@@ -814,8 +878,12 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
     if (pm.npiece > 0) {
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
         PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->near_stream, ctx->ev_fork, 0));
-        amat_near_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, ctx->near_stream>>>(
-            ctx->pt, ctx->pt_diag, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, ctx->boys, thr, stop);
+        if (ctx->amat_blocks)
+            amat_near_stored_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, ctx->near_stream>>>(
+                ctx->amat_blocks, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, stop);
+        else
+            amat_near_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, ctx->near_stream>>>(
+                ctx->pt, ctx->pt_diag, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, ctx->boys, thr, stop);
         PCM_LAUNCH_CHECK(ctx);
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
         { ctx->launches[2]++; ctx->launch_total++; }
@@ -827,6 +895,22 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[2]++; ctx->launch_total++; }
     if (pm.npiece > 0) PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
+    return PCM_OK;
+}
+// evaluates the near patches of A once (pcm_setup), if they fit the budget
+int fill_amat_blocks(pcm_ctx *ctx) {
+    const PatchMap &pm = ctx->amat_map;
+    ctx->amat_blocks = nullptr;
+    double budget_gb = 16.0;
+    if (const char *e = getenv("PCM_NEAR_STORE_GB")) budget_gb = atof(e);
+    const double need = (double)pm.nnear * SUB * SUB * 8.0;
+    if (ctx->opt.store_near == 0 || pm.npiece == 0 || need > budget_gb * 1e9) return PCM_OK;
+    int rc = dev_alloc_t(ctx, &ctx->amat_blocks, (size_t)pm.nnear * SUB * SUB);
+    if (rc) return rc;
+    const double thr = TFAR_AMAT * 2.0 / (ctx->zeta_min * ctx->zeta_min);
+    amat_near_fill_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB>>>(ctx->pt, ctx->pt_diag, (int)ctx->M, pm.start, pm.list, pm.pstart,
+                                                                           pm.piece_rg, pm.npiece, ctx->amat_blocks, ctx->boys, thr);
+    PCM_LAUNCH_CHECK(ctx);
     return PCM_OK;
 }
 int launch_amatvec_partials(pcm_ctx *ctx, const double *q_sorted, const int *stop, cudaStream_t s) {

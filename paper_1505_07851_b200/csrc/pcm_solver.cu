@@ -735,6 +735,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     int rc;
     const int saved_timing = ctx->timing;
     ctx->timing = 0;
+    ctx->cg_ev_n = 0;
     const unsigned gb = (unsigned)cdiv(M, 256);
 #define CG_TRY(expr) do { rc = (expr); if (rc) { ctx->timing = saved_timing; return rc; } } while (0)
 #define CG_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { ctx->timing = saved_timing; \
@@ -778,7 +779,10 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         rr = h[2];
         if (hc[CTL_STOP]) break;
         for (int k = 0; k < batch; ++k) {
+            const bool ev = saved_timing && ctx->cg_ev_n < pcm_ctx::CG_EV;
+            if (ev) CG_CUDA(cudaEventRecord(ctx->cg_ev[2 * ctx->cg_ev_n], s));
             CG_TRY(launch_amatvec_partials(ctx, p, ctl, s));
+            if (ev) { CG_CUDA(cudaEventRecord(ctx->cg_ev[2 * ctx->cg_ev_n + 1], s)); ctx->cg_ev_n++; }
             cg_matvec_reduce_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, amat_parts(ctx), p, Ap, scal, scal + 16, ctl);
             ctx->launch_total += 1;
             CG_TRY(update(0));

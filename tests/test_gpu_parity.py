@@ -257,6 +257,11 @@ def test_amatvec_parity(pcm, orc, torch_cuda, M):
     col = pcm.pcm_amatvec(ctx, dev(torch_cuda, e)).cpu().numpy()
     ref = np.array([orc.a_entry(s, i, M // 2) for i in range(M)])
     assert_parity(col, ref, f"A column, M = {M}")
+    # the near patches stored at setup (default) and re-evaluated in every call give the same bits
+    ctx2 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s.xyz, s.zeta, s.switch,
+                         store_near=False)
+    np.testing.assert_array_equal(pcm.pcm_amatvec(ctx2, dev(torch_cuda, q)).cpu().numpy(), y)
+    pcm.pcm_destroy(ctx2)
 
 
 def test_amatvec_coincident_and_mixed_exponents(pcm, orc, torch_cuda):
@@ -270,3 +275,6 @@ def test_amatvec_coincident_and_mixed_exponents(pcm, orc, torch_cuda):
     y = pcm.pcm_amatvec(ctx, dev(torch_cuda, q)).cpu().numpy()
     assert np.isfinite(y).all()
     assert_parity(y, orc.amatvec(s, q), "A q with coincident points and zeta from 0.2 to 30")
+    ctx2 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s.xyz, s.zeta, s.switch,
+                         store_near=False)
+    np.testing.assert_array_equal(pcm.pcm_amatvec(ctx2, dev(torch_cuda, q)).cpu().numpy(), y)
