@@ -134,6 +134,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     if ((rc = dev_alloc_t(ctx, &ctx->ypart, (size_t)ctx->ypart_slots * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->colpart, (size_t)std::max<int64_t>(ctx->plan_amat.xb, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->cg_vec, (size_t)6 * std::max<int64_t>(M, 1)))) return fail(rc);
+    if ((rc = dev_alloc_t(ctx, &ctx->cg_part, (size_t)(M / 32 + 2)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->cg_scal, (size_t)1024))) return fail(rc);
     e = cudaMemset(ctx->cg_scal, 0, 1024 * 8);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->cg_scal_host, 64 * sizeof(double));

@@ -29,18 +29,30 @@ struct AmatParts {
     const int64_t *pstart;
     int slots, chunk_len, RB, tile;
 };
-__device__ __forceinline__ double amat_row_sum(const AmatParts &a, int M, int k) {
-    const int r0 = k / a.RB * a.RB;
+// A 256-thread block sums the rows k0 .. k0+31: warp `part` (0..7) of the block adds, for row k0 + lane, every 8th term
+// of each of the three lists (coalesced across the lanes), the eight partial sums are then added in order by warp 0.
+// Returns the row sum in the threads of warp 0 (0.0 for rows >= M); s_tmp: shared, 8 * 32 doubles; all 256 threads call.
+constexpr int AMAT_RED_PARTS = 8;
+__device__ __forceinline__ double amat_row_sum_block(const AmatParts &a, int M, int k0, double *s_tmp) {
+    const int lane = threadIdx.x & 31, part = threadIdx.x >> 5;
+    const int k = k0 + lane;
     double s = 0.0;
-    for (int c = r0 / a.chunk_len; c < a.slots; ++c) s += a.ypart[(size_t)c * M + k];
-    const int nsym = (k / a.tile * a.tile) / a.RB;
-    double u = 0.0;
-    for (int rb = 0; rb < nsym; ++rb) u += a.colpart[(size_t)rb * M + k];
-    s += u;
-    const int64_t rg = k / 32;
+    if (k < M) {
+        const int r0 = k / a.RB * a.RB;
+        for (int c = r0 / a.chunk_len + part; c < a.slots; c += AMAT_RED_PARTS) s += a.ypart[(size_t)c * M + k];
+        const int nsym = (k / a.tile * a.tile) / a.RB;
+        for (int rb = part; rb < nsym; rb += AMAT_RED_PARTS) s += a.colpart[(size_t)rb * M + k];
+        const int64_t rg = k / 32;
+        for (int64_t e = a.pstart[rg] + part; e < a.pstart[rg + 1]; e += AMAT_RED_PARTS) s += a.near[e * 32 + lane];
+    }
+    s_tmp[part * 32 + lane] = s;
+    __syncthreads();
     double t = 0.0;
-    for (int64_t e = a.pstart[rg]; e < a.pstart[rg + 1]; ++e) t += a.near[e * 32 + (k & 31)];
-    return s + t;
+    if (part == 0) {
+#pragma unroll
+        for (int q = 0; q < AMAT_RED_PARTS; ++q) t += s_tmp[q * 32 + lane];
+    }
+    return t;
 }
 
 AmatParts amat_parts(const pcm_ctx *ctx);  // pcm_kernels.cu

@@ -166,6 +166,7 @@ struct pcm_ctx {
     double *colpart = nullptr;  // amatvec column partial sums of the symmetric sweep [plan_amat.xb][M]
     int amat_R = 4;             // row groups per warp of the A q kernel (row block = 128 amat_R points)
     double *cg_vec = nullptr;   // 6 M doubles: r, z, p, Ap, x, b (sorted point order)
+    double *cg_part = nullptr;  // [ceil(M/32)] per-CTA partial dot products of cg_matvec_reduce_kernel
     double *cg_scal = nullptr;  // device scalars
     double *cg_scal_host = nullptr;  // pinned
     double *io_a = nullptr, *io_b = nullptr;  // staging for the *_host calls

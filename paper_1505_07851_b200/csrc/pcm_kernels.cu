@@ -394,10 +394,11 @@ __global__ void reduce_slots_kernel(const double *__restrict__ part, int64_t n, 
 }
 
 // y[idx ? idx[k] : k] = the partial sums of row k of the symmetric A q sweep, in amat_row_sum's fixed order
-__global__ void amat_reduce_kernel(AmatParts parts, int M, double *__restrict__ out, const int32_t *__restrict__ idx) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= M) return;
-    out[idx ? idx[k] : k] = amat_row_sum(parts, M, k);
+__global__ void __launch_bounds__(256) amat_reduce_kernel(AmatParts parts, int M, double *__restrict__ out, const int32_t *__restrict__ idx) {
+    __shared__ double s_tmp[AMAT_RED_PARTS * 32];
+    const double t = amat_row_sum_block(parts, M, blockIdx.x * 32, s_tmp);
+    const int k = blockIdx.x * 32 + threadIdx.x;
+    if (threadIdx.x < 32 && k < M) out[idx ? idx[k] : k] = t;
 }
 AmatParts amat_parts(const pcm_ctx *ctx) {
     AmatParts a;
@@ -932,7 +933,7 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
     if ((rc = launch_amatvec_kernels(ctx, q, idx, nullptr, s))) return rc;
     for (int i = 2; i <= 6; ++i)
         if ((rc = mark(ctx, i, s))) return rc;
-    amat_reduce_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(amat_parts(ctx), M, y, idx);
+    amat_reduce_kernel<<<(unsigned)ceil_div(M, 32), 256, 0, s>>>(amat_parts(ctx), M, y, idx);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return mark(ctx, 7, s);

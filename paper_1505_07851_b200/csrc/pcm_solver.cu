@@ -347,22 +347,25 @@ __device__ __forceinline__ double ordered_sum(const double *partial, int n) {
     return block_sum(s);
 }
 
-// Ap = sum of the A q partial-sum slots + near pieces (sorted order), pAp = p.Ap
+// Ap = sum of the A q partial sums (sorted order), pAp = p.Ap.  One CTA per 32 rows (amat_row_sum_block); the per-CTA
+// dot products go to partial[blockIdx.x], the last CTA adds them in index order.
 __global__ void __launch_bounds__(DOT_THREADS) cg_matvec_reduce_kernel(int M, AmatParts parts,
                                                                        const double *__restrict__ p, double *__restrict__ Ap,
                                                                        double *__restrict__ scal, double *__restrict__ partial,
                                                                        int *__restrict__ ctl) {
+    __shared__ double s_tmp[AMAT_RED_PARTS * 32];
     if (*((volatile int *)&ctl[CTL_STOP])) return;
-    double dot = 0.0;
-    for (int k = blockIdx.x * DOT_THREADS + threadIdx.x; k < M; k += DOT_BLOCKS * DOT_THREADS) {
-        const double s = amat_row_sum(parts, M, k);
-        Ap[k] = s;
-        dot = fma(p[k], s, dot);
+    const double t = amat_row_sum_block(parts, M, blockIdx.x * 32, s_tmp);
+    const int k = blockIdx.x * 32 + threadIdx.x;
+    if (threadIdx.x < 32) {
+        double dot = 0.0;
+        if (k < M) { Ap[k] = t; dot = p[k] * t; }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) dot += __shfl_down_sync(0xffffffffu, dot, o);
+        if (threadIdx.x == 0) partial[blockIdx.x] = dot;
     }
-    dot = block_sum(dot);
-    if (threadIdx.x == 0) partial[blockIdx.x] = dot;
     if (last_block(ctl)) {
-        const double pAp = ordered_sum(partial, DOT_BLOCKS);
+        const double pAp = ordered_sum(partial, (int)gridDim.x);
         if (threadIdx.x == 0) { scal[1] = pAp; ctl[CTL_TICKET] = 0; }
     }
 }
@@ -408,11 +411,26 @@ __global__ void __launch_bounds__(DOT_THREADS) cg_update_rbj_kernel(int M, int b
         rr = fma(ri, ri, rr);
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < n; i += DOT_THREADS) {
+    // z = M_b^-1 r: np threads per row, each over every np-th column (inv is symmetric: the column read is coalesced
+    // across the rows), the np partial sums added in order through shared memory
+    const int np = n >= DOT_THREADS ? 1 : DOT_THREADS / n;
+    const int rpp = DOT_THREADS / np;            // rows per pass (>= n when n < DOT_THREADS)
+    const int part = threadIdx.x / rpp, il = threadIdx.x - part * rpp;
+    double *s_part = s_r + block;                // [np][rpp] <= DOT_THREADS doubles
+    for (int i0 = 0; i0 < n; i0 += rpp) {
+        const int i = i0 + il;
         double s = 0.0;
-        for (int j = 0; j < n; ++j) s = fma(a[(size_t)j * n + i], s_r[j], s);  // inv is symmetric: column read is coalesced
-        z[idx[i]] = s;
-        rz = fma(s_r[i], s, rz);
+        if (i < n && part < np)
+            for (int j = part; j < n; j += np) s = fma(a[(size_t)j * n + i], s_r[j], s);
+        s_part[threadIdx.x] = s;
+        __syncthreads();
+        if (part == 0 && i < n) {
+            double t = 0.0;
+            for (int q = 0; q < np; ++q) t += s_part[q * rpp + il];
+            z[idx[i]] = t;
+            rz = fma(s_r[i], t, rz);
+        }
+        __syncthreads();
     }
     rr = block_sum(rr);
     rz = block_sum(rz);
@@ -743,7 +761,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     auto update = [&](int init) -> int {
         if (precond == 2) {
             const int block = (int)ctx->rbj_block;
-            cg_update_rbj_kernel<<<(unsigned)ctx->rbj_nblocks, DOT_THREADS, (size_t)block * 8, s>>>(
+            cg_update_rbj_kernel<<<(unsigned)ctx->rbj_nblocks, DOT_THREADS, ((size_t)block + DOT_THREADS) * 8, s>>>(
                 M, block, ctx->rbj_order, ctx->rbj_inv, p, Ap, x, r, z, scal, partial, ctl, tol, max_iter, init);
         } else {
             cg_update_diag_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, precond == 1 ? ctx->pt_diag : nullptr, p, Ap, x, r, z, scal,
@@ -783,7 +801,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
             if (ev) CG_CUDA(cudaEventRecord(ctx->cg_ev[2 * ctx->cg_ev_n], s));
             CG_TRY(launch_amatvec_partials(ctx, p, ctl, s));
             if (ev) { CG_CUDA(cudaEventRecord(ctx->cg_ev[2 * ctx->cg_ev_n + 1], s)); ctx->cg_ev_n++; }
-            cg_matvec_reduce_kernel<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(M, amat_parts(ctx), p, Ap, scal, scal + 16, ctl);
+            cg_matvec_reduce_kernel<<<(unsigned)cdiv(M, 32), DOT_THREADS, 0, s>>>(M, amat_parts(ctx), p, Ap, scal, ctx->cg_part, ctl);
             ctx->launch_total += 1;
             CG_TRY(update(0));
         }
