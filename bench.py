@@ -58,6 +58,22 @@ def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
 
+# ----------------------------------------------------------------------------- N > 1: replicas only
+def max_over_ranks(ms: float, dist, device) -> float:
+    """The contract's timing rule: the slowest rank's device time.  dist = torch.distributed (initialised) or None."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world: int, units_per_step: float, ms_per_step: float) -> float:
+    """Whole-job throughput of `world` independent replicas of the step (weak scaling: every rank does the same work)."""
+    return world * units_per_step / (ms_per_step * 1e-3)
+
+
 # ----------------------------------------------------------------------------- clocks
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
@@ -282,13 +298,9 @@ def run_ours(args):
     pot_ms = [e[0].elapsed_time(e[1]) for e in ev]
     solve_ms = [e[1].elapsed_time(e[2]) for e in ev]
     fock_ms = [e[2].elapsed_time(e[3]) for e in ev]
-    total_ms = sum(step_ms)
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(sum(step_ms), dist, dev)
     ms_per_step = total_ms / args.steps
-    value = world * units_per_step / (ms_per_step * 1e-3)
+    value = job_value(world, units_per_step, ms_per_step)
 
     if rank != 0:
         if dist is not None:

@@ -77,7 +77,7 @@ def full(request, pcm, torch_cuda):
     torch = torch_cuda
     cfg = request.param
     w = synth.make_workload(cfg)
-    ctx = pcm.setup_from_workload(w.basis, w.surface)
+    ctx = pcm.setup_from_workload(w.basis, w.surface, gradient=True)
     P = torch.as_tensor(w.P, dtype=torch.float64, device="cuda")
     q = torch.as_tensor(w.q, dtype=torch.float64, device="cuda")
     v = pcm.pcm_potential(ctx, P)
@@ -98,6 +98,28 @@ def test_fullsize_counts(full, pcm):
     assert info.products_total < info.prim_pairs_total < info.prim_pairs_unscreened
     assert (info.prim_pairs[5] > 0) == (cfg == 3)         # dd pairs only with the configs[3] d shells
     assert info.prim_pair_points == float(info.prim_pairs_total) * w.surface.M
+
+
+def test_fullsize_gradient_sampled(full, pcm, orc):
+    """pcm_gradient (Eq. 14/22) at full size: sampled shell centres (every angular momentum) and points against the oracle,
+    translation invariance on the full output (the sum of all shell and point gradients vanishes)."""
+    cfg, w, ctx, P, q, v, F = full
+    gs, gp = pcm.pcm_gradient(ctx, P, q)
+    gs, gp = gs.cpu().numpy(), gp.cpu().numpy()
+    rng = np.random.default_rng(700 + cfg)
+    l = np.asarray(w.basis.shell_l)
+    shells = sorted({int(s) for la in (0, 1, 2) if (l == la).any() for s in rng.choice(np.flatnonzero(l == la), size=3, replace=False)})
+    pts = np.sort(rng.choice(w.surface.M, size=12, replace=False))
+    rs, rp = orc.gradient(w.basis, w.surface, w.P, w.q, shells=shells, points=pts)
+    # every component is a sum over all M points of q_k x (derivative integrals of magnitude O(1)) that largely cancels:
+    # no fp64 summation order can promise an absolute error below a few eps ||q||_1, so the absolute floor of the
+    # north_star tolerance is widened by 64 eps ||q||_1 (1e-11 at configs[2], 4e-11 at configs[3]; DESIGN.md 3)
+    floor = ATOL + 64 * np.finfo(float).eps * np.abs(w.q).sum()
+    for got, ref, what in ((gs[shells], rs, "shell centres"), (gp[pts], rp, "points")):
+        err = np.abs(got - ref)
+        assert np.all(err <= RTOL * np.abs(ref) + floor), f"config {cfg}: gradient on sampled {what}: max err {err.max():.3e} (floor {floor:.1e})"
+    scale = np.abs(gs).sum(0) + np.abs(gp).sum(0)
+    assert np.all(np.abs(gs.sum(0) + gp.sum(0)) <= 1e-12 * scale), "the gradients of a translation-invariant energy must sum to zero"
 
 
 def test_fullsize_potential_sampled(full, orc):
