@@ -164,6 +164,7 @@ struct pcm_ctx {
     double *ypart = nullptr;    // amatvec row partial sums [slots][M]
     int64_t ypart_slots = 0;
     double *colpart = nullptr;  // amatvec column partial sums of the symmetric sweep [plan_amat.xb][M]
+    int amat_tile = 256;        // column tile of the A q kernel (128 for small M)
     int amat_R = 4;             // row groups per warp of the A q kernel (row block = 128 amat_R points)
     double *cg_vec = nullptr;   // 6 M doubles: r, z, p, Ap, x, b (sorted point order)
     double *cg_part = nullptr;  // [ceil(M/32)] per-CTA partial dot products of cg_matvec_reduce_kernel

@@ -35,6 +35,7 @@ struct Blocking { int R, C; };
 // A q: R = 4 (row blocks of 512) for large M, R = 2 (row blocks of 256, four times the blocks) below AMAT_R4_MIN points
 constexpr int AMAT_C = 2;
 constexpr int64_t AMAT_R4_MIN = 60000;
+constexpr int64_t AMAT_T128_MAX = 30000;
 __host__ __device__ constexpr Blocking fock_blocking(int L) {
     return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{2, 2} : L == 2 ? Blocking{1, 4} : Blocking{1, 2};
 }
@@ -106,19 +107,19 @@ __device__ __forceinline__ void stage_points(const double4 *__restrict__ pt, con
 // in a fixed order.  Per evaluation 13 FP64 instructions + 1/R DADD for two entries of A instead of 12 per entry.
 // Column sums: a lane adds its R rows in registers, the 32 lanes are then summed through a [16][33] shared-memory
 // transpose per warp (one DADD per column and lane), the 4 warps at the end of the tile.
-template <int R, int C>
+template <int R, int C, int TILE>
 __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ q,
                                                       const int32_t *__restrict__ qidx, int M, int chunk_len,
                                                       double *__restrict__ out, double *__restrict__ colpart,
                                                       const uint8_t *__restrict__ farmap, int64_t nbyte, int64_t nrg,
                                                       const int *__restrict__ stop) {
-    constexpr int NS = PT_TILE / SUB;
+    constexpr int NS = TILE / SUB;
     constexpr int RB = TPB * R;
     constexpr int NW = TPB / 32;
-    static_assert(RB % PT_TILE == 0, "row blocks must be whole column tiles");
-    __shared__ double4 s_pt[PT_TILE];       // x, y, z, q
+    static_assert(RB % TILE == 0, "row blocks must be whole column tiles");
+    __shared__ double4 s_pt[TILE];       // x, y, z, q
     __shared__ double s_c[NW][16 * 33];     // per warp: [column of the half group][lane]
-    __shared__ double s_cs[NW][PT_TILE];    // per warp: column sums of the tile
+    __shared__ double s_cs[NW][TILE];    // per warp: column sums of the tile
     if (stop && *stop) return;  // a converged CG solve: the iterations queued behind it are no-ops
     const int r0 = blockIdx.x * RB;
     const int jbeg = blockIdx.y * chunk_len, jend = min(M, jbeg + chunk_len);
@@ -141,8 +142,8 @@ __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict_
         y[r] = 0.0;
     }
     double *sc = s_c[warp];
-    for (int base = max(jbeg, r0); base < jend; base += PT_TILE) {
-        const int nst = (min(PT_TILE, jend - base) + SUB - 1) / SUB;
+    for (int base = max(jbeg, r0); base < jend; base += TILE) {
+        const int nst = (min(TILE, jend - base) + SUB - 1) / SUB;
         const bool sym = base >= r0 + RB;
         const unsigned bits = far_bits<R, NS>(farmap, nbyte, rg0, nrg, base / SUB, lane);
         __syncthreads();
@@ -403,7 +404,7 @@ __global__ void __launch_bounds__(256) amat_reduce_kernel(AmatParts parts, int M
 AmatParts amat_parts(const pcm_ctx *ctx) {
     AmatParts a;
     a.ypart = ctx->ypart; a.colpart = ctx->colpart; a.near = ctx->near_amat; a.pstart = ctx->amat_map.pstart;
-    a.slots = (int)ctx->plan_amat.chunks; a.chunk_len = (int)ctx->plan_amat.chunk_len; a.RB = TPB * ctx->amat_R; a.tile = PT_TILE;
+    a.slots = (int)ctx->plan_amat.chunks; a.chunk_len = (int)ctx->plan_amat.chunk_len; a.RB = TPB * ctx->amat_R; a.tile = ctx->amat_tile;
     return a;
 }
 
@@ -843,9 +844,12 @@ int plan_all(pcm_ctx *ctx) {
     if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 2 || r == 4) ctx->amat_R = r; }
     double aw = 8.0;
     if (const char *e = getenv("PCM_AMAT_WAVES")) aw = atof(e);
-    ctx->plan_amat = ctx->amat_R == 4
-        ? make_plan(ctx->M, TPB * 4, ctx->M, PT_TILE, wave_of(ctx, amatvec_kernel<4, AMAT_C>), 0.5, aw)
-        : make_plan(ctx->M, TPB * 2, ctx->M, PT_TILE, wave_of(ctx, amatvec_kernel<2, AMAT_C>), 0.5, aw);
+    // small M: column tiles of 128 (four times the work items of the same sweep, so that the SMs stay evenly loaded)
+    ctx->amat_tile = (ctx->amat_R == 2 && ctx->M < AMAT_T128_MAX) ? 128 : 256;
+    if (const char *e = getenv("PCM_AMAT_TILE")) { const int t = atoi(e); if ((t == 128 && ctx->amat_R == 2) || t == 256) ctx->amat_tile = t; }
+    ctx->plan_amat = ctx->amat_R == 4 ? make_plan(ctx->M, TPB * 4, ctx->M, 256, wave_of(ctx, amatvec_kernel<4, AMAT_C, 256>), 0.5, aw)
+                     : ctx->amat_tile == 256 ? make_plan(ctx->M, TPB * 2, ctx->M, 256, wave_of(ctx, amatvec_kernel<2, AMAT_C, 256>), 0.5, aw)
+                                             : make_plan(ctx->M, TPB * 2, ctx->M, 128, wave_of(ctx, amatvec_kernel<2, AMAT_C, 128>), 0.5, aw);
     if (getenv("PCM_VERBOSE")) fprintf(stderr, "[pcm] amat plan: R %d xb %lld chunks %lld chunk_len %lld\n", ctx->amat_R,
                                        (long long)ctx->plan_amat.xb, (long long)ctx->plan_amat.chunks, (long long)ctx->plan_amat.chunk_len);
     plan_class<0>(ctx); plan_class<1>(ctx); plan_class<2>(ctx); plan_class<3>(ctx); plan_class<4>(ctx);
@@ -890,9 +894,11 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
         { ctx->launches[2]++; ctx->launch_total++; }
     }
     if (ctx->amat_R == 4)
-        amatvec_kernel<4, AMAT_C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+        amatvec_kernel<4, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+    else if (ctx->amat_tile == 256)
+        amatvec_kernel<2, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
     else
-        amatvec_kernel<2, AMAT_C><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+        amatvec_kernel<2, AMAT_C, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[2]++; ctx->launch_total++; }
     if (pm.npiece > 0) PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
