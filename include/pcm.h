@@ -146,6 +146,14 @@ int pcm_pivot_order(uint64_t seed, int64_t M, int64_t *perm_host);
 int pcm_rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, void *stream);
 
 /*
+ * pcm_rbj_build_async -- the same build queued on `stream` without synchronising, so that it can overlap other work
+ * (A and the preconditioner depend on the geometry only: e.g. queue it on a side stream while pcm_potential runs).
+ * The next pcm_cg_solve with precond = 2 (or pcm_rbj_get, or the next build) waits for it, orders its own stream after
+ * it and returns the build's error, if any.  Argument errors are still returned at once.
+ */
+int pcm_rbj_build_async(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, void *stream);
+
+/*
  * pcm_rbj_get -- copy the block structure back (for inspection and tests).  Any pointer may be NULL.
  * order_host[M]: indices block after block, pivot first then by descending A_kj; bstart_host[nblocks+1];
  * inv_host: the inverse blocks, row-major, back to back (sum of n_b^2 doubles).  Synchronous.

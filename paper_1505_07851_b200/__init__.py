@@ -30,7 +30,7 @@ EXPORTS = (
     "pcm_rbj_build", "pcm_rbj_get", "pcm_cg_solve", "pcm_potential_host", "pcm_fock_host", "pcm_amatvec_host",
     "pcm_cg_solve_host", "pcm_get_info", "pcm_set_timing", "pcm_last_kernel_ms", "pcm_last_class_ms",
     "pcm_launch_count", "pcm_fp64_peak", "pcm_set_nuclei", "pcm_nuclear_potential", "pcm_rhs", "pcm_energy",
-    "pcm_cg_threshold", "pcm_gradient", "pcm_last_cg_matvec_ms",
+    "pcm_cg_threshold", "pcm_gradient", "pcm_last_cg_matvec_ms", "pcm_rbj_build_async",
     "pcm_schwarz_bound", "pcm_last_error", "pcm_destroy",
 )
 
@@ -81,6 +81,7 @@ def lib(build: bool = False):
         L.pcm_amatvec.argtypes = [vp, vp, vp, vp]
         L.pcm_pivot_order.argtypes = [C.c_uint64, C.c_int64, vp]
         L.pcm_rbj_build.argtypes = [vp, C.c_int, C.c_uint64, vp, vp]
+        L.pcm_rbj_build_async.argtypes = [vp, C.c_int, C.c_uint64, vp, vp]
         L.pcm_rbj_get.argtypes = [vp, vp, vp, vp]
         L.pcm_cg_solve.argtypes = [vp, vp, vp, C.c_double, C.c_int, C.c_int, C.c_int, _ip, _dp, vp]
         L.pcm_potential_host.argtypes = [vp, vp, C.c_int64, vp]
@@ -297,6 +298,12 @@ def pcm_rbj_build(ctx: Context, block: int, seed: int = 0, pivot_order=None, str
     po = None if pivot_order is None else _np(pivot_order, np.int64)
     _check(lib().pcm_rbj_build(ctx.handle, int(block), C.c_uint64(seed & 0xFFFFFFFFFFFFFFFF), _hp(po), _stream(stream)),
            ctx.handle)
+
+
+def pcm_rbj_build_async(ctx: Context, block: int, seed: int = 0, pivot_order=None, stream=None):
+    """pcm_rbj_build queued on `stream` without synchronising; the next pcm_cg_solve(precond=2) completes it."""
+    po = None if pivot_order is None else _np(pivot_order, np.int64)
+    _check(lib().pcm_rbj_build_async(ctx.handle, int(block), C.c_uint64(seed & 0xFFFFFFFFFFFFFFFF), _hp(po), _stream(stream)), ctx.handle)
 
 
 def pcm_rbj_get(ctx: Context):

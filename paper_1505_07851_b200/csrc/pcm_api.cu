@@ -12,7 +12,6 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
                   const double *pt_zeta, const double *pt_switch);
 const char *setup_error_text();
 void pivot_order(uint64_t seed, int64_t M, int64_t *perm);
-int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s);
 int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter, int precond, int use_x0, int *iters,
              double *resid, cudaStream_t s);
 }  // namespace pcm
@@ -43,6 +42,7 @@ static void free_ctx(pcm_ctx *ctx) {
     for (auto &e : ctx->cg_ev) if (e) cudaEventDestroy(e);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->near_stream) cudaStreamDestroy(ctx->near_stream);
+    if (ctx->ev_rbj) { if (ctx->rbj_pending) cudaEventSynchronize(ctx->ev_rbj); cudaEventDestroy(ctx->ev_rbj); }
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     delete[] ctx->rbj_bstart_host;
@@ -102,6 +102,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     }
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_rbj, cudaEventDisableTiming);
     if (e != cudaSuccess) { ctx->err = std::string("cudaStreamCreate: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
     for (auto &ev : ctx->ev) {
         e = cudaEventCreate(&ev);
@@ -239,11 +240,21 @@ int pcm_pivot_order(uint64_t seed, int64_t M, int64_t *perm_host) {
 int pcm_rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, void *stream) {
     PCM_CHECK_CTX(ctx);
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
-    return rbj_build(ctx, block, seed, pivot_order_host, (cudaStream_t)stream);
+    return rbj_build(ctx, block, seed, pivot_order_host, (cudaStream_t)stream, false, false);
+}
+
+int pcm_rbj_build_async(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return rbj_build(ctx, block, seed, pivot_order_host, (cudaStream_t)stream, true, false);
 }
 
 int pcm_rbj_get(pcm_ctx *ctx, int64_t *order_host, int64_t *bstart_host, double *inv_host) {
     PCM_CHECK_CTX(ctx);
+    {
+        int rcf = rbj_finish(ctx, ctx->own_stream);
+        if (rcf) return rcf;
+    }
     if (ctx->rbj_block == 0) return set_error(ctx, PCM_ERR_STATE, "pcm_rbj_get: no RBJ preconditioner built");
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
     const int64_t M = ctx->M, l = ctx->rbj_block, nb = ctx->rbj_nblocks;

@@ -101,6 +101,7 @@ struct pcm_ctx {
     // Vectors crossing the C ABI (v, q, y, b, x) are in the caller's order; the kernels gather/scatter through s2c.
     double4 *pt = nullptr;      // (x, y, z, 1/zeta^2)
     double *pt_diag = nullptr;  // A_kk = zeta_k sqrt(2/pi)/S_k
+    double *pt_boxes = nullptr; // [ceil(M/32)][6] bounding boxes of the groups of 32 sorted points
     pcm::PatchMap amat_map;     // rows and columns = groups of 32 sorted points
     int32_t *s2c = nullptr;     // [M] device
     std::vector<int32_t> s2c_host, c2s_host;
@@ -179,6 +180,13 @@ struct pcm_ctx {
     int64_t *rbj_bstart_host = nullptr;
     double *rbj_inv = nullptr;       // inverse blocks back to back (block b at b*l*l)
     double *rbj_partial = nullptr;   // [2][rbj_nblocks] per-block r.r and r.z of the CG update kernel
+    // asynchronous build (pcm_rbj_build_async): status in cg_scal_host[32..], completed by rbj_finish
+    bool rbj_pending = false;
+    cudaEvent_t ev_rbj = nullptr;
+    uint64_t rbj_last_seed = 0;
+    bool rbj_perm_seeded = false;
+    std::vector<int32_t> rbj_perm_sorted;   // pivot order of the last build, sorted point numbering
+    std::vector<int64_t> rbj_last_perm;     // caller-given pivot order of the last build (empty: seeded)
     char *rbj_arena = nullptr;       // grow-only allocation holding the three arrays above and the build scratch
     size_t rbj_arena_bytes = 0;
 
@@ -220,6 +228,8 @@ int launch_nuclear_potential(pcm_ctx *ctx, double *u, cudaStream_t s);
 int launch_rhs(pcm_ctx *ctx, const double *u, const double *v, double f, double *b, cudaStream_t s);
 int energy_terms(pcm_ctx *ctx, const double *u, const double *v, const double *q, double f, double *terms_host, cudaStream_t s);
 int launch_gradient(pcm_ctx *ctx, const double *P, int64_t ldp, const double *q, double *g_shell, double *g_point, cudaStream_t s);
+int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s, bool async, bool force_global);
+int rbj_finish(pcm_ctx *ctx, cudaStream_t s);
 int plan_all(pcm_ctx *ctx);
 int fill_amat_blocks(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);

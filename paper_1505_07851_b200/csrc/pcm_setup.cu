@@ -340,6 +340,12 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         if ((rc = upload(ctx, &ctx->pt_diag, diag))) return rc;
         if ((rc = upload(ctx, &ctx->s2c, s2c))) return rc;
         // A q patches: far-field radius^2 of a pair of points is at most TFAR_AMAT (1/zeta_i^2 + 1/zeta_j^2)
+        {   // bounding boxes of the groups of 32 sorted points (lo xyz, hi xyz) for the RBJ neighbourhood search
+            std::vector<double> b6((size_t)std::max<int64_t>(ng, 1) * 6, 0.0);
+            for (int64_t g = 0; g < ng; ++g)
+                for (int d = 0; d < 6; ++d) b6[(size_t)g * 6 + d] = box[(size_t)g * 7 + d];
+            if ((rc = upload(ctx, &ctx->pt_boxes, b6))) return rc;
+        }
         GroupBoxes amat_boxes = ptboxes;
         for (int64_t g = 0; g < ng; ++g) amat_boxes.b[(size_t)g * 7 + 6] = TFAR_AMAT * 2.0 / (zmin * zmin);
         if ((rc = build_patch_map(ctx, amat_boxes, amat_boxes, ctx->amat_map))) return rc;

@@ -242,6 +242,173 @@ __global__ void __launch_bounds__(RBJ_THREADS) rbj_select_kernel(const double4 *
 }
 
 // ---------------------------------------------------------------------------------------------
+// RBJ block selection, neighbourhood version: ONE CTA, no grid barrier.  A_kj = erf(zeta' r)/r <= 1/r, so if every
+// unassigned point within a radius rho of the pivot is a candidate and the take-th largest candidate key tau exceeds
+// 1/rho, no point outside can enter the block: the l-1 largest over the candidates are the l-1 largest over all
+// unassigned points -- the same block the global row scan of rbj_select_kernel finds, for a few hundred evaluations
+// and a few block-level barriers per step instead of M evaluations and two grid barriers.  The candidates are the
+// unassigned points of the groups of 32 (Hilbert order) whose bounding box is closer than rho; rho adapts from step to
+// step (1.25/tau of the previous block) and grows when the test fails or too few candidates are found.  Selection among
+// the candidates is the same as in rbj_select_kernel: histogram cut on the top 16 key bits, then ranking by (key
+// descending, caller index ascending).  Used for block sizes <= 256; err = 3 asks the host to fall back.
+// ---------------------------------------------------------------------------------------------
+constexpr int RBL_THREADS = 1024;
+constexpr int RBL_RAW = 3072;   // candidate capacity (raw)
+constexpr int RBL_CAP = 1024;   // candidates above the histogram cut that are ranked
+
+struct RblShared {
+    int hist[RBJ_BINS];
+    int scan[RBJ_BINS];
+    double rkey[RBL_RAW];
+    int ridx[RBL_RAW];
+    double ckey[RBL_CAP];
+    int cidx[RBL_CAP];
+    int ccal[RBL_CAP];
+    int pivot, nraw, ncut, bstar, ngl, all_in, ok;
+    double rho, tau;
+};
+
+__global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const double4 *__restrict__ pt, int M, int block,
+                                                                       const int32_t *__restrict__ perm,
+                                                                       const int32_t *__restrict__ s2c,
+                                                                       int32_t *__restrict__ order,
+                                                                       unsigned char *__restrict__ assigned,
+                                                                       const double *__restrict__ boxes, int ng,
+                                                                       int *__restrict__ gcount, int *__restrict__ glist,
+                                                                       int *__restrict__ err, const double *__restrict__ boys0) {
+    extern __shared__ __align__(16) unsigned char rbl_smem[];
+    RblShared &S = *reinterpret_cast<RblShared *>(rbl_smem);
+    const int tid = threadIdx.x;
+    for (int g = tid; g < ng; g += RBL_THREADS) gcount[g] = min(32, M - g * 32);
+    if (tid == 0) S.rho = 6.0;
+    __syncthreads();
+    long long pos = 0, filled = 0;
+    while (filled < M) {
+        // ---- pivot: first unassigned index of the pivot order
+        if (tid == 0) S.pivot = M;
+        __syncthreads();
+        while (true) {
+            const long long p = pos + tid;
+            if (p < M && !assigned[perm[p]]) atomicMin(&S.pivot, (int)p);
+            __syncthreads();
+            if (S.pivot < M || pos + RBL_THREADS >= M) break;
+            pos += RBL_THREADS;
+            __syncthreads();
+        }
+        const int ppos = S.pivot;
+        if (ppos >= M) { if (tid == 0) *err = 2; return; }
+        pos = ppos;
+        const int k = perm[ppos];
+        const int take = (int)min((long long)block - 1, (long long)M - filled - 1);
+        const double4 pk = pt[k];
+        __syncthreads();
+        if (tid == 0) { assigned[k] = 1; atomicSub(&gcount[k >> 5], 1); }
+        __syncthreads();
+        if (take > 0) {
+            while (true) {
+                // ---- candidate groups: bounding box closer than rho and something unassigned in it
+                const double rho = S.rho, rho2 = rho * rho;
+                if (tid == 0) { S.ngl = 0; S.nraw = 0; S.ncut = 0; S.all_in = 1; S.ok = 0; }
+                for (int t = tid; t < RBJ_BINS; t += RBL_THREADS) S.hist[t] = 0;
+                __syncthreads();
+                for (int g = tid; g < ng; g += RBL_THREADS) {
+                    if (gcount[g] <= 0) continue;
+                    const double *b = boxes + (size_t)g * 6;
+                    const double gx = fmax(fmax(b[0] - pk.x, pk.x - b[3]), 0.0), gy = fmax(fmax(b[1] - pk.y, pk.y - b[4]), 0.0),
+                                 gz = fmax(fmax(b[2] - pk.z, pk.z - b[5]), 0.0);
+                    if (gx * gx + gy * gy + gz * gz < rho2) glist[atomicAdd(&S.ngl, 1)] = g;
+                    else S.all_in = 0;
+                }
+                __syncthreads();
+                const int ngl = S.ngl;
+                // ---- keys of the unassigned points of those groups
+                for (int t = tid; t < ngl * 32; t += RBL_THREADS) {
+                    const int j = glist[t >> 5] * 32 + (t & 31);
+                    if (j < M && !assigned[j]) {
+                        const double4 b = pt[j];
+                        const double dx = pk.x - b.x, dy = pk.y - b.y, dz = pk.z - b.z;
+                        const double a = amat_entry(fma(dz, dz, fma(dy, dy, dx * dx)), pk.w, b.w, boys0);
+                        const int slot = atomicAdd(&S.nraw, 1);
+                        if (slot < RBL_RAW) { S.rkey[slot] = a; S.ridx[slot] = j; }
+                        atomicAdd(&S.hist[rbj_bucket(a)], 1);
+                    }
+                }
+                __syncthreads();
+                const int nraw = S.nraw;
+                if (nraw > RBL_RAW) { if (tid == 0) *err = 3; return; }
+                if (nraw < take) {   // not enough unassigned points within rho (all_in cannot be set: take <= unassigned)
+                    __syncthreads();
+                    if (tid == 0) { S.rho = rho * 1.6; err[1] += 1; }
+                    __syncthreads();
+                    continue;
+                }
+                // ---- histogram cut: b* = the largest bucket b with count(bucket >= b) >= take
+                {
+                    const int lane = tid & 31, warp = tid >> 5;
+                    const int h = S.hist[tid];
+                    int v = h;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_down_sync(0xffffffffu, v, o); if (lane + o < 32) v += u; }
+                    if (lane == 0) S.scan[warp] = v;
+                    __syncthreads();
+                    if (warp == 0) {
+                        const int w = S.scan[lane];
+                        int x = w;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_down_sync(0xffffffffu, x, o); if (lane + o < 32) x += u; }
+                        S.scan[32 + lane] = x - w;   // keys in the buckets of the higher warps
+                    }
+                    __syncthreads();
+                    const int ge = v + S.scan[32 + warp], gt = ge - h;
+                    if (gt < take && ge >= take) S.bstar = tid;
+                }
+                __syncthreads();
+                const int bstar = S.bstar;
+                for (int c = tid; c < nraw; c += RBL_THREADS) {
+                    const double a = S.rkey[c];
+                    if (rbj_bucket(a) >= bstar) {
+                        const int slot = atomicAdd(&S.ncut, 1);
+                        if (slot < RBL_CAP) { S.ckey[slot] = a; S.cidx[slot] = S.ridx[c]; S.ccal[slot] = s2c[S.ridx[c]]; }
+                    }
+                }
+                __syncthreads();
+                const int n = S.ncut;
+                if (n > RBL_CAP || n < take) { if (tid == 0) *err = n < take ? 1 : 3; return; }
+                // ---- rank by (key descending, caller index ascending); tau = the take-th largest key
+                int rank = n;
+                if (tid < n) {
+                    const double key = S.ckey[tid];
+                    const int ci = S.ccal[tid];
+                    rank = 0;
+                    for (int o = 0; o < n; ++o) rank += (S.ckey[o] > key) || (S.ckey[o] == key && S.ccal[o] < ci);
+                    if (rank == take - 1) S.tau = key;
+                }
+                __syncthreads();
+                if (tid == 0) {
+                    const double tau = S.tau;
+                    S.ok = S.all_in || tau * rho > 1.0;          // tau > 1/rho: nothing outside rho can reach the block
+                    S.rho = S.ok ? fmax(1.25 / tau, 1.0) : fmax(rho * 1.6, 1.0001 / tau);
+                }
+                __syncthreads();
+                if (!S.ok) { if (tid == 0) err[1] += 1; continue; }
+                if (tid == 0) { err[2] += n; err[3] += nraw; }
+                if (rank < take) {
+                    const int j = S.cidx[tid];
+                    assigned[j] = 1;
+                    order[filled + 1 + rank] = j;
+                    atomicSub(&gcount[j >> 5], 1);
+                }
+                break;
+            }
+        }
+        if (tid == 0) order[filled] = k;
+        filled += 1 + take;
+        pos += 1;
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Block inversion: one thread block per diagonal block.  fill -> Cholesky (right-looking, in place, lower)
 // -> W = L^-1 (one column per thread) -> inv = W^T W.  n x n row-major, in global memory (L2 resident).
 // ---------------------------------------------------------------------------------------------
@@ -253,6 +420,10 @@ __global__ void rbj_invert_kernel(const double4 *__restrict__ pt, const double *
     double *a = inv + (size_t)blockIdx.x * block * block;
     double *w = work + (size_t)blockIdx.x * block * block;
     const int32_t *idx = order + start;
+    {   // a failed selection (asynchronous build: the host has not looked yet) leaves `order` undefined
+        const int e0 = *((volatile int *)err);
+        if (e0 == 1 || e0 == 2 || e0 == 3) return;
+    }
     for (int e = threadIdx.x; e < n * n; e += blockDim.x) {
         const int r = e / n, c = e - r * n;
         a[e] = a_entry(pt, diag, idx[r], idx[c], boys0);
@@ -631,28 +802,61 @@ int energy_terms(pcm_ctx *ctx, const double *u, const double *v, const double *q
 // ---------------------------------------------------------------------------------------------
 // host drivers
 // ---------------------------------------------------------------------------------------------
-int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s) {
+// Completes an asynchronous build: orders `s` after it, reads its status and, in the (capacity) case the neighbourhood
+// selection gave up, repeats the build synchronously with the global row scan.
+int rbj_finish(pcm_ctx *ctx, cudaStream_t s) {
+    if (!ctx->rbj_pending) return PCM_OK;
+    ctx->rbj_pending = false;
+    PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_rbj, 0));
+    PCM_CUDA(ctx, cudaEventSynchronize(ctx->ev_rbj));
+    const int h_err = *reinterpret_cast<const int *>(ctx->cg_scal_host + 32);
+    if (h_err == 3) {
+        std::vector<int64_t> perm = ctx->rbj_last_perm;
+        return rbj_build(ctx, (int)ctx->rbj_block, ctx->rbj_last_seed, perm.empty() ? nullptr : perm.data(), s, false, true);
+    }
+    if (h_err) {
+        ctx->rbj_block = 0; ctx->rbj_nblocks = 0; ctx->info.rbj_block = 0; ctx->info.rbj_nblocks = 0;
+        if (h_err == 1 || h_err == 2) return set_error(ctx, PCM_ERR_STATE, "pcm_rbj_build: block selection did not cover all points");
+        return set_error(ctx, PCM_ERR_NUMERIC, "pcm_rbj_build: a diagonal block of A is not positive definite");
+    }
+    return PCM_OK;
+}
+
+// async: everything is queued on s and the call returns; rbj_finish (pcm_cg_solve, pcm_rbj_get, the next build) completes it.
+int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s, bool async, bool force_global) {
     const int64_t M = ctx->M;
     if (block < 1) return set_error(ctx, PCM_ERR_ARG, "pcm_rbj_build: block < 1");
+    {   // a build still in flight owns the arena
+        int rcf = rbj_finish(ctx, s);
+        if (rcf) return rcf;
+    }
     if (M == 0) { ctx->rbj_block = block; ctx->rbj_nblocks = 0; return PCM_OK; }
     const bool verbose = getenv("PCM_VERBOSE") != nullptr;
     auto now = []() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); };
     const double t0 = now();
     if ((int64_t)block > M) block = (int)M;
-    std::vector<int64_t> perm64((size_t)M);
+    std::vector<int32_t> &perm = ctx->rbj_perm_sorted;  // pivot order in the library's sorted point numbering
     if (pivot_order_host) {
         std::vector<char> seen((size_t)M, 0);
         for (int64_t i = 0; i < M; ++i) {
             const int64_t v = pivot_order_host[i];
             if (v < 0 || v >= M || seen[v]) return set_error(ctx, PCM_ERR_ARG, "pcm_rbj_build: pivot order is not a permutation");
             seen[v] = 1;
-            perm64[i] = v;
         }
-    } else {
+        if (pivot_order_host != ctx->rbj_last_perm.data()) ctx->rbj_last_perm.assign(pivot_order_host, pivot_order_host + M);
+        perm.resize((size_t)M);
+        for (int64_t i = 0; i < M; ++i) perm[i] = ctx->c2s_host[(size_t)pivot_order_host[i]];
+        ctx->rbj_perm_seeded = false;
+    } else if (!(ctx->rbj_perm_seeded && ctx->rbj_last_seed == seed && (int64_t)perm.size() == M)) {
+        // the seeded order is a pure function of (seed, M): kept for the next build with the same seed
+        std::vector<int64_t> perm64((size_t)M);
         pivot_order(seed, M, perm64.data());
+        perm.resize((size_t)M);
+        for (int64_t i = 0; i < M; ++i) perm[i] = ctx->c2s_host[(size_t)perm64[i]];
+        ctx->rbj_last_perm.clear();
+        ctx->rbj_perm_seeded = true;
     }
-    std::vector<int32_t> perm((size_t)M);  // pivot order in the library's sorted point numbering
-    for (int64_t i = 0; i < M; ++i) perm[i] = ctx->c2s_host[(size_t)perm64[i]];
+    ctx->rbj_last_seed = seed;
 
     const int64_t nb = cdiv(M, block);
     // RBJ storage and build scratch live in one grow-only device arena (no allocation when a build is repeated)
@@ -704,8 +908,37 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
 
     double t1 = 0, t2 = 0;
     if (verbose) { cudaStreamSynchronize(s); t1 = now(); }
+    // block sizes up to 256: the single-CTA neighbourhood selection; it reports err = 3 (capacity) to fall back
+    bool local_done = false;
+    if (block <= 256 && !force_global && !getenv("PCM_RBJ_GLOBAL")) {
+        const int ng = (int)cdiv(M, 32);
+        int *d_gcount = (int *)w.cand_idx, *d_glist = d_gcount + ng;   // scratch of the global path, 2 M ints
+        RBJ_TRY(cudaFuncSetAttribute(rbj_select_local_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RblShared)));
+        rbj_select_local_kernel<<<1, RBL_THREADS, sizeof(RblShared), s>>>(ctx->pt, (int)M, block, d_perm, ctx->s2c, ctx->rbj_order,
+                                                                           w.assigned, ctx->pt_boxes, ng, d_gcount, d_glist, d_err,
+                                                                           ctx->boys);
+        RBJ_TRY(cudaGetLastError());
+        ctx->launch_total += 1;
+        int h_e = 0;
+        if (async) {   // the status is read by rbj_finish; the inversion below is a no-op on a failed selection
+            local_done = true;
+        } else {
+        RBJ_TRY(cudaMemcpyAsync(&h_e, d_err, 4, cudaMemcpyDeviceToHost, s));
+        RBJ_TRY(cudaStreamSynchronize(s));
+        if (verbose) {
+            int h4[4];
+            cudaMemcpy(h4, d_err, 16, cudaMemcpyDeviceToHost);
+            fprintf(stderr, "[pcm] rbj local: retries %d, ranked candidates %d, raw candidates %d over %lld blocks\n", h4[1], h4[2], h4[3], (long long)nb);
+        }
+        if (h_e == 0) local_done = true;
+        else if (h_e == 3) {   // start over with the global row scan
+            RBJ_TRY(cudaMemsetAsync(w.assigned, 0, (size_t)M, s));
+            RBJ_TRY(cudaMemsetAsync(small, 0, 64, s));
+        }
+        }
+    }
     // one cooperative launch: all CTAs must be co-resident for the grid barrier
-    {
+    if (!local_done) {
         int per_sm = 0;
         RBJ_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rbj_select_kernel, RBJ_THREADS, 0));
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(cdiv(M, RBJ_THREADS), (int64_t)std::max(per_sm, 1) * ctx->sm_count));
@@ -723,6 +956,14 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     if (verbose) { cudaStreamSynchronize(s); t2 = now(); }
     rbj_invert_kernel<<<(unsigned)nb, 256, 0, s>>>(ctx->pt, ctx->pt_diag, (int)M, block, ctx->rbj_order, ctx->rbj_inv, d_work, d_err, ctx->boys);
     RBJ_TRY(cudaGetLastError());
+    if (async) {
+        RBJ_TRY(cudaMemcpyAsync(ctx->cg_scal_host + 32, d_err, 16, cudaMemcpyDeviceToHost, s));
+        RBJ_TRY(cudaEventRecord(ctx->ev_rbj, s));
+        ctx->rbj_pending = true;
+        ctx->rbj_block = block; ctx->rbj_nblocks = nb;
+        ctx->info.rbj_block = block; ctx->info.rbj_nblocks = nb;
+        return PCM_OK;
+    }
     int h_err = 0;
     RBJ_TRY(cudaMemcpyAsync(&h_err, d_err, 4, cudaMemcpyDeviceToHost, s));
     RBJ_TRY(cudaStreamSynchronize(s));
@@ -743,6 +984,10 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
              int *iters, double *resid, cudaStream_t s) {
     const int M = (int)ctx->M;
     if (precond < 0 || precond > 2) return set_error(ctx, PCM_ERR_ARG, "pcm_cg_solve: precond must be 0, 1 or 2");
+    if (precond == 2) {
+        int rcf = rbj_finish(ctx, s);
+        if (rcf) return rcf;
+    }
     if (precond == 2 && ctx->rbj_block == 0) return set_error(ctx, PCM_ERR_STATE, "pcm_cg_solve: RBJ requested before pcm_rbj_build");
     if (M == 0) { if (iters) *iters = 0; if (resid) resid[0] = resid[1] = 0.0; return PCM_OK; }
     // all solver vectors live in the library's sorted point order; b is gathered on entry, x scattered on exit

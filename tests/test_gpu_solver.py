@@ -148,3 +148,28 @@ def test_cg_warm_start_max_iter_and_errors(pcm, orc, sys2500, torch_cuda):
         pcm.pcm_cg_solve(fresh, dev(torch_cuda, b), precond=2)   # RBJ before pcm_rbj_build
     with pytest.raises(pcm.PcmError):
         pcm.pcm_cg_solve(fresh, dev(torch_cuda, b), precond=9)
+
+
+def test_rbj_build_async_equals_sync(pcm, orc, sys2500, torch_cuda):
+    """pcm_rbj_build_async on a side stream: same blocks and inverses as the synchronous build, completed by pcm_cg_solve
+    (or pcm_rbj_get); the seeded pivot order is reused from the previous build with the same seed."""
+    torch = torch_cuda
+    s, A, q_true, ctx = sys2500
+    pcm.pcm_rbj_build(ctx, 64, seed=5)
+    o1, b1, i1 = pcm.pcm_rbj_get(ctx)
+    side = torch.cuda.Stream()
+    pcm.pcm_rbj_build_async(ctx, 32, seed=9, stream=side)      # something else in between
+    pcm.pcm_rbj_build_async(ctx, 64, seed=5, stream=side)      # waits for the pending one first
+    b = dev(torch, A @ q_true)
+    x, it, rr, rt, ok = pcm.pcm_cg_solve(ctx, b, tol=1e-10, max_iter=500, precond=2)
+    assert ok and np.abs(x.cpu().numpy() - q_true).max() < 1e-8
+    o2, b2, i2 = pcm.pcm_rbj_get(ctx)
+    assert np.array_equal(o1, o2) and np.array_equal(b1, b2) and all(np.array_equal(a, c) for a, c in zip(i1, i2))
+    pcm.pcm_rbj_build(ctx, 64, seed=5)
+    x2, it2, *_ = pcm.pcm_cg_solve(ctx, b, tol=1e-10, max_iter=500, precond=2)
+    assert it2 == it and torch.equal(x, x2)
+    pcm.pcm_rbj_build_async(ctx, 64, seed=5, stream=side)
+    o3, _, _ = pcm.pcm_rbj_get(ctx)                            # pcm_rbj_get completes a pending build too
+    assert np.array_equal(o1, o3)
+    with pytest.raises(pcm.PcmError):
+        pcm.pcm_rbj_build_async(ctx, 0, seed=1, stream=side)
