@@ -45,6 +45,10 @@ SWEEP_M = (10_000, 50_000, 100_000, 200_000)
 # Algorithmic fp64 work per (Hermite product, point) in the far field, counted from the kernel's arithmetic
 # (DESIGN.md "Roofline"): [FP64-pipe instructions, flops (FMA = 2)] per unit for L = 0..4, potential and Fock.
 # geometry 3 DADD + (1 DMUL + 2 DFMA) + rsqrt (2 DMUL + 3 DFMA) = 11 instr / 16 flop, then seeds and recursion.
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the hot kernels on the bench workload, from the ncu --set full
+# captures summarised in profiles/r1c_ncu_full_summary.csv (a profiler number cannot be taken live).
+TRAFFIC = {"amatvec": 379648.0, "potential": [1715200.0, 2185216.0, 1097216.0, None, None],
+           "fock": [1546496.0, 1363712.0, 639488.0, None, None]}
 WORK = {
     # A q: the sweep is symmetric -- one evaluation of 1/r_ij serves A_ij and A_ji; unit = one pair evaluation
     # (M^2/2 per call): geometry 6 + rsqrt 5 + two FMAs + 1/4 DADD of the column reduction = 13.25 instr, 20.25 flop.
@@ -330,7 +334,10 @@ def run_ours(args):
                 if op == "amatvec" else f"{op}_kernel<L={Ld}>", "launches_per_step": per_step,
                 "share_of_step": ms_dom * per_step / ms_per_step, "all_hot_kernels": kernels,
                 "achieved": achieved, "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                "traffic": TRAFFIC["amatvec"] if op == "amatvec" else TRAFFIC[op][Ld],
+                "traffic_source": "bytes per launch, ncu --set full capture in profiles/r1c_ncu_full_summary.csv",
+                "algorithmic_bytes": (48.0 * M if op == "amatvec" else 40.0 * M + (32.0 + 8.0 * [1, 4, 10, 20, 35][Ld]) * float(info.products[Ld])),
                 "fp64_pipe_frac": n_units * instr * 2.0 / (ms_dom * 1e-3) * 1e-12 / peak_tflops,
                 "units_per_launch": n_units, "flop_per_unit": flop, "fp64_instr_per_unit": instr, "ms_per_launch": ms_dom,
                 "peak_source": "measured live: pcm_fp64_peak DFMA chain (nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2)",
@@ -380,7 +387,7 @@ def run_ours(args):
     pcm.pcm_set_nuclei(ctx, w.atom_xyz, synth.nuclear_charges(w.elements))
     f_eps = (78.39 - 1.0) / 78.39
     gms, glue_ms = [], []
-    for k in range(3 + 5):
+    for k in range(0 if args.no_extras else 3 + 5):
         flush.zero_()
         ge[0].record(stream)
         pcm.pcm_gradient(ctx, P, q, stream=stream)
@@ -394,9 +401,10 @@ def run_ours(args):
         if k >= 3:
             gms.append(ge[0].elapsed_time(ge[1]))
             glue_ms.append((ge[1].elapsed_time(ge[2]), ge[2].elapsed_time(ge[3])))
-    line["gradient"] = {"ms": min(gms), "ms_median": statistics.median(gms), "prim_pair_point_per_s": info.prim_pair_points / (min(gms) * 1e-3),
+    if not args.no_extras:
+      line["gradient"] = {"ms": min(gms), "ms_median": statistics.median(gms), "prim_pair_point_per_s": info.prim_pair_points / (min(gms) * 1e-3),
                         "note": "pcm_gradient: Fock sweep at Hermite order L+1 and a three-accumulator point sweep; not part of the step"}
-    line["glue"] = {"bz_plus_rhs_ms": min(g[0] for g in glue_ms), "energy_ms": min(g[1] for g in glue_ms),
+      line["glue"] = {"bz_plus_rhs_ms": min(g[0] for g in glue_ms), "energy_ms": min(g[1] for g in glue_ms),
                     "energy_hartree": float(en[3])}
 
     # ---- A q sweep of configs[4] (BASELINE metric: A q FP64 fraction; HBM GB/s reported as asked)
@@ -525,6 +533,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] A q sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing (cpu_baseline)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the gradient / glue timings that follow the timed region")
     ap.add_argument("--mode", default="step", choices=["step", "kernels"], help="kernels: only the three hot calls (for ncu)")
     ap.add_argument("--config", type=int, default=CONFIG_INDEX, help="--mode kernels: BASELINE.json config index 0..3")
     ap.add_argument("--amat-m", type=int, default=50_000, help="--mode kernels: surface points of the A q call")
