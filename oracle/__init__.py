@@ -60,6 +60,8 @@ def lib():
         L.orc_prim_deriv.argtypes = [C.c_int, C.c_double, _dp, C.c_int, C.c_double, _dp, C.c_double, _dp, _dp, _dp]
         L.orc_gradient.argtypes = basis + [C.c_long, _dp, _dp, _dp, _dp, C.c_long, C.c_double, C.c_long, C.c_void_p,
                                            C.c_long, C.c_void_p, _dp, _dp]
+        L.orc_switching.argtypes = [C.c_long, _dp, _dp, _lp, C.c_long, _dp, _dp, _dp]
+        L.orc_surface_gradient.argtypes = [C.c_long, _dp, _dp, _lp, C.c_long, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp]
         L.orc_bz.argtypes = [C.c_long, _dp, _dp, C.c_long, _dp, _dp, _dp]
         L.orc_rhs.argtypes = [C.c_long, _dp, _dp, C.c_double, _dp]
         L.orc_energy.argtypes = [C.c_long, _dp, _dp, _dp, _dp, C.c_double, _dp]
@@ -282,3 +284,24 @@ def gradient(basis, surface, P, q, shells=None, points=None, cutoff: float = 1e-
     lib().orc_gradient(*_basis_args(basis), surface.M, _f(surface.xyz).reshape(-1), _f(surface.zeta), _f(q), Pm.reshape(-1),
                        Pm.shape[1], float(cutoff), nS, _ptr(sS), nK, _ptr(sK), gs.reshape(-1), gp.reshape(-1))
     return gs, gp
+
+
+# ------------------------------------------------------------------ ISWIG switching function and surface gradient terms
+def switching(surface, atom_xyz, atom_radius) -> np.ndarray:
+    """S_k of Eq. 9 (product over the atoms that do not own point k; surface.atom is the owner)."""
+    S = np.zeros(surface.M)
+    a = _f(atom_xyz).reshape(-1)
+    own = np.ascontiguousarray(surface.atom, np.int64)
+    lib().orc_switching(surface.M, _f(surface.xyz).reshape(-1), _f(surface.zeta), own, len(a) // 3, a, _f(atom_radius), S)
+    return S
+
+
+def surface_gradient(surface, atom_xyz, atom_radius, z, q, f: float):
+    """Gradient of (B z).q + q.A q/(2 f) at fixed q (A_kk through the S_k of Eq. 9): (g_point [M, 3], g_atom [N, 3])."""
+    a = _f(atom_xyz).reshape(-1)
+    n = len(a) // 3
+    gp, ga = np.zeros((surface.M, 3)), np.zeros((n, 3))
+    own = np.ascontiguousarray(surface.atom, np.int64)
+    lib().orc_surface_gradient(surface.M, _f(surface.xyz).reshape(-1), _f(surface.zeta), own, n, a, _f(atom_radius), _f(z), _f(q),
+                               float(f), gp.reshape(-1), ga.reshape(-1))
+    return gp, ga

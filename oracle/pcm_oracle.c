@@ -826,3 +826,83 @@ void orc_gradient(int nshell, const int *l, const double *xyz, const int *nprim,
     }
     free(mask); free(moff); free(po); free(bo);
 }
+
+/* ------------------------------------------------------------------------------------
+ * ISWIG switching function (Eq. 9) and the surface terms of the gradient (Eq. 14):
+ *   S_k = prod_{J != I(k)} S_wf(r_k, R_J),   I(k) = the atom that owns point k,
+ *   S_wf = 1 - (1/2) { erf[zeta_k (R_J - d)] + erf[zeta_k (R_J + d)] },  d = |r_k - R_J|, R_J = cavity radius of atom J.
+ * Gradient of  E_s = (B z).q + (1/2f) q.A q  at fixed q with respect to point positions r_k and atom positions R_J
+ * (as nuclei and as sphere centres), everything else held fixed -- the caller adds a point's row to its owning atom,
+ * because "each MS point only moves with the atom on which it is centered".  With g(z', r) =
+ * d/dr [erf(z' r)/r] = (2 z'/sqrt pi) exp(-z'^2 r^2)/r - erf(z' r)/r^2   (0 at r = 0):
+ *   B term      z_J q_k g(zeta_k, d_kJ) (r_k - R_J)/d_kJ                      -> + point k, - atom J
+ *   A, k != l   (1/f) q_k q_l g(zeta'_kl, r_kl) (r_k - r_l)/r_kl             -> point k  (both orders of the pair)
+ *   A_kk        -(1/2f) q_k^2 A_kk (dS_wf/dd)/S_wf (r_k - R_J)/d_kJ, J != I(k) -> + point k, - atom J,
+ *               dS_wf/dd = (zeta_k/sqrt pi) { exp[-zeta_k^2 (R_J - d)^2] - exp[-zeta_k^2 (R_J + d)^2] }
+ * ---------------------------------------------------------------------------------- */
+static double swf(double zeta, double R, double d) { return 1.0 - 0.5 * (erf(zeta * (R - d)) + erf(zeta * (R + d))); }
+static double dswf(double zeta, double R, double d) {
+    return zeta / sqrt(ORC_PI) * (exp(-zeta * zeta * (R - d) * (R - d)) - exp(-zeta * zeta * (R + d) * (R + d)));
+}
+static double dcoul(double zp, double r) {
+    if (r == 0.0) return 0.0;
+    return 2.0 * zp / sqrt(ORC_PI) * exp(-zp * zp * r * r) / r - erf(zp * r) / (r * r);
+}
+
+void orc_switching(long M, const double *pt_xyz, const double *pt_zeta, const long *pt_atom, long N, const double *atom_xyz,
+                   const double *atom_radius, double *S) {
+#pragma omp parallel for schedule(static)
+    for (long k = 0; k < M; ++k) {
+        double s = 1.0;
+        for (long J = 0; J < N; ++J) {
+            if (J == pt_atom[k]) continue;
+            double dx = pt_xyz[3 * k] - atom_xyz[3 * J], dy = pt_xyz[3 * k + 1] - atom_xyz[3 * J + 1],
+                   dz = pt_xyz[3 * k + 2] - atom_xyz[3 * J + 2];
+            s *= swf(pt_zeta[k], atom_radius[J], sqrt(dx * dx + dy * dy + dz * dz));
+        }
+        S[k] = s;
+    }
+}
+
+void orc_surface_gradient(long M, const double *pt_xyz, const double *pt_zeta, const long *pt_atom, long N,
+                          const double *atom_xyz, const double *atom_radius, const double *z, const double *q, double f,
+                          double *g_point, double *g_atom) {
+    double *S = malloc(sizeof(double) * (size_t)(M > 0 ? M : 1));
+    orc_switching(M, pt_xyz, pt_zeta, pt_atom, N, atom_xyz, atom_radius, S);
+    /* per (point, atom) pair force, kept so that the atom rows can be summed in point order afterwards */
+    double *pa = calloc((size_t)(M > 0 ? M : 1) * (size_t)(N > 0 ? N : 1) * 3, sizeof(double));
+#pragma omp parallel for schedule(static)
+    for (long k = 0; k < M; ++k) {
+        double sum[3] = {0, 0, 0}, comp[3] = {0, 0, 0};
+        const double zk = pt_zeta[k], akk = zk * sqrt(2.0 / ORC_PI) / S[k];
+        for (long J = 0; J < N; ++J) {
+            double e[3] = {pt_xyz[3 * k] - atom_xyz[3 * J], pt_xyz[3 * k + 1] - atom_xyz[3 * J + 1], pt_xyz[3 * k + 2] - atom_xyz[3 * J + 2]};
+            double d = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+            if (d == 0.0) continue;
+            double w = z[J] * q[k] * dcoul(zk, d);
+            if (J != pt_atom[k]) w += -0.5 / f * q[k] * q[k] * akk * dswf(zk, atom_radius[J], d) / swf(zk, atom_radius[J], d);
+            for (int x = 0; x < 3; ++x) {
+                double t = w * e[x] / d;
+                nsum(&sum[x], &comp[x], t);
+                pa[((size_t)k * N + J) * 3 + x] = t;
+            }
+        }
+        for (long l = 0; l < M; ++l) {
+            if (l == k) continue;
+            double e[3] = {pt_xyz[3 * k] - pt_xyz[3 * l], pt_xyz[3 * k + 1] - pt_xyz[3 * l + 1], pt_xyz[3 * k + 2] - pt_xyz[3 * l + 2]};
+            double r = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+            if (r == 0.0) continue;
+            double zl = pt_zeta[l], zp = zk * zl / sqrt(zk * zk + zl * zl);
+            double w = q[k] * q[l] / f * dcoul(zp, r);
+            for (int x = 0; x < 3; ++x) nsum(&sum[x], &comp[x], w * e[x] / r);
+        }
+        for (int x = 0; x < 3; ++x) g_point[3 * k + x] = sum[x] + comp[x];
+    }
+    for (long J = 0; J < N; ++J)
+        for (int x = 0; x < 3; ++x) {
+            double s = 0.0, c = 0.0;
+            for (long k = 0; k < M; ++k) nsum(&s, &c, -pa[((size_t)k * N + J) * 3 + x]);
+            g_atom[3 * J + x] = s + c;
+        }
+    free(pa); free(S);
+}

@@ -20,5 +20,6 @@ from .generators import (  # noqa: F401
     make_workload,
     make_solver_points,
     nuclear_charges,
+    cavity_radii,
     CONFIG_ATOMS,
 )

@@ -25,6 +25,11 @@ _VDW = {"H": 1.20, "C": 1.70, "N": 1.55, "O": 1.52}
 _Z = {"H": 1.0, "C": 6.0, "N": 7.0, "O": 8.0}
 
 
+def cavity_radii(elements) -> np.ndarray:
+    """Cavity radius of every atom in bohr: 1.2 x the van der Waals radius, as make_surface uses."""
+    return np.array([_CAVITY_SCALE * _VDW[e] * ANGSTROM for e in elements], dtype=np.float64)
+
+
 def nuclear_charges(elements) -> np.ndarray:
     """The vector z of Eq. 1 (nuclear charges of the solute's atoms)."""
     return np.array([_Z[e] for e in elements], dtype=np.float64)
