@@ -383,8 +383,9 @@ def run_ours(args):
                    "api": "pcm_rbj_build_async || pcm_potential_host, pcm_cg_solve_host, pcm_fock_host"}
 
     # ---- SURVEY 8(f) rows built so far, timed outside the step: the PCM gradient term (Eq. 14/22) and the glue of Eq. 1/4/13
-    ge = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ge = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
     pcm.pcm_set_nuclei(ctx, w.atom_xyz, synth.nuclear_charges(w.elements))
+    pcm.pcm_set_cavity(ctx, synth.cavity_radii(w.elements), w.surface.atom)
     f_eps = (78.39 - 1.0) / 78.39
     gms, glue_ms = [], []
     for k in range(0 if args.no_extras else 3 + 5):
@@ -397,15 +398,17 @@ def run_ours(args):
         ge[2].record(stream)
         en = pcm.pcm_energy(ctx, u, v, q, f_eps, stream=stream)
         ge[3].record(stream)
+        pcm.pcm_surface_gradient(ctx, q, f_eps, stream=stream)
+        ge[4].record(stream)
         torch.cuda.synchronize()
         if k >= 3:
             gms.append(ge[0].elapsed_time(ge[1]))
-            glue_ms.append((ge[1].elapsed_time(ge[2]), ge[2].elapsed_time(ge[3])))
+            glue_ms.append((ge[1].elapsed_time(ge[2]), ge[2].elapsed_time(ge[3]), ge[3].elapsed_time(ge[4])))
     if not args.no_extras:
       line["gradient"] = {"ms": min(gms), "ms_median": statistics.median(gms), "prim_pair_point_per_s": info.prim_pair_points / (min(gms) * 1e-3),
                         "note": "pcm_gradient: Fock sweep at Hermite order L+1 and a three-accumulator point sweep; not part of the step"}
       line["glue"] = {"bz_plus_rhs_ms": min(g[0] for g in glue_ms), "energy_ms": min(g[1] for g in glue_ms),
-                    "energy_hartree": float(en[3])}
+                    "surface_gradient_ms": min(g[2] for g in glue_ms), "energy_hartree": float(en[3])}
 
     # ---- A q sweep of configs[4] (BASELINE metric: A q FP64 fraction; HBM GB/s reported as asked)
     if not args.no_sweep:

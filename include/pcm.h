@@ -218,6 +218,29 @@ int pcm_gradient(pcm_ctx *ctx, const double *P_dev, int64_t ldp, const double *q
                  void *stream);
 
 /*
+ * ISWIG cavity quantities (Eq. 9) and the surface terms of the gradient (Eq. 14).
+ *
+ * pcm_switching -- S_k = prod_{J != owner(k)} S_wf(r_k, R_J), S_wf = 1 - {erf[zeta_k (R_J - d)] + erf[zeta_k (R_J + d)]}/2,
+ * d = |r_k - R_J|, R_J = cavity radius of atom J, evaluated on the device.  Standalone (no context: S_k is an input of
+ * pcm_setup; the paper drops points with S_k < 1e-8, PAPER.md:106 -- the caller filters).  All arrays HOST: pt_xyz 3*npoint,
+ * pt_zeta npoint, pt_atom npoint (owning atom, -1 = none), atom_xyz 3*natom, atom_radius natom, S npoint (out).
+ * device: CUDA ordinal, -1 = current.  Synchronous.
+ *
+ * pcm_set_cavity -- after pcm_set_nuclei: the cavity radius of each of those atoms and the owning atom of every surface
+ * point (HOST; caller's point order).  Needed by pcm_surface_gradient only.
+ *
+ * pcm_surface_gradient -- gradient of E_s = (B z).q + q.A q/(2f) at fixed q (A_kk = zeta_k sqrt(2/pi)/S_k as given to
+ * pcm_setup, its derivative through Eq. 9):  g_point[3k + x] = dE_s/d(x of point k) with every atom fixed,
+ * g_atom[3J + x] = dE_s/d(x of atom J, as nucleus and as sphere centre) with every point fixed; the caller adds a
+ * point's row to the atom it moves with.  Together with pcm_gradient (times -1: c = -v) this is all of
+ * Eq. 14.  q_dev: DEVICE M; g_point_dev: DEVICE 3*M; g_atom_dev: DEVICE 3*natom (either may be NULL).  Asynchronous.
+ */
+int pcm_switching(int64_t npoint, const double *pt_xyz_host, const double *pt_zeta_host, const int32_t *pt_atom_host, int natom,
+                  const double *atom_xyz_host, const double *atom_radius_host, double *S_host, int device);
+int pcm_set_cavity(pcm_ctx *ctx, const double *atom_radius_host, const int32_t *pt_atom_host);
+int pcm_surface_gradient(pcm_ctx *ctx, const double *q_dev, double f, double *g_point_dev, double *g_atom_dev, void *stream);
+
+/*
  * Host-buffer forms of the four hot calls: same semantics, every array is a HOST pointer; the call
  * copies inputs to the device, runs the device path on the context's own stream, copies the result back
  * and synchronises.  These are what bench.py's end-to-end figure times.

@@ -30,7 +30,7 @@ EXPORTS = (
     "pcm_rbj_build", "pcm_rbj_get", "pcm_cg_solve", "pcm_potential_host", "pcm_fock_host", "pcm_amatvec_host",
     "pcm_cg_solve_host", "pcm_get_info", "pcm_set_timing", "pcm_last_kernel_ms", "pcm_last_class_ms",
     "pcm_launch_count", "pcm_fp64_peak", "pcm_set_nuclei", "pcm_nuclear_potential", "pcm_rhs", "pcm_energy",
-    "pcm_cg_threshold", "pcm_gradient", "pcm_last_cg_matvec_ms", "pcm_rbj_build_async",
+    "pcm_cg_threshold", "pcm_gradient", "pcm_last_cg_matvec_ms", "pcm_rbj_build_async", "pcm_switching", "pcm_set_cavity", "pcm_surface_gradient",
     "pcm_schwarz_bound", "pcm_last_error", "pcm_destroy",
 )
 
@@ -101,6 +101,9 @@ def lib(build: bool = False):
         L.pcm_energy.argtypes = [vp, vp, vp, vp, C.c_double, _dp, vp]
         L.pcm_cg_threshold.argtypes = [C.c_double, C.c_double, _dp]
         L.pcm_gradient.argtypes = [vp, vp, C.c_int64, vp, vp, vp, vp]
+        L.pcm_switching.argtypes = [C.c_int64, vp, vp, vp, C.c_int, vp, vp, vp, C.c_int]
+        L.pcm_set_cavity.argtypes = [vp, vp, vp]
+        L.pcm_surface_gradient.argtypes = [vp, vp, C.c_double, vp, vp, vp]
         L.pcm_schwarz_bound.argtypes = [C.c_int, C.c_double, vp, C.c_int, C.c_double, vp, _dp]
         L.pcm_last_error.argtypes = [vp]
         L.pcm_last_error.restype = C.c_char_p
@@ -151,6 +154,8 @@ class Context:
         self.nbf = nbf
         self.M = M
         self.device = device
+        self.nshell = 0
+        self.natom = 0
 
     def __del__(self):
         try:
@@ -243,6 +248,7 @@ def pcm_set_nuclei(ctx: Context, atom_xyz, z) -> None:
     if len(xyz) != 3 * len(zz):
         raise ValueError("atom_xyz must hold 3 doubles per nuclear charge")
     _check(lib().pcm_set_nuclei(ctx.handle, len(zz), _hp(xyz), _hp(zz)), ctx.handle)
+    ctx.natom = len(zz)
 
 
 def pcm_nuclear_potential(ctx: Context, u=None, stream=None):
@@ -280,6 +286,35 @@ def pcm_gradient(ctx: Context, P, q, stream=None):
     _check(lib().pcm_gradient(ctx.handle, C.c_void_p(P.data_ptr()), P.stride(0), _dev(q, ctx.M), C.c_void_p(gs.data_ptr()),
                               C.c_void_p(gp.data_ptr()), _stream(stream)), ctx.handle)
     return gs, gp
+
+
+def pcm_switching(pt_xyz, pt_zeta, pt_atom, atom_xyz, atom_radius, device: int = -1) -> np.ndarray:
+    """S_k of Eq. 9 (device arithmetic, host arrays)."""
+    px, pz = _np(pt_xyz, np.float64).reshape(-1), _np(pt_zeta, np.float64)
+    pa = _np(pt_atom, np.int32)
+    ax, ar = _np(atom_xyz, np.float64).reshape(-1), _np(atom_radius, np.float64)
+    S = np.zeros(len(pz))
+    _check(lib().pcm_switching(len(pz), _hp(px), _hp(pz), _hp(pa), len(ar), _hp(ax), _hp(ar), _hp(S), int(device)))
+    return S
+
+
+def pcm_set_cavity(ctx: Context, atom_radius, pt_atom) -> None:
+    ar, pa = _np(atom_radius, np.float64), _np(pt_atom, np.int32)
+    if len(pa) != ctx.M:
+        raise ValueError("pt_atom must have one entry per surface point")
+    if len(ar) != ctx.natom:
+        raise ValueError("atom_radius must have one entry per atom given to pcm_set_nuclei")
+    _check(lib().pcm_set_cavity(ctx.handle, _hp(ar), _hp(pa)), ctx.handle)
+
+
+def pcm_surface_gradient(ctx: Context, q, f: float, stream=None):
+    """(g_point [M, 3], g_atom [natom, 3]) of (B z).q + q.A q/(2 f) at fixed q (Eq. 14 surface terms)."""
+    import torch
+    gp = torch.empty((ctx.M, 3), dtype=torch.float64, device=q.device)
+    ga = torch.empty((ctx.natom, 3), dtype=torch.float64, device=q.device)
+    _check(lib().pcm_surface_gradient(ctx.handle, _dev(q, ctx.M), float(f), C.c_void_p(gp.data_ptr()), C.c_void_p(ga.data_ptr()),
+                                      _stream(stream)), ctx.handle)
+    return gp, ga
 
 
 def pcm_cg_threshold(diis_prev: float, delta_min: float = 1e-6) -> float:

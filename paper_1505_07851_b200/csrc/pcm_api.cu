@@ -185,6 +185,7 @@ int pcm_set_nuclei(pcm_ctx *ctx, int natom, const double *atom_xyz_host, const d
     }
     PCM_CUDA(ctx, cudaMemcpy(ctx->atoms, at.data(), at.size() * sizeof(double4), cudaMemcpyHostToDevice));
     ctx->natom = natom;
+    ctx->cavity_set = false;   // radii belong to the atom list
     return PCM_OK;
 }
 
@@ -221,6 +222,46 @@ int pcm_gradient(pcm_ctx *ctx, const double *P_dev, int64_t ldp, const double *q
     if ((ctx->nbf > 0 && !P_dev) || (ctx->M > 0 && !q_dev) || ldp < ctx->nbf) return set_error(ctx, PCM_ERR_ARG, "pcm_gradient: bad argument");
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
     return launch_gradient(ctx, P_dev, ldp, q_dev, g_shell_dev, g_point_dev, (cudaStream_t)stream);
+}
+
+int pcm_switching(int64_t npoint, const double *pt_xyz_host, const double *pt_zeta_host, const int32_t *pt_atom_host, int natom,
+                  const double *atom_xyz_host, const double *atom_radius_host, double *S_host, int device) {
+    if (npoint < 0 || natom < 0 || (npoint > 0 && (!pt_xyz_host || !pt_zeta_host || !pt_atom_host || !S_host)) ||
+        (natom > 0 && (!atom_xyz_host || !atom_radius_host)))
+        return set_error(nullptr, PCM_ERR_ARG, "pcm_switching: bad argument");
+    if (device >= 0) {
+        cudaError_t e = cudaSetDevice(device);
+        if (e != cudaSuccess) return set_error(nullptr, PCM_ERR_CUDA, std::string("pcm_switching: ") + cudaGetErrorString(e));
+    }
+    return switching_host(npoint, pt_xyz_host, pt_zeta_host, pt_atom_host, natom, atom_xyz_host, atom_radius_host, S_host);
+}
+
+int pcm_set_cavity(pcm_ctx *ctx, const double *atom_radius_host, const int32_t *pt_atom_host) {
+    PCM_CHECK_CTX(ctx);
+    if (ctx->natom < 0) return set_error(ctx, PCM_ERR_STATE, "pcm_set_cavity: call pcm_set_nuclei first");
+    if ((ctx->natom > 0 && !atom_radius_host) || (ctx->M > 0 && !pt_atom_host)) return set_error(ctx, PCM_ERR_ARG, "pcm_set_cavity: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    std::vector<int32_t> own((size_t)std::max<int64_t>(ctx->M, 1), -1);
+    for (int64_t s = 0; s < ctx->M; ++s) {
+        const int32_t a = pt_atom_host[ctx->s2c_host[(size_t)s]];
+        if (a < -1 || a >= ctx->natom) return set_error(ctx, PCM_ERR_ARG, "pcm_set_cavity: owner index out of range");
+        own[(size_t)s] = a;
+    }
+    int rc;
+    if ((rc = dev_alloc_t(ctx, &ctx->atom_radius, (size_t)std::max<int64_t>(ctx->natom, 1)))) return rc;
+    if ((rc = dev_alloc_t(ctx, &ctx->pt_owner, own.size()))) return rc;
+    if (ctx->natom > 0) PCM_CUDA(ctx, cudaMemcpy(ctx->atom_radius, atom_radius_host, (size_t)ctx->natom * 8, cudaMemcpyHostToDevice));
+    PCM_CUDA(ctx, cudaMemcpy(ctx->pt_owner, own.data(), own.size() * 4, cudaMemcpyHostToDevice));
+    ctx->cavity_set = true;
+    return PCM_OK;
+}
+
+int pcm_surface_gradient(pcm_ctx *ctx, const double *q_dev, double f, double *g_point_dev, double *g_atom_dev, void *stream) {
+    PCM_CHECK_CTX(ctx);
+    if (!ctx->cavity_set) return set_error(ctx, PCM_ERR_STATE, "pcm_surface_gradient: call pcm_set_nuclei and pcm_set_cavity first");
+    if ((ctx->M > 0 && !q_dev) || !(f != 0.0)) return set_error(ctx, PCM_ERR_ARG, "pcm_surface_gradient: bad argument");
+    PCM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_surface_gradient(ctx, q_dev, f, g_point_dev, g_atom_dev, (cudaStream_t)stream);
 }
 
 int pcm_cg_threshold(double diis_prev, double delta_min, double *delta_out) {

@@ -135,6 +135,12 @@ struct pcm_ctx {
     // nuclei (pcm_set_nuclei): (x, y, z, charge)
     int64_t natom = -1;
     double4 *atoms = nullptr;
+    // cavity (pcm_set_cavity): radius of every atom's sphere, owning atom of every point (sorted point order)
+    double *atom_radius = nullptr;
+    int32_t *pt_owner = nullptr;
+    bool cavity_set = false;
+    double *surf_scratch = nullptr;   // pcm_surface_gradient partial sums (grow-only)
+    size_t surf_scratch_n = 0;
 
     // pcm_gradient (pcm_options.gradient): derivative tables and the shell bookkeeping of the pair transform
     int64_t nshell = 0;
@@ -230,6 +236,9 @@ int energy_terms(pcm_ctx *ctx, const double *u, const double *v, const double *q
 int launch_gradient(pcm_ctx *ctx, const double *P, int64_t ldp, const double *q, double *g_shell, double *g_point, cudaStream_t s);
 int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order_host, cudaStream_t s, bool async, bool force_global);
 int rbj_finish(pcm_ctx *ctx, cudaStream_t s);
+int launch_surface_gradient(pcm_ctx *ctx, const double *q, double f, double *g_point, double *g_atom, cudaStream_t s);
+int switching_host(int64_t M, const double *xyz, const double *zeta, const int32_t *owner, int natom, const double *atom_xyz,
+                   const double *atom_radius, double *S);
 int plan_all(pcm_ctx *ctx);
 int fill_amat_blocks(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
