@@ -841,13 +841,15 @@ static void plan_class(pcm_ctx *ctx) {
 int plan_all(pcm_ctx *ctx) {
     // symmetric sweep: about half of the (row block, chunk) grid has work
     ctx->amat_R = ctx->M >= AMAT_R4_MIN ? 4 : 2;
-    if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 2 || r == 4) ctx->amat_R = r; }
+    if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 1 || r == 2 || r == 4) ctx->amat_R = r; }
     double aw = 8.0;
     if (const char *e = getenv("PCM_AMAT_WAVES")) aw = atof(e);
     // small M: column tiles of 128 (four times the work items of the same sweep, so that the SMs stay evenly loaded)
-    ctx->amat_tile = (ctx->amat_R == 2 && ctx->M < AMAT_T128_MAX) ? 128 : 256;
+    ctx->amat_tile = (ctx->amat_R <= 2 && ctx->M < AMAT_T128_MAX) ? 128 : 256;
     if (const char *e = getenv("PCM_AMAT_TILE")) { const int t = atoi(e); if ((t == 128 && ctx->amat_R == 2) || t == 256) ctx->amat_tile = t; }
-    ctx->plan_amat = ctx->amat_R == 4 ? make_plan(ctx->M, TPB * 4, ctx->M, 256, wave_of(ctx, amatvec_kernel<4, AMAT_C, 256>), 0.5, aw)
+    if (ctx->amat_R == 1) ctx->amat_tile = 128;
+    ctx->plan_amat = ctx->amat_R == 1 ? make_plan(ctx->M, TPB * 1, ctx->M, 128, wave_of(ctx, amatvec_kernel<1, 4, 128>), 0.5, aw) :
+                     ctx->amat_R == 4 ? make_plan(ctx->M, TPB * 4, ctx->M, 256, wave_of(ctx, amatvec_kernel<4, AMAT_C, 256>), 0.5, aw)
                      : ctx->amat_tile == 256 ? make_plan(ctx->M, TPB * 2, ctx->M, 256, wave_of(ctx, amatvec_kernel<2, AMAT_C, 256>), 0.5, aw)
                                              : make_plan(ctx->M, TPB * 2, ctx->M, 128, wave_of(ctx, amatvec_kernel<2, AMAT_C, 128>), 0.5, aw);
     if (getenv("PCM_VERBOSE")) fprintf(stderr, "[pcm] amat plan: R %d xb %lld chunks %lld chunk_len %lld\n", ctx->amat_R,
@@ -893,7 +895,9 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
         { ctx->launches[2]++; ctx->launch_total++; }
     }
-    if (ctx->amat_R == 4)
+    if (ctx->amat_R == 1)
+        amatvec_kernel<1, 4, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+    else if (ctx->amat_R == 4)
         amatvec_kernel<4, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
     else if (ctx->amat_tile == 256)
         amatvec_kernel<2, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
