@@ -51,8 +51,9 @@ TRAFFIC = {"amatvec": 379648.0, "potential": [1715200.0, 2185216.0, 1097216.0, N
            "fock": [1546496.0, 1363712.0, 639488.0, None, None]}
 WORK = {
     # A q: the sweep is symmetric -- one evaluation of 1/r_ij serves A_ij and A_ji; unit = one pair evaluation
-    # (M^2/2 per call): geometry 6 + rsqrt 5 + two FMAs + 1/4 DADD of the column reduction = 13.25 instr, 20.25 flop.
-    "amatvec": [(13.25, 20.25)],
+    # (M^2/2 per call), R = 4 kernel: local-origin geometry 4 + 3/16 (1 DADD + 3 DFMA, the row shift amortised over 32
+    # columns), rsqrt 5 (2 DMUL + 3 DFMA), two FMAs, 1/4 DADD of the column reduction = 11.44 instr, 19.4 flop.
+    "amatvec": [(11.44, 19.4)],
     "potential": [(12, 18), (18, 27), (32, 51), (57, 94), (97, 164)],
     "fock": [(12, 18), (18, 28), (30, 46), (54, 84), (94, 150)],
 }

@@ -32,9 +32,11 @@ constexpr int PT_TILE = 256;  // surface points staged per shared-memory tile (F
 // holds R whole row groups and every skip/run decision is warp-uniform.
 // ---------------------------------------------------------------------------------------------
 struct Blocking { int R, C; };
-// A q: R = 4 (row blocks of 512) for large M, R = 2 (row blocks of 256, four times the blocks) below AMAT_R4_MIN points
+// A q: R = 4 (row blocks of 512, column tiles of 256) from AMAT_R4_MIN points on; below, R = 1 with column tiles of 128
+// (work items of 128 x 128 evaluations: sixteen times as many, so that a 9k-point sweep still loads 148 SMs evenly).
+// R = 2 remains selectable (PCM_AMAT_R) for experiments.
 constexpr int AMAT_C = 2;
-constexpr int64_t AMAT_R4_MIN = 60000;
+constexpr int64_t AMAT_R4_MIN = 20000;
 constexpr int64_t AMAT_T128_MAX = 30000;
 __host__ __device__ constexpr Blocking fock_blocking(int L) {
     return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{2, 2} : L == 2 ? Blocking{1, 4} : Blocking{1, 2};
@@ -101,12 +103,44 @@ __device__ __forceinline__ void stage_points(const double4 *__restrict__ pt, con
 
 // Symmetric sweep: A_ij = A_ji, so an evaluation 1/r_ij serves row i (y_i += q_j/r) and column j (y_j += q_i/r).
 // Block (rb, chunk) owns the rows [rb RB, (rb+1) RB), RB = TPB R, and the column tiles of its chunk that do not lie
-// before its rows:  tiles inside the row range (the diagonal band) are swept the plain way, rows only; tiles beyond it
-// are swept once for both triangles.  Row sums go to out[chunk][i] (only chunks that reach the row's block are written,
-// amat_first_slot), column sums to colpart[rb][j] (only rb < amat_sym_blocks(j) are written); amat_row_sum adds them
-// in a fixed order.  Per evaluation 13 FP64 instructions + 1/R DADD for two entries of A instead of 12 per entry.
+// before its rows:  tiles inside the row range (the diagonal band) are swept for the rows only; tiles beyond it are
+// swept once for both triangles.  Row sums go to out[chunk][i] (only chunks that reach the row's block are written),
+// column sums to colpart[rb][j] (only the row blocks before the tile of j); amat_row_sum_block adds them in a fixed order.
 // Column sums: a lane adds its R rows in registers, the 32 lanes are then summed through a [16][33] shared-memory
 // transpose per warp (one DADD per column and lane), the 4 warps at the end of the tile.
+//
+// Geometry in local coordinates: the 32 columns of a group are staged relative to their first point o as
+// (-2 (b - o), |b - o|^2), a row is shifted once per group (a - o, |a - o|^2: 6 instructions per 32 evaluations),
+// and r^2 = |a - o|^2 + |b - o|^2 - 2 (a - o).(b - o) costs 1 DADD + 3 DFMA instead of 3 DADD + DMUL + 2 DFMA.  |b - o| is
+// the extent of 32 neighbouring points and far patches are further apart than that, so the cancellation costs a few ulp
+// of r^2 (<= 20 eps for a gap of 2 bohr and an extent of 3.5).  Per evaluation 11.4 FP64 instructions (R = 4) for two
+// entries of A: geometry 4 + 3/16, rsqrt 5, two FMAs, 1/R DADD of the column reduction.
+__device__ __forceinline__ double r2_local(double alx, double aly, double alz, double a2, const double4 &b) {
+    return fma(alx, b.x, fma(aly, b.y, fma(alz, b.z, a2 + b.w)));
+}
+
+// stages the columns [base, base + nst*32) of the chunk ending at jend: s_pt = (-2 (b - o), |b - o|^2), s_q = charge,
+// s_org[g] = origin o of column group g (its first point).
+// Padding columns sit on the origin with zero charge.
+__device__ __forceinline__ void stage_points_local(const double4 *__restrict__ pt, const double *__restrict__ q,
+                                                   const int32_t *__restrict__ qidx, int base, int jend, int nst, double4 *s_pt,
+                                                   double *s_q, double4 *s_org) {
+    for (int t = threadIdx.x; t < nst * SUB; t += TPB) {
+        const int j = base + t, jo = min(base + (t & ~31), jend - 1);
+        const double4 o = pt[jo];
+        if ((t & 31) == 0) s_org[t >> 5] = o;
+        if (j < jend) {
+            const double4 b = pt[j];
+            const double x = b.x - o.x, y = b.y - o.y, z = b.z - o.z;
+            s_pt[t] = make_double4(-2.0 * x, -2.0 * y, -2.0 * z, fma(z, z, fma(y, y, x * x)));
+            s_q[t] = q[qidx ? qidx[j] : j];
+        } else {
+            s_pt[t] = make_double4(0.0, 0.0, 0.0, 0.0);
+            s_q[t] = 0.0;
+        }
+    }
+}
+
 template <int R, int C, int TILE>
 __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ q,
                                                       const int32_t *__restrict__ qidx, int M, int chunk_len,
@@ -117,28 +151,25 @@ __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict_
     constexpr int RB = TPB * R;
     constexpr int NW = TPB / 32;
     static_assert(RB % TILE == 0, "row blocks must be whole column tiles");
-    __shared__ double4 s_pt[TILE];       // x, y, z, q
+    __shared__ double4 s_pt[TILE];          // -2 (b - o), |b - o|^2
+    __shared__ double s_q[TILE];            // column charges
+    __shared__ double4 s_org[TILE / 32];    // origin of every column group
     __shared__ double s_c[NW][16 * 33];     // per warp: [column of the half group][lane]
-    __shared__ double s_cs[NW][TILE];    // per warp: column sums of the tile
+    __shared__ double s_cs[NW][TILE];       // per warp: column sums of the tile
     if (stop && *stop) return;  // a converged CG solve: the iterations queued behind it are no-ops
     const int r0 = blockIdx.x * RB;
     const int jbeg = blockIdx.y * chunk_len, jend = min(M, jbeg + chunk_len);
-    if (jend <= r0) return;     // the chunk lies before the rows: the blocks of those rows cover it (amat_first_slot)
+    if (jend <= r0) return;     // the chunk lies before the rows: the blocks of those rows cover it
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t rg0 = ((int64_t)blockIdx.x * NW + warp) * R;
-    double ax[R], ay[R], az[R], qa[R], y[R];
+    double qa[R], y[R], ax[R], ay[R], az[R];
     int ii[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         ii[r] = (int)(rg0 + r) * SUB + lane;
-        if (ii[r] < M) {
-            const double4 a = pt[ii[r]];
-            ax[r] = a.x; ay[r] = a.y; az[r] = a.z;
-            qa[r] = q[qidx ? qidx[ii[r]] : ii[r]];
-        } else {  // padding: far from everything (and from the column padding), zero charge
-            ax[r] = ay[r] = az[r] = -3e8;
-            qa[r] = 0.0;
-        }
+        qa[r] = ii[r] < M ? q[qidx ? qidx[ii[r]] : ii[r]] : 0.0;   // padding rows: zero charge, their sums are not stored
+        const double4 a = pt[min(ii[r], M - 1)];
+        ax[r] = ii[r] < M ? a.x : a.x + 3e8; ay[r] = a.y; az[r] = a.z;   // padding rows: far away
         y[r] = 0.0;
     }
     double *sc = s_c[warp];
@@ -147,102 +178,76 @@ __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict_
         const bool sym = base >= r0 + RB;
         const unsigned bits = far_bits<R, NS>(farmap, nbyte, rg0, nrg, base / SUB, lane);
         __syncthreads();
-        stage_points(pt, q, qidx, base, jend, nst, s_pt);
+        stage_points_local(pt, q, qidx, base, jend, nst, s_pt, s_q, s_org);
         __syncthreads();
         for (int st = 0; st < nst; ++st) {
-            const double4 *sp = s_pt + st * SUB;
             const unsigned m = row_mask<R>(bits, st);
-            if (!sym) {
-                if (m == (1u << R) - 1u) {
-#pragma unroll 1
-                    for (int t = 0; t < SUB; t += C) {
-                        double4 b[C];
-                        double r2[C][R];
-#pragma unroll
-                        for (int c = 0; c < C; ++c) b[c] = sp[t + c];
-#pragma unroll
-                        for (int c = 0; c < C; ++c)
-#pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const double dx = ax[r] - b[c].x, dy = ay[r] - b[c].y, dz = az[r] - b[c].z;
-                                r2[c][r] = fma(dz, dz, fma(dy, dy, dx * dx));
-                            }
-#pragma unroll
-                        for (int c = 0; c < C; ++c)
-#pragma unroll
-                            for (int r = 0; r < R; ++r) y[r] = fma(b[c].w, rsqrt_fast(r2[c][r]), y[r]);
-                    }
-                } else if (m) {
-#pragma unroll 1
-                    for (int t = 0; t < SUB; ++t) {
-                        const double4 b = sp[t];
-#pragma unroll
-                        for (int r = 0; r < R; ++r)
-                            if ((m >> r) & 1u) {
-                                const double dx = ax[r] - b.x, dy = ay[r] - b.y, dz = az[r] - b.z;
-                                y[r] = fma(b.w, rsqrt_fast(fma(dz, dz, fma(dy, dy, dx * dx))), y[r]);
-                            }
-                    }
-                }
+            if (m == 0) {
+                if (sym) s_cs[warp][st * SUB + lane] = 0.0;
                 continue;
             }
-            if (m == 0) {
-                s_cs[warp][st * SUB + lane] = 0.0;
-                continue;
+            // the rows of this thread relative to the column group's origin
+            const double4 o = s_org[st];
+            double alx[R], aly[R], alz[R], a2[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                alx[r] = ax[r] - o.x; aly[r] = ay[r] - o.y; alz[r] = az[r] - o.z;
+                a2[r] = fma(alz[r], alz[r], fma(aly[r], aly[r], alx[r] * alx[r]));
             }
 #pragma unroll 1
             for (int half = 0; half < 2; ++half) {
+                const double4 *sp = s_pt + st * SUB + half * 16;
+                const double *sq = s_q + st * SUB + half * 16;
                 if (m == (1u << R) - 1u) {
 #pragma unroll 1
                     for (int t = 0; t < 16; t += C) {
                         double4 b[C];
-                        double r2[C][R], cc[C];
+                        double qb[C], r2[C][R], cc[C];
 #pragma unroll
-                        for (int c = 0; c < C; ++c) b[c] = sp[half * 16 + t + c];
+                        for (int c = 0; c < C; ++c) { b[c] = sp[t + c]; qb[c] = sq[t + c]; }
 #pragma unroll
                         for (int c = 0; c < C; ++c)
 #pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const double dx = ax[r] - b[c].x, dy = ay[r] - b[c].y, dz = az[r] - b[c].z;
-                                r2[c][r] = fma(dz, dz, fma(dy, dy, dx * dx));
-                            }
+                            for (int r = 0; r < R; ++r) r2[c][r] = r2_local(alx[r], aly[r], alz[r], a2[r], b[c]);
 #pragma unroll
                         for (int c = 0; c < C; ++c) {
                             cc[c] = 0.0;
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
                                 const double rs = rsqrt_fast(r2[c][r]);
-                                y[r] = fma(b[c].w, rs, y[r]);
+                                y[r] = fma(qb[c], rs, y[r]);
                                 cc[c] = fma(qa[r], rs, cc[c]);
                             }
-                            sc[(t + c) * 33 + lane] = cc[c];
+                            if (sym) sc[(t + c) * 33 + lane] = cc[c];
                         }
                     }
                 } else {
 #pragma unroll 1
                     for (int t = 0; t < 16; ++t) {
-                        const double4 b = sp[half * 16 + t];
+                        const double4 b = sp[t];
+                        const double qb = sq[t];
                         double cc = 0.0;
 #pragma unroll
                         for (int r = 0; r < R; ++r)
                             if ((m >> r) & 1u) {
-                                const double dx = ax[r] - b.x, dy = ay[r] - b.y, dz = az[r] - b.z;
-                                const double rs = rsqrt_fast(fma(dz, dz, fma(dy, dy, dx * dx)));
-                                y[r] = fma(b.w, rs, y[r]);
+                                const double rs = rsqrt_fast(r2_local(alx[r], aly[r], alz[r], a2[r], b));
+                                y[r] = fma(qb, rs, y[r]);
                                 cc = fma(qa[r], rs, cc);
                             }
-                        sc[t * 33 + lane] = cc;
+                        if (sym) sc[t * 33 + lane] = cc;
                     }
                 }
-                __syncwarp();
-                // lane l sums column (l & 15) over the lanes [16 (l >> 4), 16 (l >> 4) + 16), fixed order
-                const double *col = sc + (lane & 15) * 33 + (lane >> 4) * 16;
-                double s = col[0];
+                if (sym) {
+                    __syncwarp();
+                    // lane l sums column (l & 15) over the lanes [16 (l >> 4), 16 (l >> 4) + 16), fixed order
+                    const double *col = sc + (lane & 15) * 33 + (lane >> 4) * 16;
+                    double s = col[0];
 #pragma unroll
-                for (int k = 1; k < 16; ++k) s += col[k];
-                const double o = __shfl_xor_sync(0xffffffffu, s, 16);
-                if (lane < 16) s_cs[warp][st * SUB + half * 16 + lane] = s + o;
-                __syncwarp();
+                    for (int k = 1; k < 16; ++k) s += col[k];
+                    const double o2 = __shfl_xor_sync(0xffffffffu, s, 16);
+                    if (lane < 16) s_cs[warp][st * SUB + half * 16 + lane] = s + o2;
+                    __syncwarp();
+                }
             }
         }
         if (sym) {
@@ -840,7 +845,7 @@ static void plan_class(pcm_ctx *ctx) {
 
 int plan_all(pcm_ctx *ctx) {
     // symmetric sweep: about half of the (row block, chunk) grid has work
-    ctx->amat_R = ctx->M >= AMAT_R4_MIN ? 4 : 2;
+    ctx->amat_R = ctx->M >= AMAT_R4_MIN ? 4 : 1;
     if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 1 || r == 2 || r == 4) ctx->amat_R = r; }
     double aw = 8.0;
     if (const char *e = getenv("PCM_AMAT_WAVES")) aw = atof(e);
