@@ -53,7 +53,9 @@ WORK = {
     # A q: the sweep is symmetric -- one evaluation of 1/r_ij serves A_ij and A_ji; unit = one pair evaluation
     # (M^2/2 per call), R = 4 kernel: local-origin geometry 4 + 3/16 (1 DADD + 3 DFMA, the row shift amortised over 32
     # columns), rsqrt 5 (2 DMUL + 3 DFMA), two FMAs, 1/4 DADD of the column reduction = 11.44 instr, 19.4 flop.
-    "amatvec": [(11.44, 19.4)],
+    # Below 20 000 points the R = 1 kernel runs: the column reduction costs a whole DADD per evaluation (12.19 instr, 20.25 flop).
+    "amatvec": [(11.44, 19.5)],
+    "amatvec_small": [(12.19, 20.25)],
     "potential": [(12, 18), (18, 27), (32, 51), (57, 94), (97, 164)],
     "fock": [(12, 18), (18, 28), (30, 46), (54, 84), (94, 150)],
 }
@@ -326,10 +328,11 @@ def run_ours(args):
     cands.append(("amatvec", 0, mv_ms, int(iters) + 1))
     op, Ld, ms_dom, per_step = max(cands, key=lambda c: c[2] * c[3])
     n_units = 0.5 * float(M) * M if op == "amatvec" else float(info.products[Ld]) * M
-    instr, flop = WORK[op][Ld]
+    wk = lambda o, L: WORK["amatvec_small" if (o == "amatvec" and M < 20000) else o][L]
+    instr, flop = wk(op, Ld)
     achieved = n_units * flop / (ms_dom * 1e-3) * 1e-12
     kernels = {f"{o}_L{L}": {"ms_per_launch": ms, "launches_per_step": n,
-                             "frac": (0.5 * float(M) * M if o == "amatvec" else float(info.products[L]) * M) * WORK[o][L][1] / (ms * 1e-3) * 1e-12 / peak_tflops}
+                             "frac": (0.5 * float(M) * M if o == "amatvec" else float(info.products[L]) * M) * wk(o, L)[1] / (ms * 1e-3) * 1e-12 / peak_tflops}
                for (o, L, ms, n) in cands if ms > 0.01}
     roofline = {"bound": "alu", "kernel": ("amatvec_kernel (CG iteration, M = %d; unit = pair evaluation of the symmetric sweep)" % M)
                 if op == "amatvec" else f"{op}_kernel<L={Ld}>", "launches_per_step": per_step,
@@ -429,7 +432,7 @@ def run_ours(args):
                 pcm.pcm_amatvec(c4, qd, yd)
                 ts.append(sum(pcm.pcm_last_kernel_ms(c4, pcm.OP_AMATVEC)[:2]))
             ms = min(ts)
-            instr, flop = WORK["amatvec"][0]
+            instr, flop = WORK["amatvec" if Ms >= 20000 else "amatvec_small"][0]
             pairs = 0.5 * float(Ms) * Ms
             tf = pairs * flop / (ms * 1e-3) * 1e-12
             sweep.append({"M": Ms, "ms": ms, "ms_median": statistics.median(ts), "entries_per_s": float(Ms) * Ms / (ms * 1e-3),
