@@ -84,3 +84,29 @@ def test_gradient_medium_sampled(pcm, orc, torch_cuda):
     check(gp[points], rp, "g_point")
     assert np.abs(gs.sum(0) + gp.sum(0)).max() < 1e-9
     pcm.pcm_destroy(ctx)
+
+
+def test_gradient_degenerate_sizes(pcm, orc, torch_cuda):
+    """no points / no shells / one primitive and one point: zeros of the right shape, and the closed form through the oracle"""
+    torch = torch_cuda
+    w = synth.make_workload(0, with_d=False)
+    b, s = w.basis, w.surface
+    ctx = pcm.pcm_setup(b.shell_l, b.shell_xyz, b.shell_nprim, b.prim_exp, b.prim_coef, np.zeros((0, 3)), np.zeros(0), gradient=True)
+    gs, gp = pcm.pcm_gradient(ctx, dev(torch, w.P), torch.zeros(0, dtype=torch.float64, device="cuda"))
+    assert gs.shape == (b.nshell, 3) and gp.shape == (0, 3) and (gs == 0).all()
+    pcm.pcm_destroy(ctx)
+    ctx = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s.xyz, s.zeta, gradient=True)
+    gs, gp = pcm.pcm_gradient(ctx, torch.zeros((0, 0), dtype=torch.float64, device="cuda"), dev(torch, w.q))
+    assert gs.shape == (0, 3) and gp.shape == (s.M, 3) and (gp == 0).all()
+    pcm.pcm_destroy(ctx)
+    one = synth.Basis(np.array([1], np.int32), np.array([[0.1, 0.2, 0.3]]), np.array([1], np.int32), np.array([0.9]),
+                      np.array([1.3]), np.array([0], np.int32), True)
+    s1 = synth.Surface(np.array([[1.0, -0.5, 0.7]]), np.array([2.2]), np.ones(1), np.zeros(1, np.int32))
+    P = np.array([[1.0, 0.2, -0.3], [0.2, 0.5, 0.1], [-0.3, 0.1, 2.0]])
+    ctx = pcm.setup_from_workload(one, s1, gradient=True)
+    gs, gp = pcm.pcm_gradient(ctx, dev(torch, P), dev(torch, [0.7]))
+    rs, rp = orc.gradient(one, s1, P, np.array([0.7]))
+    check(gs.cpu().numpy(), rs, "one p shell, one point: g_shell")
+    check(gp.cpu().numpy(), rp, "one p shell, one point: g_point")
+    assert np.abs(gs.cpu().numpy() + gp.cpu().numpy()).max() < 1e-14      # two bodies: equal and opposite
+    pcm.pcm_destroy(ctx)
