@@ -342,7 +342,7 @@ static int grad_reduce_herm(pcm_ctx *ctx, cudaStream_t s) {
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
     const int64_t plane = (int64_t)nherm(L + 1) * c.npad;
-    reduce_herm_kernel<<<(unsigned)ceil_div(plane, 256), 256, 0, s>>>(c.gherm, plane, (int)ctx->plan_gfock[L].chunks, c.npad,
+    reduce_herm_kernel<<<(unsigned)ceil_div(plane, 32), 256, 0, s>>>(c.gherm, plane, (int)ctx->plan_gfock[L].chunks, c.npad,
                                                                       nherm(L + 1), c.near_gfock, c.fock_map.pstart);
     PCM_LAUNCH_CHECK(ctx);
     ctx->launch_total++;

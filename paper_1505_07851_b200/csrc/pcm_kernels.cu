@@ -383,20 +383,29 @@ struct NearRefs {
     const int64_t *pstart[MAXL + 1];
     int count;
 };
-// out[idx ? idx[k] : k] = sum_slots part[slot][k] + sum of the near pieces of row k  (fixed order)
-__global__ void reduce_slots_kernel(const double *__restrict__ part, int64_t n, int slots, double *__restrict__ out,
-                                    const int32_t *__restrict__ idx, NearRefs nr) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n) return;
+// out[idx ? idx[k] : k] = sum_slots part[slot][k] + sum of the near pieces of row k.  A 256-thread block sums 32 rows:
+// warp w adds every 8th slot (and every 8th near piece of every class) for row lane, coalesced across the lanes; the
+// eight partial sums are then added in order.  Fixed order, so the result is bit-reproducible.
+__global__ void __launch_bounds__(256) reduce_slots_kernel(const double *__restrict__ part, int64_t n, int slots,
+                                                           double *__restrict__ out, const int32_t *__restrict__ idx, NearRefs nr) {
+    __shared__ double s_tmp[8 * 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t k = (int64_t)blockIdx.x * 32 + lane;
     double s = 0.0;
-    for (int c = 0; c < slots; ++c) s += part[(size_t)c * n + k];
-    const int64_t rg = k / SUB, lane = k % SUB;
-    for (int c = 0; c < nr.count; ++c) {
-        double t = 0.0;
-        for (int64_t q = nr.pstart[c][rg]; q < nr.pstart[c][rg + 1]; ++q) t += nr.near[c][q * SUB + lane];
-        s += t;
+    if (k < n) {
+        for (int c = w; c < slots; c += 8) s += part[(size_t)c * n + k];
+        const int64_t rg = k / SUB;
+        for (int c = 0; c < nr.count; ++c)
+            for (int64_t q = nr.pstart[c][rg] + w; q < nr.pstart[c][rg + 1]; q += 8) s += nr.near[c][q * SUB + lane];
     }
-    out[idx ? idx[k] : k] = s;
+    s_tmp[w * 32 + lane] = s;
+    __syncthreads();
+    if (w == 0 && k < n) {
+        double t = 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) t += s_tmp[q * 32 + lane];
+        out[idx ? idx[k] : k] = t;
+    }
 }
 
 // y[idx ? idx[k] : k] = the partial sums of row k of the symmetric A q sweep, in amat_row_sum's fixed order
@@ -556,17 +565,27 @@ __global__ void __launch_bounds__(TPB) fock_near_kernel(const double4 *__restric
     for (int h = 0; h < NH; ++h) out[h * SUB] = sink.acc[h];
 }
 
-// herm[0][h][i] = sum_c herm[c][h][i] + sum of the near pieces of product i  (fixed order); plane = nh * npad
-__global__ void reduce_herm_kernel(double *__restrict__ herm, int64_t plane, int chunks, int64_t npad, int nh,
-                                   const double *__restrict__ near, const int64_t *__restrict__ pstart) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= plane) return;
-    double s = herm[k];
-    for (int c = 1; c < chunks; ++c) s += herm[(size_t)c * plane + k];
-    const int64_t h = k / npad, i = k - h * npad, rg = i / SUB, lane = i % SUB;
-    double t = 0.0;
-    for (int64_t q = pstart[rg]; q < pstart[rg + 1]; ++q) t += near[((size_t)q * nh + h) * SUB + lane];
-    herm[k] = s + t;
+// herm[0][h][i] = sum_c herm[c][h][i] + sum of the near pieces of product i; plane = nh * npad.  As reduce_slots_kernel:
+// a 256-thread block sums 32 consecutive elements, warp w taking every 8th chunk and every 8th near piece (fixed order).
+__global__ void __launch_bounds__(256) reduce_herm_kernel(double *__restrict__ herm, int64_t plane, int chunks, int64_t npad, int nh,
+                                                          const double *__restrict__ near, const int64_t *__restrict__ pstart) {
+    __shared__ double s_tmp[8 * 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t k = (int64_t)blockIdx.x * 32 + lane;   // npad is a multiple of 32: the 32 elements share h and the row group
+    double s = 0.0;
+    if (k < plane) {
+        for (int c = w; c < chunks; c += 8) s += herm[(size_t)c * plane + k];
+        const int64_t h = k / npad, i = k - h * npad, rg = i / SUB;
+        for (int64_t q = pstart[rg] + w; q < pstart[rg + 1]; q += 8) s += near[((size_t)q * nh + h) * SUB + lane];
+    }
+    s_tmp[w * 32 + lane] = s;
+    __syncthreads();
+    if (w == 0 && k < plane) {
+        double t = 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) t += s_tmp[q * 32 + lane];
+        herm[k] = t;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -759,6 +778,53 @@ __global__ void density_to_hermite_kernel(int64_t n, int64_t first, int64_t npad
     }
 #pragma unroll
     for (int h = 0; h < NH; ++h) herm[(size_t)h * npad + i] = D[h];
+}
+
+// The same transform with one warp per product (used for L >= 2, where a product has several members of up to 25
+// components each): lane = component (a, b) of the member, members in order, then a fixed-order butterfly over the lanes.
+template <int L>
+__global__ void __launch_bounds__(128) density_to_hermite_warp_kernel(int64_t n, int64_t first, int64_t npad,
+                                                                      const int64_t *__restrict__ pm_start,
+                                                                      const int32_t *__restrict__ pm_list, const int32_t *__restrict__ m_sp,
+                                                                      const int32_t *__restrict__ m_cls, const int64_t *__restrict__ m_goff,
+                                                                      const double *__restrict__ G, const int32_t *__restrict__ sp_i0,
+                                                                      const int32_t *__restrict__ sp_j0, const int32_t *__restrict__ sp_dims,
+                                                                      const double *__restrict__ P, int64_t ldp, double *__restrict__ herm) {
+    constexpr int NH = nherm(L);
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (i >= npad) return;
+    double D[NH];
+#pragma unroll
+    for (int h = 0; h < NH; ++h) D[h] = 0.0;
+    if (i < n) {
+        const int64_t g = first + i;
+        for (int64_t e = pm_start[g]; e < pm_start[g + 1]; ++e) {
+            const int m = pm_list[e];
+            const int sp = m_sp[m];
+            const int dims = sp_dims[sp], na = dims & 0xff, nb = (dims >> 8) & 0xff, diag = dims >> 16;
+            const int i0 = sp_i0[sp], j0 = sp_j0[sp];
+            const int Lm = m_cls[m] & 0xff;
+            const int nhm = (Lm + 1) * (Lm + 2) * (Lm + 3) / 6;
+            const double *gm = G + m_goff[m];
+            for (int ab = lane; ab < na * nb; ab += 32) {
+                const int a = ab / nb, b = ab - a * nb;
+                double pw = P[(size_t)(i0 + a) * ldp + j0 + b];
+                if (!diag) pw += P[(size_t)(j0 + b) * ldp + i0 + a];
+                const double *row = gm + (size_t)ab * nhm;
+#pragma unroll
+                for (int h = 0; h < NH; ++h)
+                    if (h < nhm) D[h] = fma(row[h], pw, D[h]);
+            }
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < NH; ++h) {
+        double v = D[h];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) herm[(size_t)h * npad + i] = v;
+    }
 }
 
 // F_ab (+)= sum_members sum_h G[ab][h] H_h(product of the member).  Thread = one component (a,b) of one shell pair;
@@ -990,7 +1056,7 @@ static int reduce_fock_class(pcm_ctx *ctx, cudaStream_t s) {
     const int64_t chunks = ctx->plan_fock[L].chunks;
     if (c.n == 0) return PCM_OK;
     const int64_t plane = (int64_t)nherm(L) * c.npad;
-    reduce_herm_kernel<<<(unsigned)ceil_div(plane, 256), 256, 0, s>>>(c.herm, plane, (int)chunks, c.npad, nherm(L), c.near_fock,
+    reduce_herm_kernel<<<(unsigned)ceil_div(plane, 32), 256, 0, s>>>(c.herm, plane, (int)chunks, c.npad, nherm(L), c.near_fock,
                                                                       c.fock_map.pstart);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
@@ -1047,9 +1113,14 @@ template <int L>
 static int launch_density_class(pcm_ctx *ctx, const double *P, int64_t ldp, cudaStream_t s) {
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
-    density_to_hermite_kernel<L><<<(unsigned)(c.npad / 128), 128, 0, s>>>(
-        c.n, c.first, c.npad, ctx->pm_start, ctx->pm_list, ctx->m_sp, ctx->m_cls, ctx->m_goff, ctx->G, ctx->sp_i0,
-        ctx->sp_j0, ctx->sp_dims, P, ldp, c.herm);
+    if (L >= 2)
+        density_to_hermite_warp_kernel<L><<<(unsigned)(c.npad / 4), 128, 0, s>>>(
+            c.n, c.first, c.npad, ctx->pm_start, ctx->pm_list, ctx->m_sp, ctx->m_cls, ctx->m_goff, ctx->G, ctx->sp_i0,
+            ctx->sp_j0, ctx->sp_dims, P, ldp, c.herm);
+    else
+        density_to_hermite_kernel<L><<<(unsigned)(c.npad / 128), 128, 0, s>>>(
+            c.n, c.first, c.npad, ctx->pm_start, ctx->pm_list, ctx->m_sp, ctx->m_cls, ctx->m_goff, ctx->G, ctx->sp_i0,
+            ctx->sp_j0, ctx->sp_dims, P, ldp, c.herm);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
@@ -1120,7 +1191,7 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
         nr.count = 0;
         for (int L = 0; L <= MAXL; ++L)
             if (ctx->cls[L].n > 0) { nr.near[nr.count] = ctx->cls[L].near_pot; nr.pstart[nr.count] = ctx->cls[L].pot_map.pstart; nr.count++; }
-        reduce_slots_kernel<<<(unsigned)ceil_div(ctx->M, 256), 256, 0, s>>>(ctx->vpart, ctx->M, (int)slot, v, ctx->s2c, nr);
+        reduce_slots_kernel<<<(unsigned)ceil_div(ctx->M, 32), 256, 0, s>>>(ctx->vpart, ctx->M, (int)slot, v, ctx->s2c, nr);
         PCM_LAUNCH_CHECK(ctx);
         { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     }
