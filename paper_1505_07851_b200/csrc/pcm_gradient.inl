@@ -160,23 +160,36 @@ __global__ void __launch_bounds__(TPB) grad_point_near_kernel(const double4 *__r
     for (int d = 0; d < 3; ++d) near[((size_t)piece * 3 + d) * SUB + lane] = g[d];
 }
 
-// g_point[3 s2c[k] + d] = -q_k (sum of the slots + the near pieces of point k), fixed order; q in the caller's order
-__global__ void grad_point_reduce_kernel(const double *__restrict__ gpart, int64_t M, int slots, const double *__restrict__ q,
-                                         const int32_t *__restrict__ s2c, NearRefs nr, double *__restrict__ g_point) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= M) return;
-    const int64_t rg = k / SUB, lane = k % SUB;
-    const int32_t kc = s2c[k];
-    const double mq = -q[kc];
-    for (int d = 0; d < 3; ++d) {
-        double s = 0.0;
-        for (int c = 0; c < slots; ++c) s += gpart[((size_t)c * 3 + d) * M + k];
-        for (int c = 0; c < nr.count; ++c) {
-            double t = 0.0;
-            for (int64_t e = nr.pstart[c][rg]; e < nr.pstart[c][rg + 1]; ++e) t += nr.near[c][((size_t)e * 3 + d) * SUB + lane];
-            s += t;
+// g_point[3 s2c[k] + d] = -q_k (sum of the slots + the near pieces of point k); q in the caller's order.  A 256-thread
+// block sums 32 points: warp w adds every 8th slot and every 8th near piece, the eight partial sums are added in order.
+__global__ void __launch_bounds__(256) grad_point_reduce_kernel(const double *__restrict__ gpart, int64_t M, int slots,
+                                                                const double *__restrict__ q, const int32_t *__restrict__ s2c,
+                                                                NearRefs nr, double *__restrict__ g_point) {
+    __shared__ double s_tmp[3][8 * 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t k = (int64_t)blockIdx.x * 32 + lane;
+    double s[3] = {0.0, 0.0, 0.0};
+    if (k < M) {
+        const int64_t rg = k / SUB;
+        for (int d = 0; d < 3; ++d) {
+            for (int c = w; c < slots; c += 8) s[d] += gpart[((size_t)c * 3 + d) * M + k];
+            for (int c = 0; c < nr.count; ++c)
+                for (int64_t e = nr.pstart[c][rg] + w; e < nr.pstart[c][rg + 1]; e += 8) s[d] += nr.near[c][((size_t)e * 3 + d) * SUB + lane];
         }
-        g_point[(size_t)kc * 3 + d] = mq * s;
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) s_tmp[d][w * 32 + lane] = s[d];
+    __syncthreads();
+    if (w == 0 && k < M) {
+        const int32_t kc = s2c[k];
+        const double mq = -q[kc];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            double t = 0.0;
+#pragma unroll
+            for (int p = 0; p < 8; ++p) t += s_tmp[d][p * 32 + lane];
+            g_point[(size_t)kc * 3 + d] = mq * t;
+        }
     }
 }
 
@@ -383,7 +396,7 @@ int launch_gradient(pcm_ctx *ctx, const double *P, int64_t ldp, const double *q,
         nr.count = 0;
         for (int L = 0; L <= MAXL; ++L)
             if (ctx->cls[L].n > 0) { nr.near[nr.count] = ctx->cls[L].near_gpoint; nr.pstart[nr.count] = ctx->cls[L].pot_map.pstart; nr.count++; }
-        grad_point_reduce_kernel<<<(unsigned)ceil_div(M, 256), 256, 0, s>>>(ctx->gpart, M, (int)slot, q, ctx->s2c, nr, g_point);
+        grad_point_reduce_kernel<<<(unsigned)ceil_div(M, 32), 256, 0, s>>>(ctx->gpart, M, (int)slot, q, ctx->s2c, nr, g_point);
         PCM_LAUNCH_CHECK(ctx);
         ctx->launch_total++;
     }
