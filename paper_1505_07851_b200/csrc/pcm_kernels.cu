@@ -101,6 +101,38 @@ __device__ __forceinline__ void stage_points(const double4 *__restrict__ pt, con
     }
 }
 
+// The stored near patches (amat_near_fill_kernel below) as the main kernel sees them: when `blocks` is set, the grid of
+// amatvec_kernel is extended by rows of CTAs (blockIdx.y >= chunks) that do the near pieces, four per CTA, so that one
+// launch does the whole product and the light, memory-bound near work fills the tail of the sweep.
+struct NearStored {
+    const double *blocks;        // [nnear][32][32], nullptr: the near pieces are done by a separate kernel
+    const int64_t *start, *pstart;
+    const int32_t *list, *piece_rg;
+    int64_t npiece;
+    double *near;                // [npiece][32]
+};
+// near[piece][lane] = sum over the piece's patches (list order) of sum_t A(lane, t) q_t (t ascending)
+__device__ __forceinline__ void amat_near_stored_piece(const NearStored &ns, const double *__restrict__ q,
+                                                       const int32_t *__restrict__ qidx, int M, int64_t piece, int lane) {
+    const int64_t rg = ns.piece_rg[piece];
+    const int64_t ebeg = ns.start[rg] + (piece - ns.pstart[rg]) * NEAR_PIECE, eend = min(ns.start[rg + 1], ebeg + NEAR_PIECE);
+    double y = 0.0;
+    for (int64_t e = ebeg; e < eend; ++e) {
+        const int j = ns.list[e] * SUB + lane;
+        const double qj = j < M ? q[qidx ? qidx[j] : j] : 0.0;
+        const double *blk = ns.blocks + (size_t)e * (SUB * SUB) + lane;
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            double a[16];
+#pragma unroll
+            for (int t = 0; t < 16; ++t) a[t] = __ldg(blk + (half * 16 + t) * SUB);
+#pragma unroll
+            for (int t = 0; t < 16; ++t) y = fma(__shfl_sync(0xffffffffu, qj, half * 16 + t), a[t], y);
+        }
+    }
+    ns.near[piece * SUB + lane] = y;
+}
+
 // Symmetric sweep: A_ij = A_ji, so an evaluation 1/r_ij serves row i (y_i += q_j/r) and column j (y_j += q_i/r).
 // Block (rb, chunk) owns the rows [rb RB, (rb+1) RB), RB = TPB R, and the column tiles of its chunk that do not lie
 // before its rows:  tiles inside the row range (the diagonal band) are swept for the rows only; tiles beyond it are
@@ -146,11 +178,17 @@ __global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict_
                                                       const int32_t *__restrict__ qidx, int M, int chunk_len,
                                                       double *__restrict__ out, double *__restrict__ colpart,
                                                       const uint8_t *__restrict__ farmap, int64_t nbyte, int64_t nrg,
-                                                      const int *__restrict__ stop) {
+                                                      const int *__restrict__ stop, int chunks, NearStored ns) {
     constexpr int NS = TILE / SUB;
     constexpr int RB = TPB * R;
     constexpr int NW = TPB / 32;
     static_assert(RB % TILE == 0, "row blocks must be whole column tiles");
+    if ((int)blockIdx.y >= chunks) {   // the extra rows of the grid: stored near pieces, one per warp
+        if (stop && *stop) return;
+        const int64_t piece = ((int64_t)(blockIdx.y - chunks) * gridDim.x + blockIdx.x) * NW + (threadIdx.x >> 5);
+        if (piece < ns.npiece) amat_near_stored_piece(ns, q, qidx, M, piece, threadIdx.x & 31);
+        return;
+    }
     __shared__ double4 s_pt[TILE];          // -2 (b - o), |b - o|^2
     __shared__ double s_q[TILE];            // column charges
     __shared__ double4 s_org[TILE / 32];    // origin of every column group
@@ -348,33 +386,6 @@ __global__ void __launch_bounds__(TPB) amat_near_fill_kernel(const double4 *__re
             blk[t * SUB + lane] = ev;
         }
     }
-}
-
-// near pieces of A q from the stored blocks: one warp per piece, lane = row; near[piece][lane] = sum over the piece's
-// patches (in list order) of sum_t A(lane, t) q_t (t ascending) -- the order amat_near_kernel uses
-__global__ void __launch_bounds__(TPB) amat_near_stored_kernel(const double *__restrict__ blocks, const double *__restrict__ q,
-                                                               const int32_t *__restrict__ qidx, int M,
-                                                               const int64_t *__restrict__ start, const int32_t *__restrict__ list,
-                                                               const int64_t *__restrict__ pstart, const int32_t *__restrict__ piece_rg,
-                                                               int64_t npiece, double *__restrict__ near, const int *__restrict__ stop) {
-    if (stop && *stop) return;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
-    if (piece >= npiece) return;
-    const int64_t rg = piece_rg[piece];
-    const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
-    double y = 0.0;
-    for (int64_t e = ebeg; e < eend; ++e) {
-        const int j = list[e] * SUB + lane;
-        const double qj = j < M ? q[qidx ? qidx[j] : j] : 0.0;
-        const double *blk = blocks + (size_t)e * (SUB * SUB) + lane;
-        double a[SUB];
-#pragma unroll
-        for (int t = 0; t < SUB; ++t) a[t] = __ldg(blk + t * SUB);
-#pragma unroll
-        for (int t = 0; t < SUB; ++t) y = fma(__shfl_sync(0xffffffffu, qj, t), a[t], y);
-    }
-    near[piece * SUB + lane] = y;
 }
 
 // sums of the near pieces, per class: near[c][piece][lane], pieces of row group rg = pstart[c][rg] .. pstart[c][rg+1]
@@ -952,31 +963,37 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
     const Plan &pl = ctx->plan_amat;
     const PatchMap &pm = ctx->amat_map;
     const double thr = TFAR_AMAT * 2.0 / (ctx->zeta_min * ctx->zeta_min);
-    dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
-    if (pm.npiece > 0) {
+    const bool stored = ctx->amat_blocks != nullptr && pm.npiece > 0;
+    NearStored ns{};
+    int64_t extra = 0;
+    if (stored) {   // one launch: the near pieces ride in extra rows of the main kernel's grid
+        ns.blocks = ctx->amat_blocks; ns.start = pm.start; ns.pstart = pm.pstart; ns.list = pm.list; ns.piece_rg = pm.piece_rg;
+        ns.npiece = pm.npiece; ns.near = ctx->near_amat;
+        extra = ceil_div(ceil_div(pm.npiece, TPB / 32), pl.xb);
+    }
+    dim3 grid((unsigned)pl.xb, (unsigned)(pl.chunks + extra));
+    const bool fork = !stored && pm.npiece > 0;
+    if (fork) {     // near patches evaluated on the fly: their own kernel on the near stream
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
         PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->near_stream, ctx->ev_fork, 0));
-        if (ctx->amat_blocks)
-            amat_near_stored_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, ctx->near_stream>>>(
-                ctx->amat_blocks, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, stop);
-        else
-            amat_near_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, ctx->near_stream>>>(
-                ctx->pt, ctx->pt_diag, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, ctx->boys, thr, stop);
+        amat_near_kernel<<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, ctx->near_stream>>>(
+            ctx->pt, ctx->pt_diag, q, idx, M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece, ctx->near_amat, ctx->boys, thr, stop);
         PCM_LAUNCH_CHECK(ctx);
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
         { ctx->launches[2]++; ctx->launch_total++; }
     }
+    const int ch = (int)pl.chunks;
     if (ctx->amat_R == 1)
-        amatvec_kernel<1, 4, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+        amatvec_kernel<1, 4, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
     else if (ctx->amat_R == 4)
-        amatvec_kernel<4, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+        amatvec_kernel<4, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
     else if (ctx->amat_tile == 256)
-        amatvec_kernel<2, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+        amatvec_kernel<2, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
     else
-        amatvec_kernel<2, AMAT_C, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop);
+        amatvec_kernel<2, AMAT_C, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[2]++; ctx->launch_total++; }
-    if (pm.npiece > 0) PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
+    if (fork) PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
     return PCM_OK;
 }
 // evaluates the near patches of A once (pcm_setup), if they fit the budget
