@@ -255,12 +255,15 @@ __global__ void __launch_bounds__(RBJ_THREADS) rbj_select_kernel(const double4 *
 constexpr int RBL_THREADS = 1024;
 constexpr int RBL_RAW = 3072;   // candidate capacity (raw)
 constexpr int RBL_CAP = 1024;   // candidates above the histogram cut that are ranked
+constexpr int RBL_GL = 1024;    // candidate groups kept in shared memory (more: the global list)
 
 struct RblShared {
     int hist[RBJ_BINS];
     int scan[RBJ_BINS];
     double rkey[RBL_RAW];
     int ridx[RBL_RAW];
+    int rcal[RBL_RAW];          // caller index of a raw candidate (tie-break key)
+    int sgl[RBL_GL];            // candidate groups (shared-memory copy of glist while they fit)
     double ckey[RBL_CAP];
     int cidx[RBL_CAP];
     int ccal[RBL_CAP];
@@ -316,20 +319,24 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                     const double *b = boxes + (size_t)g * 6;
                     const double gx = fmax(fmax(b[0] - pk.x, pk.x - b[3]), 0.0), gy = fmax(fmax(b[1] - pk.y, pk.y - b[4]), 0.0),
                                  gz = fmax(fmax(b[2] - pk.z, pk.z - b[5]), 0.0);
-                    if (gx * gx + gy * gy + gz * gz < rho2) glist[atomicAdd(&S.ngl, 1)] = g;
-                    else S.all_in = 0;
+                    if (gx * gx + gy * gy + gz * gz < rho2) {
+                        const int slot = atomicAdd(&S.ngl, 1);
+                        if (slot < RBL_GL) S.sgl[slot] = g;
+                        glist[slot] = g;
+                    } else S.all_in = 0;
                 }
                 __syncthreads();
                 const int ngl = S.ngl;
                 // ---- keys of the unassigned points of those groups
                 for (int t = tid; t < ngl * 32; t += RBL_THREADS) {
-                    const int j = glist[t >> 5] * 32 + (t & 31);
+                    const int j = (ngl <= RBL_GL ? S.sgl[t >> 5] : glist[t >> 5]) * 32 + (t & 31);
                     if (j < M && !assigned[j]) {
+                        const int cal = s2c[j];
                         const double4 b = pt[j];
                         const double dx = pk.x - b.x, dy = pk.y - b.y, dz = pk.z - b.z;
                         const double a = amat_entry(fma(dz, dz, fma(dy, dy, dx * dx)), pk.w, b.w, boys0);
                         const int slot = atomicAdd(&S.nraw, 1);
-                        if (slot < RBL_RAW) { S.rkey[slot] = a; S.ridx[slot] = j; }
+                        if (slot < RBL_RAW) { S.rkey[slot] = a; S.ridx[slot] = j; S.rcal[slot] = cal; }
                         atomicAdd(&S.hist[rbj_bucket(a)], 1);
                     }
                 }
@@ -368,7 +375,7 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                     const double a = S.rkey[c];
                     if (rbj_bucket(a) >= bstar) {
                         const int slot = atomicAdd(&S.ncut, 1);
-                        if (slot < RBL_CAP) { S.ckey[slot] = a; S.cidx[slot] = S.ridx[c]; S.ccal[slot] = s2c[S.ridx[c]]; }
+                        if (slot < RBL_CAP) { S.ckey[slot] = a; S.cidx[slot] = S.ridx[c]; S.ccal[slot] = S.rcal[c]; }
                     }
                 }
                 __syncthreads();
