@@ -39,9 +39,22 @@ __device__ __forceinline__ double amat_row_sum_block(const AmatParts &a, int M, 
     double s = 0.0;
     if (k < M) {
         const int r0 = k / a.RB * a.RB;
-        for (int c = r0 / a.chunk_len + part; c < a.slots; c += AMAT_RED_PARTS) s += a.ypart[(size_t)c * M + k];
+        // four loads in flight per loop (the partial sums come from L2), same summation order
+        int c = r0 / a.chunk_len + part;
+        for (; c + 3 * AMAT_RED_PARTS < a.slots; c += 4 * AMAT_RED_PARTS) {
+            const double v0 = a.ypart[(size_t)c * M + k], v1 = a.ypart[(size_t)(c + AMAT_RED_PARTS) * M + k],
+                         v2 = a.ypart[(size_t)(c + 2 * AMAT_RED_PARTS) * M + k], v3 = a.ypart[(size_t)(c + 3 * AMAT_RED_PARTS) * M + k];
+            s += v0; s += v1; s += v2; s += v3;
+        }
+        for (; c < a.slots; c += AMAT_RED_PARTS) s += a.ypart[(size_t)c * M + k];
         const int nsym = (k / a.tile * a.tile) / a.RB;
-        for (int rb = part; rb < nsym; rb += AMAT_RED_PARTS) s += a.colpart[(size_t)rb * M + k];
+        int rb = part;
+        for (; rb + 3 * AMAT_RED_PARTS < nsym; rb += 4 * AMAT_RED_PARTS) {
+            const double v0 = a.colpart[(size_t)rb * M + k], v1 = a.colpart[(size_t)(rb + AMAT_RED_PARTS) * M + k],
+                         v2 = a.colpart[(size_t)(rb + 2 * AMAT_RED_PARTS) * M + k], v3 = a.colpart[(size_t)(rb + 3 * AMAT_RED_PARTS) * M + k];
+            s += v0; s += v1; s += v2; s += v3;
+        }
+        for (; rb < nsym; rb += AMAT_RED_PARTS) s += a.colpart[(size_t)rb * M + k];
         const int64_t rg = k / 32;
         for (int64_t e = a.pstart[rg] + part; e < a.pstart[rg + 1]; e += AMAT_RED_PARTS) s += a.near[e * 32 + lane];
     }

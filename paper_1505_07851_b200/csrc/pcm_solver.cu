@@ -598,8 +598,17 @@ __global__ void __launch_bounds__(DOT_THREADS) cg_update_rbj_kernel(int M, int b
     for (int i0 = 0; i0 < n; i0 += rpp) {
         const int i = i0 + il;
         double s = 0.0;
-        if (i < n && part < np)
-            for (int j = part; j < n; j += np) s = fma(a[(size_t)j * n + i], s_r[j], s);
+        if (i < n && part < np) {
+            int j = part;
+            for (; j + 7 * np < n; j += 8 * np) {
+                double v[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) v[u] = __ldg(a + (size_t)(j + u * np) * n + i);
+#pragma unroll
+                for (int u = 0; u < 8; ++u) s = fma(v[u], s_r[j + u * np], s);
+            }
+            for (; j < n; j += np) s = fma(__ldg(a + (size_t)j * n + i), s_r[j], s);
+        }
         s_part[threadIdx.x] = s;
         __syncthreads();
         if (part == 0 && i < n) {
@@ -618,6 +627,155 @@ __global__ void __launch_bounds__(DOT_THREADS) cg_update_rbj_kernel(int M, int b
         const double srz = ordered_sum(partial + gridDim.x, gridDim.x);
         cg_finish(srr, srz, scal, ctl, tol, max_iter, init);
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// One cooperative kernel for everything of a PCG iteration that follows the A q sweep (RBJ preconditioner):
+//   phase 1  Ap = row sums of the sweep's partial sums, per-task p.Ap        -- grid barrier --
+//   phase 2  alpha; x += alpha p, r -= alpha Ap, z = M_b^-1 r per RBJ block, per-block r.r and r.z   -- grid barrier --
+//   phase 3  beta, convergence test (CTA 0 records them), p = z + beta p
+// Every CTA adds the per-task partial sums itself, in index order, so all of them hold the same alpha and beta without a
+// broadcast, and the numbers are those of the three separate kernels (cg_matvec_reduce, cg_update_rbj, cg_direction)
+// bit for bit.  At M ~ 10^4 those three launches and their tails cost as much as half an A q sweep; here they are two
+// barriers.  The barrier is sense-reversing and self-resetting (count, generation in ctl[3], ctl[4]); the launch is
+// cooperative, so all CTAs are resident; the spin is bounded and raises ctl[5] instead of hanging.
+// ---------------------------------------------------------------------------------------------
+enum { CTL_BAR_COUNT = 3, CTL_BAR_GEN = 4, CTL_BAR_ERR = 5 };
+
+__device__ __forceinline__ void grid_sync(int *ctl, unsigned G) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        volatile int *gen = ctl + CTL_BAR_GEN;
+        const int g = *gen;
+        __threadfence();
+        if (atomicAdd(ctl + CTL_BAR_COUNT, 1) == (int)G - 1) {
+            ctl[CTL_BAR_COUNT] = 0;
+            __threadfence();
+            atomicAdd(ctl + CTL_BAR_GEN, 1);
+        } else {
+            long long spins = 0;
+            while (*gen == g) {
+                if (++spins > (1ll << 27)) { ctl[CTL_BAR_ERR] = 1; break; }
+            }
+        }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+struct CgFused {
+    int M, block, nblocks, max_iter;
+    AmatParts parts;
+    const int32_t *order;
+    const double *inv;
+    double *p, *Ap, *x, *r, *z, *scal, *part1, *part2;
+    int *ctl;
+    double tol;
+};
+
+__global__ void __launch_bounds__(DOT_THREADS) cg_fused_rbj_kernel(CgFused a) {
+    extern __shared__ double s_dyn[];       // [max(block, 0) + DOT_THREADS]
+    __shared__ double s_bc[3];
+    int *ctl = a.ctl;
+    if (*((volatile int *)&ctl[CTL_STOP])) return;
+    const unsigned G = gridDim.x;
+    const int M = a.M, tid = threadIdx.x;
+    const int iters0 = *((volatile int *)&ctl[CTL_ITERS]);
+    const double rz_old = a.scal[0];
+    // ---- phase 1
+    const int ntask1 = (M + 31) / 32;
+    for (int task = blockIdx.x; task < ntask1; task += G) {
+        const double t = amat_row_sum_block(a.parts, M, task * 32, s_dyn);
+        const int k = task * 32 + tid;
+        if (tid < 32) {
+            double dot = 0.0;
+            if (k < M) { a.Ap[k] = t; dot = a.p[k] * t; }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) dot += __shfl_down_sync(0xffffffffu, dot, o);
+            if (tid == 0) a.part1[task] = dot;
+        }
+        __syncthreads();
+    }
+    grid_sync(ctl, G);
+    {
+        const double pAp = ordered_sum(a.part1, ntask1);
+        if (tid == 0) s_bc[0] = pAp;
+        __syncthreads();
+    }
+    const double pAp = s_bc[0];
+    const double alpha = rz_old / pAp;
+    // ---- phase 2: the body of cg_update_rbj_kernel, one RBJ block per pass
+    const int block = a.block;
+    double *s_r = s_dyn, *s_part = s_dyn + block;
+    for (int b = blockIdx.x; b < a.nblocks; b += G) {
+        const long long start = (long long)b * block;
+        const int n = (int)min((long long)block, (long long)M - start);
+        const double *am = a.inv + (size_t)b * block * block;
+        const int32_t *idx = a.order + start;
+        double rr = 0.0, rz = 0.0;
+        for (int j = tid; j < n; j += DOT_THREADS) {
+            const int i = idx[j];
+            a.x[i] = fma(alpha, a.p[i], a.x[i]);
+            const double ri = fma(-alpha, a.Ap[i], a.r[i]);
+            a.r[i] = ri;
+            s_r[j] = ri;
+            rr = fma(ri, ri, rr);
+        }
+        __syncthreads();
+        const int np = n >= DOT_THREADS ? 1 : DOT_THREADS / n;
+        const int rpp = DOT_THREADS / np;
+        const int part = tid / rpp, il = tid - part * rpp;
+        for (int i0 = 0; i0 < n; i0 += rpp) {
+            const int i = i0 + il;
+            double sacc = 0.0;
+            if (i < n && part < np) {
+                // eight loads in flight (the inverse block comes from L2), same summation order
+                int j = part;
+                for (; j + 7 * np < n; j += 8 * np) {
+                    double v[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) v[u] = __ldg(am + (size_t)(j + u * np) * n + i);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) sacc = fma(v[u], s_r[j + u * np], sacc);
+                }
+                for (; j < n; j += np) sacc = fma(__ldg(am + (size_t)j * n + i), s_r[j], sacc);
+            }
+            s_part[tid] = sacc;
+            __syncthreads();
+            if (part == 0 && i < n) {
+                double t = 0.0;
+                for (int q = 0; q < np; ++q) t += s_part[q * rpp + il];
+                a.z[idx[i]] = t;
+                rz = fma(s_r[i], t, rz);
+            }
+            __syncthreads();
+        }
+        rr = block_sum(rr);
+        rz = block_sum(rz);
+        if (tid == 0) { a.part2[b] = rr; a.part2[a.nblocks + b] = rz; }
+        __syncthreads();
+    }
+    grid_sync(ctl, G);
+    {
+        const double srr = ordered_sum(a.part2, a.nblocks);
+        const double srz = ordered_sum(a.part2 + a.nblocks, a.nblocks);
+        if (tid == 0) { s_bc[1] = srr; s_bc[2] = srz; }
+        __syncthreads();
+    }
+    const double srr = s_bc[1], srz = s_bc[2];
+    const double beta = srz / rz_old;
+    const bool stop = !(sqrt(srr) > a.tol) || iters0 + 1 >= a.max_iter;
+    if (blockIdx.x == 0 && tid == 0) {
+        a.scal[1] = pAp;
+        a.scal[5] = beta;
+        a.scal[0] = srz;
+        a.scal[2] = srr;
+        ctl[CTL_ITERS] = iters0 + 1;
+        if (stop) ctl[CTL_STOP] = 1;
+    }
+    // ---- phase 3 (a converged solve keeps p, as cg_direction_kernel does)
+    if (!stop)
+        for (int i = blockIdx.x * DOT_THREADS + tid; i < M; i += (int)G * DOT_THREADS) a.p[i] = fma(beta, a.p[i], a.z[i]);
 }
 
 // Jacobi (C = diag(A)^-1) or no preconditioner (diag == nullptr)
@@ -1038,7 +1196,31 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         CG_CUDA(cudaMemcpyAsync(r, b, (size_t)M * 8, cudaMemcpyDeviceToDevice, s));
     }
     CG_TRY(update(1));  // z = C r, p = z, rz, rr; raises STOP if already converged (or max_iter == 0)
-    const int batch = 4;
+    // RBJ: everything after the sweep in one cooperative kernel (cg_fused_rbj_kernel)
+    bool fused = precond == 2 && !getenv("PCM_CG_UNFUSED");
+    CgFused fa{};
+    int fgrid = 0;
+    size_t fsmem = 0;
+    if (fused) {
+        const int block = (int)ctx->rbj_block;
+        fsmem = ((size_t)block + DOT_THREADS) * 8;
+        int per_sm = 0;
+        if (fsmem > 48 * 1024 ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cg_fused_rbj_kernel, DOT_THREADS, fsmem) != cudaSuccess || per_sm < 1) {
+            fused = false;
+            (void)cudaGetLastError();
+        } else {
+            const int64_t want = std::max<int64_t>(cdiv(M, 32), ctx->rbj_nblocks);
+            fgrid = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)per_sm * ctx->sm_count));
+            fa.M = M; fa.block = block; fa.nblocks = (int)ctx->rbj_nblocks; fa.max_iter = max_iter;
+            fa.parts = amat_parts(ctx);
+            fa.order = ctx->rbj_order; fa.inv = ctx->rbj_inv;
+            fa.p = p; fa.Ap = Ap; fa.x = x; fa.r = r; fa.z = z; fa.scal = scal; fa.part1 = ctx->cg_part; fa.part2 = ctx->rbj_partial;
+            fa.ctl = ctl; fa.tol = tol;
+        }
+    }
+    int batch = 8;   // iterations queued per read-back of the device-side convergence flag
+    if (const char *e = getenv("PCM_CG_BATCH")) batch = std::max(1, atoi(e));
     int it = 0;
     double rr = 0.0;
     while (true) {
@@ -1047,15 +1229,22 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         const int *hc = reinterpret_cast<const int *>(h + 8);
         it = hc[CTL_ITERS];
         rr = h[2];
+        if (hc[CTL_BAR_ERR]) { ctx->timing = saved_timing; return set_error(ctx, PCM_ERR_STATE, "pcm_cg_solve: grid barrier timed out"); }
         if (hc[CTL_STOP]) break;
         for (int k = 0; k < batch; ++k) {
             const bool ev = saved_timing && ctx->cg_ev_n < pcm_ctx::CG_EV;
             if (ev) CG_CUDA(cudaEventRecord(ctx->cg_ev[2 * ctx->cg_ev_n], s));
             CG_TRY(launch_amatvec_partials(ctx, p, ctl, s));
             if (ev) { CG_CUDA(cudaEventRecord(ctx->cg_ev[2 * ctx->cg_ev_n + 1], s)); ctx->cg_ev_n++; }
-            cg_matvec_reduce_kernel<<<(unsigned)cdiv(M, 32), DOT_THREADS, 0, s>>>(M, amat_parts(ctx), p, Ap, scal, ctx->cg_part, ctl);
-            ctx->launch_total += 1;
-            CG_TRY(update(0));
+            if (fused) {
+                void *args[] = {&fa};
+                CG_CUDA(cudaLaunchCooperativeKernel((const void *)cg_fused_rbj_kernel, dim3((unsigned)fgrid), dim3(DOT_THREADS), args, fsmem, s));
+                ctx->launch_total += 1;
+            } else {
+                cg_matvec_reduce_kernel<<<(unsigned)cdiv(M, 32), DOT_THREADS, 0, s>>>(M, amat_parts(ctx), p, Ap, scal, ctx->cg_part, ctl);
+                ctx->launch_total += 1;
+                CG_TRY(update(0));
+            }
         }
     }
     const double rn = std::sqrt(rr);
