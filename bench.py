@@ -53,9 +53,9 @@ WORK = {
     # A q: the sweep is symmetric -- one evaluation of 1/r_ij serves A_ij and A_ji; unit = one pair evaluation
     # (M^2/2 per call), R = 4 kernel: local-origin geometry 4 + 3/16 (1 DADD + 3 DFMA, the row shift amortised over 32
     # columns), rsqrt 5 (2 DMUL + 3 DFMA), two FMAs, 1/4 DADD of the column reduction = 11.44 instr, 19.4 flop.
-    # Below 20 000 points the R = 1 kernel runs: the column reduction costs a whole DADD per evaluation (12.19 instr, 20.25 flop).
+    # Below 20 000 points the R = 2 kernel runs: row shift 6/32 per row, half a DADD of column reduction (11.69 instr, 19.75 flop).
     "amatvec": [(11.44, 19.5)],
-    "amatvec_small": [(12.19, 20.25)],
+    "amatvec_small": [(11.69, 19.75)],
     "potential": [(12, 18), (18, 27), (32, 51), (57, 94), (97, 164)],
     "fock": [(12, 18), (18, 28), (30, 46), (54, 84), (94, 150)],
 }

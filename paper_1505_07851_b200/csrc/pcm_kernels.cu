@@ -32,12 +32,9 @@ constexpr int PT_TILE = 256;  // surface points staged per shared-memory tile (F
 // holds R whole row groups and every skip/run decision is warp-uniform.
 // ---------------------------------------------------------------------------------------------
 struct Blocking { int R, C; };
-// A q: R = 4 (row blocks of 512, column tiles of 256) from AMAT_R4_MIN points on; below, R = 1 with column tiles of 128
-// (work items of 128 x 128 evaluations: sixteen times as many, so that a 9k-point sweep still loads 148 SMs evenly).
-// R = 2 remains selectable (PCM_AMAT_R) for experiments.
+// A q blocking (plan_all): R = 4 / tile 256 from AMAT_R4_MIN points on, R = 2 / tile 64 below
 constexpr int AMAT_C = 2;
 constexpr int64_t AMAT_R4_MIN = 20000;
-constexpr int64_t AMAT_T128_MAX = 30000;
 __host__ __device__ constexpr Blocking fock_blocking(int L) {
     return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{2, 2} : L == 2 ? Blocking{1, 4} : Blocking{1, 2};
 }
@@ -921,19 +918,20 @@ static void plan_class(pcm_ctx *ctx) {
 }
 
 int plan_all(pcm_ctx *ctx) {
-    // symmetric sweep: about half of the (row block, chunk) grid has work
-    ctx->amat_R = ctx->M >= AMAT_R4_MIN ? 4 : 1;
-    if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 1 || r == 2 || r == 4) ctx->amat_R = r; }
+    // symmetric sweep: about half of the (row block, chunk) grid has work.  From AMAT_R4_MIN points on: row blocks of 512
+    // (R = 4) and column tiles of 256; below: row blocks of 256 (R = 2) and tiles of 64, i.e. 16 times as many, smaller
+    // work items, so that a 9k-point sweep still loads 148 SMs evenly.  PCM_AMAT_R / PCM_AMAT_TILE override (experiments).
+    ctx->amat_R = ctx->M >= AMAT_R4_MIN ? 4 : 2;
+    ctx->amat_tile = ctx->amat_R == 4 ? 256 : 64;
+    if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 2 || r == 4) ctx->amat_R = r; }
+    if (const char *e = getenv("PCM_AMAT_TILE")) { const int t = atoi(e); if (t == 64 || t == 128 || t == 256) ctx->amat_tile = t; }
+    if (ctx->amat_R == 4) ctx->amat_tile = 256;
     double aw = 8.0;
     if (const char *e = getenv("PCM_AMAT_WAVES")) aw = atof(e);
-    // small M: column tiles of 128 (four times the work items of the same sweep, so that the SMs stay evenly loaded)
-    ctx->amat_tile = (ctx->amat_R <= 2 && ctx->M < AMAT_T128_MAX) ? 128 : 256;
-    if (const char *e = getenv("PCM_AMAT_TILE")) { const int t = atoi(e); if ((t == 128 && ctx->amat_R == 2) || t == 256) ctx->amat_tile = t; }
-    if (ctx->amat_R == 1) ctx->amat_tile = 128;
-    ctx->plan_amat = ctx->amat_R == 1 ? make_plan(ctx->M, TPB * 1, ctx->M, 128, wave_of(ctx, amatvec_kernel<1, 4, 128>), 0.5, aw) :
-                     ctx->amat_R == 4 ? make_plan(ctx->M, TPB * 4, ctx->M, 256, wave_of(ctx, amatvec_kernel<4, AMAT_C, 256>), 0.5, aw)
-                     : ctx->amat_tile == 256 ? make_plan(ctx->M, TPB * 2, ctx->M, 256, wave_of(ctx, amatvec_kernel<2, AMAT_C, 256>), 0.5, aw)
-                                             : make_plan(ctx->M, TPB * 2, ctx->M, 128, wave_of(ctx, amatvec_kernel<2, AMAT_C, 128>), 0.5, aw);
+    ctx->plan_amat = ctx->amat_R == 4       ? make_plan(ctx->M, TPB * 4, ctx->M, 256, wave_of(ctx, amatvec_kernel<4, AMAT_C, 256>), 0.5, aw)
+                     : ctx->amat_tile == 64  ? make_plan(ctx->M, TPB * 2, ctx->M, 64, wave_of(ctx, amatvec_kernel<2, AMAT_C, 64>), 0.5, aw)
+                     : ctx->amat_tile == 128 ? make_plan(ctx->M, TPB * 2, ctx->M, 128, wave_of(ctx, amatvec_kernel<2, AMAT_C, 128>), 0.5, aw)
+                                             : make_plan(ctx->M, TPB * 2, ctx->M, 256, wave_of(ctx, amatvec_kernel<2, AMAT_C, 256>), 0.5, aw);
     if (getenv("PCM_VERBOSE")) fprintf(stderr, "[pcm] amat plan: R %d xb %lld chunks %lld chunk_len %lld\n", ctx->amat_R,
                                        (long long)ctx->plan_amat.xb, (long long)ctx->plan_amat.chunks, (long long)ctx->plan_amat.chunk_len);
     plan_class<0>(ctx); plan_class<1>(ctx); plan_class<2>(ctx); plan_class<3>(ctx); plan_class<4>(ctx);
@@ -983,14 +981,14 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
         { ctx->launches[2]++; ctx->launch_total++; }
     }
     const int ch = (int)pl.chunks;
-    if (ctx->amat_R == 1)
-        amatvec_kernel<1, 4, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
-    else if (ctx->amat_R == 4)
-        amatvec_kernel<4, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
-    else if (ctx->amat_tile == 256)
-        amatvec_kernel<2, AMAT_C, 256><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
-    else
-        amatvec_kernel<2, AMAT_C, 128><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, pm.nbyte, pm.nrg, stop, ch, ns);
+#define PCM_AMAT_LAUNCH(R_, T_)                                                                                                   \
+    amatvec_kernel<R_, AMAT_C, T_><<<grid, TPB, 0, s>>>(ctx->pt, q, idx, M, (int)pl.chunk_len, ctx->ypart, ctx->colpart, pm.far, \
+                                                        pm.nbyte, pm.nrg, stop, ch, ns)
+    if (ctx->amat_R == 4) PCM_AMAT_LAUNCH(4, 256);
+    else if (ctx->amat_tile == 64) PCM_AMAT_LAUNCH(2, 64);
+    else if (ctx->amat_tile == 128) PCM_AMAT_LAUNCH(2, 128);
+    else PCM_AMAT_LAUNCH(2, 256);
+#undef PCM_AMAT_LAUNCH
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[2]++; ctx->launch_total++; }
     if (fork) PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
