@@ -913,8 +913,10 @@ template <int L>
 static void plan_class(pcm_ctx *ctx) {
     constexpr Blocking fb = fock_blocking(L), pb = pot_blocking(L);
     const ClassData &c = ctx->cls[L];
-    ctx->plan_fock[L] = make_plan(c.npad, TPB * fb.R, ctx->M, PT_TILE, wave_of(ctx, fock_kernel<L, fb.R, fb.C>));
-    ctx->plan_pot[L] = make_plan(ctx->M, TPB * pb.R, c.npad, pot_tile(L), wave_of(ctx, potential_kernel<L, pb.R, pb.C>));
+    double iw = 4.0;
+    if (const char *e = getenv("PCM_INT_WAVES")) iw = atof(e);
+    ctx->plan_fock[L] = make_plan(c.npad, TPB * fb.R, ctx->M, PT_TILE, wave_of(ctx, fock_kernel<L, fb.R, fb.C>), 1.0, iw);
+    ctx->plan_pot[L] = make_plan(ctx->M, TPB * pb.R, c.npad, pot_tile(L), wave_of(ctx, potential_kernel<L, pb.R, pb.C>), 1.0, iw);
 }
 
 int plan_all(pcm_ctx *ctx) {
