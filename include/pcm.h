@@ -80,6 +80,8 @@ typedef struct pcm_info {
     int64_t rbj_block;                 /* 0 until pcm_rbj_build */
     int64_t rbj_nblocks;
     int64_t device_bytes;              /* device memory held by the context */
+    int64_t amat_near_patches;         /* 32 x 32 patches of A that are not far field (evaluated with erf) */
+    int64_t amat_stored_bytes;         /* bytes of those patches kept on the device (0: re-evaluated in every A q) */
 } pcm_info;
 
 /* Fills *opt with the defaults listed above. */

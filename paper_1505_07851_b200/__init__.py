@@ -47,7 +47,8 @@ class pcm_info(C.Structure):
                 ("products", C.c_int64 * PCM_NL), ("products_total", C.c_int64),
                 ("prim_pair_points", C.c_double), ("product_points", C.c_double),
                 ("zeta_min", C.c_double), ("zeta_max", C.c_double),
-                ("rbj_block", C.c_int64), ("rbj_nblocks", C.c_int64), ("device_bytes", C.c_int64)]
+                ("rbj_block", C.c_int64), ("rbj_nblocks", C.c_int64), ("device_bytes", C.c_int64),
+                ("amat_near_patches", C.c_int64), ("amat_stored_bytes", C.c_int64)]
 
 
 class PcmError(RuntimeError):

@@ -142,6 +142,8 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { ctx->err = std::string("pcm_setup: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
     ctx->info.device_bytes = ctx->device_bytes;
+    ctx->info.amat_near_patches = ctx->amat_map.nnear;
+    ctx->info.amat_stored_bytes = ctx->amat_blocks ? ctx->amat_map.nnear * 32 * 32 * 8 : 0;
     *out = ctx;
     return PCM_OK;
 }
