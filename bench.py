@@ -58,7 +58,7 @@ WORK = {
     "amatvec": [(11.44, 19.5)],
     "amatvec_small": [(11.69, 19.75)],
     "potential": [(12, 18), (18, 27), (32, 51), (57, 94), (97, 164)],
-    "fock": [(12, 18), (18, 28), (30, 46), (54, 84), (94, 150)],
+    "fock": [(12, 18), (17, 27), (28, 44), (51, 81), (90, 146)],   # the charge multiplies the first seed only
 }
 
 

@@ -83,6 +83,17 @@ __device__ __forceinline__ void seeds_far(double R2, double (&g)[L + 1]) {
         for (int n = 1; n <= L; ++n) g[n] = g[n - 1] * (u * (double)(-(2 * n - 1)));
     }
 }
+// the same seeds times a common factor w (the point's charge in the Fock sweep): one multiplication instead of L + 1
+template <int L>
+__device__ __forceinline__ void seeds_far_scaled(double R2, double w, double (&g)[L + 1]) {
+    const double ri = rsqrt_fast(R2);
+    g[0] = ri * w;
+    if (L > 0) {
+        const double u = ri * ri;
+#pragma unroll
+        for (int n = 1; n <= L; ++n) g[n] = g[n - 1] * (u * (double)(-(2 * n - 1)));
+    }
+}
 
 // General seeds: g_n = (w/kappa) (-2 rho)^n F_n(rho R2), w = sqrt(rho/p) = 1/sqrt(1 + p/zeta^2).
 // F_L by an 8-term Taylor expansion about the nearest table row, lower orders by downward recursion

@@ -445,9 +445,7 @@ template <int L>
 __device__ __forceinline__ void fock_far_unit(const double4 &A, const double4 &pc, FockSink<L> &sink) {
     const double x = A.x - pc.x, y = A.y - pc.y, z = A.z - pc.z;
     double g[L + 1];
-    seeds_far<L>(fma(z, z, fma(y, y, x * x)), g);
-#pragma unroll
-    for (int n = 0; n <= L; ++n) g[n] *= pc.w;
+    seeds_far_scaled<L>(fma(z, z, fma(y, y, x * x)), pc.w, g);
     hermite_R<L>(x, y, z, g, sink);
 }
 
