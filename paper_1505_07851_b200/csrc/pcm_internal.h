@@ -197,8 +197,8 @@ struct pcm_ctx {
     size_t rbj_arena_bytes = 0;
 
     cudaStream_t own_stream = nullptr;
-    // the near kernels run on near_stream, forked from and joined back into the caller's stream around the main
-    // kernels of the same call, so that their latency-bound work fills what the FP64-bound main kernels leave idle
+    // the near kernels run on near_stream (low priority), forked from and joined back into the caller's stream around the
+    // main kernels of the same call, so that their latency-bound work fills what the FP64-bound main kernels leave idle
     cudaStream_t near_stream = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     // events: 0 start, 1 after the pre-transform, 2+L after the class-L main kernel, 7 end, 8 CG residual read-back
