@@ -417,15 +417,19 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
 
 // ---------------------------------------------------------------------------------------------
 // Block inversion: one thread block per diagonal block.  fill -> Cholesky (right-looking, in place, lower)
-// -> W = L^-1 (one column per thread) -> inv = W^T W.  n x n row-major, in global memory (L2 resident).
+// -> W = L^-1 (one column per thread) -> inv = W^T W.  n x n row-major; the two n x n work arrays live in shared memory
+// when they fit (use_smem: 2 n^2 doubles of dynamic shared memory, block sizes up to ~100), otherwise in global memory
+// (L2 resident).  Same arithmetic either way.
 // ---------------------------------------------------------------------------------------------
 __global__ void rbj_invert_kernel(const double4 *__restrict__ pt, const double *__restrict__ diag, int M, int block,
                                   const int32_t *__restrict__ order, double *__restrict__ inv, double *__restrict__ work,
-                                  int *__restrict__ err, const double *__restrict__ boys0) {
+                                  int *__restrict__ err, const double *__restrict__ boys0, int use_smem) {
+    extern __shared__ double s_blk[];
     const long long start = (long long)blockIdx.x * block;
     const int n = (int)min((long long)block, (long long)M - start);
-    double *a = inv + (size_t)blockIdx.x * block * block;
-    double *w = work + (size_t)blockIdx.x * block * block;
+    double *ga = inv + (size_t)blockIdx.x * block * block;
+    double *a = use_smem ? s_blk : ga;
+    double *w = use_smem ? s_blk + (size_t)block * block : work + (size_t)blockIdx.x * block * block;
     const int32_t *idx = order + start;
     {   // a failed selection (asynchronous build: the host has not looked yet) leaves `order` undefined
         const int e0 = *((volatile int *)err);
@@ -447,10 +451,10 @@ __global__ void rbj_invert_kernel(const double4 *__restrict__ pt, const double *
         __syncthreads();
         for (int i = j + threadIdx.x; i < n; i += blockDim.x) a[(size_t)i * n + j] = (i == j) ? s : a[(size_t)i * n + j] * is;
         __syncthreads();
-        const int m = n - j - 1;  // trailing update a[i][c] -= L[i][j] L[c][j], j < c <= i
-        for (int e = threadIdx.x; e < m * m; e += blockDim.x) {
-            const int i = j + 1 + e / m, c = j + 1 + e % m;
-            if (c <= i) a[(size_t)i * n + c] -= a[(size_t)i * n + j] * a[(size_t)c * n + j];
+        // trailing update a[i][c] -= L[i][j] L[c][j], j < c <= i: 16 x 16 threads stride over (i, c), no integer division
+        for (int i = j + 1 + (int)(threadIdx.x >> 4); i < n; i += (int)(blockDim.x >> 4)) {
+            const double lij = a[(size_t)i * n + j];
+            for (int c = j + 1 + (int)(threadIdx.x & 15); c <= i; c += 16) a[(size_t)i * n + c] -= lij * a[(size_t)c * n + j];
         }
         __syncthreads();
     }
@@ -475,6 +479,10 @@ __global__ void rbj_invert_kernel(const double4 *__restrict__ pt, const double *
     for (int e = threadIdx.x; e < n * n; e += blockDim.x) {
         const int r = e / n, c = e - r * n;
         if (c > r) a[(size_t)r * n + c] = a[(size_t)c * n + r];
+    }
+    if (use_smem) {
+        __syncthreads();
+        for (int e = threadIdx.x; e < n * n; e += blockDim.x) ga[e] = a[e];
     }
 }
 
@@ -1121,7 +1129,13 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     ctx->launch_total += 1;
     RBJ_TRY(cudaGetLastError());
     if (verbose) { cudaStreamSynchronize(s); t2 = now(); }
-    rbj_invert_kernel<<<(unsigned)nb, 256, 0, s>>>(ctx->pt, ctx->pt_diag, (int)M, block, ctx->rbj_order, ctx->rbj_inv, d_work, d_err, ctx->boys);
+    {
+        const size_t inv_smem = (size_t)2 * block * block * 8;
+        const int use_smem = inv_smem <= 160 * 1024;
+        if (use_smem) RBJ_TRY(cudaFuncSetAttribute(rbj_invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)inv_smem));
+        rbj_invert_kernel<<<(unsigned)nb, 256, use_smem ? inv_smem : 0, s>>>(ctx->pt, ctx->pt_diag, (int)M, block, ctx->rbj_order, ctx->rbj_inv,
+                                                                            d_work, d_err, ctx->boys, use_smem);
+    }
     RBJ_TRY(cudaGetLastError());
     if (async) {
         RBJ_TRY(cudaMemcpyAsync(ctx->cg_scal_host + 32, d_err, 16, cudaMemcpyDeviceToHost, s));
