@@ -57,7 +57,8 @@ WORK = {
     # Below 20 000 points the R = 2 kernel runs: row shift 6/32 per row, half a DADD of column reduction (11.69 instr, 19.75 flop).
     "amatvec": [(11.44, 19.5)],
     "amatvec_small": [(11.69, 19.75)],
-    "potential": [(12, 18), (17, 26), (32, 51), (57, 94), (97, 164)],   # L = 1: contracted before the seeds (pot_far_unit<1>)
+    # L = 1, 2, 3: contracted before the seeds, Horner in u = 1/R^2 (pot_far_unit<1..3>); L = 4: generic recursion
+    "potential": [(12, 18), (17, 26), (28, 45), (51, 85), (97, 164)],
     "fock": [(12, 18), (17, 27), (28, 44), (51, 81), (90, 146)],   # the charge multiplies the first seed only
 }
 

@@ -611,6 +611,9 @@ struct PotSink {
 
 template <int L>
 __host__ __device__ constexpr int pot_rec() { return (4 + nherm(L) + 1) / 2 * 2; }      // main kernel: centre, pad, D_h
+// potential_kernel's own record: for L = 3 four more slots (the first-order coefficients of the third-order block)
+template <int L>
+__host__ __device__ constexpr int pot_rec_main() { return pot_rec<L>() + (L == 3 ? 4 : 0); }
 template <int L>
 __host__ __device__ constexpr int pot_rec_near() { return (4 + nherm(L) + 2 + 1) / 2 * 2; }  // + (p, 1/kappa)
 
@@ -637,13 +640,56 @@ __device__ __forceinline__ void pot_far_unit<1>(const double *rec, const double4
     v = fma(ri, fma(-u, s, rec[4]), v);
 }
 
+// L = 2 contracted the same way: with g1 = -u g0, g2 = 3 u^2 g0 and R_200 = g1 + x^2 g2, R_110 = x y g2, ...
+//   D.R = g0 [ D_000 - u (D_1 . r + tr) + 3 u^2 (r^T D_2 r) ],  tr = D_200 + D_020 + D_002 (staged in the record's pad slot),
+// 28 FP64 instructions per evaluation instead of the ~36 of the generic recursion followed by the contraction.
+template <>
+__device__ __forceinline__ void pot_far_unit<2>(const double *rec, const double4 &c, double &v) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+    const double2 h23 = *reinterpret_cast<const double2 *>(rec + 2);
+    const double x = h01.x - c.x, y = h01.y - c.y, z = h23.x - c.z;
+    const double ri = rsqrt_fast(fma(z, z, fma(y, y, x * x)));
+    const double u = ri * ri;
+    // components: 4 = (2,0,0), 5 = (1,1,0), 6 = (1,0,1), 7 = (0,2,0), 8 = (0,1,1), 9 = (0,0,2)
+    const double q2 = fma(x, fma(rec[8], x, fma(rec[9], y, rec[10] * z)), fma(y, fma(rec[11], y, rec[12] * z), z * (rec[13] * z)));
+    const double lin = fma(rec[5], x, fma(rec[6], y, fma(rec[7], z, h23.y)));
+    const double e1 = fma(u * 3.0, q2, -lin);
+    v = fma(ri, fma(u, e1, rec[4]), v);
+}
+
+// L = 3: R_300 = 3 x g2 + x^3 g3, R_210 = y g2 + x^2 y g3, R_111 = x y z g3, ... and g3 = -15 u^3 g0, so
+//   D.R = g0 [ D_000 - u (D_1 . r + tr) + 3 u^2 (r^T D_2 r + l . r) - 15 u^3 C_3(r) ],
+// C_3 the cubic form of the third-order block, l = (3 D_300 + D_120 + D_102, 3 D_030 + D_210 + D_012, 3 D_003 + D_201 + D_021)
+// staged behind the record (slots 24..26) and tr in the pad slot.  51 FP64 instructions per evaluation.
+template <>
+__device__ __forceinline__ void pot_far_unit<3>(const double *rec, const double4 &c, double &v) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+    const double2 h23 = *reinterpret_cast<const double2 *>(rec + 2);
+    const double x = h01.x - c.x, y = h01.y - c.y, z = h23.x - c.z;
+    const double ri = rsqrt_fast(fma(z, z, fma(y, y, x * x)));
+    const double u = ri * ri;
+    const double *D = rec + 4;
+    // third order: 10 = (3,0,0), 11 = (2,1,0), 12 = (2,0,1), 13 = (1,2,0), 14 = (1,1,1), 15 = (1,0,2), 16 = (0,3,0),
+    // 17 = (0,2,1), 18 = (0,1,2), 19 = (0,0,3)
+    const double A = fma(D[10], x, fma(D[11], y, D[12] * z));
+    const double B = fma(y, fma(D[13], y, D[14] * z), (D[15] * z) * z);
+    const double Cc = fma(y * y, fma(D[16], y, D[17] * z), (z * z) * fma(D[18], y, D[19] * z));
+    const double c3 = fma(x, fma(x, A, B), Cc);
+    double q2 = fma(x, fma(D[4], x, fma(D[5], y, D[6] * z)), fma(y, fma(D[7], y, D[8] * z), z * (D[9] * z)));
+    q2 = fma(rec[24], x, fma(rec[25], y, fma(rec[26], z, q2)));
+    const double lin = fma(D[1], x, fma(D[2], y, fma(D[3], z, h23.y)));
+    const double e2 = fma(u * -5.0, c3, q2);
+    const double e1 = fma(u * 3.0, e2, -lin);
+    v = fma(ri, fma(u, e1, D[0]), v);
+}
+
 template <int L, int R, int C>
 __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restrict__ prodA, const double *__restrict__ herm,
                                                         int64_t npad, int chunk_len, const double4 *__restrict__ pt, int M,
                                                         double *__restrict__ vpart, const uint8_t *__restrict__ farmap,
                                                         int64_t nbyte, int64_t nrg) {
     constexpr int NH = nherm(L);
-    constexpr int REC = pot_rec<L>();
+    constexpr int REC = pot_rec_main<L>();
     constexpr int TILE = pot_tile(L), NS = TILE / SUB;
     __shared__ __align__(16) double s_rec[TILE * REC];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -671,6 +717,18 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
         for (int t = threadIdx.x; t < cnt * NH; t += TPB) {
             const int h = t / cnt, i = t - h * cnt;  // consecutive threads read consecutive products of one component
             s_rec[i * REC + 4 + h] = herm[(size_t)h * npad + base + i];
+        }
+        if (L == 2 || L == 3) {   // pot_far_unit<2>, <3> want the trace of the second-order block in the pad slot
+            __syncthreads();
+            for (int t = threadIdx.x; t < cnt; t += TPB) {
+                double *r = s_rec + t * REC;
+                r[3] = r[4 + 4] + r[4 + 7] + r[4 + 9];
+                if (L == 3) {     // and the first-order coefficients of the third-order block behind the record
+                    r[24] = fma(3.0, r[4 + 10], r[4 + 13] + r[4 + 15]);
+                    r[25] = fma(3.0, r[4 + 16], r[4 + 11] + r[4 + 18]);
+                    r[26] = fma(3.0, r[4 + 19], r[4 + 12] + r[4 + 17]);
+                }
+            }
         }
         __syncthreads();
         for (int st = 0; st < nst; ++st) {
