@@ -278,11 +278,24 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                                                                        unsigned char *__restrict__ assigned,
                                                                        const double *__restrict__ boxes, int ng,
                                                                        int *__restrict__ gcount, int *__restrict__ glist,
-                                                                       int *__restrict__ err, const double *__restrict__ boys0) {
+                                                                       int *__restrict__ err, const double *__restrict__ boys0,
+                                                                       int cache) {
     extern __shared__ __align__(16) unsigned char rbl_smem[];
     RblShared &S = *reinterpret_cast<RblShared *>(rbl_smem);
     const int tid = threadIdx.x;
-    for (int g = tid; g < ng; g += RBL_THREADS) gcount[g] = min(32, M - g * 32);
+    // cache != 0: the assigned flags, the per-group counts and the group boxes live in shared memory behind S
+    // (every step reads them several times in dependent order; from L2 that is most of a step's latency)
+    double *s_bx = reinterpret_cast<double *>(rbl_smem + (sizeof(RblShared) + 15) / 16 * 16);
+    int *s_gc = reinterpret_cast<int *>(s_bx + (size_t)6 * ng);
+    unsigned char *s_asg = reinterpret_cast<unsigned char *>(s_gc + ng);
+    unsigned char *asg = cache ? s_asg : assigned;
+    int *gc = cache ? s_gc : gcount;
+    const double *bx = cache ? s_bx : boxes;
+    if (cache) {
+        for (int i = tid; i < 6 * ng; i += RBL_THREADS) s_bx[i] = boxes[i];
+        for (int i = tid; i < M; i += RBL_THREADS) s_asg[i] = 0;
+    }
+    for (int g = tid; g < ng; g += RBL_THREADS) gc[g] = min(32, M - g * 32);
     if (tid == 0) S.rho = 6.0;
     __syncthreads();
     long long pos = 0, filled = 0;
@@ -292,7 +305,7 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
         __syncthreads();
         while (true) {
             const long long p = pos + tid;
-            if (p < M && !assigned[perm[p]]) atomicMin(&S.pivot, (int)p);
+            if (p < M && !asg[perm[p]]) atomicMin(&S.pivot, (int)p);
             __syncthreads();
             if (S.pivot < M || pos + RBL_THREADS >= M) break;
             pos += RBL_THREADS;
@@ -305,7 +318,7 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
         const int take = (int)min((long long)block - 1, (long long)M - filled - 1);
         const double4 pk = pt[k];
         __syncthreads();
-        if (tid == 0) { assigned[k] = 1; atomicSub(&gcount[k >> 5], 1); }
+        if (tid == 0) { asg[k] = 1; atomicSub(&gc[k >> 5], 1); }
         __syncthreads();
         if (take > 0) {
             while (true) {
@@ -315,8 +328,8 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                 for (int t = tid; t < RBJ_BINS; t += RBL_THREADS) S.hist[t] = 0;
                 __syncthreads();
                 for (int g = tid; g < ng; g += RBL_THREADS) {
-                    if (gcount[g] <= 0) continue;
-                    const double *b = boxes + (size_t)g * 6;
+                    if (gc[g] <= 0) continue;
+                    const double *b = bx + (size_t)g * 6;
                     const double gx = fmax(fmax(b[0] - pk.x, pk.x - b[3]), 0.0), gy = fmax(fmax(b[1] - pk.y, pk.y - b[4]), 0.0),
                                  gz = fmax(fmax(b[2] - pk.z, pk.z - b[5]), 0.0);
                     if (gx * gx + gy * gy + gz * gz < rho2) {
@@ -330,12 +343,18 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                 // ---- keys of the unassigned points of those groups
                 for (int t = tid; t < ngl * 32; t += RBL_THREADS) {
                     const int j = (ngl <= RBL_GL ? S.sgl[t >> 5] : glist[t >> 5]) * 32 + (t & 31);
-                    if (j < M && !assigned[j]) {
+                    // whole warps run this loop (ngl * 32 items): one slot reservation per warp instead of one per candidate
+                    const bool live = j < M && !asg[j];
+                    const unsigned live_mask = __ballot_sync(0xffffffffu, live);
+                    int wbase = 0;
+                    if ((tid & 31) == 0 && live_mask) wbase = atomicAdd(&S.nraw, __popc(live_mask));
+                    wbase = __shfl_sync(0xffffffffu, wbase, 0);
+                    if (live) {
                         const int cal = s2c[j];
                         const double4 b = pt[j];
                         const double dx = pk.x - b.x, dy = pk.y - b.y, dz = pk.z - b.z;
                         const double a = amat_entry(fma(dz, dz, fma(dy, dy, dx * dx)), pk.w, b.w, boys0);
-                        const int slot = atomicAdd(&S.nraw, 1);
+                        const int slot = wbase + __popc(live_mask & ((1u << (tid & 31)) - 1u));
                         if (slot < RBL_RAW) { S.rkey[slot] = a; S.ridx[slot] = j; S.rcal[slot] = cal; }
                         atomicAdd(&S.hist[rbj_bucket(a)], 1);
                     }
@@ -401,9 +420,9 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                 if (tid == 0) { err[2] += n; err[3] += nraw; }
                 if (rank < take) {
                     const int j = S.cidx[tid];
-                    assigned[j] = 1;
+                    asg[j] = 1;
                     order[filled + 1 + rank] = j;
-                    atomicSub(&gcount[j >> 5], 1);
+                    atomicSub(&gc[j >> 5], 1);
                 }
                 break;
             }
@@ -1088,10 +1107,13 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     if (block <= 256 && (M <= 30000 || getenv("PCM_RBJ_LOCAL")) && !force_global && !getenv("PCM_RBJ_GLOBAL")) {
         const int ng = (int)cdiv(M, 32);
         int *d_gcount = (int *)w.cand_idx, *d_glist = d_gcount + ng;   // scratch of the global path, 2 M ints
-        RBJ_TRY(cudaFuncSetAttribute(rbj_select_local_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RblShared)));
-        rbj_select_local_kernel<<<1, RBL_THREADS, sizeof(RblShared), s>>>(ctx->pt, (int)M, block, d_perm, ctx->s2c, ctx->rbj_order,
-                                                                           w.assigned, ctx->pt_boxes, ng, d_gcount, d_glist, d_err,
-                                                                           ctx->boys);
+        const size_t base_smem = (sizeof(RblShared) + 15) / 16 * 16;
+        const size_t cache_smem = base_smem + (size_t)ng * 6 * 8 + (size_t)ng * 4 + (size_t)M + 16;
+        const int cache = cache_smem <= 200 * 1024;
+        const size_t smem = cache ? cache_smem : base_smem;
+        RBJ_TRY(cudaFuncSetAttribute(rbj_select_local_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        rbj_select_local_kernel<<<1, RBL_THREADS, smem, s>>>(ctx->pt, (int)M, block, d_perm, ctx->s2c, ctx->rbj_order, w.assigned,
+                                                              ctx->pt_boxes, ng, d_gcount, d_glist, d_err, ctx->boys, cache);
         RBJ_TRY(cudaGetLastError());
         ctx->launch_total += 1;
         int h_e = 0;
