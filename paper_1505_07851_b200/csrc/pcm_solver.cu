@@ -267,6 +267,7 @@ struct RblShared {
     double ckey[RBL_CAP];
     int cidx[RBL_CAP];
     int ccal[RBL_CAP];
+    int crank[RBL_CAP];
     int pivot, nraw, ncut, bstar, ngl, all_in, ok;
     double rho, tau;
 };
@@ -401,15 +402,20 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                 const int n = S.ncut;
                 if (n > RBL_CAP || n < take) { if (tid == 0) *err = n < take ? 1 : 3; return; }
                 // ---- rank by (key descending, caller index ascending); tau = the take-th largest key
-                int rank = n;
-                if (tid < n) {
-                    const double key = S.ckey[tid];
-                    const int ci = S.ccal[tid];
-                    rank = 0;
-                    for (int o = 0; o < n; ++o) rank += (S.ckey[o] > key) || (S.ckey[o] == key && S.ccal[o] < ci);
-                    if (rank == take - 1) S.tau = key;
+                // one warp per candidate, the lanes stride over the others (n^2 / 1024 comparisons per thread)
+                for (int cand = tid >> 5; cand < n; cand += RBL_THREADS / 32) {
+                    const double key = S.ckey[cand];
+                    const int ci = S.ccal[cand];
+                    int cnt = 0;
+                    for (int o = tid & 31; o < n; o += 32) cnt += (S.ckey[o] > key) || (S.ckey[o] == key && S.ccal[o] < ci);
+                    cnt = __reduce_add_sync(0xffffffffu, cnt);
+                    if ((tid & 31) == 0) {
+                        S.crank[cand] = cnt;
+                        if (cnt == take - 1) S.tau = key;
+                    }
                 }
                 __syncthreads();
+                const int rank = tid < n ? S.crank[tid] : n;
                 if (tid == 0) {
                     const double tau = S.tau;
                     S.ok = S.all_in || tau * rho > 1.0;          // tau > 1/rho: nothing outside rho can reach the block
