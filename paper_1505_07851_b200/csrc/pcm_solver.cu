@@ -1108,9 +1108,9 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     if (verbose) { cudaStreamSynchronize(s); t1 = now(); }
     // block sizes up to 256: the single-CTA neighbourhood selection; it reports err = 3 (capacity) to fall back
     bool local_done = false;
-    // (measured: 1.24 vs 1.64 ms at M = 8 930, equal at 50k, 101 vs 90 ms at 200k, where scanning 6 250 group boxes per block
-    // with one CTA costs more than the two grid barriers of the global scan)
-    if (block <= 256 && (M <= 30000 || getenv("PCM_RBJ_LOCAL")) && !force_global && !getenv("PCM_RBJ_GLOBAL")) {
+    // (measured: 0.8 vs 1.6 ms at M = 8 930, 6.1 vs 9.6 ms at 50k, 86 vs 78 ms at 200k, where scanning 6 250 group boxes per
+    // block with one CTA costs more than the two grid barriers of the global scan)
+    if (block <= 256 && (M <= 100000 || getenv("PCM_RBJ_LOCAL")) && !force_global && !getenv("PCM_RBJ_GLOBAL")) {
         const int ng = (int)cdiv(M, 32);
         int *d_gcount = (int *)w.cand_idx, *d_glist = d_gcount + ng;   // scratch of the global path, 2 M ints
         const size_t base_smem = (sizeof(RblShared) + 15) / 16 * 16;
