@@ -34,9 +34,6 @@ constexpr int PT_TILE = 256;  // surface points staged per shared-memory tile (F
 struct Blocking { int R, C; };
 // A q blocking (plan_all): R = 4 / tile 256 from AMAT_R4_MIN points on, R = 2 / tile 64 below
 constexpr int AMAT_C = 2;
-#ifndef AMAT_MINB
-#define AMAT_MINB 1
-#endif
 constexpr int64_t AMAT_R4_MIN = 20000;
 __host__ __device__ constexpr Blocking fock_blocking(int L) {
     return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{2, 2} : L == 2 ? Blocking{1, 4} : Blocking{1, 2};
@@ -174,7 +171,7 @@ __device__ __forceinline__ void stage_points_local(const double4 *__restrict__ p
 }
 
 template <int R, int C, int TILE>
-__global__ void __launch_bounds__(TPB, AMAT_MINB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ q,
+__global__ void __launch_bounds__(TPB) amatvec_kernel(const double4 *__restrict__ pt, const double *__restrict__ q,
                                                       const int32_t *__restrict__ qidx, int M, int chunk_len,
                                                       double *__restrict__ out, double *__restrict__ colpart,
                                                       const uint8_t *__restrict__ farmap, int64_t nbyte, int64_t nrg,
