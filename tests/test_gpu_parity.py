@@ -261,6 +261,9 @@ def test_amatvec_parity(pcm, orc, torch_cuda, M):
     ctx2 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s.xyz, s.zeta, s.switch,
                          store_near=False)
     np.testing.assert_array_equal(pcm.pcm_amatvec(ctx2, dev(torch_cuda, q)).cpu().numpy(), y)
+    i1, i2 = pcm.pcm_get_info(ctx), pcm.pcm_get_info(ctx2)
+    assert i1.amat_near_patches == i2.amat_near_patches >= (M + 31) // 32        # at least the diagonal patches
+    assert i1.amat_stored_bytes == i1.amat_near_patches * 32 * 32 * 8 and i2.amat_stored_bytes == 0
     pcm.pcm_destroy(ctx2)
 
 
