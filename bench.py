@@ -46,10 +46,10 @@ SWEEP_M = (10_000, 50_000, 100_000, 200_000)
 # (DESIGN.md "Roofline"): [FP64-pipe instructions, flops (FMA = 2)] per unit for L = 0..4, potential and Fock.
 # geometry 3 DADD + (1 DMUL + 2 DFMA) + rsqrt (2 DMUL + 3 DFMA) = 11 instr / 16 flop, then seeds and recursion.
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the hot kernels on the bench workload, from the ncu --set full
-# captures summarised in profiles/r1d_ncu_full_summary.csv (a profiler number cannot be taken live).  The A q launch
+# captures summarised in profiles/r1e_ncu_full_summary.csv (a profiler number cannot be taken live).  The A q launch
 # streams its stored near patches (50.3 MB on configs[1]; ncu flushes L2 between replays, in the step they stay in L2).
-TRAFFIC = {"amatvec": 50.83e6, "potential": [1715200.0, 2185216.0, 1097216.0, None, None],
-           "fock": [1546496.0, 1363712.0, 639488.0, None, None]}
+TRAFFIC = {"amatvec": 50.81e6, "potential": [1715456.0, 2184704.0, 1097216.0, None, None],
+           "fock": [1547008.0, 1363712.0, 639232.0, None, None]}
 WORK = {
     # A q: the sweep is symmetric -- one evaluation of 1/r_ij serves A_ij and A_ji; unit = one pair evaluation
     # (M^2/2 per call), R = 4 kernel: local-origin geometry 4 + 3/16 (1 DADD + 3 DFMA, the row shift amortised over 32
@@ -342,7 +342,7 @@ def run_ours(args):
                 "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                 "traffic": TRAFFIC["amatvec"] if op == "amatvec" else TRAFFIC[op][Ld],
-                "traffic_source": "bytes per launch, ncu --set full capture in profiles/r1d_ncu_full_summary.csv",
+                "traffic_source": "bytes per launch, ncu --set full capture in profiles/r1e_ncu_full_summary.csv",
                 "algorithmic_bytes": (48.0 * M + float(info.amat_stored_bytes) if op == "amatvec" else 40.0 * M + (32.0 + 8.0 * [1, 4, 10, 20, 35][Ld]) * float(info.products[Ld])),
                 "fp64_pipe_frac": n_units * instr * 2.0 / (ms_dom * 1e-3) * 1e-12 / peak_tflops,
                 "units_per_launch": n_units, "flop_per_unit": flop, "fp64_instr_per_unit": instr, "ms_per_launch": ms_dom,
