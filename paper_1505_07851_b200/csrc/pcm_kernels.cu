@@ -39,7 +39,7 @@ __host__ __device__ constexpr Blocking fock_blocking(int L) {
     return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{2, 2} : L == 2 ? Blocking{1, 4} : Blocking{1, 2};
 }
 __host__ __device__ constexpr Blocking pot_blocking(int L) {
-    return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{4, 1} : L == 2 ? Blocking{2, 2} : L == 3 ? Blocking{1, 2} : Blocking{1, 1};
+    return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{4, 1} : L == 2 ? Blocking{2, 2} : L == 3 ? Blocking{2, 2} : Blocking{1, 1};
 }
 __host__ __device__ constexpr int pot_tile(int L) { return L <= 2 ? 256 : 64; }  // products staged per tile (8 or 2 groups)
 
