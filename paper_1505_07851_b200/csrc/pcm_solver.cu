@@ -1256,6 +1256,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         } else {
             const int64_t want = std::max<int64_t>(cdiv(M, 32), ctx->rbj_nblocks);
             fgrid = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)per_sm * ctx->sm_count));
+            if (const char *e = getenv("PCM_CG_GRID")) fgrid = std::max(1, std::min(fgrid, atoi(e)));
             fa.M = M; fa.block = block; fa.nblocks = (int)ctx->rbj_nblocks; fa.max_iter = max_iter;
             fa.parts = amat_parts(ctx);
             fa.order = ctx->rbj_order; fa.inv = ctx->rbj_inv;
