@@ -42,6 +42,50 @@ __device__ __forceinline__ void pot_grad_far_unit(const double *rec, const doubl
     g[0] = sink.gx; g[1] = sink.gy; g[2] = sink.gz;
 }
 
+// Classes L = 0, 1, 2 (all of an s/p basis) without the Hermite recursion: the far unit of the potential is g0 F(u, r),
+// g0 = 1/R, u = 1/R^2, F = D_0 - u (D_1.r + tr) + 3 u^2 Q_2(r) (pot_far_unit<1>, <2>), and with dg0/dr = -u g0 r, du/dr = -2 u^2 r
+//   sum_h D_h Rt_{h+1_d} = d/dr_d [g0 F] = g0 u [ -r_d (D_0 - 3 u (D_1.r + tr) + 15 u^2 Q_2) - D_1,d + 3 u dQ_2/dr_d ]
+// (the odd double factorials 1, 3, 15 again).  17 / 24 / 45 FP64 instructions instead of 21 / 40 / 75.
+template <>
+__device__ __forceinline__ void pot_grad_far_unit<0>(const double *rec, const double4 &c, double (&g)[3]) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+    const double x = h01.x - c.x, y = h01.y - c.y, z = rec[2] - c.z;
+    const double ri = rsqrt_fast(fma(z, z, fma(y, y, x * x)));
+    const double t = -(ri * ri) * (ri * rec[4]);
+    g[0] = fma(t, x, g[0]); g[1] = fma(t, y, g[1]); g[2] = fma(t, z, g[2]);
+}
+template <>
+__device__ __forceinline__ void pot_grad_far_unit<1>(const double *rec, const double4 &c, double (&g)[3]) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+    const double x = h01.x - c.x, y = h01.y - c.y, z = rec[2] - c.z;
+    const double ri = rsqrt_fast(fma(z, z, fma(y, y, x * x)));
+    const double u = ri * ri;
+    const double s = fma(rec[5], x, fma(rec[6], y, rec[7] * z));
+    const double a = fma(u * -3.0, s, rec[4]);           // D_0 - 3 u D_1.r
+    const double mc = -(ri * u);                         // -g0 u
+    g[0] = fma(mc, fma(x, a, rec[5]), g[0]);
+    g[1] = fma(mc, fma(y, a, rec[6]), g[1]);
+    g[2] = fma(mc, fma(z, a, rec[7]), g[2]);
+}
+template <>
+__device__ __forceinline__ void pot_grad_far_unit<2>(const double *rec, const double4 &c, double (&g)[3]) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+    const double x = h01.x - c.x, y = h01.y - c.y, z = rec[2] - c.z;
+    const double ri = rsqrt_fast(fma(z, z, fma(y, y, x * x)));
+    const double u = ri * ri;
+    const double *D = rec + 4;   // 4 = (2,0,0), 5 = (1,1,0), 6 = (1,0,1), 7 = (0,2,0), 8 = (0,1,1), 9 = (0,0,2)
+    const double qx = fma(D[4] + D[4], x, fma(D[5], y, D[6] * z));   // dQ_2/dx
+    const double qy = fma(D[5], x, fma(D[7] + D[7], y, D[8] * z));
+    const double qz = fma(D[6], x, fma(D[8], y, (D[9] + D[9]) * z));
+    const double q2 = 0.5 * fma(x, qx, fma(y, qy, z * qz));          // Euler: r.dQ_2/dr = 2 Q_2
+    const double lin = fma(D[1], x, fma(D[2], y, fma(D[3], z, (D[4] + D[7]) + D[9])));
+    const double a = fma(u, fma(u * 15.0, q2, -3.0 * lin), D[0]);    // D_0 - 3 u lin + 15 u^2 Q_2
+    const double u3 = u * 3.0, mc = -(ri * u);
+    g[0] = fma(mc, fma(x, a, fma(-u3, qx, D[1])), g[0]);
+    g[1] = fma(mc, fma(y, a, fma(-u3, qy, D[2])), g[1]);
+    g[2] = fma(mc, fma(z, a, fma(-u3, qz, D[3])), g[2]);
+}
+
 // far patches: rows = R points per thread, columns = products of class L staged in shared memory (as potential_kernel)
 template <int L, int R, int C>
 __global__ void __launch_bounds__(TPB) grad_point_kernel(const double4 *__restrict__ prodA, const double *__restrict__ herm,
