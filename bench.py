@@ -239,7 +239,7 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    pcm.lib()
+    pcm.lib(build=True)
     dev = torch.device("cuda", local)
 
     t0 = time.perf_counter()
@@ -465,7 +465,7 @@ def run_kernels(args):
     import torch
     import paper_1505_07851_b200 as pcm
     torch.cuda.set_device(0)
-    pcm.lib()
+    pcm.lib(build=True)
     w = synth.make_workload(args.config)
     ctx = pcm.setup_from_workload(w.basis, w.surface, gradient=True)
     s4, q4, _ = synth.make_solver_points(args.amat_m)

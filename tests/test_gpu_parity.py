@@ -25,7 +25,7 @@ def torch_cuda():
 @pytest.fixture(scope="module")
 def pcm():
     import paper_1505_07851_b200 as m
-    m.lib()
+    m.lib(build=True)   # compiles the library first if it is missing or stale (nvcc is in the image)
     return m
 
 
