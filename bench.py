@@ -239,7 +239,11 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    pcm.lib(build=True)
+    if rank == 0:
+        pcm.lib(build=True)          # compiles the library first if it is missing or stale; one rank only
+    if dist is not None:
+        dist.barrier()
+    pcm.lib()
     dev = torch.device("cuda", local)
 
     t0 = time.perf_counter()
