@@ -8,7 +8,13 @@
  *                           F_mu,nu = sum_k q_k (mu|J_k|nu)          (Eq. 10, dF^S = -F),
  *   - the matrix A of Eq. 2 / 3 / 8 and the product A q,
  *   - textbook preconditioned CG (section 4b) with the Jacobi and the randomized
- *     block-Jacobi (RBJ, section 4b-ii) preconditioners.
+ *     block-Jacobi (RBJ, section 4b-ii) preconditioners,
+ *   - the rest of a C-PCM step: B z (Eq. 4), the right-hand side of Eq. 1, the energy of Eq. 13,
+ *     the dynamic CG threshold of Eq. 21                       (pins: tests/test_oracle_glue.py),
+ *   - the gradient of E = v.q with respect to shell centres and surface points, i.e. the
+ *     one-electron term of Eq. 14 / Eq. 22                     (pins: tests/test_oracle_gradient.py),
+ *   - the ISWIG switching function of Eq. 9 and the surface terms of Eq. 14 (grad B, grad A
+ *     including A_kk through S_k)                              (pins: tests/test_oracle_surface.py).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
  * legs may call this file.  It shares no code, table, constant generator or helper with
