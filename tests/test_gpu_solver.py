@@ -173,3 +173,25 @@ def test_rbj_build_async_equals_sync(pcm, orc, sys2500, torch_cuda):
     assert np.array_equal(o1, o3)
     with pytest.raises(pcm.PcmError):
         pcm.pcm_rbj_build_async(ctx, 0, seed=1, stream=side)
+
+
+def test_fused_cg_and_neighbourhood_selection_are_exact_rewrites(pcm, orc, sys2500, torch_cuda, monkeypatch):
+    """DESIGN.md claims that (i) the one-CTA neighbourhood block selection finds the blocks of the global row scan and
+    (ii) the fused cooperative CG kernel reproduces the separate kernels bit for bit.  Both have a switch."""
+    torch = torch_cuda
+    s, A, q_true, ctx = sys2500
+    b = dev(torch, A @ q_true)
+    monkeypatch.delenv("PCM_RBJ_GLOBAL", raising=False)
+    monkeypatch.delenv("PCM_CG_UNFUSED", raising=False)
+    pcm.pcm_rbj_build(ctx, 48, seed=11)
+    o_local, b_local, inv_local = pcm.pcm_rbj_get(ctx)
+    x_fused, it_fused, rr_fused, _, ok = pcm.pcm_cg_solve(ctx, b, tol=1e-10, max_iter=500, precond=2)
+    assert ok
+    monkeypatch.setenv("PCM_CG_UNFUSED", "1")
+    x_sep, it_sep, rr_sep, _, ok = pcm.pcm_cg_solve(ctx, b, tol=1e-10, max_iter=500, precond=2)
+    assert ok and it_sep == it_fused and rr_sep == rr_fused and torch.equal(x_sep, x_fused)
+    monkeypatch.setenv("PCM_RBJ_GLOBAL", "1")
+    pcm.pcm_rbj_build(ctx, 48, seed=11)
+    o_glob, b_glob, inv_glob = pcm.pcm_rbj_get(ctx)
+    assert np.array_equal(o_local, o_glob) and np.array_equal(b_local, b_glob)
+    assert all(np.array_equal(a, c) for a, c in zip(inv_local, inv_glob))
