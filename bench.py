@@ -96,7 +96,7 @@ class ClockSampler:
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20",
                                           "-i", str(self.idx)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._pump, daemon=True)
             self.thread.start()
@@ -105,19 +105,24 @@ class ClockSampler:
 
     def _pump(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
 
-    def stop(self):
+    def stop(self, window=None):
+        """window = (t0, t1) in time.perf_counter(): only the samples that arrived inside it count (the sampler is started
+        before the warm-up steps because nvidia-smi needs ~0.1 s to deliver its first line); all samples if none did."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.25)
+        time.sleep(0.05)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
         sm, mx, reasons, power = [], [], set(), []
-        for ln in self.lines:
+        lines = list(self.lines)
+        inside = [ln for (t, ln) in lines if window and window[0] <= t <= window[1] + 0.02]
+        scope = "timed region" if inside else "warm-up + timed region"
+        for ln in (inside if inside else [ln for (_, ln) in lines]):
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 9:
                 continue
@@ -131,7 +136,7 @@ class ClockSampler:
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(power), "samples": len(sm),
-                "reasons": sorted(reasons)}
+                "sampled_over": scope, "reasons": sorted(reasons)}
 
 
 def load_peaks():
@@ -273,18 +278,18 @@ def run_ours(args):
         pcm.pcm_fock(ctx, q, F, stream=stream)
         return it, rr, rt, ok
 
+    peak_tflops = pcm.pcm_fp64_peak(ctx, 10)
+    sampler = ClockSampler(local)
+    sampler.start()                          # before the warm-up: its first line takes ~0.1 s
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
-    peak_tflops = pcm.pcm_fp64_peak(ctx, 10)
 
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
     cls_pot, cls_fock, main_ms, cg_mv = [], [], [], []
-    sampler = ClockSampler(local)
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
-    sampler.start()
     launches0 = pcm.pcm_launch_count(ctx)
     wall0 = time.perf_counter()
     iters = None
@@ -307,7 +312,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
     launches = pcm.pcm_launch_count(ctx) - launches0
-    clocks = sampler.stop()
+    clocks = sampler.stop(window=(wall0, wall0 + wall))
     if dist is not None:
         dist.barrier()
     step_ms = [e[0].elapsed_time(e[3]) for e in ev]
