@@ -62,6 +62,8 @@ def lib():
                                            C.c_long, C.c_void_p, _dp, _dp]
         L.orc_switching.argtypes = [C.c_long, _dp, _dp, _lp, C.c_long, _dp, _dp, _dp]
         L.orc_surface_gradient.argtypes = [C.c_long, _dp, _dp, _lp, C.c_long, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp]
+        L.orc_build_cavity.restype = C.c_long
+        L.orc_build_cavity.argtypes = [C.c_long, _dp, _dp, C.c_long, _dp, _dp, C.c_double, C.c_double, _dp, _dp, _dp, _lp, _lp]
         L.orc_bz.argtypes = [C.c_long, _dp, _dp, C.c_long, _dp, _dp, _dp]
         L.orc_rhs.argtypes = [C.c_long, _dp, _dp, C.c_double, _dp]
         L.orc_energy.argtypes = [C.c_long, _dp, _dp, _dp, _dp, C.c_double, _dp]
@@ -305,3 +307,19 @@ def surface_gradient(surface, atom_xyz, atom_radius, z, q, f: float):
     lib().orc_surface_gradient(surface.M, _f(surface.xyz).reshape(-1), _f(surface.zeta), own, n, a, _f(atom_radius), _f(z), _f(q),
                                float(f), gp.reshape(-1), ga.reshape(-1))
     return gp, ga
+
+
+# ------------------------------------------------------------------ ISWIG cavity construction (Eq. 7, Eq. 9, the 1e-8 screening)
+def build_cavity(atom_xyz, atom_radius, unit_grid, weights, zeta_tab: float, s_min: float = 1e-8):
+    """Points r = R_I + rad_I u_g of every atom with zeta = zeta_tab/(rad_I sqrt(w_g)) (Eq. 7) and S of Eq. 9, those with
+    S >= s_min kept, atom after atom.  Returns (synth-shaped surface fields) xyz [n,3], zeta [n], S [n],
+    atom [n], node [n]."""
+    a = _f(atom_xyz).reshape(-1)
+    N = len(a) // 3
+    u = _f(unit_grid).reshape(-1)
+    G = len(u) // 3
+    cap = max(N * G, 1)
+    xyz, zeta, S = np.zeros(3 * cap), np.zeros(cap), np.zeros(cap)
+    own, node = np.zeros(cap, np.int64), np.zeros(cap, np.int64)
+    n = lib().orc_build_cavity(N, a, _f(atom_radius), G, u, _f(weights), float(zeta_tab), float(s_min), xyz, zeta, S, own, node)
+    return xyz[:3 * n].reshape(n, 3).copy(), zeta[:n].copy(), S[:n].copy(), own[:n].copy(), node[:n].copy()

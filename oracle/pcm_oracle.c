@@ -14,7 +14,10 @@
  *   - the gradient of E = v.q with respect to shell centres and surface points, i.e. the
  *     one-electron term of Eq. 14 / Eq. 22                     (pins: tests/test_oracle_gradient.py),
  *   - the ISWIG switching function of Eq. 9 and the surface terms of Eq. 14 (grad B, grad A
- *     including A_kk through S_k)                              (pins: tests/test_oracle_surface.py).
+ *     including A_kk through S_k)                              (pins: tests/test_oracle_surface.py),
+ *   - the ISWIG cavity construction itself: sphere points per atom from a given unit-sphere
+ *     quadrature, zeta_k of Eq. 7, S_k of Eq. 9, the S_k >= 1e-8 screening of PAPER.md:106
+ *                                                              (pins: tests/test_oracle_cavity.py).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
  * legs may call this file.  It shares no code, table, constant generator or helper with
@@ -911,4 +914,38 @@ void orc_surface_gradient(long M, const double *pt_xyz, const double *pt_zeta, c
             g_atom[3 * J + x] = s + c;
         }
     free(pa); free(S);
+}
+
+/* ------------------------------------------------------------------------------------
+ * ISWIG cavity construction (Eq. 7 and Eq. 9, PAPER.md:106 the 1e-8 screening).
+ * Every atom I (centre R_I, cavity radius rad_I) carries the same unit-sphere quadrature: nodes u_g, |u_g| = 1, with
+ * weights w_g, sum_g w_g = 4 pi (the paper uses Lebedev grids; the grid is an INPUT here).  For every (I, g):
+ *     r     = R_I + rad_I u_g
+ *     zeta  = zeta_tab / (rad_I sqrt(w_g))                                     Eq. 7
+ *     S     = prod_{J != I} S_wf(r, R_J)                                       Eq. 9 (reading R13: J runs over the other atoms)
+ * and the point is kept iff S >= s_min ("MS points with a switching function value less than this threshold are
+ * ignored"; the paper's threshold is 1e-8).  Output order: atom after atom, node index ascending.
+ * The arrays must hold N*G entries; the return value is the number of points kept.
+ * Pins: tests/test_oracle_cavity.py.
+ * ---------------------------------------------------------------------------------- */
+long orc_build_cavity(long N, const double *atom_xyz, const double *atom_radius, long G, const double *unit, const double *w,
+                      double zeta_tab, double s_min, double *pt_xyz, double *pt_zeta, double *pt_S, long *pt_atom, long *pt_node) {
+    long n = 0;
+    for (long I = 0; I < N; ++I)
+        for (long g = 0; g < G; ++g) {
+            double r[3];
+            for (int x = 0; x < 3; ++x) r[x] = atom_xyz[3 * I + x] + atom_radius[I] * unit[3 * g + x];
+            double zeta = zeta_tab / (atom_radius[I] * sqrt(w[g]));
+            double S = 1.0;
+            for (long J = 0; J < N; ++J) {
+                if (J == I) continue;
+                double dx = r[0] - atom_xyz[3 * J], dy = r[1] - atom_xyz[3 * J + 1], dz = r[2] - atom_xyz[3 * J + 2];
+                S *= swf(zeta, atom_radius[J], sqrt(dx * dx + dy * dy + dz * dz));
+            }
+            if (!(S >= s_min)) continue;
+            pt_xyz[3 * n] = r[0]; pt_xyz[3 * n + 1] = r[1]; pt_xyz[3 * n + 2] = r[2];
+            pt_zeta[n] = zeta; pt_S[n] = S; pt_atom[n] = I; pt_node[n] = g;
+            ++n;
+        }
+    return n;
 }
