@@ -243,6 +243,40 @@ int pcm_set_cavity(pcm_ctx *ctx, const double *atom_radius_host, const int32_t *
 int pcm_surface_gradient(pcm_ctx *ctx, const double *q_dev, double f, double *g_point_dev, double *g_atom_dev, void *stream);
 
 /*
+ * ISWIG cavity construction on the device: the surface points of a molecule from its atoms.
+ *
+ * pcm_build_cavity -- every atom I (centre R_I, cavity radius rad_I; the paper: 1.2 x Bondi) carries the same unit-sphere
+ * quadrature of ngrid nodes u_g (unit vectors) with weights w_g > 0, sum w_g = 4 pi.  The paper uses Lebedev grids; the
+ * grid is an INPUT here (any quadrature of the sphere).  For every (I, g):
+ *     r_k = R_I + rad_I u_g,   zeta_k = zeta_tab / (rad_I sqrt(w_g))   (Eq. 7; zeta_tab = the tabulated exponent of the
+ *     quadrature level),   S_k = prod_{J != I} S_wf(r_k, R_J)   (Eq. 9)
+ * and the point is kept iff S_k >= s_min ("MS points with a switching function value less than this threshold are
+ * ignored"; the paper's value is 1e-8).  The kept points are in (atom, node) order.  All arrays HOST:
+ * atom_xyz 3*natom (bohr), atom_radius natom (> 0), grid_xyz 3*ngrid, grid_weight ngrid.  device: CUDA ordinal, -1 =
+ * current.  On success *out owns DEVICE arrays of the kept points (pcm_cavity_device) until pcm_cavity_destroy.
+ * Synchronous.  natom = 0 or ngrid = 0 give an empty cavity.  Errors: PCM_ERR_ARG, PCM_ERR_ALLOC, PCM_ERR_CUDA.
+ *
+ * pcm_cavity_size -- number of kept points.
+ * pcm_cavity_get -- copies to HOST arrays (any may be NULL): pt_xyz 3*n, pt_zeta n, pt_switch n (S_k), pt_atom n (owning
+ * atom I), pt_node n (grid node g).
+ * pcm_cavity_device -- the DEVICE arrays themselves (owned by the cavity; any out pointer may be NULL).
+ * pcm_setup_cavity -- pcm_setup with npoint, pt_xyz, pt_zeta and pt_switch taken from the cavity (no caller-side copy of
+ * the points); the context also remembers the cavity's radii and owners, so that after pcm_set_nuclei with the same
+ * natom atoms pcm_surface_gradient works without pcm_set_cavity.  Point k of the context is point k of the cavity.
+ */
+typedef struct pcm_cavity pcm_cavity;
+int pcm_build_cavity(pcm_cavity **out, int natom, const double *atom_xyz_host, const double *atom_radius_host, int ngrid,
+                     const double *grid_xyz_host, const double *grid_weight_host, double zeta_tab, double s_min, int device);
+int pcm_cavity_size(const pcm_cavity *cav, int64_t *npoint);
+int pcm_cavity_get(const pcm_cavity *cav, double *pt_xyz_host, double *pt_zeta_host, double *pt_switch_host, int32_t *pt_atom_host,
+                   int32_t *pt_node_host);
+int pcm_cavity_device(const pcm_cavity *cav, const double **xyz_dev, const double **zeta_dev, const double **switch_dev,
+                      const int32_t **atom_dev, const int32_t **node_dev);
+int pcm_cavity_destroy(pcm_cavity *cav);
+int pcm_setup_cavity(pcm_ctx **out, int nshell, const int *shell_l, const double *shell_xyz, const int *shell_nprim,
+                     const double *prim_exp, const double *prim_coef, const pcm_cavity *cav, const pcm_options *opt);
+
+/*
  * Host-buffer forms of the four hot calls: same semantics, every array is a HOST pointer; the call
  * copies inputs to the device, runs the device path on the context's own stream, copies the result back
  * and synchronises.  These are what bench.py's end-to-end figure times.

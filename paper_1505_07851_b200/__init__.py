@@ -32,6 +32,7 @@ EXPORTS = (
     "pcm_launch_count", "pcm_fp64_peak", "pcm_set_nuclei", "pcm_nuclear_potential", "pcm_rhs", "pcm_energy",
     "pcm_cg_threshold", "pcm_gradient", "pcm_last_cg_matvec_ms", "pcm_rbj_build_async", "pcm_switching", "pcm_set_cavity", "pcm_surface_gradient",
     "pcm_schwarz_bound", "pcm_last_error", "pcm_destroy",
+    "pcm_build_cavity", "pcm_cavity_size", "pcm_cavity_get", "pcm_cavity_device", "pcm_cavity_destroy", "pcm_setup_cavity",
 )
 
 
@@ -105,6 +106,12 @@ def lib(build: bool = False):
         L.pcm_switching.argtypes = [C.c_int64, vp, vp, vp, C.c_int, vp, vp, vp, C.c_int]
         L.pcm_set_cavity.argtypes = [vp, vp, vp]
         L.pcm_surface_gradient.argtypes = [vp, vp, C.c_double, vp, vp, vp]
+        L.pcm_build_cavity.argtypes = [C.POINTER(vp), C.c_int, vp, vp, C.c_int, vp, vp, C.c_double, C.c_double, C.c_int]
+        L.pcm_cavity_size.argtypes = [vp, _lp]
+        L.pcm_cavity_get.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.pcm_cavity_device.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+        L.pcm_cavity_destroy.argtypes = [vp]
+        L.pcm_setup_cavity.argtypes = [C.POINTER(vp), C.c_int, vp, vp, vp, vp, vp, vp, C.POINTER(pcm_options)]
         L.pcm_schwarz_bound.argtypes = [C.c_int, C.c_double, vp, C.c_int, C.c_double, vp, _dp]
         L.pcm_last_error.argtypes = [vp]
         L.pcm_last_error.restype = C.c_char_p
@@ -138,13 +145,29 @@ def _stream(stream):
     return C.c_void_p(stream.cuda_stream)
 
 
-def _dev(t, n=None):
+def _dev(t, n=None, ctx=None, strided=False):
+    """Device address of a CUDA float64 tensor: contiguous (unless `strided`: a row-major matrix with its own leading
+    dimension), at least n elements, on the context's device."""
     import torch
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
         raise TypeError("expected a CUDA float64 tensor")
     if n is not None and t.numel() < n:
         raise ValueError("tensor too small")
+    if not strided and not t.is_contiguous():
+        raise ValueError("expected a contiguous tensor")
+    if ctx is not None and t.device.index != ctx.device:
+        raise ValueError(f"tensor is on cuda:{t.device.index}, the context on cuda:{ctx.device}")
     return C.c_void_p(t.data_ptr())
+
+
+def _matrix(t, n, what):
+    """(device address, leading dimension) of a row-major n x n CUDA float64 matrix."""
+    if n > 0 and (t.dim() != 2 or t.shape[0] < n or t.shape[1] < n or (t.shape[1] > 1 and t.stride(1) != 1)):
+        raise ValueError(f"{what} must be a row-major matrix of at least {n} x {n}")
+    ld = t.stride(0) if t.dim() == 2 and t.shape[0] > 1 else max(n, 1)
+    if ld < n:
+        raise ValueError(f"{what}: leading dimension {ld} < {n}")
+    return ld
 
 
 class Context:
@@ -187,6 +210,10 @@ def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_z
     px = _np(pt_xyz, np.float64).reshape(-1)
     pz = _np(pt_zeta, np.float64)
     ps = None if pt_switch is None else _np(pt_switch, np.float64)
+    if len(sx) != 3 * len(sl) or len(sn) != len(sl) or len(pe) != int(sn.sum()) or len(pc) != len(pe):
+        raise ValueError("pcm_setup: shell_xyz must hold 3 doubles per shell, prim_exp / prim_coef sum(shell_nprim) entries")
+    if len(px) != 3 * len(pz) or (ps is not None and len(ps) != len(pz)):
+        raise ValueError("pcm_setup: pt_xyz must hold 3 doubles per point, pt_switch one")
     if device < 0:
         device = torch.cuda.current_device()
     torch.cuda.init()
@@ -218,10 +245,8 @@ def pcm_potential(ctx: Context, P, v=None, stream=None):
     import torch
     if v is None:
         v = torch.empty(ctx.M, dtype=torch.float64, device=P.device)
-    ldp = P.stride(0) if P.dim() == 2 and P.shape[0] > 1 else max(ctx.nbf, 1)
-    if P.dim() == 2 and P.shape[1] > 1 and P.stride(1) != 1:
-        raise ValueError("P must be row-major")
-    _check(lib().pcm_potential(ctx.handle, _dev(P), ldp, _dev(v, ctx.M), _stream(stream)), ctx.handle)
+    ldp = _matrix(P, ctx.nbf, "P")
+    _check(lib().pcm_potential(ctx.handle, _dev(P, None, ctx, strided=True), ldp, _dev(v, ctx.M, ctx), _stream(stream)), ctx.handle)
     return v
 
 
@@ -230,8 +255,8 @@ def pcm_fock(ctx: Context, q, F=None, accumulate: bool = False, stream=None):
     if F is None:
         F = torch.empty((ctx.nbf, ctx.nbf), dtype=torch.float64, device=q.device)
         accumulate = False
-    ldf = F.stride(0) if F.dim() == 2 and F.shape[0] > 1 else max(ctx.nbf, 1)
-    _check(lib().pcm_fock(ctx.handle, _dev(q, ctx.M), _dev(F), ldf, 1 if accumulate else 0, _stream(stream)), ctx.handle)
+    ldf = _matrix(F, ctx.nbf, "F")
+    _check(lib().pcm_fock(ctx.handle, _dev(q, ctx.M, ctx), _dev(F, None, ctx, strided=True), ldf, 1 if accumulate else 0, _stream(stream)), ctx.handle)
     return F
 
 
@@ -239,7 +264,7 @@ def pcm_amatvec(ctx: Context, q, y=None, stream=None):
     import torch
     if y is None:
         y = torch.empty(ctx.M, dtype=torch.float64, device=q.device)
-    _check(lib().pcm_amatvec(ctx.handle, _dev(q, ctx.M), _dev(y, ctx.M), _stream(stream)), ctx.handle)
+    _check(lib().pcm_amatvec(ctx.handle, _dev(q, ctx.M, ctx), _dev(y, ctx.M, ctx), _stream(stream)), ctx.handle)
     return y
 
 
@@ -297,6 +322,84 @@ def pcm_switching(pt_xyz, pt_zeta, pt_atom, atom_xyz, atom_radius, device: int =
     S = np.zeros(len(pz))
     _check(lib().pcm_switching(len(pz), _hp(px), _hp(pz), _hp(pa), len(ar), _hp(ax), _hp(ar), _hp(S), int(device)))
     return S
+
+
+class Cavity:
+    """Owner of a ``pcm_cavity*`` (device arrays of the kept surface points)."""
+
+    def __init__(self, handle, natom):
+        self.handle = handle
+        self.natom = natom
+
+    @property
+    def npoint(self) -> int:
+        n = C.c_int64(0)
+        _check(lib().pcm_cavity_size(self.handle, C.byref(n)))
+        return int(n.value)
+
+    def __del__(self):
+        try:
+            pcm_cavity_destroy(self)
+        except Exception:
+            pass
+
+
+def pcm_build_cavity(atom_xyz, atom_radius, grid_xyz, grid_weight, zeta_tab: float, s_min: float = 1e-8, device: int = -1) -> Cavity:
+    """ISWIG cavity of Eq. 7 / Eq. 9 with the S_k >= s_min screening, built on the device (include/pcm.h)."""
+    ax, ar = _np(atom_xyz, np.float64).reshape(-1), _np(atom_radius, np.float64)
+    gx, gw = _np(grid_xyz, np.float64).reshape(-1), _np(grid_weight, np.float64)
+    if len(ax) != 3 * len(ar) or len(gx) != 3 * len(gw):
+        raise ValueError("atom_xyz / grid_xyz must hold 3 doubles per radius / weight")
+    h = C.c_void_p()
+    _check(lib().pcm_build_cavity(C.byref(h), len(ar), _hp(ax), _hp(ar), len(gw), _hp(gx), _hp(gw), float(zeta_tab), float(s_min), int(device)))
+    return Cavity(h, len(ar))
+
+
+def pcm_cavity_get(cav: Cavity):
+    """(xyz [n, 3], zeta [n], S [n], atom [n], node [n]) as host arrays."""
+    n = cav.npoint
+    xyz, zeta, S = np.zeros((n, 3)), np.zeros(n), np.zeros(n)
+    atom, node = np.zeros(n, np.int32), np.zeros(n, np.int32)
+    _check(lib().pcm_cavity_get(cav.handle, _hp(xyz), _hp(zeta), _hp(S), _hp(atom), _hp(node)))
+    return xyz, zeta, S, atom, node
+
+
+def pcm_cavity_device(cav: Cavity):
+    """Raw device addresses (xyz, zeta, S, atom, node) of the cavity's arrays."""
+    p = [C.c_void_p() for _ in range(5)]
+    _check(lib().pcm_cavity_device(cav.handle, *[C.byref(x) for x in p]))
+    return tuple(x.value for x in p)
+
+
+def pcm_cavity_destroy(cav: Cavity) -> None:
+    if cav is not None and getattr(cav, "handle", None):
+        h, cav.handle = cav.handle, None
+        lib().pcm_cavity_destroy(h)
+
+
+def pcm_setup_cavity(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, cav: Cavity, *, screen_eps: float = 1e-12,
+                     d_pure: bool = True, merge_products: bool = True, gradient: bool = False, store_near: bool = True) -> Context:
+    """pcm_setup with the surface points of a built cavity."""
+    import torch
+    sl = _np(shell_l, np.int32)
+    sx = _np(shell_xyz, np.float64).reshape(-1)
+    sn = _np(shell_nprim, np.int32)
+    pe = _np(prim_exp, np.float64)
+    pc = _np(prim_coef, np.float64)
+    if len(sx) != 3 * len(sl) or len(sn) != len(sl) or len(pe) != int(sn.sum()) or len(pc) != len(pe):
+        raise ValueError("pcm_setup_cavity: inconsistent shell array lengths")
+    opt = pcm_options_default()
+    opt.screen_eps = float(screen_eps)
+    opt.d_pure = 1 if d_pure else 0
+    opt.merge_products = 1 if merge_products else 0
+    opt.gradient = 1 if gradient else 0
+    opt.store_near = 1 if store_near else 0
+    h = C.c_void_p()
+    _check(lib().pcm_setup_cavity(C.byref(h), len(sl), _hp(sl), _hp(sx), _hp(sn), _hp(pe), _hp(pc), cav.handle, C.byref(opt)), None)
+    ctx = Context(h, 0, cav.npoint, torch.cuda.current_device())
+    ctx.nbf = int(pcm_get_info(ctx).nbf)
+    ctx.nshell = len(sl)
+    return ctx
 
 
 def pcm_set_cavity(ctx: Context, atom_radius, pt_atom) -> None:
@@ -367,7 +470,7 @@ def pcm_cg_solve(ctx: Context, b, x=None, tol: float = 1e-8, max_iter: int = 100
         use_x0 = False
     it = C.c_int(0)
     resid = (C.c_double * 2)()
-    rc = _check(lib().pcm_cg_solve(ctx.handle, _dev(b, ctx.M), _dev(x, ctx.M), float(tol), int(max_iter), int(precond),
+    rc = _check(lib().pcm_cg_solve(ctx.handle, _dev(b, ctx.M, ctx), _dev(x, ctx.M, ctx), float(tol), int(max_iter), int(precond),
                                    1 if use_x0 else 0, C.byref(it), resid, _stream(stream)), ctx.handle)
     return x, int(it.value), float(resid[0]), float(resid[1]), rc == PCM_OK
 

@@ -192,6 +192,8 @@ int pcm_set_nuclei(pcm_ctx *ctx, int natom, const double *atom_xyz_host, const d
     PCM_CUDA(ctx, cudaMemcpy(ctx->atoms, at.data(), at.size() * sizeof(double4), cudaMemcpyHostToDevice));
     ctx->natom = natom;
     ctx->cavity_set = false;   // radii belong to the atom list
+    if (ctx->cav_natom == natom && natom >= 0 && (int64_t)ctx->cav_owner_host.size() == ctx->M)   // context of pcm_setup_cavity
+        return pcm_set_cavity(ctx, ctx->cav_radius_host.data(), ctx->cav_owner_host.data());
     return PCM_OK;
 }
 

@@ -139,6 +139,10 @@ struct pcm_ctx {
     double *atom_radius = nullptr;
     int32_t *pt_owner = nullptr;
     bool cavity_set = false;
+    // a context made by pcm_setup_cavity remembers the cavity's atoms: pcm_set_nuclei with as many atoms re-registers them
+    int cav_natom = -1;
+    std::vector<double> cav_radius_host;
+    std::vector<int32_t> cav_owner_host;   // caller (= cavity) point order
     double *surf_scratch = nullptr;   // pcm_surface_gradient partial sums (grow-only)
     size_t surf_scratch_n = 0;
 
