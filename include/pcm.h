@@ -59,7 +59,11 @@ typedef struct pcm_options {
     int store_near;        /* 1 (default): the patches of A that are not in the far field (the entries that need erf) are
                               evaluated once at pcm_setup and kept on the device (8 KB per 32 x 32 patch, up to 16 GB; beyond
                               that, or with 0, they are re-evaluated in every pcm_amatvec).  Same values either way. */
-    int reserved[2];
+    int cg_path;           /* pcm_cg_solve / pcm_amatvec: 0 (default) = one persistent cooperative kernel per solve and one launch per
+                              A q below 20 000 points, separate kernel launches above; 1 = always separate launches (the
+                              reference path); 2 = the persistent kernel at any size its buffers allow.  Same recurrences; the
+                              two paths add the partial sums of A q in different (each fixed) orders */
+    int reserved[1];
 } pcm_options;
 
 typedef struct pcm_info {

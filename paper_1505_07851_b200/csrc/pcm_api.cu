@@ -135,6 +135,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     ctx->ypart_slots = ctx->plan_amat.chunks;
     if ((rc = dev_alloc_t(ctx, &ctx->near_amat, (size_t)ctx->amat_map.npiece * 32))) return fail(rc);
     if ((rc = fill_amat_blocks(ctx))) return fail(rc);
+    if ((rc = plan_sweep(ctx))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->vpart, (size_t)std::max<int64_t>(ctx->vpart_slots, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->ypart, (size_t)ctx->ypart_slots * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->colpart, (size_t)std::max<int64_t>(ctx->plan_amat.xb, 1) * std::max<int64_t>(M, 1)))) return fail(rc);

@@ -59,8 +59,31 @@ struct PatchMap {
     int64_t npiece = 0;
     int64_t *pstart = nullptr;  // [nrg + 1] CSR: pieces of each row group
     int32_t *piece_rg = nullptr;  // [npiece]
+    // host copies, kept for the A q map only (plan_sweep partitions the sweep from them)
+    std::vector<uint8_t> far_host;
+    std::vector<int64_t> start_host, pstart_host;
+    std::vector<int32_t> piece_rg_host;
 };
 constexpr int NEAR_PIECE = 4;
+
+// Warp-granular partition of the symmetric A q sweep and the buffers of the persistent PCG kernel (pcm_cgp.cu); built by
+// plan_sweep at pcm_setup for cavities below AMAT_PERSIST_MAX points whose near patches are stored.
+constexpr int64_t AMAT_PERSIST_MAX = 20000;
+struct SweepPlan {
+    bool ready = false;
+    int grid = 0, nwarp = 0, ng = 0, nrb = 0, nslot = 0;
+    int64_t nstrip = 0;
+    size_t smem = 0;
+    int2 *strip = nullptr;            // [nstrip] (row block, column group | far mask of the 4 row groups << 24)
+    int64_t *seg_start = nullptr;     // [nwarp + 1] strips of every warp
+    int32_t *seg_slot0 = nullptr;     // [nwarp + 1] first row-sum slot of every warp
+    int32_t *rb_slot_start = nullptr; // [nrb + 1] slots of every row block (consecutive)
+    double4 *colloc = nullptr;        // [M] (-2 (b - o), |b - o|^2), o = first point of the column's group
+    double4 *org = nullptr;           // [ng] o
+    double *yslot = nullptr;          // [nslot][128] row sums of a (segment, row block) run
+    double *colpart = nullptr;        // [nrb][M] column sums of a row block
+    double *pbuf = nullptr;           // [M] second buffer of the CG direction
+};
 
 struct ClassData {        // products of one total angular momentum L, padded to a multiple of 128
     int64_t n = 0;        // products
@@ -166,6 +189,7 @@ struct pcm_ctx {
 
     // fixed work partitions (sizes and SM count only; set once in pcm_setup by plan_all)
     pcm::Plan plan_pot[pcm::MAXL + 1], plan_fock[pcm::MAXL + 1], plan_amat;
+    pcm::SweepPlan cgp;
 
     // scratch
     double *vpart = nullptr;    // potential partial sums [slots][M]
@@ -244,6 +268,10 @@ int launch_surface_gradient(pcm_ctx *ctx, const double *q, double f, double *g_p
 int switching_host(int64_t M, const double *xyz, const double *zeta, const int32_t *owner, int natom, const double *atom_xyz,
                    const double *atom_radius, double *S);
 int plan_all(pcm_ctx *ctx);
+int plan_sweep(pcm_ctx *ctx);
+int cgp_matvec(pcm_ctx *ctx, const double *q, const int32_t *idx, double *y, cudaStream_t s);
+int cgp_solve(pcm_ctx *ctx, double *r, double *z, double *p, double *Ap, double *x, double tol, int max_iter, int precond, cudaStream_t s);
+bool cgp_can_solve(const pcm_ctx *ctx, int precond);
 int fill_amat_blocks(pcm_ctx *ctx);
 int fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
 void build_boys_tables(std::vector<double> &tab);

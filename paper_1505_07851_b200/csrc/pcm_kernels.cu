@@ -1096,6 +1096,13 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
     int rc;
     if ((rc = mark(ctx, 0, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
+    if (ctx->cgp.ready && ctx->opt.cg_path != 1) {   // small cavities: sweep, grid barrier and row sums in one cooperative launch
+        if ((rc = cgp_matvec(ctx, q, idx, y, s))) return rc;
+        ctx->launches[2]++;
+        for (int i = 2; i <= 7; ++i)
+            if ((rc = mark(ctx, i, s))) return rc;
+        return PCM_OK;
+    }
     if ((rc = launch_amatvec_kernels(ctx, q, idx, nullptr, s))) return rc;
     for (int i = 2; i <= 6; ++i)
         if ((rc = mark(ctx, i, s))) return rc;

@@ -239,7 +239,7 @@ static double box_gap2(const double *a, const double *b) {
     return s;
 }
 // patch (rg, cg) is far when the boxes are further apart than both groups' far-field radii (1 % margin)
-static int build_patch_map(pcm_ctx *ctx, const GroupBoxes &rows, const GroupBoxes &cols, PatchMap &pm) {
+static int build_patch_map(pcm_ctx *ctx, const GroupBoxes &rows, const GroupBoxes &cols, PatchMap &pm, bool keep_host = false) {
     const int64_t nrg = rows.n(), ncg = cols.n(), nbyte = (ncg + 7) / 8;
     pm.nrg = nrg; pm.ncg = ncg; pm.nbyte = nbyte;
     std::vector<uint8_t> far((size_t)std::max<int64_t>(nrg * nbyte, 1), 0);
@@ -282,7 +282,9 @@ static int build_patch_map(pcm_ctx *ctx, const GroupBoxes &rows, const GroupBoxe
     if ((rc = upload(ctx, &pm.start, start))) return rc;
     if ((rc = upload(ctx, &pm.pstart, pstart))) return rc;
     if ((rc = upload(ctx, &pm.piece_rg, piece_rg))) return rc;
-    return upload(ctx, &pm.list, list);
+    if ((rc = upload(ctx, &pm.list, list))) return rc;
+    if (keep_host) { pm.far_host = std::move(far); pm.start_host = std::move(start); pm.pstart_host = std::move(pstart); pm.piece_rg_host = std::move(piece_rg); }
+    return PCM_OK;
 }
 
 static int class_of(int la, int lb) {
@@ -348,7 +350,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         }
         GroupBoxes amat_boxes = ptboxes;
         for (int64_t g = 0; g < ng; ++g) amat_boxes.b[(size_t)g * 7 + 6] = TFAR_AMAT * 2.0 / (zmin * zmin);
-        if ((rc = build_patch_map(ctx, amat_boxes, amat_boxes, ctx->amat_map))) return rc;
+        if ((rc = build_patch_map(ctx, amat_boxes, amat_boxes, ctx->amat_map, npoint < 4 * AMAT_PERSIST_MAX))) return rc;
     }
     {
         std::vector<double> tab;

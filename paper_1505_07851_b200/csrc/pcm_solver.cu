@@ -1240,6 +1240,19 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         CG_CUDA(cudaMemsetAsync(x, 0, (size_t)M * 8, s));
         CG_CUDA(cudaMemcpyAsync(r, b, (size_t)M * 8, cudaMemcpyDeviceToDevice, s));
     }
+    int it = 0;
+    double rr = 0.0;
+    // below AMAT_PERSIST_MAX points: every iteration inside one persistent cooperative kernel (pcm_cgp.cu)
+    const bool persistent = ctx->opt.cg_path != 1 && cgp_can_solve(ctx, precond);
+    if (persistent) {
+        CG_TRY(cgp_solve(ctx, r, z, p, Ap, x, tol, max_iter, precond, s));
+        CG_CUDA(cudaMemcpyAsync(h, scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CG_CUDA(cudaStreamSynchronize(s));
+        const int *hc = reinterpret_cast<const int *>(h + 8);
+        it = hc[CTL_ITERS];
+        rr = h[2];
+        if (hc[CTL_BAR_ERR]) { ctx->timing = saved_timing; return set_error(ctx, PCM_ERR_STATE, "pcm_cg_solve: grid barrier timed out"); }
+    } else {
     CG_TRY(update(1));  // z = C r, p = z, rz, rr; raises STOP if already converged (or max_iter == 0)
     // RBJ: everything after the sweep in one cooperative kernel (cg_fused_rbj_kernel)
     bool fused = precond == 2 && !getenv("PCM_CG_UNFUSED");
@@ -1267,8 +1280,6 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     }
     int batch = 8;   // iterations queued per read-back of the device-side convergence flag
     if (const char *e = getenv("PCM_CG_BATCH")) batch = std::max(1, atoi(e));
-    int it = 0;
-    double rr = 0.0;
     while (true) {
         CG_CUDA(cudaMemcpyAsync(h, scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
         CG_CUDA(cudaStreamSynchronize(s));
@@ -1293,6 +1304,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
             }
         }
     }
+    }
     const double rn = std::sqrt(rr);
     // true residual
     CG_TRY(launch_amatvec_sorted(ctx, x, Ap, s));
@@ -1308,6 +1320,8 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     ctx->timing = saved_timing;
     if (iters) *iters = it;
     if (resid) { resid[0] = rn; resid[1] = std::sqrt(h[4]); }
+    if (!std::isfinite(rn) || !std::isfinite(h[4]))
+        return set_error(ctx, PCM_ERR_NUMERIC, "pcm_cg_solve: the residual is not finite (non-finite right-hand side, or p.Ap = 0)");
     return rn > tol ? PCM_NOT_CONVERGED : PCM_OK;
 }
 

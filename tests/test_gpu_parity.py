@@ -257,10 +257,15 @@ def test_amatvec_parity(pcm, orc, torch_cuda, M):
     col = pcm.pcm_amatvec(ctx, dev(torch_cuda, e)).cpu().numpy()
     ref = np.array([orc.a_entry(s, i, M // 2) for i in range(M)])
     assert_parity(col, ref, f"A column, M = {M}")
-    # the near patches stored at setup (default) and re-evaluated in every call give the same bits
-    ctx2 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s.xyz, s.zeta, s.switch,
-                         store_near=False)
-    np.testing.assert_array_equal(pcm.pcm_amatvec(ctx2, dev(torch_cuda, q)).cpu().numpy(), y)
+    # the near patches stored at setup (default) and re-evaluated in every call give the same bits (both through the
+    # separate-launch path: without stored patches the one-launch sweep of pcm_cgp.cu is not used)
+    z0, zi = np.zeros(0), np.zeros(0, np.int32)
+    ctx1 = pcm.pcm_setup(zi, np.zeros((0, 3)), zi, z0, z0, s.xyz, s.zeta, s.switch, cg_path=1)
+    ctx2 = pcm.pcm_setup(zi, np.zeros((0, 3)), zi, z0, z0, s.xyz, s.zeta, s.switch, store_near=False)
+    y1 = pcm.pcm_amatvec(ctx1, dev(torch_cuda, q)).cpu().numpy()
+    np.testing.assert_array_equal(pcm.pcm_amatvec(ctx2, dev(torch_cuda, q)).cpu().numpy(), y1)
+    assert_parity(y1, orc.amatvec(s, q), f"A q (separate launches), M = {M}")
+    pcm.pcm_destroy(ctx1)
     i1, i2 = pcm.pcm_get_info(ctx), pcm.pcm_get_info(ctx2)
     assert i1.amat_near_patches == i2.amat_near_patches >= (M + 31) // 32        # at least the diagonal patches
     assert i1.amat_stored_bytes == i1.amat_near_patches * 32 * 32 * 8 and i2.amat_stored_bytes == 0

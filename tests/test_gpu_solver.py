@@ -34,9 +34,9 @@ def dev(torch, a):
     return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda")
 
 
-def points_ctx(pcm, s):
+def points_ctx(pcm, s, **kw):
     z = np.zeros(0)
-    return pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), z, z, s.xyz, s.zeta, s.switch)
+    return pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), z, z, s.xyz, s.zeta, s.switch, **kw)
 
 
 @pytest.fixture(scope="module")
@@ -179,7 +179,8 @@ def test_fused_cg_and_neighbourhood_selection_are_exact_rewrites(pcm, orc, sys25
     """DESIGN.md claims that (i) the one-CTA neighbourhood block selection finds the blocks of the global row scan and
     (ii) the fused cooperative CG kernel reproduces the separate kernels bit for bit.  Both have a switch."""
     torch = torch_cuda
-    s, A, q_true, ctx = sys2500
+    s, A, q_true, _ = sys2500
+    ctx = points_ctx(pcm, s, cg_path=1)            # the separate-launch path (below 20k points the default is the persistent kernel)
     b = dev(torch, A @ q_true)
     monkeypatch.delenv("PCM_RBJ_GLOBAL", raising=False)
     monkeypatch.delenv("PCM_CG_UNFUSED", raising=False)
@@ -195,3 +196,50 @@ def test_fused_cg_and_neighbourhood_selection_are_exact_rewrites(pcm, orc, sys25
     o_glob, b_glob, inv_glob = pcm.pcm_rbj_get(ctx)
     assert np.array_equal(o_local, o_glob) and np.array_equal(b_local, b_glob)
     assert all(np.array_equal(a, c) for a, c in zip(inv_local, inv_glob))
+
+
+@pytest.mark.parametrize("M", [300, 2500, 9000])
+def test_persistent_solve_equals_the_separate_launch_path(pcm, orc, torch_cuda, M):
+    """Below 20k points pcm_cg_solve runs every iteration inside one persistent cooperative kernel and pcm_amatvec is one
+    launch (pcm_cgp.cu); pcm_options.cg_path = 1 keeps the separate launches.  Same recurrences, another (fixed) order of the
+    A q partial sums: A q agrees to rounding, the iteration counts are equal (up to one, when the residual of an iteration sits
+    at the tolerance) and the solutions agree to 1e-11 where the counts are equal."""
+    torch = torch_cuda
+    s, q, q_true = synth.make_solver_points(M, seed=1004)
+    cp, cr = points_ctx(pcm, s), points_ctx(pcm, s, cg_path=1)
+    qd = dev(torch, q)
+    yp, yr = pcm.pcm_amatvec(cp, qd).cpu().numpy(), pcm.pcm_amatvec(cr, qd).cpu().numpy()
+    assert np.all(np.abs(yp - yr) <= 1e-13 * np.abs(yr) + 1e-15)
+    assert np.array_equal(pcm.pcm_amatvec(cp, qd).cpu().numpy(), yp)                 # fixed order: bit-reproducible
+    if M <= 2500:
+        ref = orc.amatvec(s, q)
+        assert np.all(np.abs(yp - ref) <= 1e-10 * np.abs(ref) + 1e-12)
+    b = pcm.pcm_amatvec(cr, dev(torch, q_true))
+    for c in (cp, cr):
+        pcm.pcm_rbj_build(c, 64, seed=7)
+    for precond in (0, 1, 2):
+        xp, itp, rrp, rtp, okp = pcm.pcm_cg_solve(cp, b, tol=1e-9, max_iter=3000, precond=precond)
+        xr, itr, rrr, rtr, okr = pcm.pcm_cg_solve(cr, b, tol=1e-9, max_iter=3000, precond=precond)
+        assert okp and okr and abs(itp - itr) <= 1, (precond, itp, itr)
+        assert rtp <= 2e-9 and float((xp - xr).abs().max()) <= (1e-11 if itp == itr else 1e-9)
+        xp2, itp2, rrp2, _, _ = pcm.pcm_cg_solve(cp, b, tol=1e-9, max_iter=3000, precond=precond)
+        assert itp2 == itp and rrp2 == rrp and torch.equal(xp, xp2)                  # bit-reproducible run to run
+    assert float((xp - dev(torch, q_true)).abs().max()) < 1e-7
+    # max_iter and warm start behave as on the reference path
+    x3, it3, rr3, _, ok3 = pcm.pcm_cg_solve(cp, b, tol=1e-9, max_iter=3, precond=2)
+    assert not ok3 and it3 == 3
+    x4, it4, _, _, ok4 = pcm.pcm_cg_solve(cp, b, x=xp.clone(), tol=1e-8, precond=2, use_x0=True)
+    assert ok4 and it4 == 0
+    for c in (cp, cr):
+        pcm.pcm_destroy(c)
+
+
+def test_cg_non_finite_right_hand_side_is_an_error(pcm, torch_cuda):
+    s, q, _ = synth.make_solver_points(300, seed=1004)
+    for path in (0, 1):
+        c = points_ctx(pcm, s, cg_path=path)
+        b = dev(torch_cuda, q)
+        b[5] = float("nan")
+        with pytest.raises(pcm.PcmError):
+            pcm.pcm_cg_solve(c, b, tol=1e-8, precond=1)
+        pcm.pcm_destroy(c)
