@@ -45,6 +45,7 @@ CONFIG_INDEX = 3
 RBJ_BLOCK = 64
 CG_TOL = 1e-8
 SWEEP_M = (10_000, 50_000, 100_000, 200_000)
+STORED_M = (2_500, 5_000, 10_000, 50_000)   # stored-A variant against the on-the-fly sweep
 SOLVER_M = (10_000, 50_000, 200_000)   # configs[4]: full pcm_cg_solve, RBJ-64 against Jacobi
 
 WORKLOADS = {
@@ -447,6 +448,53 @@ def amat_and_solver_sweep(pcm, torch, dev, flush, model, peak_tflops, with_solve
     return sweep, solver
 
 
+def stored_a_comparison(pcm, torch, dev, flush, hbm_gbs):
+    """the stored-A variant against the on-the-fly sweep, same persistent-kernel path, same
+    bits.  Stored, an A q streams 4 M^2 bytes of far-field 1/r values plus the stored near patches; `warm` = back-to-back calls
+    (what a CG iteration sees: L2-resident when it fits), `cold` = L2 flushed before the call."""
+    out = []
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    z, zi = np.zeros(0), np.zeros(0, np.int32)
+    for Ms in STORED_M:
+        s4, q4, _ = synth.make_solver_points(Ms)
+        qd = torch.as_tensor(q4, dtype=torch.float64, device=dev)
+        yd = torch.empty_like(qd)
+        rec = {"M": Ms}
+        for name, sf in (("stored", 1), ("on_the_fly", -1)):
+            c = pcm.pcm_setup(zi, np.zeros((0, 3)), zi, z, z, s4.xyz, s4.zeta, s4.switch, cg_path=2, store_far=sf)
+            info = pcm.pcm_get_info(c)
+            if not info.amat_persistent or (sf == 1 and info.amat_far_stored_bytes == 0):
+                rec[name] = None
+                pcm.pcm_destroy(c)
+                continue
+            pcm.pcm_set_timing(c, True)
+            cold, warm = [], []
+            for _ in range(3):
+                pcm.pcm_amatvec(c, qd, yd)
+            for _ in range(5):
+                flush.zero_()
+                pcm.pcm_amatvec(c, qd, yd)
+                cold.append(sum(pcm.pcm_last_kernel_ms(c, pcm.OP_AMATVEC)[:2]))
+            for _ in range(8):
+                pcm.pcm_amatvec(c, qd, yd)
+                warm.append(sum(pcm.pcm_last_kernel_ms(c, pcm.OP_AMATVEC)[:2]))
+            nbytes = float(info.amat_far_stored_bytes + info.amat_stored_bytes)
+            rec[name] = {"ms_cold": min(cold), "ms_warm": min(warm), "bytes_streamed": nbytes}
+            if sf == 1:
+                rec[name].update({"bound": "hbm", "achieved_gbs_cold": nbytes / (min(cold) * 1e-3) * 1e-9,
+                                  "frac_of_hbm_peak_cold": nbytes / (min(cold) * 1e-3) * 1e-9 / hbm_gbs,
+                                  "achieved_gbs_warm": nbytes / (min(warm) * 1e-3) * 1e-9})
+            pcm.pcm_destroy(c)
+        c = pcm.pcm_setup(zi, np.zeros((0, 3)), zi, z, z, s4.xyz, s4.zeta, s4.switch)
+        info = pcm.pcm_get_info(c)
+        rec["default_choice"] = ("stored" if info.amat_far_stored_bytes else "on_the_fly") + (" (persistent kernel)" if info.amat_persistent else " (separate launches)")
+        pcm.pcm_destroy(c)
+        out.append(rec)
+    return {"rule": "pcm_options.store_far = 0: the far field is stored when far + near bytes <= 96 MB (resident in the 126 MB L2), i.e. M <~ 4 500; "
+                    "above that the on-the-fly sweep is used (from HBM the stored form needs 4 M^2 B / 6.5 TB/s, no faster than the arithmetic)",
+            "cases": out}
+
+
 def run_ours(args):
     import torch
     import paper_1505_07851_b200 as pcm
@@ -684,6 +732,7 @@ def run_ours(args):
     # ---- A q sweep and the solver on configs[4] (BASELINE metric: A q FP64 fraction; HBM GB/s reported as asked)
     if not args.no_sweep:
         line["amatvec"], line["solver"] = amat_and_solver_sweep(pcm, torch, dev, flush, model, peak_tflops)
+        line["amatvec_stored"] = stored_a_comparison(pcm, torch, dev, flush, float(peaks.get("hbm_gbs", 6650.0)))
 
     # ---- the oracle on the host cores (reported baseline, not the target)
     if world == 1 and not args.no_cpu:

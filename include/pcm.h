@@ -63,7 +63,10 @@ typedef struct pcm_options {
                               A q below 20 000 points, separate kernel launches above; 1 = always separate launches (the
                               reference path); 2 = the persistent kernel at any size its buffers allow.  Same recurrences; the
                               two paths add the partial sums of A q in different (each fixed) orders */
-    int reserved[1];
+    int store_far;         /* the stored-A variant (PAPER.md:106 stores all of A) for the far field of the persistent path: 0 (default) =
+                              keep the far-field 1/r values too (4 M^2 bytes) when they and the stored near patches stay resident
+                              in L2 (<= 96 MB: about M <= 4 500); 1 = whenever device memory allows; -1 = never.  Same values,
+                              same summation order: the result does not depend on it */
 } pcm_options;
 
 typedef struct pcm_info {
@@ -86,6 +89,8 @@ typedef struct pcm_info {
     int64_t device_bytes;              /* device memory held by the context */
     int64_t amat_near_patches;         /* 32 x 32 patches of A that are not far field (evaluated with erf) */
     int64_t amat_stored_bytes;         /* bytes of those patches kept on the device (0: re-evaluated in every A q) */
+    int64_t amat_far_stored_bytes;     /* bytes of the stored far field (pcm_options.store_far; 0: evaluated on the fly) */
+    int64_t amat_persistent;           /* 1: pcm_cg_solve / pcm_amatvec use the persistent-kernel path (pcm_options.cg_path) */
 } pcm_info;
 
 /* Fills *opt with the defaults listed above. */

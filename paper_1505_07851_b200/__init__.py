@@ -38,7 +38,7 @@ EXPORTS = (
 
 class pcm_options(C.Structure):
     _fields_ = [("screen_eps", C.c_double), ("d_pure", C.c_int), ("device", C.c_int), ("merge_products", C.c_int),
-                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("reserved", C.c_int * 1)]
+                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("store_far", C.c_int)]
 
 
 class pcm_info(C.Structure):
@@ -49,7 +49,8 @@ class pcm_info(C.Structure):
                 ("prim_pair_points", C.c_double), ("product_points", C.c_double),
                 ("zeta_min", C.c_double), ("zeta_max", C.c_double),
                 ("rbj_block", C.c_int64), ("rbj_nblocks", C.c_int64), ("device_bytes", C.c_int64),
-                ("amat_near_patches", C.c_int64), ("amat_stored_bytes", C.c_int64)]
+                ("amat_near_patches", C.c_int64), ("amat_stored_bytes", C.c_int64), ("amat_far_stored_bytes", C.c_int64),
+                ("amat_persistent", C.c_int64)]
 
 
 class PcmError(RuntimeError):
@@ -197,7 +198,7 @@ def pcm_options_default() -> pcm_options:
 
 def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_zeta, pt_switch=None, *,
               screen_eps: float = 1e-12, d_pure: bool = True, device: int = -1, merge_products: bool = True,
-              gradient: bool = False, store_near: bool = True, cg_path: int = 0) -> Context:
+              gradient: bool = False, store_near: bool = True, cg_path: int = 0, store_far: int = 0) -> Context:
     """Host numpy arrays in, context out (include/pcm.h: pcm_setup)."""
     import torch
     if not torch.cuda.is_available():
@@ -225,6 +226,7 @@ def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_z
     opt.gradient = 1 if gradient else 0
     opt.store_near = 1 if store_near else 0
     opt.cg_path = int(cg_path)
+    opt.store_far = int(store_far)
     h = C.c_void_p()
     rc = lib().pcm_setup(C.byref(h), len(sl), _hp(sl), _hp(sx), _hp(sn), _hp(pe), _hp(pc), len(pz), _hp(px), _hp(pz),
                          _hp(ps), C.byref(opt))

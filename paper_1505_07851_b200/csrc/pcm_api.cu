@@ -149,6 +149,8 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     ctx->info.device_bytes = ctx->device_bytes;
     ctx->info.amat_near_patches = ctx->amat_map.nnear;
     ctx->info.amat_stored_bytes = ctx->amat_blocks ? ctx->amat_map.nnear * 32 * 32 * 8 : 0;
+    ctx->info.amat_far_stored_bytes = ctx->cgp.far_bytes;
+    ctx->info.amat_persistent = ctx->cgp.ready ? 1 : 0;
     *out = ctx;
     return PCM_OK;
 }

@@ -42,6 +42,7 @@ struct CgpArgs {
     const int64_t *seg_start;
     const int32_t *seg_slot0, *rb_slot_start;
     double *yslot, *colpart;
+    double *afar;              // stored far field: [half strip][16 columns][4 row groups][32 lanes] values of 1/r (0 where near), or nullptr
     // stored near patches (PatchMap of A): pieces of <= NEAR_PIECE patches of one row group
     const double *nblk;
     const int64_t *nstart, *npstart;
@@ -149,6 +150,9 @@ struct PSrc {
 // The warp's share of the sweep: its segment of far half-strips, with the stored near patches of its near pieces streamed
 // through shared memory underneath (one half patch per half strip, copied asynchronously while the previous half strip
 // computes), and the columns of the next strip prefetched the same way.
+// MODE 0: 1/r evaluated on the fly; MODE 1: evaluated and written to a.afar (pcm_setup, no sums needed); MODE 2: read from a.afar
+// (the stored-A variant of the paper, PAPER.md:106 -- same FMAs in the same order, so the result equals MODE 0 bit for bit).
+template <int MODE>
 __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int gw, int lane, double *wsm) {
     constexpr int R = CGP_R, C = CGP_C;
     const int M = a.M;
@@ -279,23 +283,37 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
         // (selected, not multiplied: a near patch may hold r = 0): three rows of wasted arithmetic at worst, but no slow
         // path whose cost the partition would have to know (near patches cluster at the start of a row block's strips).
         const bool full = m == (1u << R) - 1u;
+        double *ah = MODE ? a.afar + (size_t)h * (16 * R * 32) + lane : nullptr;
 #pragma unroll 1
         for (int t = 0; t < 16; t += C) {
             double4 b[C];
             double qb[C], r2[C][R], cc[C];
 #pragma unroll
             for (int c = 0; c < C; ++c) { b[c] = sp[t + c]; qb[c] = sq[t + c]; }
+            if (MODE == 2) {
 #pragma unroll
-            for (int c = 0; c < C; ++c)
+                for (int c = 0; c < C; ++c)
 #pragma unroll
-                for (int r = 0; r < R; ++r) r2[c][r] = fma(alx[r], b[c].x, fma(aly[r], b[c].y, fma(alz[r], b[c].z, a2[r] + b[c].w)));
+                    for (int r = 0; r < R; ++r) r2[c][r] = __ldg(ah + ((t + c) * R + r) * 32);     // the stored 1/r itself
+            } else {
+#pragma unroll
+                for (int c = 0; c < C; ++c)
+#pragma unroll
+                    for (int r = 0; r < R; ++r) r2[c][r] = fma(alx[r], b[c].x, fma(aly[r], b[c].y, fma(alz[r], b[c].z, a2[r] + b[c].w)));
+            }
 #pragma unroll
             for (int c = 0; c < C; ++c) {
                 cc[c] = 0.0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    double rs = rsqrt_fast(r2[c][r]);
-                    if (!full && !((m >> r) & 1u)) rs = 0.0;
+                    double rs;
+                    if (MODE == 2) {
+                        rs = r2[c][r];
+                    } else {
+                        rs = rsqrt_fast(r2[c][r]);
+                        if (!full && !((m >> r) & 1u)) rs = 0.0;
+                        if (MODE == 1) ah[((t + c) * R + r) * 32] = rs;
+                    }
                     y[r] = fma(qb[c], rs, y[r]);
                     cc[c] = fma(qa[r], rs, cc[c]);
                 }
@@ -467,6 +485,7 @@ __device__ __forceinline__ void cgp_update(const CgpArgs &a, const double *p, do
     }
 }
 
+template <int MODE>
 __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
     extern __shared__ double dyn[];
     __shared__ double s_w[CGP_WARPS];
@@ -491,7 +510,7 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
         cgp_stamp(a, iters, 0);
         unsigned long long t0 = 0;
         if (a.dbg && iters == 1 && tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
-        cgp_sweep(a, pv, gw, lane, wsm);
+        cgp_sweep<MODE>(a, pv, gw, lane, wsm);
         if (a.dbg && iters == 1) {
             __syncthreads();
             if (tid == 0) { unsigned long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); a.dbg[CGP_DBG_ITERS * 8 + blockIdx.x] = t1 - t0; }
@@ -542,12 +561,14 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
 }
 
 // y = A q with the same sweep and row sums: one launch, one grid barrier
+template <int MODE>
 __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_matvec_kernel(CgpArgs a) {
     extern __shared__ double dyn[];
     const unsigned G = gridDim.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     PSrc pv{a.q, nullptr, a.qidx, 0.0};
-    cgp_sweep(a, pv, blockIdx.x * CGP_WARPS + warp, lane, dyn + warp * CGP_WSMEM2);
+    cgp_sweep<MODE>(a, pv, blockIdx.x * CGP_WARPS + warp, lane, dyn + warp * CGP_WSMEM2);
+    if (MODE == 1) return;      // filling the store: the sums are not needed
     cgp_grid_sync(a.ctl, G);
     for (int g0 = blockIdx.x * CGP_TEAMS; g0 < a.ng; g0 += (int)G * CGP_TEAMS) {
         const int g = g0 + warp / CGP_TW;
@@ -571,6 +592,8 @@ static int upload2(pcm_ctx *ctx, T **dst, const std::vector<T> &src) {
     return PCM_OK;
 }
 
+static CgpArgs cgp_args(pcm_ctx *ctx);
+
 // Builds the warp-granular partition for contexts whose A q sweep is latency-dominated (M < AMAT_PERSIST_MAX) and whose
 // near patches are stored.  Leaves ctx->cgp.ready = false otherwise (the separate-launch path is used).
 int plan_sweep(pcm_ctx *ctx) {
@@ -584,9 +607,12 @@ int plan_sweep(pcm_ctx *ctx) {
     if (pm.far_host.empty()) return PCM_OK;
     int per_sm = 0;
     const size_t smem = (size_t)CGP_WARPS * CGP_WSMEM2 * 8;
-    if (cudaFuncSetAttribute(cgp_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(cgp_matvec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cgp_solve_kernel, CGP_THREADS, smem) != cudaSuccess || per_sm < 1) {
+    if (cudaFuncSetAttribute(cgp_solve_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(cgp_solve_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(cgp_matvec_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(cgp_matvec_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(cgp_matvec_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cgp_solve_kernel<0>, CGP_THREADS, smem) != cudaSuccess || per_sm < 1) {
         (void)cudaGetLastError();
         return PCM_OK;
     }
@@ -680,6 +706,33 @@ int plan_sweep(pcm_ctx *ctx) {
     PCM_CUDA(ctx, cudaMemset(sp.yslot, 0, (size_t)std::max<int32_t>(nslot, 1) * CGP_ROWS * 8));
     sp.smem = smem;
     sp.ready = true;
+    // The stored-A variant (PAPER.md:106 stores all of A): the far field kept as the sweep consumes it, 16 KB per half strip,
+    // M^2/2 values in all.  It replaces ~9 FP64 instructions and a MUFU per pair by an 8-byte load, i.e. it trades the FP64 pipe
+    // for memory bandwidth: from HBM that is a tie at best (4 M^2 bytes per product: 400 MB at M = 10k = 61 us at 6.5 TB/s
+    // against ~59 us of arithmetic), from L2 it wins.  Rule (store_far = 0): store when the far field and the stored near
+    // patches together stay resident in L2; store_far = 1 stores whenever memory allows (measurements), -1 never.
+    {
+        const double far_bytes = (double)nhalf * 16.0 * CGP_R * 32.0 * 8.0;
+        const double near_bytes = ctx->amat_blocks ? (double)pm.nnear * 1024.0 * 8.0 : 0.0;
+        double l2_budget = 96e6;           // of the 126 MB L2: the vectors, partial sums and inverse blocks need room too
+        if (const char *e = getenv("PCM_STORE_FAR_L2_MB")) l2_budget = atof(e) * 1e6;
+        size_t free_b = 0, total_b = 0;
+        cudaMemGetInfo(&free_b, &total_b);
+        const bool fits_mem = far_bytes < 0.5 * (double)free_b;
+        const bool want = ctx->opt.store_far == 1 ? fits_mem : (ctx->opt.store_far == 0 && far_bytes + near_bytes <= l2_budget && fits_mem);
+        sp.far_bytes = 0;
+        if (want && nhalf > 0) {
+            if ((rc = dev_alloc_t(ctx, &sp.afar, (size_t)nhalf * 16 * CGP_R * 32))) return rc;
+            CgpArgs a = cgp_args(ctx);
+            a.afar = sp.afar;
+            a.q = sp.pbuf; a.qidx = nullptr; a.y = nullptr;     // any finite vector: only the 1/r values are kept
+            PCM_CUDA(ctx, cudaMemset(sp.pbuf, 0, (size_t)M * 8));
+            void *args[] = {&a};
+            PCM_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)cgp_matvec_kernel<1>, dim3((unsigned)sp.grid), dim3(CGP_THREADS), args, smem, 0));
+            PCM_CUDA(ctx, cudaDeviceSynchronize());
+            sp.far_bytes = (int64_t)far_bytes;
+        }
+    }
     if (getenv("PCM_VERBOSE")) {
         double mx = 0.0;
         for (int w = 0; w < sp.nwarp; ++w) {
@@ -706,6 +759,7 @@ static CgpArgs cgp_args(pcm_ctx *ctx) {
     a.pt = ctx->pt; a.colloc = sp.colloc; a.org = sp.org;
     a.strip = sp.strip; a.seg_start = sp.seg_start; a.seg_slot0 = sp.seg_slot0; a.rb_slot_start = sp.rb_slot_start;
     a.yslot = sp.yslot; a.colpart = sp.colpart;
+    a.afar = sp.afar;
     a.nblk = ctx->amat_blocks; a.nstart = pm.start; a.npstart = pm.pstart; a.nlist = pm.list; a.npiece_rg = pm.piece_rg;
     a.npiece = pm.npiece; a.near = ctx->near_amat;
     if (const char *e = getenv("PCM_CGP_DEBUG")) { if (atoi(e) & 1) a.npiece = 0; }   // timing experiments only (wrong results)
@@ -720,7 +774,8 @@ int cgp_matvec(pcm_ctx *ctx, const double *q, const int32_t *idx, double *y, cud
     CgpArgs a = cgp_args(ctx);
     a.q = q; a.qidx = idx; a.y = y;
     void *args[] = {&a};
-    PCM_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)cgp_matvec_kernel, dim3((unsigned)ctx->cgp.grid), dim3(CGP_THREADS), args, ctx->cgp.smem, s));
+    const void *k = a.afar ? (const void *)cgp_matvec_kernel<2> : (const void *)cgp_matvec_kernel<0>;
+    PCM_CUDA(ctx, cudaLaunchCooperativeKernel(k, dim3((unsigned)ctx->cgp.grid), dim3(CGP_THREADS), args, ctx->cgp.smem, s));
     ctx->launch_total += 1;
     return PCM_OK;
 }
@@ -744,7 +799,8 @@ int cgp_solve(pcm_ctx *ctx, double *r, double *z, double *p, double *Ap, double 
         PCM_CUDA(ctx, cudaMemsetAsync(a.dbg, 0, (CGP_DBG_ITERS * 8 + 1024) * 8, s));
     }
     void *args[] = {&a};
-    PCM_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)cgp_solve_kernel, dim3((unsigned)ctx->cgp.grid), dim3(CGP_THREADS), args, smem, s));
+    const void *k = a.afar ? (const void *)cgp_solve_kernel<2> : (const void *)cgp_solve_kernel<0>;
+    PCM_CUDA(ctx, cudaLaunchCooperativeKernel(k, dim3((unsigned)ctx->cgp.grid), dim3(CGP_THREADS), args, smem, s));
     ctx->launch_total += 1;
     if (verbose) {   // CTA 0's view of the phases: sweep, wait, row sums, wait, update, wait (microseconds)
         unsigned long long h[CGP_DBG_ITERS * 8 + 1024];

@@ -83,6 +83,8 @@ struct SweepPlan {
     double *yslot = nullptr;          // [nslot][128] row sums of a (segment, row block) run
     double *colpart = nullptr;        // [nrb][M] column sums of a row block
     double *pbuf = nullptr;           // [M] second buffer of the CG direction
+    double *afar = nullptr;           // stored far field [2 nstrip][16][4][32] (nullptr: evaluated on the fly)
+    int64_t far_bytes = 0;
 };
 
 struct ClassData {        // products of one total angular momentum L, padded to a multiple of 128

@@ -243,3 +243,50 @@ def test_cg_non_finite_right_hand_side_is_an_error(pcm, torch_cuda):
         with pytest.raises(pcm.PcmError):
             pcm.pcm_cg_solve(c, b, tol=1e-8, precond=1)
         pcm.pcm_destroy(c)
+
+
+@pytest.mark.parametrize("M", [700, 3000])
+def test_stored_far_field_equals_the_on_the_fly_sweep(pcm, orc, torch_cuda, M):
+    """SURVEY.md 8(f) rank 3 ('A is explicitly stored'): pcm_options.store_far keeps the far-field 1/r values the
+    sweep would evaluate (on top of the stored near patches), and the sweep reads them back in the same order -- A q and the
+    solve are bit-identical to the on-the-fly path, and equal to the oracle.  The default stores when everything fits in L2."""
+    torch = torch_cuda
+    s, q, q_true = synth.make_solver_points(M, seed=1004)
+    c_store, c_fly, c_auto = points_ctx(pcm, s, store_far=1), points_ctx(pcm, s, store_far=-1), points_ctx(pcm, s)
+    i_store, i_fly, i_auto = (pcm.pcm_get_info(c) for c in (c_store, c_fly, c_auto))
+    assert i_store.amat_persistent == 1 and i_fly.amat_persistent == 1
+    assert i_fly.amat_far_stored_bytes == 0 and i_store.amat_far_stored_bytes > 0
+    assert i_auto.amat_far_stored_bytes == i_store.amat_far_stored_bytes          # a few MB: resident in L2, the rule stores
+    assert i_store.amat_far_stored_bytes + i_store.amat_stored_bytes >= 8 * (M * (M - 1) // 2)   # every pair is stored once at least
+    qd = dev(torch, q)
+    ys, yf = pcm.pcm_amatvec(c_store, qd).cpu().numpy(), pcm.pcm_amatvec(c_fly, qd).cpu().numpy()
+    assert np.array_equal(ys, yf)
+    ref = orc.amatvec(s, q)
+    assert np.all(np.abs(ys - ref) <= 1e-10 * np.abs(ref) + 1e-12)
+    e = np.zeros(M)
+    e[M // 3] = 1.0
+    col = pcm.pcm_amatvec(c_store, dev(torch, e)).cpu().numpy()
+    refc = np.array([orc.a_entry(s, i, M // 3) for i in range(M)])
+    assert np.all(np.abs(col - refc) <= 1e-10 * np.abs(refc) + 1e-12)            # single stored entries
+    b = dev(torch, orc.amatvec(s, q_true))
+    for c in (c_store, c_fly):
+        pcm.pcm_rbj_build(c, 64, seed=7)
+    for precond in (1, 2):
+        xs, its, rrs, _, oks = pcm.pcm_cg_solve(c_store, b, tol=1e-9, precond=precond)
+        xf, itf, rrf, _, okf = pcm.pcm_cg_solve(c_fly, b, tol=1e-9, precond=precond)
+        assert oks and okf and its == itf and rrs == rrf and torch.equal(xs, xf)
+    assert float((xs - dev(torch, q_true)).abs().max()) < 1e-7
+    for c in (c_store, c_fly, c_auto):
+        pcm.pcm_destroy(c)
+
+
+def test_store_far_rule_leaves_large_cavities_on_the_fly(pcm):
+    s, _, _ = synth.make_solver_points(9000, seed=1004)
+    c = points_ctx(pcm, s)
+    info = pcm.pcm_get_info(c)
+    assert info.amat_persistent == 1 and info.amat_far_stored_bytes == 0      # 4 M^2 = 324 MB does not stay in L2
+    pcm.pcm_destroy(c)
+    s, _, _ = synth.make_solver_points(30000, seed=1004)
+    c = points_ctx(pcm, s)
+    assert pcm.pcm_get_info(c).amat_persistent == 0                            # 20k points and more: separate launches
+    pcm.pcm_destroy(c)
