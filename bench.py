@@ -533,7 +533,7 @@ def run_ours(args):
     q = torch.zeros(M, dtype=torch.float64, device=dev)
     F = torch.empty((nbf, nbf), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
-    pcm.pcm_set_timing(ctx, True)
+    pcm.pcm_set_timing(ctx, False)      # the library's own per-kernel events serialise the class kernels: off in the timed region
     stream = torch.cuda.current_stream()
     side = torch.cuda.Stream(device=dev, priority=-1)   # the RBJ build depends on the geometry only: it overlaps pcm_potential
 
@@ -571,10 +571,6 @@ def run_ours(args):
         pcm.pcm_fock(ctx, q, F, stream=stream)
         ev[k][3].record(stream)
         ev[k][3].synchronize()
-        cls_pot.append(pcm.pcm_last_class_ms(ctx, pcm.OP_POTENTIAL))
-        cls_fock.append(pcm.pcm_last_class_ms(ctx, pcm.OP_FOCK))
-        main_ms.append((pcm.pcm_last_kernel_ms(ctx, pcm.OP_POTENTIAL), pcm.pcm_last_kernel_ms(ctx, pcm.OP_FOCK)))
-        cg_mv.append(pcm.pcm_last_cg_matvec_ms(ctx)[0])
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
     launches = pcm.pcm_launch_count(ctx) - launches0
@@ -590,6 +586,22 @@ def run_ours(args):
     ms_per_step = total_ms / args.steps
     value = job_value(world, units_per_step, ms_per_step)
     whole_ms = max_over_ranks(sum(step_ms), dist, dev) / args.steps
+
+    # ---- kernel breakdown (outside the timed region): the same calls with the library's per-kernel events on, which runs the class
+    # kernels one after the other -- the per-class times and roofline fractions come from here
+    pcm.pcm_set_timing(ctx, True)
+    for k in range(1 + 3):
+        flush.zero_()
+        pcm.pcm_potential(ctx, P, v, stream=stream)
+        flush.zero_()
+        pcm.pcm_fock(ctx, q, F, stream=stream)
+        torch.cuda.synchronize()
+        if k >= 1:
+            cls_pot.append(pcm.pcm_last_class_ms(ctx, pcm.OP_POTENTIAL))
+            cls_fock.append(pcm.pcm_last_class_ms(ctx, pcm.OP_FOCK))
+            main_ms.append((pcm.pcm_last_kernel_ms(ctx, pcm.OP_POTENTIAL), pcm.pcm_last_kernel_ms(ctx, pcm.OP_FOCK)))
+    pcm.pcm_cg_solve(ctx, v, q.clone(), tol=CG_TOL, max_iter=2000, precond=2, stream=stream)
+    cg_mv.append(pcm.pcm_last_cg_matvec_ms(ctx)[0])
 
     if rank != 0:
         if dist is not None:
@@ -619,13 +631,15 @@ def run_ours(args):
         "frac": 0.5 * float(M) * M * wa["flop"] / (mv_ms * 1e-3) * 1e-12 / peak_tflops if mv_ms > 0 else None}
     tpu = wk["traffic_per_unit"]
     roofline = {"bound": "alu", "kernel": f"{op}_kernel<L={Ld}> on {WORKLOADS[args.config].split(':')[0]}", "launches_per_step": 1,
-                "share_of_step": ms_dom / ms_per_step, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "share_of_step": min(1.0, ms_dom / ms_per_step), "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "peak_nominal": 148 * 64 * 2 * 1.965e-3, "frac_of_nominal": achieved / (148 * 64 * 2 * 1.965e-3),
                 "traffic": tpu * n_units if tpu is not None else None,
                 "traffic_source": (f"dram__bytes_read.sum + dram__bytes_write.sum per unit from {model['_source']['file']} x the units of this launch"
                                    if tpu is not None else "no ncu capture of this kernel under profiles/: null"),
                 "algorithmic_bytes": 40.0 * M + (32.0 + 8.0 * [1, 4, 10, 20, 35][Ld]) * float(info.products[Ld]),
                 "fp64_pipe_frac": n_units * wk["instr"] * 2.0 / (ms_dom * 1e-3) * 1e-12 / peak_tflops,
+                "timed": "launch duration from the library's CUDA events in the breakdown pass after the timed region (class kernels one after the "
+                         "other); in the timed region the five class kernels of a call run concurrently on five streams",
                 "units_per_launch": n_units, "flop_per_unit": wk["flop"], "fp64_instr_per_unit": wk["instr"], "work_source": wk["source"],
                 "work_capture": model.get("_source"), "ms_per_launch": ms_dom, "all_hot_kernels": kernels,
                 "peak_source": "measured live: pcm_fp64_peak DFMA chain (MEASURED_PEAKS.json has no fp64 entry; nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2)",

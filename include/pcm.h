@@ -67,6 +67,10 @@ typedef struct pcm_options {
                               keep the far-field 1/r values too (4 M^2 bytes) when they and the stored near patches stay resident
                               in L2 (<= 96 MB: about M <= 4 500); 1 = whenever device memory allows; -1 = never.  Same values,
                               same summation order: the result does not depend on it */
+    int serial_classes;    /* 1: pcm_potential / pcm_fock launch their per-class kernels one after the other on the caller's stream
+                              (as with pcm_set_timing on); 0 (default): concurrently on five internal streams joined back into
+                              it.  Same results */
+    int reserved[3];
 } pcm_options;
 
 typedef struct pcm_info {

@@ -38,7 +38,7 @@ EXPORTS = (
 
 class pcm_options(C.Structure):
     _fields_ = [("screen_eps", C.c_double), ("d_pure", C.c_int), ("device", C.c_int), ("merge_products", C.c_int),
-                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("store_far", C.c_int)]
+                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("store_far", C.c_int), ("serial_classes", C.c_int), ("reserved", C.c_int * 3)]
 
 
 class pcm_info(C.Structure):

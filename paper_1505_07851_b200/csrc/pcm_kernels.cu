@@ -610,7 +610,9 @@ template <int L>
 __host__ __device__ constexpr int pot_rec() { return (4 + nherm(L) + 1) / 2 * 2; }      // main kernel: centre, pad, D_h
 // potential_kernel's own record: for L = 3 four more slots (the first-order coefficients of the third-order block)
 template <int L>
-__host__ __device__ constexpr int pot_rec_main() { return pot_rec<L>() + (L == 3 ? 4 : 0); }
+__host__ __device__ constexpr int pot_rec_main() { return pot_rec<L>() + (L == 3 ? 4 : 0) + (L == 1 ? 2 : 0); }
+// L = 0, 1: the main kernel works in the local coordinates of its row block (pot_local_unit below)
+__host__ __device__ constexpr bool pot_local(int L) { return L <= 1; }
 template <int L>
 __host__ __device__ constexpr int pot_rec_near() { return (4 + nherm(L) + 2 + 1) / 2 * 2; }  // + (p, 1/kappa)
 
@@ -680,6 +682,28 @@ __device__ __forceinline__ void pot_far_unit<3>(const double *rec, const double4
     v = fma(ri, fma(u, e1, D[0]), v);
 }
 
+// L = 0, 1 in local coordinates, as the A q sweep: with o the first point of the CTA's row block, a = C - o (the point, in
+// registers with |a|^2) and the record staged as (-2 (P - o), |P - o|^2, D_h[, D_1 . (P - o)]),
+//   R^2 = |a|^2 + |P - o|^2 - 2 a . (P - o)                      1 DADD + 3 DFMA instead of 3 DADD + DMUL + 2 DFMA,
+//   D_1 . (P - C) = D_1 . (P - o) - D_1 . a                      3 DFMA instead of 3 DADD + DMUL + 2 DFMA (x, y, z are never formed):
+// 10 and 15 FP64 instructions per evaluation instead of 12 and 17.  The cancellation costs (|a| + |P - o|)^2 / R^2 ulps of R^2
+// (|a| <= the extent of the 512 points of a row block; a few tens of ulps for the closest far products, as in amatvec_kernel).
+template <int L>
+__device__ __forceinline__ void pot_local_unit(const double *rec, const double4 &a, double &v) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+    const double2 h23 = *reinterpret_cast<const double2 *>(rec + 2);
+    const double ri = rsqrt_fast(fma(a.x, h01.x, fma(a.y, h01.y, fma(a.z, h23.x, a.w + h23.y))));
+    if (L == 0) {
+        v = fma(rec[4], ri, v);
+    } else {
+        const double u = ri * ri;
+        const double ms = fma(rec[5], a.x, fma(rec[6], a.y, fma(rec[7], a.z, -rec[8])));     // -(D_1 . (P - C))
+        v = fma(ri, fma(u, ms, rec[4]), v);
+    }
+}
+
+// (forcing the old occupancy back with a minimum-blocks launch bound -- 64 / 72 instead of 72 / 80 registers -- measured slower
+// for L = 0 and no different for L = 1)
 template <int L, int R, int C>
 __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restrict__ prodA, const double *__restrict__ herm,
                                                         int64_t npad, int chunk_len, const double4 *__restrict__ pt, int M,
@@ -694,10 +718,16 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
     double4 c[R];
     int kk[R];
     double v[R];
+    double4 org = make_double4(0.0, 0.0, 0.0, 0.0);
+    if (pot_local(L)) org = pt[min((int)blockIdx.x * (TPB * R), M - 1)];      // origin of the row block's local coordinates
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         kk[r] = (int)(rg0 + r) * SUB + lane;
         c[r] = pt[min(kk[r], M - 1)];
+        if (pot_local(L)) {       // (a, |a|^2), a = C - o
+            c[r].x -= org.x; c[r].y -= org.y; c[r].z -= org.z;
+            c[r].w = fma(c[r].z, c[r].z, fma(c[r].y, c[r].y, c[r].x * c[r].x));
+        }
         v[r] = 0.0;
     }
     // products [pbeg, pend): pend <= npad, both multiples of 32 (the padding carries zero density)
@@ -709,11 +739,23 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
         for (int t = threadIdx.x; t < cnt; t += TPB) {
             const double4 a = prodA[base + t];
             double *r = s_rec + t * REC;
-            r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = 0.0;
+            if (pot_local(L)) {
+                const double x = a.x - org.x, y = a.y - org.y, z = a.z - org.z;
+                r[0] = -2.0 * x; r[1] = -2.0 * y; r[2] = -2.0 * z; r[3] = fma(z, z, fma(y, y, x * x));
+            } else {
+                r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = 0.0;
+            }
         }
         for (int t = threadIdx.x; t < cnt * NH; t += TPB) {
             const int h = t / cnt, i = t - h * cnt;  // consecutive threads read consecutive products of one component
             s_rec[i * REC + 4 + h] = herm[(size_t)h * npad + base + i];
+        }
+        if (L == 1) {             // pot_local_unit<1> wants D_1 . (P - o) behind the record
+            __syncthreads();
+            for (int t = threadIdx.x; t < cnt; t += TPB) {
+                double *r = s_rec + t * REC;
+                r[8] = -0.5 * fma(r[5], r[0], fma(r[6], r[1], r[7] * r[2]));
+            }
         }
         if (L == 2 || L == 3) {   // pot_far_unit<2>, <3> want the trace of the second-order block in the pad slot
             __syncthreads();
@@ -737,14 +779,20 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
 #pragma unroll
                     for (int cc = 0; cc < C; ++cc)
 #pragma unroll
-                        for (int r = 0; r < R; ++r) pot_far_unit<L>(sr + (t + cc) * REC, c[r], v[r]);
+                        for (int r = 0; r < R; ++r) {
+                            if (pot_local(L)) pot_local_unit<L>(sr + (t + cc) * REC, c[r], v[r]);
+                            else pot_far_unit<L>(sr + (t + cc) * REC, c[r], v[r]);
+                        }
                 }
             } else if (R > 1 && m) {
 #pragma unroll 1
                 for (int t = 0; t < SUB; ++t) {
 #pragma unroll
                     for (int r = 0; r < R; ++r)
-                        if ((m >> r) & 1u) pot_far_unit<L>(sr + t * REC, c[r], v[r]);
+                        if ((m >> r) & 1u) {
+                            if (pot_local(L)) pot_local_unit<L>(sr + t * REC, c[r], v[r]);
+                            else pot_far_unit<L>(sr + t * REC, c[r], v[r]);
+                        }
                 }
             }
         }
@@ -1172,11 +1220,24 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
         if ((rc = launch_fock_near<3>(ctx, q, ctx->near_stream))) return rc;
         if ((rc = launch_fock_near<4>(ctx, q, ctx->near_stream))) return rc;
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
-        if ((rc = launch_fock_class<0>(ctx, q, s)) || (rc = mark(ctx, 2, s))) return rc;
-        if ((rc = launch_fock_class<1>(ctx, q, s)) || (rc = mark(ctx, 3, s))) return rc;
-        if ((rc = launch_fock_class<2>(ctx, q, s)) || (rc = mark(ctx, 4, s))) return rc;
-        if ((rc = launch_fock_class<3>(ctx, q, s)) || (rc = mark(ctx, 5, s))) return rc;
-        if ((rc = launch_fock_class<4>(ctx, q, s)) || (rc = mark(ctx, 6, s))) return rc;
+        if (ctx->timing || ctx->opt.serial_classes) {
+            if ((rc = launch_fock_class<0>(ctx, q, s)) || (rc = mark(ctx, 2, s))) return rc;
+            if ((rc = launch_fock_class<1>(ctx, q, s)) || (rc = mark(ctx, 3, s))) return rc;
+            if ((rc = launch_fock_class<2>(ctx, q, s)) || (rc = mark(ctx, 4, s))) return rc;
+            if ((rc = launch_fock_class<3>(ctx, q, s)) || (rc = mark(ctx, 5, s))) return rc;
+            if ((rc = launch_fock_class<4>(ctx, q, s)) || (rc = mark(ctx, 6, s))) return rc;
+        } else {   // concurrent class kernels, as in launch_potential
+            for (int L = 0; L <= MAXL; ++L) PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->cls_stream[L], ctx->ev_fork, 0));
+            if ((rc = launch_fock_class<1>(ctx, q, ctx->cls_stream[1]))) return rc;
+            if ((rc = launch_fock_class<2>(ctx, q, ctx->cls_stream[2]))) return rc;
+            if ((rc = launch_fock_class<0>(ctx, q, ctx->cls_stream[0]))) return rc;
+            if ((rc = launch_fock_class<3>(ctx, q, ctx->cls_stream[3]))) return rc;
+            if ((rc = launch_fock_class<4>(ctx, q, ctx->cls_stream[4]))) return rc;
+            for (int L = 0; L <= MAXL; ++L) {
+                PCM_CUDA(ctx, cudaEventRecord(ctx->ev_cls[L], ctx->cls_stream[L]));
+                PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_cls[L], 0));
+            }
+        }
         PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
     } else {
         for (int i = 2; i <= 6; ++i)
@@ -1231,8 +1292,9 @@ static int launch_potential_near(pcm_ctx *ctx, cudaStream_t s) {
     return PCM_OK;
 }
 
+// slot: first partial-sum slot of the class (fixed by the class order, whatever the launch order)
 template <int L>
-static int launch_potential_class(pcm_ctx *ctx, int64_t &slot, cudaStream_t s) {
+static int launch_potential_class(pcm_ctx *ctx, int64_t slot, cudaStream_t s) {
     constexpr Blocking pb = pot_blocking(L);
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
@@ -1242,7 +1304,6 @@ static int launch_potential_class(pcm_ctx *ctx, int64_t &slot, cudaStream_t s) {
     potential_kernel<L, pb.R, pb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
                                                          ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);
-    slot += pl.chunks;
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
 }
@@ -1269,12 +1330,29 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
     if ((rc = launch_potential_near<3>(ctx, ctx->near_stream))) return rc;
     if ((rc = launch_potential_near<4>(ctx, ctx->near_stream))) return rc;
     PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
-    int64_t slot = 0;
-    if ((rc = launch_potential_class<0>(ctx, slot, s)) || (rc = mark(ctx, 2, s))) return rc;
-    if ((rc = launch_potential_class<1>(ctx, slot, s)) || (rc = mark(ctx, 3, s))) return rc;
-    if ((rc = launch_potential_class<2>(ctx, slot, s)) || (rc = mark(ctx, 4, s))) return rc;
-    if ((rc = launch_potential_class<3>(ctx, slot, s)) || (rc = mark(ctx, 5, s))) return rc;
-    if ((rc = launch_potential_class<4>(ctx, slot, s)) || (rc = mark(ctx, 6, s))) return rc;
+    int64_t base[MAXL + 2] = {0};
+    for (int L = 0; L <= MAXL; ++L) base[L + 1] = base[L] + (ctx->cls[L].n > 0 ? ctx->plan_pot[L].chunks : 0);
+    const int64_t slot = base[MAXL + 1];
+    if (ctx->timing || ctx->opt.serial_classes) {   // per-class events: the class kernels run one after the other on s
+        if ((rc = launch_potential_class<0>(ctx, base[0], s)) || (rc = mark(ctx, 2, s))) return rc;
+        if ((rc = launch_potential_class<1>(ctx, base[1], s)) || (rc = mark(ctx, 3, s))) return rc;
+        if ((rc = launch_potential_class<2>(ctx, base[2], s)) || (rc = mark(ctx, 4, s))) return rc;
+        if ((rc = launch_potential_class<3>(ctx, base[3], s)) || (rc = mark(ctx, 5, s))) return rc;
+        if ((rc = launch_potential_class<4>(ctx, base[4], s)) || (rc = mark(ctx, 6, s))) return rc;
+    } else {
+        // the five class kernels on five streams: the tail of one class overlaps the body of the next (each launch is only a few
+        // waves: PAPER.md:160 launches its per-class kernels sequentially); the longest-running classes are queued first
+        for (int L = 0; L <= MAXL; ++L) PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->cls_stream[L], ctx->ev_fork, 0));
+        if ((rc = launch_potential_class<1>(ctx, base[1], ctx->cls_stream[1]))) return rc;
+        if ((rc = launch_potential_class<2>(ctx, base[2], ctx->cls_stream[2]))) return rc;
+        if ((rc = launch_potential_class<0>(ctx, base[0], ctx->cls_stream[0]))) return rc;
+        if ((rc = launch_potential_class<3>(ctx, base[3], ctx->cls_stream[3]))) return rc;
+        if ((rc = launch_potential_class<4>(ctx, base[4], ctx->cls_stream[4]))) return rc;
+        for (int L = 0; L <= MAXL; ++L) {
+            PCM_CUDA(ctx, cudaEventRecord(ctx->ev_cls[L], ctx->cls_stream[L]));
+            PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_cls[L], 0));
+        }
+    }
     PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
     if (slot == 0) {
         PCM_CUDA(ctx, cudaMemsetAsync(v, 0, (size_t)ctx->M * 8, s));
