@@ -70,7 +70,10 @@ typedef struct pcm_options {
     int serial_classes;    /* 1: pcm_potential / pcm_fock launch their per-class kernels one after the other on the caller's stream
                               (as with pcm_set_timing on); 0 (default): concurrently on five internal streams joined back into
                               it.  Same results */
-    int reserved[3];
+    int tma_tiles;         /* 1: pcm_fock brings its surface-point tiles into shared memory with TMA bulk copies (cp.async.bulk +
+                              mbarrier, double-buffered) from a per-call packed (x, y, z, q) array instead of per-thread loads;
+                              0 (default).  Same results bit for bit */
+    int reserved[2];
 } pcm_options;
 
 typedef struct pcm_info {

@@ -139,6 +139,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
         ctx->vpart_slots += (c.n > 0) ? ctx->plan_pot[L].chunks : 0;
     }
     ctx->ypart_slots = ctx->plan_amat.chunks;
+    if (ctx->opt.tma_tiles && (rc = dev_alloc_t(ctx, &ctx->ptq, (size_t)std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->near_amat, (size_t)ctx->amat_map.npiece * 32))) return fail(rc);
     if ((rc = fill_amat_blocks(ctx))) return fail(rc);
     if ((rc = plan_sweep(ctx))) return fail(rc);

@@ -125,6 +125,7 @@ struct pcm_ctx {
     // points, stored in Morton order ("sorted index" s); the caller's index of sorted point s is s2c[s].
     // Vectors crossing the C ABI (v, q, y, b, x) are in the caller's order; the kernels gather/scatter through s2c.
     double4 *pt = nullptr;      // (x, y, z, 1/zeta^2)
+    double4 *ptq = nullptr;     // (x, y, z, q_k) in sorted order, packed per pcm_fock call (pcm_options.tma_tiles)
     double *pt_diag = nullptr;  // A_kk = zeta_k sqrt(2/pi)/S_k
     double *pt_boxes = nullptr; // [ceil(M/32)][6] bounding boxes of the groups of 32 sorted points
     pcm::PatchMap amat_map;     // rows and columns = groups of 32 sorted points

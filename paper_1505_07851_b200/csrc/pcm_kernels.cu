@@ -19,6 +19,10 @@ namespace pcm {
 
 constexpr int TPB = 128;   // threads per block of the hot kernels ("1 x 128", still a good size)
 constexpr int SUB = 32;    // rows / columns per classified group
+// Below this many (product, point) evaluations per call the class kernels run one after the other: the fork / join of five
+// streams costs ~20 us, more than the tails it hides (measured: configs[1] 0.876 -> 0.896 ms, configs[2] 7.99 -> 8.02 ms with
+// the streams, configs[3] 86.6 -> 85.6 ms).
+constexpr double CONCURRENT_CLASSES_MIN = 2e10;
 constexpr int PT_TILE = 256;  // surface points staged per shared-memory tile (Fock, A q): 8 groups = one byte of the far map
 
 // ---------------------------------------------------------------------------------------------
@@ -498,6 +502,115 @@ __global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ p
                 }
             }
         }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t ip = (rg0 + r) * SUB + lane;
+        if (ip < npad) {
+            double *out = herm + (size_t)blockIdx.y * NH * npad + ip;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) out[(size_t)h * npad] = sink[r].acc[h];
+        }
+    }
+}
+
+// ---- the same sweep with the point tiles brought in by the TMA unit (cp.async.bulk, 1-D) --------------------------------
+// north_star: "surface-point tiles staged in shared memory (TMA where tiles are regular)".  The tiles become regular once
+// the charges are gathered into the library's sorted point order and packed with the coordinates, ptq[k] = (x, y, z, q_k)
+// (pack_points_kernel, M x 32 B per call): a tile is then 256 x 32 B = 8 KB of contiguous memory.  One elected thread issues
+// the bulk copy of tile i + 1 into the other buffer while the CTA computes on tile i; completion is an mbarrier transaction
+// count, so the two __syncthreads() per tile of fock_kernel become one (the buffer hand-back) plus the mbarrier wait.
+// Selected by pcm_options.tma_tiles (measured against fock_kernel: DESIGN.md "Tried").
+__global__ void pack_points_kernel(const double4 *__restrict__ pt, const double *__restrict__ q, const int32_t *__restrict__ qidx, int M,
+                                   double4 *__restrict__ ptq) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= M) return;
+    const double4 p = pt[k];
+    ptq[k] = make_double4(p.x, p.y, p.z, q[qidx ? qidx[k] : k]);
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
+    const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(dst)),
+                 "l"(src), "r"(bytes), "r"(b)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned done = 0;
+    while (!done) {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done) : "r"(b), "r"(parity) : "memory");
+    }
+}
+
+template <int L, int R, int C>
+__global__ void __launch_bounds__(TPB) fock_tma_kernel(const double4 *__restrict__ prodA, int64_t npad, const double4 *__restrict__ ptq, int M,
+                                                       int chunk_len, double *__restrict__ herm, const uint8_t *__restrict__ farmap,
+                                                       int64_t nbyte, int64_t nrg) {
+    constexpr int NH = nherm(L);
+    constexpr int NS = PT_TILE / SUB;
+    __shared__ __align__(128) double4 s_pt[2][PT_TILE];  // x, y, z, q
+    __shared__ __align__(8) uint64_t s_bar[2];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
+    double4 A[R];
+    FockSink<L> sink[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        A[r] = prodA[min((rg0 + r) * SUB + lane, npad - 1)];
+#pragma unroll
+        for (int h = 0; h < NH; ++h) sink[r].acc[h] = 0.0;
+    }
+    const int kbeg = blockIdx.y * chunk_len, kend = min(M, kbeg + chunk_len);
+    if (threadIdx.x == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && kbeg < kend) tma_load_1d(s_pt[0], ptq + kbeg, (unsigned)min(PT_TILE, kend - kbeg) * 32u, &s_bar[0]);
+    int it = 0;
+    for (int base = kbeg; base < kend; base += PT_TILE, ++it) {
+        const int buf = it & 1;
+        const int cnt = min(PT_TILE, kend - base), nst = (cnt + SUB - 1) / SUB;
+        const unsigned bits = far_bits<R, NS>(farmap, nbyte, rg0, nrg, base / SUB, lane);
+        // the next tile into the other buffer (every thread left it at the __syncthreads() that closed the previous tile)
+        if (threadIdx.x == 0 && base + PT_TILE < kend)
+            tma_load_1d(s_pt[buf ^ 1], ptq + base + PT_TILE, (unsigned)min(PT_TILE, kend - base - PT_TILE) * 32u, &s_bar[buf ^ 1]);
+        mbar_wait(&s_bar[buf], (unsigned)(it >> 1) & 1u);
+        if (cnt < nst * SUB) {     // ragged last group: padding points far from everything, zero charge
+            for (int t = cnt + threadIdx.x; t < nst * SUB; t += TPB) s_pt[buf][t] = make_double4(3e8, 3e8, 3e8, 0.0);
+            __syncthreads();
+        }
+        for (int st = 0; st < nst; ++st) {
+            const double4 *sp = s_pt[buf] + st * SUB;
+            const unsigned m = row_mask<R>(bits, st);
+            if (m == (1u << R) - 1u) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; t += C) {
+#pragma unroll
+                    for (int c = 0; c < C; ++c) {
+                        const double4 pc = sp[t + c];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) fock_far_unit<L>(A[r], pc, sink[r]);
+                    }
+                }
+            } else if (R > 1 && m) {
+#pragma unroll 1
+                for (int t = 0; t < SUB; ++t) {
+                    const double4 pc = sp[t];
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+                        if ((m >> r) & 1u) fock_far_unit<L>(A[r], pc, sink[r]);
+                }
+            }
+        }
+        __syncthreads();           // this buffer may be refilled from now on
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -1183,8 +1296,12 @@ static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s) {
     const Plan &pl = ctx->plan_fock[L];
     const PatchMap &pm = c.fock_map;
     dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
-    fock_kernel<L, fb.R, fb.C><<<grid, TPB, 0, s>>>(c.prodA, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, (int)pl.chunk_len, c.herm,
-                                                    pm.far, pm.nbyte, pm.nrg);
+    if (ctx->opt.tma_tiles && ctx->ptq)
+        fock_tma_kernel<L, fb.R, fb.C><<<grid, TPB, 0, s>>>(c.prodA, c.npad, ctx->ptq, (int)ctx->M, (int)pl.chunk_len, c.herm, pm.far, pm.nbyte,
+                                                            pm.nrg);
+    else
+        fock_kernel<L, fb.R, fb.C><<<grid, TPB, 0, s>>>(c.prodA, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, (int)pl.chunk_len, c.herm,
+                                                        pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
@@ -1211,6 +1328,11 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
     if ((rc = mark(ctx, 0, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
     if (ctx->M > 0) {
+        if (ctx->opt.tma_tiles && ctx->ptq) {   // (x, y, z, q) in sorted order: the regular tiles the bulk copies want
+            pack_points_kernel<<<(unsigned)ceil_div(ctx->M, 256), 256, 0, s>>>(ctx->pt, q, ctx->s2c, (int)ctx->M, ctx->ptq);
+            PCM_LAUNCH_CHECK(ctx);
+            { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+        }
         // near kernels of all classes on the near stream, concurrently with the main kernels on s
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
         PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->near_stream, ctx->ev_fork, 0));
@@ -1220,7 +1342,7 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
         if ((rc = launch_fock_near<3>(ctx, q, ctx->near_stream))) return rc;
         if ((rc = launch_fock_near<4>(ctx, q, ctx->near_stream))) return rc;
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
-        if (ctx->timing || ctx->opt.serial_classes) {
+        if (ctx->timing || ctx->opt.serial_classes || ctx->info.product_points < CONCURRENT_CLASSES_MIN) {
             if ((rc = launch_fock_class<0>(ctx, q, s)) || (rc = mark(ctx, 2, s))) return rc;
             if ((rc = launch_fock_class<1>(ctx, q, s)) || (rc = mark(ctx, 3, s))) return rc;
             if ((rc = launch_fock_class<2>(ctx, q, s)) || (rc = mark(ctx, 4, s))) return rc;
@@ -1333,7 +1455,7 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
     int64_t base[MAXL + 2] = {0};
     for (int L = 0; L <= MAXL; ++L) base[L + 1] = base[L] + (ctx->cls[L].n > 0 ? ctx->plan_pot[L].chunks : 0);
     const int64_t slot = base[MAXL + 1];
-    if (ctx->timing || ctx->opt.serial_classes) {   // per-class events: the class kernels run one after the other on s
+    if (ctx->timing || ctx->opt.serial_classes || ctx->info.product_points < CONCURRENT_CLASSES_MIN) {   // per-class events: the class kernels run one after the other on s
         if ((rc = launch_potential_class<0>(ctx, base[0], s)) || (rc = mark(ctx, 2, s))) return rc;
         if ((rc = launch_potential_class<1>(ctx, base[1], s)) || (rc = mark(ctx, 3, s))) return rc;
         if ((rc = launch_potential_class<2>(ctx, base[2], s)) || (rc = mark(ctx, 4, s))) return rc;

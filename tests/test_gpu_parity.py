@@ -286,3 +286,25 @@ def test_amatvec_coincident_and_mixed_exponents(pcm, orc, torch_cuda):
     ctx2 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0), s.xyz, s.zeta, s.switch,
                          store_near=False)
     np.testing.assert_array_equal(pcm.pcm_amatvec(ctx2, dev(torch_cuda, q)).cpu().numpy(), y)
+
+
+def test_fock_tma_tiles_and_serial_classes_give_the_same_bits(pcm, orc, torch_cuda):
+    """pcm_options.tma_tiles (point tiles brought in by cp.async.bulk + mbarrier from a packed (x, y, z, q) array) and
+    pcm_options.serial_classes (class kernels one after the other instead of on five streams) change how the work is moved and
+    scheduled, not what is computed: F and v are bit-identical to the default path, ragged tiles included."""
+    torch = torch_cuda
+    for cfg, kw in ((0, dict(with_d=True)), (1, dict(n_atoms=40))):
+        w = synth.make_workload(cfg, **kw)
+        b, s = w.basis, w.surface
+        qd, Pd = dev(torch, w.q), dev(torch, w.P)
+        ref = pcm.setup_from_workload(b, s)
+        F0, v0 = pcm.pcm_fock(ref, qd).cpu().numpy(), pcm.pcm_potential(ref, Pd).cpu().numpy()
+        assert_parity(v0[:64], orc.potential(b, s, w.P, points=np.arange(64)), "v")
+        for opts in (dict(tma_tiles=True), dict(serial_classes=True), dict(tma_tiles=True, serial_classes=True)):
+            c = pcm.setup_from_workload(b, s, **opts)
+            assert np.array_equal(pcm.pcm_fock(c, qd).cpu().numpy(), F0), opts
+            assert np.array_equal(pcm.pcm_potential(c, Pd).cpu().numpy(), v0), opts
+            pcm.pcm_set_timing(c, True)
+            assert np.array_equal(pcm.pcm_fock(c, qd).cpu().numpy(), F0), opts
+            pcm.pcm_destroy(c)
+        pcm.pcm_destroy(ref)
