@@ -24,7 +24,8 @@
  *   - the context owns COPIES of everything given to pcm_setup; the caller owns P, q, b, v, F, y, x.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Hot calls
  *     are asynchronous with respect to the host unless stated otherwise.
- *   - a context must not be used from two host threads at once (it owns scratch buffers).
+ *   - a context must not be used from two host threads at once, and calls on one context must be stream-ordered (it owns
+ *     scratch buffers, internal streams and events); the one exception is pcm_rbj_build_async, made to overlap another call.
  *   - there is no CPU fallback: every call fails with PCM_ERR_CUDA if the device is unusable.
  */
 #ifndef PCM_B200_H
@@ -61,8 +62,10 @@ typedef struct pcm_options {
                               that, or with 0, they are re-evaluated in every pcm_amatvec).  Same values either way. */
     int cg_path;           /* pcm_cg_solve / pcm_amatvec: 0 (default) = one persistent cooperative kernel per solve and one launch per
                               A q below 20 000 points, separate kernel launches above; 1 = always separate launches (the
-                              reference path); 2 = the persistent kernel at any size its buffers allow.  Same recurrences; the
-                              two paths add the partial sums of A q in different (each fixed) orders */
+                              reference path); 2 = the persistent kernel at any size its buffers allow; 3 = separate launches with
+                              every CG vector operation in a kernel of its own (no fused update kernel: the bit-exactness
+                              reference of path 1).  Same recurrences; paths 0/2 and 1/3 add the partial sums of A q in different
+                              (each fixed) orders */
     int store_far;         /* the stored-A variant (PAPER.md:106 stores all of A) for the far field of the persistent path: 0 (default) =
                               keep the far-field 1/r values too (4 M^2 bytes) when they and the stored near patches stay resident
                               in L2 (<= 96 MB: about M <= 4 500); 1 = whenever device memory allows; -1 = never.  Same values,
@@ -73,7 +76,9 @@ typedef struct pcm_options {
     int tma_tiles;         /* 1: pcm_fock brings its surface-point tiles into shared memory with TMA bulk copies (cp.async.bulk +
                               mbarrier, double-buffered) from a per-call packed (x, y, z, q) array instead of per-thread loads;
                               0 (default).  Same results bit for bit */
-    int reserved[2];
+    int rbj_global_scan;   /* 1: pcm_rbj_build selects every block with the cooperative global row scan instead of the one-CTA
+                              neighbourhood search (same blocks; the default uses the scan only above 150 000 points or l > 256) */
+    int reserved[1];
 } pcm_options;
 
 typedef struct pcm_info {
@@ -187,7 +192,12 @@ int pcm_rbj_get(pcm_ctx *ctx, int64_t *order_host, int64_t *bstart_host, double 
  * tol is the absolute Euclidean norm of the recurrence residual (the paper's delta).
  * iters (HOST, may be NULL): matrix-vector products after the initial residual.
  * resid (HOST, may be NULL): resid[0] = final recurrence ||r||, resid[1] = true ||b - A x|| recomputed at exit.
- * Synchronous: reads the residual norm back every iteration.  Returns PCM_OK or PCM_NOT_CONVERGED.
+ * Synchronous.  Below 20 000 points the iterations run inside one persistent kernel and the host reads the outcome once;
+ * above, iterations are queued eight at a time between read-backs of the device-side convergence flag.  Returns PCM_OK,
+ * PCM_NOT_CONVERGED, or PCM_ERR_NUMERIC when the residual is not finite (non-finite b, p.Ap = 0).
+ * SURVEY.md 8(b) proposed `block` and `seed` as arguments of this call: they are arguments of pcm_rbj_build[_async], because
+ * the preconditioner depends on the geometry only and is built once for many solves; precond = 2 uses the last build and
+ * fails with PCM_ERR_STATE if there is none.
  */
 int pcm_cg_solve(pcm_ctx *ctx, const double *b_dev, double *x_dev, double tol, int max_iter, int precond, int use_x0,
                  int *iters, double *resid, void *stream);

@@ -102,9 +102,9 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
         int prio_lo = 0, prio_hi = 0;
         cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
         // low priority: the near kernels (branchy, ~40 % of the FP64 pipe) then fill the tails of the main kernels instead
-        // of displacing them (measured 2-3 % on pcm_potential / pcm_fock; PCM_NEAR_PRIO=1 restores high priority)
-        const char *pe = getenv("PCM_NEAR_PRIO");
-        e = cudaStreamCreateWithPriority(&ctx->near_stream, cudaStreamNonBlocking, (pe && atoi(pe) == 1) ? prio_hi : prio_lo);
+        // of displacing them (measured 2-3 % on pcm_potential / pcm_fock against a high-priority stream)
+        (void)prio_hi;
+        e = cudaStreamCreateWithPriority(&ctx->near_stream, cudaStreamNonBlocking, prio_lo);
     }
     for (int L = 0; L <= MAXL && e == cudaSuccess; ++L) {
         e = cudaStreamCreateWithFlags(&ctx->cls_stream[L], cudaStreamNonBlocking);

@@ -601,7 +601,7 @@ int plan_sweep(pcm_ctx *ctx) {
     sp.ready = false;
     const int64_t M = ctx->M;
     const PatchMap &pm = ctx->amat_map;
-    if (M == 0 || ctx->opt.cg_path == 1) return PCM_OK;
+    if (M == 0 || ctx->opt.cg_path == 1 || ctx->opt.cg_path == 3) return PCM_OK;
     if (ctx->opt.cg_path == 0 && M >= AMAT_PERSIST_MAX) return PCM_OK;
     if (pm.npiece > 0 && ctx->amat_blocks == nullptr) return PCM_OK;      // near patches not stored: classic path
     if (pm.far_host.empty()) return PCM_OK;
@@ -624,7 +624,6 @@ int plan_sweep(pcm_ctx *ctx) {
     const int64_t ng = pm.nrg, nrb = cdiv2(ng, CGP_R), nbyte = pm.nbyte;
     sp.ng = (int)ng; sp.nrb = (int)nrb;
     // strips with at least one far patch
-    const bool dbg_full = getenv("PCM_CGP_DEBUG") && (atoi(getenv("PCM_CGP_DEBUG")) & 2);   // timing experiments only (wrong results)
     std::vector<int2> strip;
     std::vector<float> cost;
     for (int64_t rb = 0; rb < nrb; ++rb)
@@ -635,13 +634,11 @@ int plan_sweep(pcm_ctx *ctx) {
                 if (rg < ng && ((pm.far_host[(size_t)rg * nbyte + cg / 8] >> (cg & 7)) & 1)) m |= 1u << r;
             }
             if (!m) continue;
-            if (dbg_full) m = 15;
             strip.push_back(make_int2((int)rb, (int)(cg | ((int64_t)m << 24))));
             cost.push_back((float)CGP_R);      // a strip costs its 4 patches whatever the mask (the near rows are computed and discarded)
         }
     // near pieces go round-robin to the warps (piece q to warp q mod nwarp), before the far segment; their cost shortens it
-    double near_cost = 0.3;
-    if (const char *e = getenv("PCM_CGP_NEAR_COST")) near_cost = atof(e);
+    const double near_cost = 0.3;    // a stored near patch against a far patch, in warp time (0.6 and 1.0 measured no different)
     std::vector<double> wnear((size_t)sp.nwarp, 0.0);
     for (int64_t q = 0; q < pm.npiece; ++q) {
         const int64_t rg = pm.piece_rg_host[q];
@@ -714,8 +711,7 @@ int plan_sweep(pcm_ctx *ctx) {
     {
         const double far_bytes = (double)nhalf * 16.0 * CGP_R * 32.0 * 8.0;
         const double near_bytes = ctx->amat_blocks ? (double)pm.nnear * 1024.0 * 8.0 : 0.0;
-        double l2_budget = 96e6;           // of the 126 MB L2: the vectors, partial sums and inverse blocks need room too
-        if (const char *e = getenv("PCM_STORE_FAR_L2_MB")) l2_budget = atof(e) * 1e6;
+        const double l2_budget = 96e6;     // of the 126 MB L2: the vectors, partial sums and inverse blocks need room too
         size_t free_b = 0, total_b = 0;
         cudaMemGetInfo(&free_b, &total_b);
         const bool fits_mem = far_bytes < 0.5 * (double)free_b;
@@ -762,7 +758,6 @@ static CgpArgs cgp_args(pcm_ctx *ctx) {
     a.afar = sp.afar;
     a.nblk = ctx->amat_blocks; a.nstart = pm.start; a.npstart = pm.pstart; a.nlist = pm.list; a.npiece_rg = pm.piece_rg;
     a.npiece = pm.npiece; a.near = ctx->near_amat;
-    if (const char *e = getenv("PCM_CGP_DEBUG")) { if (atoi(e) & 1) a.npiece = 0; }   // timing experiments only (wrong results)
     a.diag = ctx->pt_diag;
     a.scal = ctx->cg_scal;
     a.ctl = reinterpret_cast<int *>(ctx->cg_scal + 8);

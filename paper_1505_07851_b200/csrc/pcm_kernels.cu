@@ -1142,8 +1142,7 @@ template <int L>
 static void plan_class(pcm_ctx *ctx) {
     constexpr Blocking fb = fock_blocking(L), pb = pot_blocking(L);
     const ClassData &c = ctx->cls[L];
-    double iw = 4.0;
-    if (const char *e = getenv("PCM_INT_WAVES")) iw = atof(e);
+    const double iw = 4.0;   // wave target of the work partition (more waves measured no different on configs[1])
     ctx->plan_fock[L] = make_plan(c.npad, TPB * fb.R, ctx->M, PT_TILE, wave_of(ctx, fock_kernel<L, fb.R, fb.C>), 1.0, iw);
     ctx->plan_pot[L] = make_plan(ctx->M, TPB * pb.R, c.npad, pot_tile(L), wave_of(ctx, potential_kernel<L, pb.R, pb.C>), 1.0, iw);
 }
@@ -1151,14 +1150,10 @@ static void plan_class(pcm_ctx *ctx) {
 int plan_all(pcm_ctx *ctx) {
     // symmetric sweep: about half of the (row block, chunk) grid has work.  From AMAT_R4_MIN points on: row blocks of 512
     // (R = 4) and column tiles of 256; below: row blocks of 256 (R = 2) and tiles of 64, i.e. 16 times as many, smaller
-    // work items, so that a 9k-point sweep still loads 148 SMs evenly.  PCM_AMAT_R / PCM_AMAT_TILE override (experiments).
+    // work items, so that a 9k-point sweep still loads 148 SMs evenly (R = 1 / tile 128 and R = 2 / tile 32 or 128 measured slower).
     ctx->amat_R = ctx->M >= AMAT_R4_MIN ? 4 : 2;
     ctx->amat_tile = ctx->amat_R == 4 ? 256 : 64;
-    if (const char *e = getenv("PCM_AMAT_R")) { const int r = atoi(e); if (r == 2 || r == 4) ctx->amat_R = r; }
-    if (const char *e = getenv("PCM_AMAT_TILE")) { const int t = atoi(e); if (t == 64 || t == 128 || t == 256) ctx->amat_tile = t; }
-    if (ctx->amat_R == 4) ctx->amat_tile = 256;
-    double aw = 8.0;
-    if (const char *e = getenv("PCM_AMAT_WAVES")) aw = atof(e);
+    const double aw = 8.0;
     ctx->plan_amat = ctx->amat_R == 4       ? make_plan(ctx->M, TPB * 4, ctx->M, 256, wave_of(ctx, amatvec_kernel<4, AMAT_C, 256>), 0.5, aw)
                      : ctx->amat_tile == 64  ? make_plan(ctx->M, TPB * 2, ctx->M, 64, wave_of(ctx, amatvec_kernel<2, AMAT_C, 64>), 0.5, aw)
                      : ctx->amat_tile == 128 ? make_plan(ctx->M, TPB * 2, ctx->M, 128, wave_of(ctx, amatvec_kernel<2, AMAT_C, 128>), 0.5, aw)
@@ -1229,8 +1224,7 @@ static int launch_amatvec_kernels(pcm_ctx *ctx, const double *q, const int32_t *
 int fill_amat_blocks(pcm_ctx *ctx) {
     const PatchMap &pm = ctx->amat_map;
     ctx->amat_blocks = nullptr;
-    double budget_gb = 16.0;
-    if (const char *e = getenv("PCM_NEAR_STORE_GB")) budget_gb = atof(e);
+    const double budget_gb = 16.0;
     const double need = (double)pm.nnear * SUB * SUB * 8.0;
     if (ctx->opt.store_near == 0 || pm.npiece == 0 || need > budget_gb * 1e9) return PCM_OK;
     int rc = dev_alloc_t(ctx, &ctx->amat_blocks, (size_t)pm.nnear * SUB * SUB);
@@ -1257,7 +1251,7 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
     int rc;
     if ((rc = mark(ctx, 0, s))) return rc;
     if ((rc = mark(ctx, 1, s))) return rc;
-    if (ctx->cgp.ready && ctx->opt.cg_path != 1) {   // small cavities: sweep, grid barrier and row sums in one cooperative launch
+    if (ctx->cgp.ready) {   // small cavities: sweep, grid barrier and row sums in one cooperative launch
         if ((rc = cgp_matvec(ctx, q, idx, y, s))) return rc;
         ctx->launches[2]++;
         for (int i = 2; i <= 7; ++i)

@@ -469,7 +469,7 @@ __global__ void rbj_invert_kernel(const double4 *__restrict__ pt, const double *
     for (int j = 0; j < n; ++j) {
         const double d = a[(size_t)j * n + j];
         if (!(d > 0.0)) {
-            if (threadIdx.x == 0) *err = 3;
+            if (threadIdx.x == 0) *err = 4;   // not positive definite (1, 2: selection failed; 3: selection capacity, host falls back)
             return;
         }
         const double s = sqrt(d), is = 1.0 / s;
@@ -1033,6 +1033,8 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     auto now = []() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); };
     const double t0 = now();
     if ((int64_t)block > M) block = (int)M;
+    // the CG update kernels keep a block's residual in shared memory: (block + 256) doubles must fit
+    if (((size_t)block + 256) * 8 > 200 * 1024) return set_error(ctx, PCM_ERR_ARG, "pcm_rbj_build: block size above 25 000 is not supported");
     std::vector<int32_t> &perm = ctx->rbj_perm_sorted;  // pivot order in the library's sorted point numbering
     if (pivot_order_host) {
         std::vector<char> seen((size_t)M, 0);
@@ -1111,7 +1113,7 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     // (measured: 0.8 vs 1.6 ms at M = 8 930, 6.1 vs 9.6 ms at 50k, 86 vs 78 ms at 200k, where scanning 6 250 group boxes per
     // block with one CTA costs more than the two grid barriers of the global scan; up to 150k the one-CTA form is kept because
     // an asynchronous build then hides behind pcm_potential on one SM instead of taking CTAs on all of them)
-    if (block <= 256 && (M <= 150000 || getenv("PCM_RBJ_LOCAL")) && !force_global && !getenv("PCM_RBJ_GLOBAL")) {
+    if (block <= 256 && M <= 150000 && !force_global && !ctx->opt.rbj_global_scan) {
         const int ng = (int)cdiv(M, 32);
         int *d_gcount = (int *)w.cand_idx, *d_glist = d_gcount + ng;   // scratch of the global path, 2 M ints
         const size_t base_smem = (sizeof(RblShared) + 15) / 16 * 16;
@@ -1216,6 +1218,8 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     auto update = [&](int init) -> int {
         if (precond == 2) {
             const int block = (int)ctx->rbj_block;
+            if (((size_t)block + DOT_THREADS) * 8 > 48 * 1024)    // large blocks: opt in to more dynamic shared memory
+                cudaFuncSetAttribute(cg_update_rbj_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(((size_t)block + DOT_THREADS) * 8));
             cg_update_rbj_kernel<<<(unsigned)ctx->rbj_nblocks, DOT_THREADS, ((size_t)block + DOT_THREADS) * 8, s>>>(
                 M, block, ctx->rbj_order, ctx->rbj_inv, p, Ap, x, r, z, scal, partial, ctl, tol, max_iter, init);
         } else {
@@ -1243,7 +1247,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     int it = 0;
     double rr = 0.0;
     // below AMAT_PERSIST_MAX points: every iteration inside one persistent cooperative kernel (pcm_cgp.cu)
-    const bool persistent = ctx->opt.cg_path != 1 && cgp_can_solve(ctx, precond);
+    const bool persistent = ctx->opt.cg_path != 1 && ctx->opt.cg_path != 3 && cgp_can_solve(ctx, precond);
     if (persistent) {
         CG_TRY(cgp_solve(ctx, r, z, p, Ap, x, tol, max_iter, precond, s));
         CG_CUDA(cudaMemcpyAsync(h, scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
@@ -1255,7 +1259,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
     } else {
     CG_TRY(update(1));  // z = C r, p = z, rz, rr; raises STOP if already converged (or max_iter == 0)
     // RBJ: everything after the sweep in one cooperative kernel (cg_fused_rbj_kernel)
-    bool fused = precond == 2 && !getenv("PCM_CG_UNFUSED");
+    bool fused = precond == 2 && ctx->opt.cg_path != 3;
     CgFused fa{};
     int fgrid = 0;
     size_t fsmem = 0;
@@ -1270,7 +1274,6 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
         } else {
             const int64_t want = std::max<int64_t>(cdiv(M, 32), ctx->rbj_nblocks);
             fgrid = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)per_sm * ctx->sm_count));
-            if (const char *e = getenv("PCM_CG_GRID")) fgrid = std::max(1, std::min(fgrid, atoi(e)));
             fa.M = M; fa.block = block; fa.nblocks = (int)ctx->rbj_nblocks; fa.max_iter = max_iter;
             fa.parts = amat_parts(ctx);
             fa.order = ctx->rbj_order; fa.inv = ctx->rbj_inv;
@@ -1278,8 +1281,7 @@ int cg_solve(pcm_ctx *ctx, const double *b_caller, double *x_caller, double tol,
             fa.ctl = ctl; fa.tol = tol;
         }
     }
-    int batch = 8;   // iterations queued per read-back of the device-side convergence flag
-    if (const char *e = getenv("PCM_CG_BATCH")) batch = std::max(1, atoi(e));
+    const int batch = 8;   // iterations queued per read-back of the device-side convergence flag
     while (true) {
         CG_CUDA(cudaMemcpyAsync(h, scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
         CG_CUDA(cudaStreamSynchronize(s));

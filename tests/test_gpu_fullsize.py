@@ -124,10 +124,16 @@ def test_fullsize_gradient_sampled(full, pcm, orc):
 
 def test_fullsize_potential_sampled(full, orc):
     cfg, w, ctx, P, q, v, F = full
+    # 96 seeded points plus the 32 points closest to a nucleus (the shell centres): those are the ones whose products take the
+    # near-field (Boys table) branch, which random sampling exercises only by chance
+    from scipy.spatial import cKDTree
     rng = np.random.default_rng(500 + cfg)
-    pts = np.sort(rng.choice(w.surface.M, size=32, replace=False))
+    dmin, _ = cKDTree(w.atom_xyz).query(w.surface.xyz)
+    close = np.argsort(dmin, kind="stable")[:32]
+    rest = np.setdiff1d(np.arange(w.surface.M), close)
+    pts = np.sort(np.concatenate([close, rng.choice(rest, size=96, replace=False)]))
     ref = orc.potential(w.basis, w.surface, w.P, points=pts)
-    assert_parity(v[pts.tolist()].cpu().numpy(), ref, f"config {cfg}: v on 32 sampled points")
+    assert_parity(v[pts.tolist()].cpu().numpy(), ref, f"config {cfg}: v on 128 points (32 closest to a nucleus + 96 sampled)")
 
 
 def test_fullsize_fock_sampled_blocks(full, orc, torch_cuda):

@@ -308,3 +308,34 @@ def test_fock_tma_tiles_and_serial_classes_give_the_same_bits(pcm, orc, torch_cu
             assert np.array_equal(pcm.pcm_fock(c, qd).cpu().numpy(), F0), opts
             pcm.pcm_destroy(c)
         pcm.pcm_destroy(ref)
+
+
+def test_shell_level_prescreen_never_drops_a_pair_eq15_keeps(pcm):
+    """pcm_setup skips whole shell pairs with a cheap shell-level estimate before it evaluates Eq. 15 per primitive pair.  The
+    estimate must be an upper bound: on adversarial shells (very diffuse and very tight exponents, d shells, coefficients from
+    1e-3 to 1e3, distances up to where the pairs die) the surviving primitive pairs equal a brute-force count with
+    pcm_schwarz_bound over every primitive pair."""
+    rng = np.random.default_rng(17)
+    nsh = 40
+    l = rng.integers(0, 3, nsh).astype(np.int32)
+    xyz = rng.uniform(-1, 1, (nsh, 3)) * np.array([30.0, 6.0, 6.0])
+    nprim = rng.integers(1, 4, nsh).astype(np.int32)
+    exps = np.exp(rng.uniform(np.log(0.01), np.log(3000.0), int(nprim.sum())))
+    coef = np.exp(rng.uniform(np.log(1e-3), np.log(1e3), int(nprim.sum()))) * rng.choice([-1.0, 1.0], int(nprim.sum()))
+    off = np.concatenate([[0], np.cumsum(nprim)])
+    pts = rng.uniform(-5, 5, (40, 3))
+    for eps in (1e-12, 1e-6):
+        ctx = pcm.pcm_setup(l, xyz, nprim, exps, coef, pts, np.full(40, 2.0), screen_eps=eps)
+        info = pcm.pcm_get_info(ctx)
+        want = 0
+        for I in range(nsh):
+            for J in range(I, nsh):
+                for i in range(off[I], off[I + 1]):
+                    for j in range(off[J], off[J + 1]):
+                        if I == J and j < i:
+                            continue
+                        b = pcm.pcm_schwarz_bound(int(l[I]), float(exps[i]), xyz[I], int(l[J]), float(exps[j]), xyz[J])
+                        want += abs(coef[i] * coef[j]) * b >= eps
+        assert info.prim_pairs_total == want, (eps, info.prim_pairs_total, want)
+        assert 0 < want < info.prim_pairs_unscreened
+        pcm.pcm_destroy(ctx)

@@ -175,27 +175,26 @@ def test_rbj_build_async_equals_sync(pcm, orc, sys2500, torch_cuda):
         pcm.pcm_rbj_build_async(ctx, 0, seed=1, stream=side)
 
 
-def test_fused_cg_and_neighbourhood_selection_are_exact_rewrites(pcm, orc, sys2500, torch_cuda, monkeypatch):
+def test_fused_cg_and_neighbourhood_selection_are_exact_rewrites(pcm, orc, sys2500, torch_cuda):
     """DESIGN.md claims that (i) the one-CTA neighbourhood block selection finds the blocks of the global row scan and
-    (ii) the fused cooperative CG kernel reproduces the separate kernels bit for bit.  Both have a switch."""
+    (ii) the fused cooperative CG update kernel of the separate-launch path reproduces the separate kernels bit for bit.
+    Both have a switch in pcm_options (cg_path = 1 / 3, rbj_global_scan)."""
     torch = torch_cuda
     s, A, q_true, _ = sys2500
-    ctx = points_ctx(pcm, s, cg_path=1)            # the separate-launch path (below 20k points the default is the persistent kernel)
+    c_fused, c_sep, c_glob = points_ctx(pcm, s, cg_path=1), points_ctx(pcm, s, cg_path=3), points_ctx(pcm, s, cg_path=1, rbj_global_scan=True)
     b = dev(torch, A @ q_true)
-    monkeypatch.delenv("PCM_RBJ_GLOBAL", raising=False)
-    monkeypatch.delenv("PCM_CG_UNFUSED", raising=False)
-    pcm.pcm_rbj_build(ctx, 48, seed=11)
-    o_local, b_local, inv_local = pcm.pcm_rbj_get(ctx)
-    x_fused, it_fused, rr_fused, _, ok = pcm.pcm_cg_solve(ctx, b, tol=1e-10, max_iter=500, precond=2)
+    for c in (c_fused, c_sep, c_glob):
+        pcm.pcm_rbj_build(c, 48, seed=11)
+    o_local, b_local, inv_local = pcm.pcm_rbj_get(c_fused)
+    x_fused, it_fused, rr_fused, _, ok = pcm.pcm_cg_solve(c_fused, b, tol=1e-10, max_iter=500, precond=2)
     assert ok
-    monkeypatch.setenv("PCM_CG_UNFUSED", "1")
-    x_sep, it_sep, rr_sep, _, ok = pcm.pcm_cg_solve(ctx, b, tol=1e-10, max_iter=500, precond=2)
+    x_sep, it_sep, rr_sep, _, ok = pcm.pcm_cg_solve(c_sep, b, tol=1e-10, max_iter=500, precond=2)
     assert ok and it_sep == it_fused and rr_sep == rr_fused and torch.equal(x_sep, x_fused)
-    monkeypatch.setenv("PCM_RBJ_GLOBAL", "1")
-    pcm.pcm_rbj_build(ctx, 48, seed=11)
-    o_glob, b_glob, inv_glob = pcm.pcm_rbj_get(ctx)
+    o_glob, b_glob, inv_glob = pcm.pcm_rbj_get(c_glob)
     assert np.array_equal(o_local, o_glob) and np.array_equal(b_local, b_glob)
     assert all(np.array_equal(a, c) for a, c in zip(inv_local, inv_glob))
+    for c in (c_fused, c_sep, c_glob):
+        pcm.pcm_destroy(c)
 
 
 @pytest.mark.parametrize("M", [300, 2500, 9000])

@@ -32,6 +32,41 @@ def close(got, ref, atol=1e-12):
     return np.all(np.abs(got - ref) <= 1e-10 * np.abs(ref) + atol)
 
 
+def term_magnitudes(s, atoms, rad, z, q, f):
+    """Per element of g_point and g_atom: the sum of the ABSOLUTE values of the terms Eq. 14's surface gradient adds up (the B
+    term per nucleus, the off-diagonal A term per point pair, the A_kk term per other sphere), with scipy's erf.  A sum of n
+    rounded terms is off by at most n eps sum|terms|; the element-wise floor of the comparison is 8 eps times this."""
+    from scipy.special import erf
+    M, N = s.M, len(rad)
+    pt, zk = s.xyz, s.zeta
+    g = lambda zp, r: np.abs(2 * zp / np.sqrt(np.pi) * np.exp(-(zp * r) ** 2) / r) + np.abs(erf(zp * r) / r ** 2)
+    mp, ma = np.zeros((M, 3)), np.zeros((N, 3))
+    akk = zk * np.sqrt(2 / np.pi) / s.switch
+    for J in range(N):
+        e = pt - atoms[J]
+        d = np.linalg.norm(e, axis=1)
+        ok = d > 0
+        w = np.zeros(M)
+        w[ok] = np.abs(z[J] * q[ok]) * g(zk[ok], d[ok])
+        other = ok & (s.atom != J)
+        a_, b_ = zk * (rad[J] - d), zk * (rad[J] + d)
+        swf = 1 - 0.5 * (erf(a_) + erf(b_))
+        dswf = zk / np.sqrt(np.pi) * (np.exp(-a_ * a_) + np.exp(-b_ * b_))
+        w[other] += 0.5 / abs(f) * q[other] ** 2 * akk[other] * dswf[other] / swf[other]
+        t = np.where(ok[:, None], w[:, None] * np.abs(e) / np.where(ok, d, 1.0)[:, None], 0.0)
+        mp += t
+        ma[J] = t.sum(0)
+    for k in range(M):
+        e = pt[k] - pt
+        r = np.linalg.norm(e, axis=1)
+        ok = r > 0
+        zp = zk[k] * zk / np.sqrt(zk[k] ** 2 + zk ** 2)
+        w = np.zeros(M)
+        w[ok] = np.abs(q[k] * q[ok] / f) * g(zp[ok], r[ok])
+        mp[k] += (w[:, None] * np.abs(e) / np.where(ok, r, 1.0)[:, None]).sum(0)
+    return mp, ma
+
+
 def points_ctx(pcm, s):
     e = np.zeros(0)
     return pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), e, e, s.xyz, s.zeta, s.switch)
@@ -103,6 +138,11 @@ def test_surface_gradient_small_exponents_and_coincidences(pcm, orc, torch_cuda)
     gp, ga = gp.cpu().numpy(), ga.cpu().numpy()
     assert np.isfinite(gp).all() and np.isfinite(ga).all()
     rp, ra = orc.surface_gradient(s, atoms, rad, z, q, 0.9)
-    scale = 1e-12 * max(1.0, np.abs(rp).max())
-    assert close(gp, rp, atol=scale) and close(ga, ra, atol=1e-12 * max(1.0, np.abs(ra).max()))
+    # element-wise: 1e-10 |ref| + 1e-12 + 8 eps x (sum of the absolute terms of that element) -- the terms reach 1e3 here (small
+    # exponents, charges up to 0.5, a nucleus 1e-3 from a point) and largely cancel, so eps x their magnitude is the rounding
+    # floor of any summation order
+    mp, ma = term_magnitudes(s, atoms, rad, z, q, 0.9)
+    eps8 = 8 * np.finfo(float).eps
+    assert np.all(np.abs(gp - rp) <= 1e-10 * np.abs(rp) + 1e-12 + eps8 * mp), np.abs(gp - rp).max()
+    assert np.all(np.abs(ga - ra) <= 1e-10 * np.abs(ra) + 1e-12 + eps8 * ma), np.abs(ga - ra).max()
     pcm.pcm_destroy(ctx)

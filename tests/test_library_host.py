@@ -71,10 +71,59 @@ def test_schwarz_bound_worked_example(L):
     ss = pcm.pcm_schwarz_bound(0, al, A, 0, be, B)
     assert ss ** 2 == pytest.approx(2 * math.pi ** 2.5 * K * K / (p * p * math.sqrt(2 * p)), rel=1e-13)
     assert ss ** 2 == pytest.approx(g["ss"], rel=1e-11)
-    # the bound is the max over Cartesian components, so it is at least the listed component's value
+    # the bound is the max over Cartesian components, so it is at least the listed component's value (the maximum itself is
+    # pinned for every class in test_schwarz_bound_every_class_by_an_independent_route)
     assert pcm.pcm_schwarz_bound(1, al, A, 0, be, B) ** 2 >= g["pxs"] * (1 - 1e-11)
     assert pcm.pcm_schwarz_bound(1, al, A, 1, be, B) ** 2 >= g["pxpz"] * (1 - 1e-11)
     assert pcm.pcm_schwarz_bound(2, al, A, 0, be, B) ** 2 >= g["dxxs"] * (1 - 1e-11)
+
+
+def _self_repulsion(a, alpha, A, b, beta, B):
+    """[chi_a chi_b|chi_a chi_b] for raw Cartesian primitives by a route that shares nothing with the library's Hermite
+    expansion: 1/r12 = (2/sqrt pi) int_0^inf exp(-t^2 r12^2) dt makes the six-dimensional integral a product of three
+    two-dimensional Gaussian integrals per t; in u = (x1 + x2)/sqrt 2, w = (x1 - x2)/sqrt 2 (x measured from P) the exponent
+    is -p u^2 - (p + 2 t^2) w^2, so each is a polynomial moment, exact by Gauss-Hermite; the t integral is adaptive."""
+    from scipy import integrate
+    A, B = np.asarray(A, float), np.asarray(B, float)
+    p = alpha + beta
+    P = (alpha * A + beta * B) / p
+    K = math.exp(-alpha * beta / p * float(((A - B) ** 2).sum()))
+    x, w = np.polynomial.hermite.hermgauss(12)        # exact to degree 23 >= 2 (2 + 2) x 2
+
+    def axis(t, d):
+        cu, cw = p, p + 2 * t * t
+        U, W = np.meshgrid(x / math.sqrt(cu), x / math.sqrt(cw), indexing="ij")
+        wt = np.outer(w / math.sqrt(cu), w / math.sqrt(cw))
+        y1, y2 = (U + W) / math.sqrt(2), (U - W) / math.sqrt(2)
+        g = lambda y: (y + P[d] - A[d]) ** a[d] * (y + P[d] - B[d]) ** b[d]
+        return float((wt * g(y1) * g(y2)).sum())
+
+    f = lambda s: (lambda t: axis(t, 0) * axis(t, 1) * axis(t, 2) / (1 - s) ** 2)(s / (1 - s))
+    val = integrate.quad(f, 0, 1, epsabs=0, epsrel=1e-12, limit=400)[0]
+    return 2 / math.sqrt(math.pi) * K * K * val
+
+
+def test_schwarz_bound_every_class_by_an_independent_route(L):
+    """Eq. 15's screening quantity for all six shell classes: pcm_schwarz_bound^2 equals the maximum over the
+    Cartesian components of [ab|ab] evaluated by _self_repulsion (numerical t-integral of Gauss-Hermite moments) -- an
+    over- or under-estimate of any component of any class fails here, not only the s-s closed form."""
+    carts = {0: [(0, 0, 0)], 1: [(1, 0, 0), (0, 1, 0), (0, 0, 1)],
+             2: [(2, 0, 0), (1, 1, 0), (1, 0, 1), (0, 2, 0), (0, 1, 1), (0, 0, 2)]}
+    e = GOLD["worked_example"]
+    cases = [(e["alpha"], e["A"], e["beta"], e["B"]), (2.3, [0.2, -0.1, 0.4], 0.35, [-0.6, 0.5, 0.1])]
+    # the s-s closed form pins the route itself first
+    al, A, be, B = cases[0]
+    pp = al + be
+    Kab = math.exp(-al * be / pp * sum((x - y) ** 2 for x, y in zip(A, B)))
+    assert _self_repulsion((0, 0, 0), al, A, (0, 0, 0), be, B) == pytest.approx(2 * math.pi ** 2.5 * Kab * Kab / (pp * pp * math.sqrt(2 * pp)), rel=1e-10)
+    g = GOLD["schwarz_worked_example"]
+    assert _self_repulsion((1, 0, 0), al, A, (0, 0, 1), be, B) == pytest.approx(g["pxpz"], rel=1e-9)     # survey-derived value
+    assert _self_repulsion((2, 0, 0), al, A, (0, 0, 0), be, B) == pytest.approx(g["dxxs"], rel=1e-9)
+    for al, A, be, B in cases:
+        for la in range(3):
+            for lb in range(la, 3):
+                ref = max(_self_repulsion(a, al, A, b, be, B) for a in carts[la] for b in carts[lb])
+                assert pcm.pcm_schwarz_bound(la, al, A, lb, be, B) ** 2 == pytest.approx(ref, rel=1e-9), (la, lb)
 
 
 def test_schwarz_bound_by_quadrature(L):
