@@ -1111,9 +1111,9 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     // block sizes up to 256: the single-CTA neighbourhood selection; it reports err = 3 (capacity) to fall back
     bool local_done = false;
     // (measured: 0.8 vs 1.6 ms at M = 8 930, 6.1 vs 9.6 ms at 50k, 86 vs 78 ms at 200k, where scanning 6 250 group boxes per
-    // block with one CTA costs more than the two grid barriers of the global scan; up to 150k the one-CTA form is kept because
-    // an asynchronous build then hides behind pcm_potential on one SM instead of taking CTAs on all of them)
-    if (block <= 256 && M <= 150000 && !force_global && !ctx->opt.rbj_global_scan) {
+    // block with one CTA costs more than the two grid barriers of the global scan; at the 102 470 points of configs[3] the
+    // one-CTA form runs out of candidate capacity after 11 ms and the scan has to run anyway)
+    if (block <= 256 && M <= 100000 && !force_global && !ctx->opt.rbj_global_scan) {
         const int ng = (int)cdiv(M, 32);
         int *d_gcount = (int *)w.cand_idx, *d_glist = d_gcount + ng;   // scratch of the global path, 2 M ints
         const size_t base_smem = (sizeof(RblShared) + 15) / 16 * 16;

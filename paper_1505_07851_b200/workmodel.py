@@ -50,6 +50,9 @@ def kernel_key(name: str) -> str | None:
     m = re.search(r"(potential|fock)_near_kernel<\s*(\d+)", name)
     if m:
         return f"{m.group(1)}_near_L{m.group(2)}"
+    m = re.search(r"cgp_matvec_kernel<\s*(\d+)", name)
+    if m:
+        return "amatvec_cgp" if m.group(1) == "0" else f"amatvec_cgp_mode{m.group(1)}"
     m = re.search(r"amatvec\w*_kernel<\s*(\d+)", name)
     if m:
         return f"amatvec_R{m.group(1)}"
@@ -122,13 +125,15 @@ def _summarise(raw_csv: str, kernel_json: str) -> list:
                 return float(r[c].replace(",", "")) if c is not None else 0.0
             except ValueError:
                 return 0.0
+        if key.startswith("amatvec_cgp_mode"):
+            continue     # the fill / stored variants of the one-launch sweep are not part of the work model
         if key.startswith("amatvec"):
             M = run["amat_M"]
             units, workload = 0.5 * M * M, f"configs[4] M={M}"
         elif key[-2] == "L" and key[-1].isdigit():
             units, workload = float(run["products_by_L"][int(key[-1])]) * run["M"], f"configs[{run['config']}]"
         else:
-            units, workload = 0.0, f"configs[{run['config']}]"
+            continue     # not a hot kernel of the work model (transforms, reductions)
         rows.append({"key": key, "kernel": name.split("(")[0].replace("void ", "").strip(), "workload": workload, "units": f"{units:.6g}",
                      "time_us": f"{val('time') / 1e3:.3f}", "dfma": f"{val('dfma'):.0f}", "dadd": f"{val('dadd'):.0f}",
                      "dmul": f"{val('dmul'):.0f}", "fp64_warp_inst": f"{val('fp64_warp_inst'):.0f}",
