@@ -44,9 +44,9 @@ UNIT = "prim-pair*point/s"
 CONFIG_INDEX = 3
 RBJ_BLOCK = 64
 CG_TOL = 1e-8
-SWEEP_M = (10_000, 50_000, 100_000, 200_000)
+SWEEP_M = (2_500, 10_000, 50_000, 100_000, 200_000)
 STORED_M = (2_500, 5_000, 10_000, 50_000)   # stored-A variant against the on-the-fly sweep
-SOLVER_M = (10_000, 50_000, 200_000)   # configs[4]: full pcm_cg_solve, RBJ-64 against Jacobi
+SOLVER_M = (2_500, 10_000, 50_000, 200_000)   # configs[4]: full pcm_cg_solve, RBJ-64 against Jacobi
 
 WORKLOADS = {
     0: "configs[0]: 12-atom chain, 6-31G-shaped s/sp shells, 50 points/atom",
@@ -454,6 +454,20 @@ def amat_and_solver_sweep(pcm, torch, dev, flush, model, peak_tflops, with_solve
                     e1.record(stream); torch.cuda.synchronize()
                     tsol.append(e0.elapsed_time(e1))
                 rec[name] = {"iters": int(it), "ms": min(tsol), "ms_per_iter": min(tsol) / max(it, 1), "converged": bool(ok), "true_resid": rt}
+            if Ms < 20000:   # the same solve through the separate-launch path (pcm_options.cg_path = 1), for comparison
+                c1 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0),
+                                   s4.xyz, s4.zeta, s4.switch, cg_path=1)
+                pcm.pcm_rbj_build(c1, RBJ_BLOCK, seed=7, stream=stream)
+                tsol, it = [], 0
+                for _ in range(3):
+                    flush.zero_()
+                    e0.record(stream)
+                    _, it, rr, rt, ok = pcm.pcm_cg_solve(c1, b, x, tol=CG_TOL, max_iter=5000, precond=2, stream=stream)
+                    e1.record(stream); torch.cuda.synchronize()
+                    tsol.append(e0.elapsed_time(e1))
+                rec["rbj64_separate_launches"] = {"iters": int(it), "ms": min(tsol), "ms_per_iter": min(tsol) / max(it, 1)}
+                rec["path"] = "persistent cooperative kernel (pcm_cgp.cu); rbj64_separate_launches = the same solve with cg_path = 1"
+                pcm.pcm_destroy(c1)
             solver.append(rec)
         pcm.pcm_destroy(c4)
     return sweep, solver
