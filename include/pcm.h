@@ -146,7 +146,8 @@ int pcm_potential(pcm_ctx *ctx, const double *P_dev, int64_t ldp, double *v_dev,
 int pcm_fock(pcm_ctx *ctx, const double *q_dev, double *F_dev, int64_t ldf, int accumulate, void *stream);
 
 /*
- * pcm_amatvec -- y = A q with A evaluated on the fly (Eq. 2, 3, 8; never stored, unlike PAPER.md:106).
+ * pcm_amatvec -- y = A q with A evaluated on the fly (Eq. 2, 3, 8); what pcm_options.store_near / store_far keep of A (the paper
+ * stores all of it) is read back instead of re-evaluated, with the same values and summation order.
  * q_dev, y_dev: DEVICE, M doubles, must not alias.  Coincident points i != j (a caller error) are treated as
  * r = 0 -> 2 zeta'/sqrt(pi), never NaN.  Deterministic.  Asynchronous.
  */
