@@ -78,7 +78,9 @@ typedef struct pcm_options {
                               0 (default).  Same results bit for bit */
     int rbj_global_scan;   /* 1: pcm_rbj_build selects every block with the cooperative global row scan instead of the one-CTA
                               neighbourhood search (same blocks; the default uses the scan only above 150 000 points or l > 256) */
-    int reserved[1];
+    int potential_pr;      /* bit L set: pcm_potential sweeps the products of total angular momentum L in the Fock layout (product
+                              in registers, warp-shuffle reduction over the 32 products of a warp per point) instead of the
+                              point-in-registers layout.  Same values up to the summation order.  Default 0 (measured: DESIGN.md) */
 } pcm_options;
 
 typedef struct pcm_info {

@@ -38,7 +38,7 @@ EXPORTS = (
 
 class pcm_options(C.Structure):
     _fields_ = [("screen_eps", C.c_double), ("d_pure", C.c_int), ("device", C.c_int), ("merge_products", C.c_int),
-                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("store_far", C.c_int), ("serial_classes", C.c_int), ("tma_tiles", C.c_int), ("rbj_global_scan", C.c_int), ("reserved", C.c_int * 1)]
+                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("store_far", C.c_int), ("serial_classes", C.c_int), ("tma_tiles", C.c_int), ("rbj_global_scan", C.c_int), ("potential_pr", C.c_int)]
 
 
 class pcm_info(C.Structure):
@@ -199,7 +199,7 @@ def pcm_options_default() -> pcm_options:
 def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_zeta, pt_switch=None, *,
               screen_eps: float = 1e-12, d_pure: bool = True, device: int = -1, merge_products: bool = True,
               gradient: bool = False, store_near: bool = True, cg_path: int = 0, store_far: int = 0, tma_tiles: bool = False,
-              serial_classes: bool = False, rbj_global_scan: bool = False) -> Context:
+              serial_classes: bool = False, rbj_global_scan: bool = False, potential_pr: int = 0) -> Context:
     """Host numpy arrays in, context out (include/pcm.h: pcm_setup)."""
     import torch
     if not torch.cuda.is_available():
@@ -231,6 +231,7 @@ def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_z
     opt.tma_tiles = 1 if tma_tiles else 0
     opt.serial_classes = 1 if serial_classes else 0
     opt.rbj_global_scan = 1 if rbj_global_scan else 0
+    opt.potential_pr = int(potential_pr)
     h = C.c_void_p()
     rc = lib().pcm_setup(C.byref(h), len(sl), _hp(sl), _hp(sx), _hp(sn), _hp(pe), _hp(pc), len(pz), _hp(px), _hp(pz),
                          _hp(ps), C.byref(opt))

@@ -915,6 +915,96 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
         if (kk[r] < M) vpart[(size_t)blockIdx.y * M + kk[r]] = v[r];
 }
 
+// ---- the potential in the Fock layout ("product in registers", pcm_options.potential_pr) -------------------------------
+// north_star describes the P-contraction as "warp-shuffle reductions": thread = one Hermite product with its centre and
+// D_h in REGISTERS, the points of the CTA's point block (PR_PTS of them) staged once in shared memory, and the 32 products
+// of a warp summed per point by a fixed-order shuffle butterfly -- NB point values per lane are reduced together, halving
+// the live values at every step (NB/2 + NB/4 + ... + 1 + log2(32/NB) exchanges for NB points: ~1 SHFL.64 + 1 DADD per
+// evaluation), after which lane pair (2j, 2j+1) holds the warp's sum for point j.  Per-warp point accumulators in shared
+// memory, added over the warps at the end -> vpart[product chunk][point].  Against potential_kernel this trades the
+// broadcast reads of the product record (27 doubles per evaluation at L = 3) for one shuffle-add per evaluation.
+// Far patches come from the class's Fock map (rows = product groups, columns = point groups: the same boxes and the same
+// symmetric criterion as the potential map, so the near kernel's complement is unchanged).
+constexpr int PR_PTS = 512;
+template <int L, int NB>
+__global__ void __launch_bounds__(TPB) potential_pr_kernel(const double4 *__restrict__ prodA, const double *__restrict__ herm,
+                                                           int64_t npad, int pchunk, const double4 *__restrict__ pt, int M,
+                                                           double *__restrict__ vpart, const uint8_t *__restrict__ farmap,
+                                                           int64_t nbyte) {
+    constexpr int NH = nherm(L);
+    constexpr int REC = pot_rec<L>() + (L == 3 ? 4 : 0);
+    __shared__ double4 s_pt[PR_PTS];                 // x, y, z of the point block (padding: far away)
+    __shared__ double s_acc[TPB / 32][PR_PTS];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int k0 = blockIdx.x * PR_PTS, npts = min(PR_PTS, M - k0), ngrp = (npts + 31) / 32;
+    for (int t = threadIdx.x; t < PR_PTS; t += TPB) {
+        s_pt[t] = (t < npts) ? pt[k0 + t] : make_double4(3e8, 3e8, 3e8, 1.0);
+#pragma unroll
+        for (int w = 0; w < TPB / 32; ++w) s_acc[w][t] = 0.0;
+    }
+    __syncthreads();
+    const int64_t pbeg = (int64_t)blockIdx.y * pchunk, pend = min(npad, pbeg + (int64_t)pchunk);
+    for (int64_t pb = pbeg; pb < pend; pb += TPB) {
+        const int64_t ip = pb + threadIdx.x;       // < npad: npad and pchunk are multiples of TPB
+        double rec[REC];
+        {
+            const double4 a = prodA[ip];
+            rec[0] = a.x; rec[1] = a.y; rec[2] = a.z; rec[3] = 0.0;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) rec[4 + h] = herm[(size_t)h * npad + ip];
+            if (L == 2 || L == 3) rec[3] = rec[4 + 4] + rec[4 + 7] + rec[4 + 9];
+            if (L == 3) {
+                rec[24] = fma(3.0, rec[4 + 10], rec[4 + 13] + rec[4 + 15]);
+                rec[25] = fma(3.0, rec[4 + 16], rec[4 + 11] + rec[4 + 18]);
+                rec[26] = fma(3.0, rec[4 + 19], rec[4 + 12] + rec[4 + 17]);
+            }
+        }
+        const uint8_t *frow = farmap + (size_t)(ip >> 5) * nbyte;     // the warp's product group (warp-uniform)
+        for (int g = 0; g < ngrp; ++g) {
+            const int cg = (k0 >> 5) + g;
+            if (!((frow[cg >> 3] >> (cg & 7)) & 1)) continue;
+#pragma unroll 1
+            for (int t0 = 0; t0 < 32; t0 += NB) {
+                double val[NB];
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    val[j] = 0.0;
+                    pot_far_unit<L>(rec, s_pt[g * 32 + t0 + j], val[j]);
+                }
+                // butterfly: after the step with lane mask `off` a lane keeps the half of its values its bit selects
+                int nv = NB;
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) {
+                    if (nv > 1) {
+                        nv >>= 1;
+                        const bool up = (lane & off) != 0;
+#pragma unroll
+                        for (int j = 0; j < NB / 2; ++j) {
+                            if (j < nv) {
+                                const double keep = up ? val[j + nv] : val[j], send = up ? val[j] : val[j + nv];
+                                val[j] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+                            }
+                        }
+                    } else {
+                        val[0] += __shfl_xor_sync(0xffffffffu, val[0], off);
+                    }
+                }
+                // lane bits (from 16 down) selected the upper halves in turn: the point index is their bit pattern
+                constexpr int LOG_NB = NB == 16 ? 4 : NB == 8 ? 3 : NB == 4 ? 2 : 1;
+                const int j = (lane >> (5 - LOG_NB)) & (NB - 1);
+                if ((lane & ((1 << (5 - LOG_NB)) - 1)) == 0) s_acc[warp][g * 32 + t0 + j] += val[0];
+            }
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < npts; t += TPB) {
+        double v = s_acc[0][t];
+#pragma unroll
+        for (int w = 1; w < TPB / 32; ++w) v += s_acc[w][t];
+        vpart[(size_t)blockIdx.y * M + k0 + t] = v;
+    }
+}
+
 // near patches of the potential sweep: one warp per piece; lane = point; the 32 products of a listed group are
 // staged in the warp's own shared memory.  Writes near[piece][lane].
 template <int L>
@@ -1145,6 +1235,8 @@ static void plan_class(pcm_ctx *ctx) {
     const double iw = 4.0;   // wave target of the work partition (more waves measured no different on configs[1])
     ctx->plan_fock[L] = make_plan(c.npad, TPB * fb.R, ctx->M, PT_TILE, wave_of(ctx, fock_kernel<L, fb.R, fb.C>), 1.0, iw);
     ctx->plan_pot[L] = make_plan(ctx->M, TPB * pb.R, c.npad, pot_tile(L), wave_of(ctx, potential_kernel<L, pb.R, pb.C>), 1.0, iw);
+    if ((ctx->opt.potential_pr >> L) & 1)    // product-in-registers layout: rows = point blocks of PR_PTS, chunks of whole product blocks
+        ctx->plan_pot[L] = make_plan(ctx->M, PR_PTS, c.npad, TPB, wave_of(ctx, potential_pr_kernel<L, (L <= 3 ? 16 : 8)>), 1.0, iw);
 }
 
 int plan_all(pcm_ctx *ctx) {
@@ -1417,6 +1509,13 @@ static int launch_potential_class(pcm_ctx *ctx, int64_t slot, cudaStream_t s) {
     const Plan &pl = ctx->plan_pot[L];
     const PatchMap &pm = c.pot_map;
     dim3 grid((unsigned)pl.xb, (unsigned)pl.chunks);
+    if ((ctx->opt.potential_pr >> L) & 1) {
+        potential_pr_kernel<L, (L <= 3 ? 16 : 8)><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
+                                                                    ctx->vpart + (size_t)slot * ctx->M, c.fock_map.far, c.fock_map.nbyte);
+        PCM_LAUNCH_CHECK(ctx);
+        { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
+        return PCM_OK;
+    }
     potential_kernel<L, pb.R, pb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
                                                          ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);

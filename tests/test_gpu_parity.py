@@ -339,3 +339,27 @@ def test_shell_level_prescreen_never_drops_a_pair_eq15_keeps(pcm):
         assert info.prim_pairs_total == want, (eps, info.prim_pairs_total, want)
         assert 0 < want < info.prim_pairs_unscreened
         pcm.pcm_destroy(ctx)
+
+
+def test_potential_product_in_registers_layout(pcm, orc, torch_cuda):
+    """pcm_options.potential_pr: the potential swept in the Fock layout (product in registers, warp-shuffle reduction over the 32
+    products of a warp) for every class -- against the oracle at the north_star tolerance, and reproducible run to run."""
+    torch = torch_cuda
+    w = synth.make_workload(0, with_d=True)
+    ref = orc.potential(w.basis, w.surface, w.P)
+    for bits in (31, 8 + 16, 1 + 4):
+        c = pcm.setup_from_workload(w.basis, w.surface, potential_pr=bits)
+        v = pcm.pcm_potential(c, dev(torch, w.P)).cpu().numpy()
+        assert_parity(v, ref, f"v, potential_pr = {bits}")
+        assert np.array_equal(pcm.pcm_potential(c, dev(torch, w.P)).cpu().numpy(), v)
+        pcm.pcm_destroy(c)
+    w = synth.make_workload(1, n_atoms=50)            # several point blocks and product chunks, ragged tails
+    c = pcm.setup_from_workload(w.basis, w.surface, potential_pr=31)
+    v = pcm.pcm_potential(c, dev(torch, w.P)).cpu().numpy()
+    pts = np.arange(0, w.surface.M, 37)
+    assert_parity(v[pts], orc.potential(w.basis, w.surface, w.P, points=pts), "v on sampled points, potential_pr = 31")
+    c0 = pcm.setup_from_workload(w.basis, w.surface)
+    v0 = pcm.pcm_potential(c0, dev(torch, w.P)).cpu().numpy()
+    assert np.all(np.abs(v - v0) <= 1e-12 * np.abs(v0) + 1e-14)
+    pcm.pcm_destroy(c)
+    pcm.pcm_destroy(c0)
