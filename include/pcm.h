@@ -322,8 +322,9 @@ int pcm_get_info(pcm_ctx *ctx, pcm_info *out);
 /*
  * Kernel timing.  pcm_set_timing(ctx, 1) makes pcm_potential (op 0), pcm_fock (op 1) and pcm_amatvec (op 2) record
  * CUDA events on the launching stream around their kernels (each op has its own event set).
- * pcm_last_kernel_ms: for the most recent timed call of `op`, ms[0] = the main integral / matvec kernels,
- * ms[1] = pre/post transforms and reductions; n_launch (may be NULL) = kernels that call launched.
+ * pcm_last_kernel_ms: for the most recent timed call of `op`, ms[0] = the main integral kernels, ms[1] = pre/post transforms
+ * and reductions (op 2: ms[0] = the whole product, sweep and row sums, ms[1] = 0); n_launch (may be NULL) = kernels that
+ * call launched.
  * pcm_last_class_ms: the same call split by total angular momentum, ms[L] = device time of the main kernel of the
  * products with L = l_a + l_b = 0..4 (op 2: ms[0] is its one kernel).  Both synchronise on the recorded events.
  */

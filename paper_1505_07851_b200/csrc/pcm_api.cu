@@ -454,6 +454,11 @@ int pcm_last_kernel_ms(pcm_ctx *ctx, int op, double ms[2], int *n_launch) {
     cudaEvent_t *ev = ctx->ev + 8 * op;
     PCM_CUDA(ctx, cudaEventSynchronize(ev[7]));
     float a = 0, b = 0, c = 0;
+    if (op == 2) {   // pcm_amatvec records one event before and one after its launches
+        PCM_CUDA(ctx, cudaEventElapsedTime(&b, ev[0], ev[7]));
+        ms[0] = b;
+        return PCM_OK;
+    }
     PCM_CUDA(ctx, cudaEventElapsedTime(&a, ev[0], ev[1]));
     PCM_CUDA(ctx, cudaEventElapsedTime(&b, ev[1], ev[6]));
     PCM_CUDA(ctx, cudaEventElapsedTime(&c, ev[6], ev[7]));
@@ -469,6 +474,13 @@ int pcm_last_class_ms(pcm_ctx *ctx, int op, double ms[PCM_NL]) {
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaEvent_t *ev = ctx->ev + 8 * op;
     PCM_CUDA(ctx, cudaEventSynchronize(ev[7]));
+    if (op == 2) {
+        float t = 0;
+        PCM_CUDA(ctx, cudaEventElapsedTime(&t, ev[0], ev[7]));
+        ms[0] = t;
+        for (int L = 1; L < PCM_NL; ++L) ms[L] = 0.0;
+        return PCM_OK;
+    }
     for (int L = 0; L < PCM_NL; ++L) {
         float t = 0;
         PCM_CUDA(ctx, cudaEventElapsedTime(&t, ev[1 + L], ev[2 + L]));

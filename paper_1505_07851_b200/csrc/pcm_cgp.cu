@@ -61,6 +61,7 @@ struct CgpArgs {
     const double *inv;
     double *r, *z, *p0, *p1, *Ap, *x, *part1, *part2, *scal;
     int *ctl;
+    int phase;                 // cgp_matvec_kernel: 0 = sweep, grid barrier, row sums (cooperative launch); 1 = sweep only; 2 = row sums only
     unsigned long long *dbg;   // PCM_VERBOSE: %globaltimer of CTA 0 at the phase boundaries of the first iterations
 };
 constexpr int CGP_DBG_ITERS = 8;
@@ -567,9 +568,9 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_matvec_kernel(CgpArgs a) {
     const unsigned G = gridDim.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     PSrc pv{a.q, nullptr, a.qidx, 0.0};
-    cgp_sweep<MODE>(a, pv, blockIdx.x * CGP_WARPS + warp, lane, dyn + warp * CGP_WSMEM2);
-    if (MODE == 1) return;      // filling the store: the sums are not needed
-    cgp_grid_sync(a.ctl, G);
+    if (a.phase != 2) cgp_sweep<MODE>(a, pv, blockIdx.x * CGP_WARPS + warp, lane, dyn + warp * CGP_WSMEM2);
+    if (MODE == 1 || a.phase == 1) return;      // filling the store, or the sweep half of a two-launch product
+    if (a.phase == 0) cgp_grid_sync(a.ctl, G);
     for (int g0 = blockIdx.x * CGP_TEAMS; g0 < a.ng; g0 += (int)G * CGP_TEAMS) {
         const int g = g0 + warp / CGP_TW;
         const double t = cgp_row_sum(a, g, dyn);
@@ -769,9 +770,18 @@ int cgp_matvec(pcm_ctx *ctx, const double *q, const int32_t *idx, double *y, cud
     CgpArgs a = cgp_args(ctx);
     a.q = q; a.qidx = idx; a.y = y;
     void *args[] = {&a};
-    const void *k = a.afar ? (const void *)cgp_matvec_kernel<2> : (const void *)cgp_matvec_kernel<0>;
-    PCM_CUDA(ctx, cudaLaunchCooperativeKernel(k, dim3((unsigned)ctx->cgp.grid), dim3(CGP_THREADS), args, ctx->cgp.smem, s));
-    ctx->launch_total += 1;
+    (void)args;
+    // Two ordinary launches (sweep; row sums) instead of one cooperative launch with a grid barrier: a cooperative launch costs
+    // ~20 us more between the events around it than its kernel runs (measured at M = 10k: 94 us against 72 us under ncu), which a
+    // single A q does not win back; inside a solve the launch happens once, so pcm_cg_solve keeps the cooperative kernel.
+    a.phase = 1;
+    if (a.afar) cgp_matvec_kernel<2><<<(unsigned)ctx->cgp.grid, CGP_THREADS, ctx->cgp.smem, s>>>(a);
+    else cgp_matvec_kernel<0><<<(unsigned)ctx->cgp.grid, CGP_THREADS, ctx->cgp.smem, s>>>(a);
+    a.phase = 2;
+    const unsigned rgrid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(cdiv2(a.ng, CGP_TEAMS), 4 * (int64_t)ctx->cgp.grid));
+    cgp_matvec_kernel<0><<<rgrid, CGP_THREADS, CGP_WARPS * 32 * 8, s>>>(a);
+    PCM_CUDA(ctx, cudaGetLastError());
+    ctx->launch_total += 2;
     return PCM_OK;
 }
 

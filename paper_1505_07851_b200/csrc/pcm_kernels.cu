@@ -1341,18 +1341,15 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
     if (M == 0) return PCM_OK;
     const int32_t *idx = caller_order ? ctx->s2c : nullptr;
     int rc;
+    // timing: one event before and one after (each event record is a command of its own on the stream, ~1 us: eight of them
+    // would be a tenth of a 10k-point product)
     if ((rc = mark(ctx, 0, s))) return rc;
-    if ((rc = mark(ctx, 1, s))) return rc;
-    if (ctx->cgp.ready) {   // small cavities: sweep, grid barrier and row sums in one cooperative launch
+    if (ctx->cgp.ready) {   // small cavities: the warp-granular sweep of pcm_cgp.cu and its row sums, two launches
         if ((rc = cgp_matvec(ctx, q, idx, y, s))) return rc;
-        ctx->launches[2]++;
-        for (int i = 2; i <= 7; ++i)
-            if ((rc = mark(ctx, i, s))) return rc;
-        return PCM_OK;
+        ctx->launches[2] += 2;
+        return mark(ctx, 7, s);
     }
     if ((rc = launch_amatvec_kernels(ctx, q, idx, nullptr, s))) return rc;
-    for (int i = 2; i <= 6; ++i)
-        if ((rc = mark(ctx, i, s))) return rc;
     amat_reduce_kernel<<<(unsigned)ceil_div(M, 32), 256, 0, s>>>(amat_parts(ctx), M, y, idx);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
