@@ -75,9 +75,11 @@ def work_of(model: dict, op: str, L: int = 0, M: int = 0, amat_key: str | None =
         rec = model.get(key)
     if rec:
         return {"key": key, "instr": rec["fp64_instr_per_unit"], "flop": rec["flop_per_unit"], "traffic_per_unit": rec["traffic_per_unit"],
+                "issue_slots": rec.get("issue_slots_per_unit"),
                 "source": f"ncu counters, {model['_source']['file']} ({rec['workload']})"}
     hw = HAND_WORK[op][L] if op in ("potential", "fock") else HAND_WORK.get(key, HAND_WORK["amatvec_R4"])
-    return {"key": key, "instr": hw[0], "flop": hw[1], "traffic_per_unit": None, "source": "hand count (no capture of this kernel under profiles/)"}
+    return {"key": key, "instr": hw[0], "flop": hw[1], "traffic_per_unit": None, "issue_slots": None,
+            "source": "hand count (no capture of this kernel under profiles/)"}
 
 
 def log(*a):
@@ -673,6 +675,10 @@ def run_ours(args):
                                    if tpu is not None else "no ncu capture of this kernel under profiles/: null"),
                 "algorithmic_bytes": 40.0 * M + (32.0 + 8.0 * [1, 4, 10, 20, 35][Ld]) * float(info.products[Ld]),
                 "fp64_pipe_frac": n_units * wk["instr"] * 2.0 / (ms_dom * 1e-3) * 1e-12 / peak_tflops,
+                # the bound these kernels actually sit on: issue cycles = 2 per FP64 warp instruction + 1 per other
+                # instruction, 592 sub-partitions issuing one cycle per clock at the SM clock sampled during the timed region
+                "issue_slot_frac": (n_units * wk["issue_slots"] / (592.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6 * ms_dom * 1e-3)
+                                    if wk.get("issue_slots") else None),
                 "timed": "launch duration from the library's CUDA events in the breakdown pass after the timed region (class kernels one after the "
                          "other); in the timed region the five class kernels of a call run concurrently on five streams",
                 "units_per_launch": n_units, "flop_per_unit": wk["flop"], "fp64_instr_per_unit": wk["instr"], "work_source": wk["source"],

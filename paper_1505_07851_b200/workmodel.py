@@ -9,6 +9,7 @@ A q sweep).  `load()` turns it into per-unit figures keyed by kernel:
     flop_per_unit        = (2 DFMA + DADD + DMUL) / units
     fp64_instr_per_unit  = (DFMA + DADD + DMUL) / units                  (thread instructions on the FP64 pipe)
     traffic_per_unit     = DRAM bytes / units
+    issue_slots_per_unit = (FP64 warp instructions + all warp instructions) / units   (an FP64 instruction takes two issue cycles)
 
 `python -m paper_1505_07851_b200.workmodel RAW.csv KERNELS.json [--no-header] >> profiles/<tag>_flops.csv`
 writes its rows from the raw `ncu --csv --page raw --print-units base` output of one `bench.py --mode kernels` run and the
@@ -27,7 +28,7 @@ import sys
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 FIELDS = ["key", "kernel", "workload", "units", "time_us", "dfma", "dadd", "dmul", "fp64_warp_inst", "dram_bytes", "regs", "grid",
-          "fp64_pipe_pct_elapsed"]
+          "fp64_pipe_pct_elapsed", "warp_inst"]
 METRICS = {
     "dfma": "sm__sass_thread_inst_executed_op_dfma_pred_on.sum",
     "dadd": "sm__sass_thread_inst_executed_op_dadd_pred_on.sum",
@@ -38,8 +39,9 @@ METRICS = {
     "time": "gpu__time_duration.sum",
     "regs": "launch__registers_per_thread",
     "pipe": "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed",
+    "warp_inst": "smsp__inst_executed.sum",
 }
-NCU_METRICS = ",".join(METRICS[k] for k in ("dfma", "dadd", "dmul", "fp64_warp_inst", "dram_read", "dram_write", "time", "regs", "pipe"))
+NCU_METRICS = ",".join(METRICS[k] for k in ("dfma", "dadd", "dmul", "fp64_warp_inst", "dram_read", "dram_write", "time", "regs", "pipe", "warp_inst"))
 
 
 def kernel_key(name: str) -> str | None:
@@ -88,6 +90,13 @@ def load(path: str | None = None) -> dict:
                "units": units, "time_us_under_ncu": float(row["time_us"]) if row.get("time_us") else None,
                "fp64_pipe_pct_elapsed": float(row["fp64_pipe_pct_elapsed"]) if row.get("fp64_pipe_pct_elapsed") else None,
                "workload": row.get("workload", "")}
+        # issue slots per unit: on this part an FP64 warp instruction holds its sub-partition's issue port for two cycles, every
+        # other instruction for one: (2 fp64 + other) = fp64 + all warp instructions, per unit
+        if row.get("warp_inst") and row.get("fp64_warp_inst"):
+            try:
+                rec["issue_slots_per_unit"] = (float(row["warp_inst"]) + float(row["fp64_warp_inst"])) / units
+            except ValueError:
+                pass
         out[key] = rec
         out.setdefault(row["key"], rec)      # first row of a key = the default (largest workload first in the file)
     out["_source"] = {"file": os.path.relpath(path, ROOT), "sha16": hashlib.sha256(raw.encode()).hexdigest()[:16]}
@@ -138,7 +147,8 @@ def _summarise(raw_csv: str, kernel_json: str) -> list:
                      "time_us": f"{val('time') / 1e3:.3f}", "dfma": f"{val('dfma'):.0f}", "dadd": f"{val('dadd'):.0f}",
                      "dmul": f"{val('dmul'):.0f}", "fp64_warp_inst": f"{val('fp64_warp_inst'):.0f}",
                      "dram_bytes": f"{val('dram_read') + val('dram_write'):.0f}", "regs": f"{val('regs'):.0f}",
-                     "grid": r[col["Grid Size"]] if "Grid Size" in col else "", "fp64_pipe_pct_elapsed": f"{val('pipe'):.2f}"})
+                     "grid": r[col["Grid Size"]] if "Grid Size" in col else "", "fp64_pipe_pct_elapsed": f"{val('pipe'):.2f}",
+                     "warp_inst": f"{val('warp_inst'):.0f}"})
     return rows
 
 
