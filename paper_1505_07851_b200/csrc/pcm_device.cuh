@@ -183,6 +183,10 @@ __device__ __forceinline__ void hermite_R(double x, double y, double z, const do
                     if (pw == 1) {
                         if (n == 0) sink.product(h, t, u, v, c, R[n + 1][h1]);
                         else R[n][h] = c * R[n + 1][h1];
+                    } else if (n == 0 && Sink::kSplit) {
+                        // a sink that accumulates: acc_h += c R1_h1 now, and (pw - 1) x [sum over evaluations of R1_h2] at the end
+                        // (hermite_lower / hermite_fixup) -- the "lower" terms of many components are the same few values
+                        sink.product(h, t, u, v, c, R[n + 1][h1]);
                     } else {
                         const double lower = (pw == 2) ? R[n + 1][h2] : (double)(pw - 1) * R[n + 1][h2];
                         const double val = fma(c, R[n + 1][h1], lower);
@@ -193,6 +197,29 @@ __device__ __forceinline__ void hermite_R(double x, double y, double z, const do
             }
         }
     }
+    if (Sink::kSplit && L >= 2) {   // the lower terms of the order-0 integrals: R^1_h2 for every h2 of degree <= L - 2, once each
+#pragma unroll
+        for (int h2 = 0; h2 < nherm(L >= 2 ? L - 2 : 0); ++h2) sink.lower(h2, R[1][h2]);
+    }
+}
+
+// For a split sink: acc[h] += (pw - 1) x accL[h2] for every component whose lowered power pw is >= 2 (the same pick_dir walk)
+template <int L>
+__device__ __forceinline__ void hermite_fixup(double (&acc)[nherm(L)], const double (&accL)[nherm(L >= 2 ? L - 2 : 0)]) {
+#pragma unroll
+    for (int d = 2; d <= L; ++d)
+#pragma unroll
+        for (int t = d; t >= 0; --t)
+#pragma unroll
+            for (int u = d - t; u >= 0; --u) {
+                const int v = d - t - u;
+                const int dir = pick_dir(t, u, v);
+                const int pw = dir == 0 ? t : (dir == 1 ? u : v);
+                if (pw >= 2) {
+                    const int h2 = dir == 0 ? hidx(t - 2, u, v) : (dir == 1 ? hidx(t, u - 2, v) : hidx(t, u, v - 2));
+                    acc[hidx(t, u, v)] = fma((double)(pw - 1), accL[h2], acc[hidx(t, u, v)]);
+                }
+            }
 }
 
 }  // namespace pcm

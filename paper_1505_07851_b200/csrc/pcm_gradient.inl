@@ -17,6 +17,8 @@
 // ---------------------------------------------------------------------------------------------
 template <int L>
 struct PotGradSink {
+    static constexpr bool kSplit = false;
+    __device__ __forceinline__ void lower(int, double) {}
     const double *D;   // D_h of the product, h < nherm(L)
     double gx, gy, gz;
     __device__ __forceinline__ void value(int, int t, int u, int v, double x) {

@@ -440,13 +440,40 @@ AmatParts amat_parts(const pcm_ctx *ctx) {
 // ---------------------------------------------------------------------------------------------
 template <int L>
 struct FockSink {
+    static constexpr bool kSplit = false;
+    __device__ __forceinline__ void lower(int, double) {}
     double acc[nherm(L)];
     __device__ __forceinline__ void value(int h, int, int, int, double v) { acc[h] += v; }
     __device__ __forceinline__ void product(int h, int, int, int, double a, double b) { acc[h] = fma(a, b, acc[h]); }
 };
 
+// The main Fock sweep accumulates the order-0 integrals in two parts: R_h = c R^1_h1 + (pw - 1) R^1_h2 (the last recursion step,
+// pw = the power being lowered).  acc_h takes the first term by FMA; the second terms of all components are multiples of the
+// few R^1_h2 with degree(h2) <= L - 2 (g_1 alone for L = 2; g_1, x g_2, y g_2, z g_2 for L = 3), which are summed once per
+// evaluation into accL and added to the components at the end of the kernel (hermite_fixup): 3 -> 1 additions per evaluation
+// at L = 2, 12 -> 4 at L = 3.  Another (still fixed) summation order than FockSink's.
+constexpr int FOCK_SPLIT_MAXL = 4;      // L = 5 (gradient of the dd class): 216 registers with it
 template <int L>
-__device__ __forceinline__ void fock_far_unit(const double4 &A, const double4 &pc, FockSink<L> &sink) {
+struct FockSinkSplit {
+    static constexpr bool kSplit = (L >= 2 && L <= FOCK_SPLIT_MAXL);
+    double acc[nherm(L)];
+    double accL[nherm(L >= 2 ? L - 2 : 0)];
+    __device__ __forceinline__ void value(int h, int, int, int, double v) { acc[h] += v; }
+    __device__ __forceinline__ void product(int h, int, int, int, double a, double b) { acc[h] = fma(a, b, acc[h]); }
+    __device__ __forceinline__ void lower(int h2, double v) { accL[h2] += v; }
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int h = 0; h < nherm(L); ++h) acc[h] = 0.0;
+#pragma unroll
+        for (int h = 0; h < nherm(L >= 2 ? L - 2 : 0); ++h) accL[h] = 0.0;
+    }
+    __device__ __forceinline__ void finish() {
+        if (kSplit) hermite_fixup<L>(acc, accL);
+    }
+};
+
+template <int L, class Sink>
+__device__ __forceinline__ void fock_far_unit(const double4 &A, const double4 &pc, Sink &sink) {
     const double x = A.x - pc.x, y = A.y - pc.y, z = A.z - pc.z;
     double g[L + 1];
     seeds_far_scaled<L>(fma(z, z, fma(y, y, x * x)), pc.w, g);
@@ -465,12 +492,11 @@ __global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ p
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
     double4 A[R];
-    FockSink<L> sink[R];
+    FockSinkSplit<L> sink[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         A[r] = prodA[min((rg0 + r) * SUB + lane, npad - 1)];
-#pragma unroll
-        for (int h = 0; h < NH; ++h) sink[r].acc[h] = 0.0;
+        sink[r].clear();
     }
     const int kbeg = blockIdx.y * chunk_len, kend = min(M, kbeg + chunk_len);
     for (int base = kbeg; base < kend; base += PT_TILE) {
@@ -505,6 +531,7 @@ __global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ p
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
+        sink[r].finish();
         const int64_t ip = (rg0 + r) * SUB + lane;
         if (ip < npad) {
             double *out = herm + (size_t)blockIdx.y * NH * npad + ip;
@@ -559,12 +586,11 @@ __global__ void __launch_bounds__(TPB) fock_tma_kernel(const double4 *__restrict
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
     double4 A[R];
-    FockSink<L> sink[R];
+    FockSinkSplit<L> sink[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         A[r] = prodA[min((rg0 + r) * SUB + lane, npad - 1)];
-#pragma unroll
-        for (int h = 0; h < NH; ++h) sink[r].acc[h] = 0.0;
+        sink[r].clear();
     }
     const int kbeg = blockIdx.y * chunk_len, kend = min(M, kbeg + chunk_len);
     if (threadIdx.x == 0) {
@@ -614,6 +640,7 @@ __global__ void __launch_bounds__(TPB) fock_tma_kernel(const double4 *__restrict
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
+        sink[r].finish();
         const int64_t ip = (rg0 + r) * SUB + lane;
         if (ip < npad) {
             double *out = herm + (size_t)blockIdx.y * NH * npad + ip;
@@ -713,6 +740,8 @@ __global__ void __launch_bounds__(256) reduce_herm_kernel(double *__restrict__ h
 // ---------------------------------------------------------------------------------------------
 template <int L>
 struct PotSink {
+    static constexpr bool kSplit = false;
+    __device__ __forceinline__ void lower(int, double) {}
     const double *D;
     double v;
     __device__ __forceinline__ void value(int h, int, int, int, double x) { v = fma(D[h], x, v); }
