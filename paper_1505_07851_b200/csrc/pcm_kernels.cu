@@ -45,6 +45,14 @@ __host__ __device__ constexpr Blocking fock_blocking(int L) {
 __host__ __device__ constexpr Blocking pot_blocking(int L) {
     return L == 0 ? Blocking{4, 2} : L == 1 ? Blocking{4, 1} : L == 2 ? Blocking{2, 2} : L == 3 ? Blocking{2, 2} : Blocking{1, 1};
 }
+// Large cavities (POT_BIG_MIN points and more) take twice the points per thread for L >= 2: the product record (14, 27, 39 doubles)
+// is then read from shared memory once per 4 (2) evaluations instead of 2 (1) -- every load is an issue slot the FP64 pipe does
+// not get -- at the price of half as many point blocks, which small cavities cannot afford (configs[1], L = 2: 0.186 -> 0.223 ms;
+// configs[3]: 24.3 -> 23.6, 11.2 -> 11.05, 4.51 -> 4.43 ms for L = 2, 3, 4).
+constexpr int64_t POT_BIG_MIN = 40000;
+__host__ __device__ constexpr Blocking pot_blocking_big(int L) {
+    return L <= 1 ? pot_blocking(L) : L <= 3 ? Blocking{4, 1} : Blocking{2, 1};
+}
 __host__ __device__ constexpr int pot_tile(int L) { return L <= 2 ? 256 : 64; }  // products staged per tile (8 or 2 groups)
 
 // far bits of the R row groups of this warp for the NS column groups starting at column group cg0 (cg0 % NS == 0,
@@ -1264,6 +1272,9 @@ static void plan_class(pcm_ctx *ctx) {
     const double iw = 4.0;   // wave target of the work partition (more waves measured no different on configs[1])
     ctx->plan_fock[L] = make_plan(c.npad, TPB * fb.R, ctx->M, PT_TILE, wave_of(ctx, fock_kernel<L, fb.R, fb.C>), 1.0, iw);
     ctx->plan_pot[L] = make_plan(ctx->M, TPB * pb.R, c.npad, pot_tile(L), wave_of(ctx, potential_kernel<L, pb.R, pb.C>), 1.0, iw);
+    constexpr Blocking pbb = pot_blocking_big(L);
+    if (ctx->M >= POT_BIG_MIN && (pbb.R != pb.R || pbb.C != pb.C))
+        ctx->plan_pot[L] = make_plan(ctx->M, TPB * pbb.R, c.npad, pot_tile(L), wave_of(ctx, potential_kernel<L, pbb.R, pbb.C>), 1.0, iw);
     if ((ctx->opt.potential_pr >> L) & 1)    // product-in-registers layout: rows = point blocks of PR_PTS, chunks of whole product blocks
         ctx->plan_pot[L] = make_plan(ctx->M, PR_PTS, c.npad, TPB, wave_of(ctx, potential_pr_kernel<L, (L <= 3 ? 16 : 8)>), 1.0, iw);
 }
@@ -1542,8 +1553,13 @@ static int launch_potential_class(pcm_ctx *ctx, int64_t slot, cudaStream_t s) {
         { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
         return PCM_OK;
     }
-    potential_kernel<L, pb.R, pb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
-                                                         ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
+    constexpr Blocking pbb = pot_blocking_big(L);
+    if (ctx->M >= POT_BIG_MIN && (pbb.R != pb.R || pbb.C != pb.C))
+        potential_kernel<L, pbb.R, pbb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
+                                                               ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
+    else
+        potential_kernel<L, pb.R, pb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
+                                                             ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
