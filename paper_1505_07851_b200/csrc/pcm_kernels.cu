@@ -802,7 +802,7 @@ __device__ __forceinline__ void pot_far_unit<2>(const double *rec, const double4
     // components: 4 = (2,0,0), 5 = (1,1,0), 6 = (1,0,1), 7 = (0,2,0), 8 = (0,1,1), 9 = (0,0,2)
     const double q2 = fma(x, fma(rec[8], x, fma(rec[9], y, rec[10] * z)), fma(y, fma(rec[11], y, rec[12] * z), z * (rec[13] * z)));
     const double lin = fma(rec[5], x, fma(rec[6], y, fma(rec[7], z, h23.y)));
-    const double e1 = fma(u * 3.0, q2, -lin);
+    const double e1 = fma(u, q2, -lin);          // the record carries 3 D_2 (pot_scale_record)
     v = fma(ri, fma(u, e1, rec[4]), v);
 }
 
@@ -827,8 +827,8 @@ __device__ __forceinline__ void pot_far_unit<3>(const double *rec, const double4
     double q2 = fma(x, fma(D[4], x, fma(D[5], y, D[6] * z)), fma(y, fma(D[7], y, D[8] * z), z * (D[9] * z)));
     q2 = fma(rec[24], x, fma(rec[25], y, fma(rec[26], z, q2)));
     const double lin = fma(D[1], x, fma(D[2], y, fma(D[3], z, h23.y)));
-    const double e2 = fma(u * -5.0, c3, q2);
-    const double e1 = fma(u * 3.0, e2, -lin);
+    const double e2 = fma(u, c3, q2);            // the record carries 3 D_2, 3 l and -15 D_3 (pot_scale_record)
+    const double e1 = fma(u, e2, -lin);
     v = fma(ri, fma(u, e1, D[0]), v);
 }
 
@@ -854,6 +854,26 @@ __device__ __forceinline__ void pot_local_unit(const double *rec, const double4 
 
 // (forcing the old occupancy back with a minimum-blocks launch bound -- 64 / 72 instead of 72 / 80 registers -- measured slower
 // for L = 0 and no different for L = 1)
+// Derived slots of a staged record r = (centre, pad, D_h ...): the trace of D_2 in the pad slot (L = 2, 3), the first-order
+// coefficients l of the third-order block behind the record (L = 3); then the constants of the Horner form are folded into the
+// coefficients -- D_2 <- 3 D_2 (L = 2, 3), l <- 3 l and D_3 <- -15 D_3 (L = 3) -- so that pot_far_unit multiplies by u only
+// (one FP64 instruction less per evaluation at L = 2, two at L = 3).
+template <int L>
+__device__ __forceinline__ void pot_scale_record(double *r) {
+    if (L == 2 || L == 3) {
+        r[3] = r[4 + 4] + r[4 + 7] + r[4 + 9];
+        if (L == 3) {
+            r[24] = 3.0 * fma(3.0, r[4 + 10], r[4 + 13] + r[4 + 15]);
+            r[25] = 3.0 * fma(3.0, r[4 + 16], r[4 + 11] + r[4 + 18]);
+            r[26] = 3.0 * fma(3.0, r[4 + 19], r[4 + 12] + r[4 + 17]);
+#pragma unroll
+            for (int h = 10; h < 20; ++h) r[4 + h] *= -15.0;
+        }
+#pragma unroll
+        for (int h = 4; h < 10; ++h) r[4 + h] *= 3.0;
+    }
+}
+
 template <int L, int R, int C>
 __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restrict__ prodA, const double *__restrict__ herm,
                                                         int64_t npad, int chunk_len, const double4 *__restrict__ pt, int M,
@@ -909,15 +929,7 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
         }
         if (L == 2 || L == 3) {   // pot_far_unit<2>, <3> want the trace of the second-order block in the pad slot
             __syncthreads();
-            for (int t = threadIdx.x; t < cnt; t += TPB) {
-                double *r = s_rec + t * REC;
-                r[3] = r[4 + 4] + r[4 + 7] + r[4 + 9];
-                if (L == 3) {     // and the first-order coefficients of the third-order block behind the record
-                    r[24] = fma(3.0, r[4 + 10], r[4 + 13] + r[4 + 15]);
-                    r[25] = fma(3.0, r[4 + 16], r[4 + 11] + r[4 + 18]);
-                    r[26] = fma(3.0, r[4 + 19], r[4 + 12] + r[4 + 17]);
-                }
-            }
+            for (int t = threadIdx.x; t < cnt; t += TPB) pot_scale_record<L>(s_rec + t * REC);
         }
         __syncthreads();
         for (int st = 0; st < nst; ++st) {
@@ -989,12 +1001,7 @@ __global__ void __launch_bounds__(TPB) potential_pr_kernel(const double4 *__rest
             rec[0] = a.x; rec[1] = a.y; rec[2] = a.z; rec[3] = 0.0;
 #pragma unroll
             for (int h = 0; h < NH; ++h) rec[4 + h] = herm[(size_t)h * npad + ip];
-            if (L == 2 || L == 3) rec[3] = rec[4 + 4] + rec[4 + 7] + rec[4 + 9];
-            if (L == 3) {
-                rec[24] = fma(3.0, rec[4 + 10], rec[4 + 13] + rec[4 + 15]);
-                rec[25] = fma(3.0, rec[4 + 16], rec[4 + 11] + rec[4 + 18]);
-                rec[26] = fma(3.0, rec[4 + 19], rec[4 + 12] + rec[4 + 17]);
-            }
+            pot_scale_record<L>(rec);
         }
         const uint8_t *frow = farmap + (size_t)(ip >> 5) * nbyte;     // the warp's product group (warp-uniform)
         for (int g = 0; g < ngrp; ++g) {
