@@ -289,3 +289,36 @@ def test_store_far_rule_leaves_large_cavities_on_the_fly(pcm):
     c = points_ctx(pcm, s)
     assert pcm.pcm_get_info(c).amat_persistent == 0                            # 20k points and more: separate launches
     pcm.pcm_destroy(c)
+
+
+def test_rbj_capacity_fallback_sync_and_async(pcm, orc, torch_cuda):
+    """5 000 points packed into a ball of radius 0.6 bohr: every unassigned point is a candidate of every pivot, which exceeds the
+    candidate capacity of the one-CTA neighbourhood selection -- it reports 'capacity' and the build repeats with the global row
+    scan.  Synchronous build, asynchronous build (completed by pcm_rbj_get) and a build forced onto the scan give the same
+    blocks; the blocks are valid against the oracle's A, and the preconditioned solve converges."""
+    torch = torch_cuda
+    rng = np.random.default_rng(23)
+    M = 5000
+    d = rng.normal(size=(M, 3))
+    xyz = d / np.linalg.norm(d, axis=1)[:, None] * 0.6 * rng.uniform(0, 1, (M, 1)) ** (1 / 3)
+    s = synth.Surface(xyz=xyz, zeta=rng.uniform(4.0, 6.0, M), switch=rng.uniform(0.2, 1.0, M), atom=np.zeros(M, np.int32))
+    c_sync, c_async, c_scan = points_ctx(pcm, s), points_ctx(pcm, s), points_ctx(pcm, s, rbj_global_scan=True)
+    pcm.pcm_rbj_build(c_sync, 64, seed=3)
+    side = torch.cuda.Stream()
+    pcm.pcm_rbj_build_async(c_async, 64, seed=3, stream=side)
+    pcm.pcm_rbj_build(c_scan, 64, seed=3)
+    o1, b1, i1 = pcm.pcm_rbj_get(c_sync)
+    o2, b2, i2 = pcm.pcm_rbj_get(c_async)          # completes the pending build (and its fallback)
+    o3, b3, i3 = pcm.pcm_rbj_get(c_scan)
+    assert sorted(o1.tolist()) == list(range(M))
+    assert np.array_equal(o1, o2) and np.array_equal(o1, o3) and np.array_equal(b1, b3)
+    assert all(np.array_equal(a, b) and np.array_equal(a, c) for a, b, c in zip(i1, i2, i3))
+    A = orc.amatrix(s)
+    blk = o1[b1[0]:b1[1]]
+    np.testing.assert_allclose(i1[0] @ A[np.ix_(blk, blk)], np.eye(len(blk)), atol=1e-7)
+    q_true = rng.uniform(-0.05, 0.05, M)
+    b = dev(torch, A @ q_true)
+    x, it, rr, rt, ok = pcm.pcm_cg_solve(c_async, b, tol=1e-8, max_iter=5000, precond=2)
+    assert ok and rt < 2e-8
+    for c in (c_sync, c_async, c_scan):
+        pcm.pcm_destroy(c)
