@@ -723,8 +723,10 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) / n_e2e * 1e3
     line["e2e"] = {"value": world * units_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": n_e2e,
-                   "h2d_bytes_per_step": int(nbf * nbf * 8 + M * 8), "d2h_bytes_per_step": int(nbf * nbf * 8 + M * 8),
-                   "api": "pcm_potential_host(P -> v) + pcm_fock_host(q -> F): pinned host buffers, P up / v down / q up / F down inside the timed region"}
+                   "h2d_bytes_per_step": int(info.components * 16 + M * 8), "d2h_bytes_per_step": int(info.components * 16 + M * 8),
+                   "dense_matrix_bytes": int(nbf * nbf * 8),
+                   "api": ("pcm_potential_host(P -> v) + pcm_fock_host(q -> F) on pinned host buffers, inside the timed region; of the dense "
+                           "P and F only the elements of surviving shell pairs cross PCIe (gathered / scattered on the host, F zero-filled there)")}
     del Ph, Fh
 
     # ---- SURVEY 8(f) rows, timed outside the step: the PCM gradient term (Eq. 14/22) and the glue of Eq. 1/4/13

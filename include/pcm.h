@@ -105,6 +105,8 @@ typedef struct pcm_info {
     int64_t amat_stored_bytes;         /* bytes of those patches kept on the device (0: re-evaluated in every A q) */
     int64_t amat_far_stored_bytes;     /* bytes of the stored far field (pcm_options.store_far; 0: evaluated on the fly) */
     int64_t amat_persistent;           /* 1: pcm_cg_solve / pcm_amatvec use the persistent-kernel path (pcm_options.cg_path) */
+    int64_t components;                /* elements (mu, nu) of P / F in blocks of surviving shell pairs I <= J: what pcm_potential reads
+                                          and pcm_fock writes (times two for the transposes of off-diagonal shell pairs) */
 } pcm_info;
 
 /* Fills *opt with the defaults listed above. */
@@ -308,7 +310,10 @@ int pcm_setup_cavity(pcm_ctx **out, int nshell, const int *shell_l, const double
 /*
  * Host-buffer forms of the four hot calls: same semantics, every array is a HOST pointer; the call
  * copies inputs to the device, runs the device path on the context's own stream, copies the result back
- * and synchronises.  These are what bench.py's end-to-end figure times.
+ * and synchronises.  These are what bench.py's end-to-end figure times.  Of P and F only the elements of
+ * surviving shell pairs cross PCIe (pcm_info.components x 16 bytes, gathered / scattered on the host with
+ * OpenMP through a pinned staging buffer owned by the context): pcm_potential_host reads no other element
+ * of P_host; pcm_fock_host zero-fills F_host (accumulate = 0) or leaves the other elements as they are.
  */
 int pcm_potential_host(pcm_ctx *ctx, const double *P_host, int64_t ldp, double *v_host);
 int pcm_fock_host(pcm_ctx *ctx, const double *q_host, double *F_host, int64_t ldf, int accumulate);

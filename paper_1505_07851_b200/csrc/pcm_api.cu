@@ -37,6 +37,8 @@ static void free_ctx(pcm_ctx *ctx) {
     cudaSetDevice(ctx->device);
     for (void *p : ctx->allocs) cudaFree(p);
     if (ctx->cg_scal_host) cudaFreeHost(ctx->cg_scal_host);
+    if (ctx->io_pin) cudaFreeHost(ctx->io_pin);
+    if (ctx->io_c) cudaFree(ctx->io_c);
     if (ctx->io_a) cudaFree(ctx->io_a);
     if (ctx->io_b) cudaFree(ctx->io_b);
     for (auto &e : ctx->ev) if (e) cudaEventDestroy(e);
@@ -158,6 +160,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     ctx->info.amat_stored_bytes = ctx->amat_blocks ? ctx->amat_map.nnear * 32 * 32 * 8 : 0;
     ctx->info.amat_far_stored_bytes = ctx->cgp.far_bytes;
     ctx->info.amat_persistent = ctx->cgp.ready ? 1 : 0;
+    ctx->info.components = ctx->ncomp;
     *out = ctx;
     return PCM_OK;
 }
@@ -346,6 +349,37 @@ int pcm_cg_solve(pcm_ctx *ctx, const double *b_dev, double *x_dev, double tol, i
 }
 
 // ---- host-buffer forms ------------------------------------------------------------------------
+// P and F are dense nbf x nbf on the host, but the path reads / writes only the elements of surviving shell pairs (a few
+// per cent at configs[3]: 2 GB of matrix, some tens of MB of components).  The host-buffer calls therefore gather those
+// elements into a pinned compact buffer (OpenMP), copy that, and scatter on the other side; the device kernels keep working
+// on a dense device image whose other elements are never read.
+namespace pcm {
+__global__ void scatter_components_kernel(int64_t nc, const int32_t *__restrict__ mu, const int32_t *__restrict__ nu,
+                                          const uint8_t *__restrict__ diag, const double *__restrict__ comp, double *__restrict__ D, int64_t ld) {
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nc) return;
+    D[(size_t)mu[c] * ld + nu[c]] = comp[2 * c];
+    if (!diag[c]) D[(size_t)nu[c] * ld + mu[c]] = comp[2 * c + 1];
+}
+__global__ void gather_components_kernel(int64_t nc, const int32_t *__restrict__ mu, const int32_t *__restrict__ nu,
+                                         const uint8_t *__restrict__ diag, const double *__restrict__ D, int64_t ld, double *__restrict__ comp) {
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nc) return;
+    comp[2 * c] = D[(size_t)mu[c] * ld + nu[c]];
+    comp[2 * c + 1] = diag[c] ? 0.0 : D[(size_t)nu[c] * ld + mu[c]];
+}
+}  // namespace pcm
+
+static int ensure_compact_io(pcm_ctx *ctx) {
+    if (ctx->io_pin && ctx->io_c) return PCM_OK;
+    const size_t bytes = std::max<size_t>((size_t)ctx->ncomp * 16, 16);
+    if (!ctx->io_pin && cudaMallocHost((void **)&ctx->io_pin, bytes) != cudaSuccess)
+        return set_error(ctx, PCM_ERR_ALLOC, "cudaMallocHost (component staging) failed");
+    if (!ctx->io_c && cudaMalloc((void **)&ctx->io_c, bytes) != cudaSuccess)
+        return set_error(ctx, PCM_ERR_ALLOC, "cudaMalloc (component staging) failed");
+    return PCM_OK;
+}
+
 static int ensure_io(pcm_ctx *ctx, double **buf, size_t *have, size_t bytes) {
     if (*have >= bytes && *buf) return PCM_OK;
     if (*buf) cudaFree(*buf);
@@ -363,11 +397,26 @@ int pcm_potential_host(pcm_ctx *ctx, const double *P_host, int64_t ldp, double *
     if (!v_host || (ctx->nbf > 0 && (!P_host || ldp < ctx->nbf))) return set_error(ctx, PCM_ERR_ARG, "pcm_potential_host: bad argument");
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
     const size_t nb = (size_t)ctx->nbf;
+    const int64_t nc = ctx->ncomp;
     int rc;
     if ((rc = ensure_io(ctx, &ctx->io_a, &ctx->io_a_bytes, nb * nb * 8))) return rc;
     if ((rc = ensure_io(ctx, &ctx->io_b, &ctx->io_b_bytes, (size_t)ctx->M * 8))) return rc;
+    if ((rc = ensure_compact_io(ctx))) return rc;
     cudaStream_t s = ctx->own_stream;
-    if (nb) PCM_CUDA(ctx, cudaMemcpy2DAsync(ctx->io_a, nb * 8, P_host, (size_t)ldp * 8, nb * 8, nb, cudaMemcpyHostToDevice, s));
+    if (nc > 0) {
+        const int32_t *mu = ctx->comp_mu_host.data(), *nu = ctx->comp_nu_host.data();
+        double *pin = ctx->io_pin;
+#pragma omp parallel for schedule(static)
+        for (int64_t c = 0; c < nc; ++c) {
+            pin[2 * c] = P_host[(size_t)mu[c] * ldp + nu[c]];
+            pin[2 * c + 1] = P_host[(size_t)nu[c] * ldp + mu[c]];
+        }
+        PCM_CUDA(ctx, cudaMemcpyAsync(ctx->io_c, pin, (size_t)nc * 16, cudaMemcpyHostToDevice, s));
+        scatter_components_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, s>>>(nc, ctx->comp_mu, ctx->comp_nu, ctx->comp_diag, ctx->io_c, ctx->io_a,
+                                                                             (int64_t)nb);
+        PCM_CUDA(ctx, cudaGetLastError());
+        ctx->launch_total += 1;
+    }
     if ((rc = launch_potential(ctx, ctx->io_a, (int64_t)nb, ctx->io_b, s))) return rc;
     PCM_CUDA(ctx, cudaMemcpyAsync(v_host, ctx->io_b, (size_t)ctx->M * 8, cudaMemcpyDeviceToHost, s));
     PCM_CUDA(ctx, cudaStreamSynchronize(s));
@@ -380,15 +429,38 @@ int pcm_fock_host(pcm_ctx *ctx, const double *q_host, double *F_host, int64_t ld
     if (!F_host || ldf < ctx->nbf || (ctx->M > 0 && !q_host)) return set_error(ctx, PCM_ERR_ARG, "pcm_fock_host: bad argument");
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
     const size_t nb = (size_t)ctx->nbf;
+    const int64_t nc = ctx->ncomp;
     int rc;
     if ((rc = ensure_io(ctx, &ctx->io_a, &ctx->io_a_bytes, nb * nb * 8))) return rc;
     if ((rc = ensure_io(ctx, &ctx->io_b, &ctx->io_b_bytes, (size_t)ctx->M * 8))) return rc;
+    if ((rc = ensure_compact_io(ctx))) return rc;
     cudaStream_t s = ctx->own_stream;
     if (ctx->M) PCM_CUDA(ctx, cudaMemcpyAsync(ctx->io_b, q_host, (size_t)ctx->M * 8, cudaMemcpyHostToDevice, s));
-    if (accumulate) PCM_CUDA(ctx, cudaMemcpy2DAsync(ctx->io_a, nb * 8, F_host, (size_t)ldf * 8, nb * 8, nb, cudaMemcpyHostToDevice, s));
-    if ((rc = launch_fock(ctx, ctx->io_b, ctx->io_a, (int64_t)nb, accumulate, s))) return rc;
-    PCM_CUDA(ctx, cudaMemcpy2DAsync(F_host, (size_t)ldf * 8, ctx->io_a, nb * 8, nb * 8, nb, cudaMemcpyDeviceToHost, s));
+    // the device image is built from zero (only its component elements come back); accumulate is applied on the host
+    if ((rc = launch_fock(ctx, ctx->io_b, ctx->io_a, (int64_t)nb, 0, s))) return rc;
+    if (nc > 0) {
+        gather_components_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, s>>>(nc, ctx->comp_mu, ctx->comp_nu, ctx->comp_diag, ctx->io_a, (int64_t)nb,
+                                                                            ctx->io_c);
+        PCM_CUDA(ctx, cudaGetLastError());
+        ctx->launch_total += 1;
+        PCM_CUDA(ctx, cudaMemcpyAsync(ctx->io_pin, ctx->io_c, (size_t)nc * 16, cudaMemcpyDeviceToHost, s));
+    }
+    if (!accumulate) {     // zero-fill on the host while the device works
+#pragma omp parallel for schedule(static)
+        for (int64_t i = 0; i < (int64_t)nb; ++i) std::memset(F_host + (size_t)i * ldf, 0, nb * 8);
+    }
     PCM_CUDA(ctx, cudaStreamSynchronize(s));
+    if (nc > 0) {
+        const int32_t *mu = ctx->comp_mu_host.data(), *nu = ctx->comp_nu_host.data();
+        const uint8_t *dg = ctx->comp_diag_host.data();
+        const double *pin = ctx->io_pin;
+        // every (mu, nu) is written by exactly one component, so the loop is race-free
+#pragma omp parallel for schedule(static)
+        for (int64_t c = 0; c < nc; ++c) {
+            F_host[(size_t)mu[c] * ldf + nu[c]] += pin[2 * c];
+            if (!dg[c]) F_host[(size_t)nu[c] * ldf + mu[c]] += pin[2 * c + 1];
+        }
+    }
     return PCM_OK;
 }
 

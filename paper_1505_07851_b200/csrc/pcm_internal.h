@@ -208,6 +208,14 @@ struct pcm_ctx {
     double *cg_part = nullptr;  // [ceil(M/32)] per-CTA partial dot products of cg_matvec_reduce_kernel
     double *cg_scal = nullptr;  // device scalars
     double *cg_scal_host = nullptr;  // pinned
+    // host-buffer calls: only the elements of P / F that belong to a surviving shell pair cross PCIe.  Per component c of the
+    // component table: its element (mu, nu) and whether the shell pair is diagonal (then (nu, mu) is a component of its own).
+    std::vector<int32_t> comp_mu_host, comp_nu_host;
+    std::vector<uint8_t> comp_diag_host;
+    int32_t *comp_mu = nullptr, *comp_nu = nullptr;   // device copies
+    uint8_t *comp_diag = nullptr;
+    double *io_pin = nullptr;                         // pinned staging, 2 ncomp doubles: (mu, nu) and (nu, mu) of every component
+    double *io_c = nullptr;                           // its device image
     double *io_a = nullptr, *io_b = nullptr;  // staging for the *_host calls
     size_t io_a_bytes = 0, io_b_bytes = 0;
 

@@ -627,6 +627,20 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
     if ((rc = upload(ctx, &ctx->sp_dims, sp_dims))) return rc;
     if ((rc = upload(ctx, &ctx->c_sp, c_sp))) return rc;
     if ((rc = upload(ctx, &ctx->c_ab, c_ab))) return rc;
+    {   // element of every component, for the compact transfers of the host-buffer calls
+        const size_t nc = c_sp.size();
+        ctx->comp_mu_host.resize(nc); ctx->comp_nu_host.resize(nc); ctx->comp_diag_host.resize(nc);
+        for (size_t c = 0; c < nc; ++c) {
+            const int sp = c_sp[c], dims = sp_dims[sp], nb = (dims >> 8) & 0xff;
+            const int a = c_ab[c] / nb, b = c_ab[c] - a * nb;
+            ctx->comp_mu_host[c] = sp_i0[sp] + a;
+            ctx->comp_nu_host[c] = sp_j0[sp] + b;
+            ctx->comp_diag_host[c] = (uint8_t)(dims >> 16);
+        }
+        if ((rc = upload(ctx, &ctx->comp_mu, ctx->comp_mu_host))) return rc;
+        if ((rc = upload(ctx, &ctx->comp_nu, ctx->comp_nu_host))) return rc;
+        if ((rc = upload(ctx, &ctx->comp_diag, ctx->comp_diag_host))) return rc;
+    }
     ctx->nshell = nshell;
     if (want_grad) {
         std::vector<int32_t> shI(pairs.size()), shJ(pairs.size());

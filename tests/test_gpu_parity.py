@@ -150,6 +150,23 @@ def test_host_buffer_forms_equal_device_forms(case, pcm, torch_cuda):
     F2 = np.full_like(F, 1.5)
     pcm.pcm_fock_host(ctx, w.q, F2, accumulate=True)
     np.testing.assert_allclose(F2 - 1.5, F, rtol=0, atol=1e-13)
+    # only the elements of surviving shell pairs cross PCIe: elements of screened-out pairs stay as they are (accumulate) or
+    # become zero, and a P that is garbage outside the surviving blocks gives the same potential
+    touched = F != 0.0
+    assert np.all(F2[~touched] == 1.5)
+    F3 = np.full_like(F, 7.0)
+    pcm.pcm_fock_host(ctx, w.q, F3, accumulate=False)
+    np.testing.assert_array_equal(F3, F)
+    info = pcm.pcm_get_info(ctx)
+    assert 0 < info.components <= ctx.nbf * ctx.nbf
+    ctx2 = pcm.setup_from_workload(w.basis, w.surface, screen_eps=1e-3)       # a screening that really drops shell pairs
+    i2 = pcm.pcm_get_info(ctx2)
+    Fs = pcm.pcm_fock(ctx2, dev(torch_cuda, w.q)).cpu().numpy()
+    if (Fs == 0.0).any():
+        Pg = np.where(Fs != 0.0, w.P, np.nan)                                   # NaN wherever the path must not look
+        np.testing.assert_array_equal(pcm.pcm_potential_host(ctx2, Pg), pcm.pcm_potential(ctx2, dev(torch_cuda, w.P)).cpu().numpy())
+        assert i2.components < ctx.nbf * ctx.nbf
+    pcm.pcm_destroy(ctx2)
 
 
 def test_runs_are_bit_reproducible(case, pcm, torch_cuda):
