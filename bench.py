@@ -680,7 +680,7 @@ def run_ours(args):
                 "issue_slot_frac": (n_units * wk["issue_slots"] / (592.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6 * ms_dom * 1e-3)
                                     if wk.get("issue_slots") else None),
                 "timed": "launch duration from the library's CUDA events in the breakdown pass after the timed region (class kernels one after the "
-                         "other); in the timed region the five class kernels of a call run concurrently on five streams",
+                         "other); in the timed region the class kernels of a call are a chain of programmatic dependent launches (tails overlap)",
                 "units_per_launch": n_units, "flop_per_unit": wk["flop"], "fp64_instr_per_unit": wk["instr"], "work_source": wk["source"],
                 "work_capture": model.get("_source"), "ms_per_launch": ms_dom, "all_hot_kernels": kernels,
                 "peak_source": "measured live: pcm_fp64_peak DFMA chain (MEASURED_PEAKS.json has no fp64 entry; nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2)",

@@ -70,14 +70,15 @@ typedef struct pcm_options {
                               keep the far-field 1/r values too (4 M^2 bytes) when they and the stored near patches stay resident
                               in L2 (<= 96 MB: about M <= 4 500); 1 = whenever device memory allows; -1 = never.  Same values,
                               same summation order: the result does not depend on it */
-    int serial_classes;    /* 1: pcm_potential / pcm_fock launch their per-class kernels one after the other on the caller's stream
-                              (as with pcm_set_timing on); 0 (default): concurrently on five internal streams joined back into
-                              it.  Same results */
+    int serial_classes;    /* 1: pcm_potential / pcm_fock launch their per-class kernels the ordinary way, each after the one before
+                              it has finished (as with pcm_set_timing on); 0 (default): as a chain of programmatic dependent
+                              launches on the caller's stream, so that a class kernel starts while the last wave of the one before
+                              it is still running.  Same results bit for bit */
     int tma_tiles;         /* 1: pcm_fock brings its surface-point tiles into shared memory with TMA bulk copies (cp.async.bulk +
                               mbarrier, double-buffered) from a per-call packed (x, y, z, q) array instead of per-thread loads;
                               0 (default).  Same results bit for bit */
     int rbj_global_scan;   /* 1: pcm_rbj_build selects every block with the cooperative global row scan instead of the one-CTA
-                              neighbourhood search (same blocks; the default uses the scan only above 150 000 points or l > 256) */
+                              neighbourhood search (same blocks; the default uses the scan only above 100 000 points or l > 256) */
     int potential_pr;      /* bit L set: pcm_potential sweeps the products of total angular momentum L in the Fock layout (product
                               in registers, warp-shuffle reduction over the 32 products of a warp per point) instead of the
                               point-in-registers layout.  Same values up to the summation order.  Default 0 (measured: DESIGN.md) */

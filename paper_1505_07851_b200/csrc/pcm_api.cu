@@ -45,8 +45,6 @@ static void free_ctx(pcm_ctx *ctx) {
     for (auto &e : ctx->cg_ev) if (e) cudaEventDestroy(e);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->near_stream) cudaStreamDestroy(ctx->near_stream);
-    for (auto &st : ctx->cls_stream) if (st) cudaStreamDestroy(st);
-    for (auto &ev : ctx->ev_cls) if (ev) cudaEventDestroy(ev);
     if (ctx->ev_rbj) { if (ctx->rbj_pending) cudaEventSynchronize(ctx->ev_rbj); cudaEventDestroy(ctx->ev_rbj); }
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
@@ -107,10 +105,6 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
         // of displacing them (measured 2-3 % on pcm_potential / pcm_fock against a high-priority stream)
         (void)prio_hi;
         e = cudaStreamCreateWithPriority(&ctx->near_stream, cudaStreamNonBlocking, prio_lo);
-    }
-    for (int L = 0; L <= MAXL && e == cudaSuccess; ++L) {
-        e = cudaStreamCreateWithFlags(&ctx->cls_stream[L], cudaStreamNonBlocking);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_cls[L], cudaEventDisableTiming);
     }
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);

@@ -241,8 +241,6 @@ struct pcm_ctx {
     cudaStream_t near_stream = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     // the class kernels of one call run concurrently on these (forked from / joined into the caller's stream), unless timing is on
-    cudaStream_t cls_stream[pcm::MAXL + 1] = {};
-    cudaEvent_t ev_cls[pcm::MAXL + 1] = {};
     // events: 0 start, 1 after the pre-transform, 2+L after the class-L main kernel, 7 end, 8 CG residual read-back
     cudaEvent_t ev[28] = {};   // ev[8*op + i], op = 0 potential, 1 fock, 2 amatvec; 24 CG; 25, 26 peak benchmark
     // CG: events around the A q launches (main + near kernels) of the first CG_EV iterations of the last timed solve

@@ -19,10 +19,6 @@ namespace pcm {
 
 constexpr int TPB = 128;   // threads per block of the hot kernels ("1 x 128", still a good size)
 constexpr int SUB = 32;    // rows / columns per classified group
-// Below this many (product, point) evaluations per call the class kernels run one after the other: the fork / join of five
-// streams costs ~20 us, more than the tails it hides (measured: configs[1] 0.876 -> 0.896 ms, configs[2] 7.99 -> 8.02 ms with
-// the streams, configs[3] 86.6 -> 85.6 ms).
-constexpr double CONCURRENT_CLASSES_MIN = 2e10;
 constexpr int PT_TILE = 256;  // surface points staged per shared-memory tile (Fock, A q): 8 groups = one byte of the far map
 
 // ---------------------------------------------------------------------------------------------
@@ -54,6 +50,17 @@ __host__ __device__ constexpr Blocking pot_blocking_big(int L) {
     return L <= 1 ? pot_blocking(L) : L <= 3 ? Blocking{4, 1} : Blocking{2, 1};
 }
 __host__ __device__ constexpr int pot_tile(int L) { return L <= 2 ? 256 : 64; }  // products staged per tile (8 or 2 groups)
+
+// ---- programmatic dependent launch (PTX griddepcontrol, sm_90+) -----------------------------------------------------------
+// The class kernels of one call are independent of one another, but each is only a few waves long at small and medium sizes
+// and its last wave leaves most of the SMs idle (PAPER.md:160 launches its per-class kernels one after the other).  A class
+// kernel therefore signals at its very start that the next launch of the stream may be scheduled, and a kernel launched with
+// the programmatic-serialization attribute (launch_class below) begins as soon as every CTA of its predecessor has started,
+// i.e. it fills the SM slots the predecessor's last wave leaves free.  Before it exits, each of its CTAs waits for the
+// predecessor to have completed, so that completion stays in launch order and the ordinary launch that follows the chain
+// (the reduction) sees all of it.  Both instructions do nothing in a kernel launched the ordinary way.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait_predecessor() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // far bits of the R row groups of this warp for the NS column groups starting at column group cg0 (cg0 % NS == 0,
 // NS = 8 or 2): bit (r * 8 + s) = patch (row group rg0 + r, column group cg0 + s) is far.  Warp-uniform result.
@@ -497,6 +504,7 @@ __global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ p
     constexpr int NH = nherm(L);
     constexpr int NS = PT_TILE / SUB;
     __shared__ double4 s_pt[PT_TILE];  // x, y, z, q
+    pdl_launch_dependents();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
     double4 A[R];
@@ -547,6 +555,7 @@ __global__ void __launch_bounds__(TPB) fock_kernel(const double4 *__restrict__ p
             for (int h = 0; h < NH; ++h) out[(size_t)h * npad] = sink[r].acc[h];
         }
     }
+    pdl_wait_predecessor();
 }
 
 // ---- the same sweep with the point tiles brought in by the TMA unit (cp.async.bulk, 1-D) --------------------------------
@@ -883,6 +892,7 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
     constexpr int REC = pot_rec_main<L>();
     constexpr int TILE = pot_tile(L), NS = TILE / SUB;
     __shared__ __align__(16) double s_rec[TILE * REC];
+    pdl_launch_dependents();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t rg0 = ((int64_t)blockIdx.x * (TPB / 32) + warp) * R;
     double4 c[R];
@@ -962,6 +972,7 @@ __global__ void __launch_bounds__(TPB) potential_kernel(const double4 *__restric
 #pragma unroll
     for (int r = 0; r < R; ++r)
         if (kk[r] < M) vpart[(size_t)blockIdx.y * M + kk[r]] = v[r];
+    pdl_wait_predecessor();
 }
 
 // ---- the potential in the Fock layout ("product in registers", pcm_options.potential_pr) -------------------------------
@@ -1405,6 +1416,23 @@ static int launch_amatvec_impl(pcm_ctx *ctx, const double *q, double *y, bool ca
 int launch_amatvec(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s) { return launch_amatvec_impl(ctx, q, y, true, s); }
 int launch_amatvec_sorted(pcm_ctx *ctx, const double *q, double *y, cudaStream_t s) { return launch_amatvec_impl(ctx, q, y, false, s); }
 
+// One class kernel; chained: with the programmatic-serialization attribute, i.e. it may start while the last wave of the launch
+// before it on s is still running (see pdl_launch_dependents above; both kernels must be class kernels of the same call).
+template <class... KArgs, class... Args>
+static cudaError_t launch_class(void (*kernel)(KArgs...), dim3 grid, cudaStream_t s, bool chained, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(TPB);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = chained ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 template <int L>
 static int launch_fock_near(pcm_ctx *ctx, const double *q, cudaStream_t s) {
     ClassData &c = ctx->cls[L];
@@ -1419,7 +1447,7 @@ static int launch_fock_near(pcm_ctx *ctx, const double *q, cudaStream_t s) {
 }
 
 template <int L>
-static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s) {
+static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s, bool chained = false) {
     constexpr Blocking fb = fock_blocking(L);
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
@@ -1430,8 +1458,8 @@ static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s) {
         fock_tma_kernel<L, fb.R, fb.C><<<grid, TPB, 0, s>>>(c.prodA, c.npad, ctx->ptq, (int)ctx->M, (int)pl.chunk_len, c.herm, pm.far, pm.nbyte,
                                                             pm.nrg);
     else
-        fock_kernel<L, fb.R, fb.C><<<grid, TPB, 0, s>>>(c.prodA, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, (int)pl.chunk_len, c.herm,
-                                                        pm.far, pm.nbyte, pm.nrg);
+        PCM_CUDA(ctx, launch_class(fock_kernel<L, fb.R, fb.C>, grid, s, chained, c.prodA, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M,
+                                   (int)pl.chunk_len, c.herm, pm.far, pm.nbyte, pm.nrg));
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
@@ -1472,23 +1500,23 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
         if ((rc = launch_fock_near<3>(ctx, q, ctx->near_stream))) return rc;
         if ((rc = launch_fock_near<4>(ctx, q, ctx->near_stream))) return rc;
         PCM_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->near_stream));
-        if (ctx->timing || ctx->opt.serial_classes || ctx->info.product_points < CONCURRENT_CLASSES_MIN) {
+        if (ctx->timing || ctx->opt.serial_classes || (ctx->opt.tma_tiles && ctx->ptq)) {   // ordinary launches, per-class events
             if ((rc = launch_fock_class<0>(ctx, q, s)) || (rc = mark(ctx, 2, s))) return rc;
             if ((rc = launch_fock_class<1>(ctx, q, s)) || (rc = mark(ctx, 3, s))) return rc;
             if ((rc = launch_fock_class<2>(ctx, q, s)) || (rc = mark(ctx, 4, s))) return rc;
             if ((rc = launch_fock_class<3>(ctx, q, s)) || (rc = mark(ctx, 5, s))) return rc;
             if ((rc = launch_fock_class<4>(ctx, q, s)) || (rc = mark(ctx, 6, s))) return rc;
-        } else {   // concurrent class kernels, as in launch_potential
-            for (int L = 0; L <= MAXL; ++L) PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->cls_stream[L], ctx->ev_fork, 0));
-            if ((rc = launch_fock_class<1>(ctx, q, ctx->cls_stream[1]))) return rc;
-            if ((rc = launch_fock_class<2>(ctx, q, ctx->cls_stream[2]))) return rc;
-            if ((rc = launch_fock_class<0>(ctx, q, ctx->cls_stream[0]))) return rc;
-            if ((rc = launch_fock_class<3>(ctx, q, ctx->cls_stream[3]))) return rc;
-            if ((rc = launch_fock_class<4>(ctx, q, ctx->cls_stream[4]))) return rc;
-            for (int L = 0; L <= MAXL; ++L) {
-                PCM_CUDA(ctx, cudaEventRecord(ctx->ev_cls[L], ctx->cls_stream[L]));
-                PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_cls[L], 0));
-            }
+        } else {   // a chain of programmatic dependent launches, as in launch_potential
+            bool ch = false;
+            if ((rc = launch_fock_class<1>(ctx, q, s, ch))) return rc;
+            ch = ch || ctx->cls[1].n > 0;
+            if ((rc = launch_fock_class<0>(ctx, q, s, ch))) return rc;
+            ch = ch || ctx->cls[0].n > 0;
+            if ((rc = launch_fock_class<2>(ctx, q, s, ch))) return rc;
+            ch = ch || ctx->cls[2].n > 0;
+            if ((rc = launch_fock_class<3>(ctx, q, s, ch))) return rc;
+            ch = ch || ctx->cls[3].n > 0;
+            if ((rc = launch_fock_class<4>(ctx, q, s, ch))) return rc;
         }
         PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
     } else {
@@ -1546,7 +1574,7 @@ static int launch_potential_near(pcm_ctx *ctx, cudaStream_t s) {
 
 // slot: first partial-sum slot of the class (fixed by the class order, whatever the launch order)
 template <int L>
-static int launch_potential_class(pcm_ctx *ctx, int64_t slot, cudaStream_t s) {
+static int launch_potential_class(pcm_ctx *ctx, int64_t slot, cudaStream_t s, bool chained = false) {
     constexpr Blocking pb = pot_blocking(L);
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
@@ -1562,11 +1590,11 @@ static int launch_potential_class(pcm_ctx *ctx, int64_t slot, cudaStream_t s) {
     }
     constexpr Blocking pbb = pot_blocking_big(L);
     if (ctx->M >= POT_BIG_MIN && (pbb.R != pb.R || pbb.C != pb.C))
-        potential_kernel<L, pbb.R, pbb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
-                                                               ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
+        PCM_CUDA(ctx, launch_class(potential_kernel<L, pbb.R, pbb.C>, grid, s, chained, c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt,
+                                   (int)ctx->M, ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg));
     else
-        potential_kernel<L, pb.R, pb.C><<<grid, TPB, 0, s>>>(c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt, (int)ctx->M,
-                                                             ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg);
+        PCM_CUDA(ctx, launch_class(potential_kernel<L, pb.R, pb.C>, grid, s, chained, c.prodA, c.herm, c.npad, (int)pl.chunk_len, ctx->pt,
+                                   (int)ctx->M, ctx->vpart + (size_t)slot * ctx->M, pm.far, pm.nbyte, pm.nrg));
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
@@ -1597,25 +1625,27 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
     int64_t base[MAXL + 2] = {0};
     for (int L = 0; L <= MAXL; ++L) base[L + 1] = base[L] + (ctx->cls[L].n > 0 ? ctx->plan_pot[L].chunks : 0);
     const int64_t slot = base[MAXL + 1];
-    if (ctx->timing || ctx->opt.serial_classes || ctx->info.product_points < CONCURRENT_CLASSES_MIN) {   // per-class events: the class kernels run one after the other on s
+    if (ctx->timing || ctx->opt.serial_classes || ctx->opt.potential_pr) {   // ordinary launches, one after the other, per-class events
         if ((rc = launch_potential_class<0>(ctx, base[0], s)) || (rc = mark(ctx, 2, s))) return rc;
         if ((rc = launch_potential_class<1>(ctx, base[1], s)) || (rc = mark(ctx, 3, s))) return rc;
         if ((rc = launch_potential_class<2>(ctx, base[2], s)) || (rc = mark(ctx, 4, s))) return rc;
         if ((rc = launch_potential_class<3>(ctx, base[3], s)) || (rc = mark(ctx, 5, s))) return rc;
         if ((rc = launch_potential_class<4>(ctx, base[4], s)) || (rc = mark(ctx, 6, s))) return rc;
     } else {
-        // the five class kernels on five streams: the tail of one class overlaps the body of the next (each launch is only a few
-        // waves: PAPER.md:160 launches its per-class kernels sequentially); the longest-running classes are queued first
-        for (int L = 0; L <= MAXL; ++L) PCM_CUDA(ctx, cudaStreamWaitEvent(ctx->cls_stream[L], ctx->ev_fork, 0));
-        if ((rc = launch_potential_class<1>(ctx, base[1], ctx->cls_stream[1]))) return rc;
-        if ((rc = launch_potential_class<2>(ctx, base[2], ctx->cls_stream[2]))) return rc;
-        if ((rc = launch_potential_class<0>(ctx, base[0], ctx->cls_stream[0]))) return rc;
-        if ((rc = launch_potential_class<3>(ctx, base[3], ctx->cls_stream[3]))) return rc;
-        if ((rc = launch_potential_class<4>(ctx, base[4], ctx->cls_stream[4]))) return rc;
-        for (int L = 0; L <= MAXL; ++L) {
-            PCM_CUDA(ctx, cudaEventRecord(ctx->ev_cls[L], ctx->cls_stream[L]));
-            PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_cls[L], 0));
-        }
+        // A chain of programmatic dependent launches on s (pdl_launch_dependents above): every class kernel after the first may
+        // start while the last wave of the one before it is still running, so the tail of one class overlaps the body of the
+        // next (PAPER.md:160 launches its per-class kernels sequentially).  The classes with the most work go first, the
+        // shortest last: its tail is the only one left.  The partial-sum slots are fixed by the class order, not the launch order.
+        bool ch = false;
+        if ((rc = launch_potential_class<1>(ctx, base[1], s, ch))) return rc;
+        ch = ch || ctx->cls[1].n > 0;
+        if ((rc = launch_potential_class<0>(ctx, base[0], s, ch))) return rc;
+        ch = ch || ctx->cls[0].n > 0;
+        if ((rc = launch_potential_class<2>(ctx, base[2], s, ch))) return rc;
+        ch = ch || ctx->cls[2].n > 0;
+        if ((rc = launch_potential_class<3>(ctx, base[3], s, ch))) return rc;
+        ch = ch || ctx->cls[3].n > 0;
+        if ((rc = launch_potential_class<4>(ctx, base[4], s, ch))) return rc;
     }
     PCM_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_join, 0));
     if (slot == 0) {

@@ -307,7 +307,7 @@ def test_amatvec_coincident_and_mixed_exponents(pcm, orc, torch_cuda):
 
 def test_fock_tma_tiles_and_serial_classes_give_the_same_bits(pcm, orc, torch_cuda):
     """pcm_options.tma_tiles (point tiles brought in by cp.async.bulk + mbarrier from a packed (x, y, z, q) array) and
-    pcm_options.serial_classes (class kernels one after the other instead of on five streams) change how the work is moved and
+    pcm_options.serial_classes (class kernels as ordinary launches instead of a chain of dependent launches) change how the work is moved and
     scheduled, not what is computed: F and v are bit-identical to the default path, ragged tiles included."""
     torch = torch_cuda
     for cfg, kw in ((0, dict(with_d=True)), (1, dict(n_atoms=40))):
@@ -325,6 +325,29 @@ def test_fock_tma_tiles_and_serial_classes_give_the_same_bits(pcm, orc, torch_cu
             assert np.array_equal(pcm.pcm_fock(c, qd).cpu().numpy(), F0), opts
             pcm.pcm_destroy(c)
         pcm.pcm_destroy(ref)
+
+
+def test_chained_class_launches_are_ordered_before_the_reduction(pcm, torch_cuda):
+    """The default path launches the class kernels of a call as a chain of programmatic dependent launches (each may start
+    while the one before it is still in its last wave).  Completion must stay in launch order so that the reduction after the
+    chain sees every partial sum: all five classes, several waves per kernel, 40 back-to-back calls, every result bit-identical
+    to the one of ordinary launches (serial_classes)."""
+    torch = torch_cuda
+    w = synth.make_workload(3, n_atoms=160, n_pts=110, seed=99)
+    qd, Pd = dev(torch, w.q), dev(torch, w.P)
+    ser = pcm.setup_from_workload(w.basis, w.surface, serial_classes=True)
+    F0, v0 = pcm.pcm_fock(ser, qd).clone(), pcm.pcm_potential(ser, Pd).clone()
+    pcm.pcm_destroy(ser)
+    ctx = pcm.setup_from_workload(w.basis, w.surface)
+    assert all(n > 0 for n in pcm.pcm_get_info(ctx).products)
+    F, v = torch.empty_like(F0), torch.empty_like(v0)
+    for it in range(40):
+        F.fill_(float("nan")); v.fill_(float("nan"))
+        pcm.pcm_potential(ctx, Pd, v)
+        pcm.pcm_fock(ctx, qd, F)
+        pcm.pcm_fock(ctx, qd, F, accumulate=False)
+        assert torch.equal(v, v0) and torch.equal(F, F0), it
+    pcm.pcm_destroy(ctx)
 
 
 def test_shell_level_prescreen_never_drops_a_pair_eq15_keeps(pcm):
