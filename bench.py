@@ -47,6 +47,7 @@ CG_TOL = 1e-8
 SWEEP_M = (2_500, 10_000, 50_000, 100_000, 200_000)
 STORED_M = (2_500, 5_000, 10_000, 50_000)   # stored-A variant against the on-the-fly sweep
 SOLVER_M = (2_500, 10_000, 50_000, 200_000)   # configs[4]: full pcm_cg_solve, RBJ-64 against Jacobi
+RBJ_SWEEP_M, RBJ_SWEEP_BLOCKS = 50000, (8, 32, 100, 256, 800)   # block-size study of PAPER.md:192-196 at one size
 
 WORKLOADS = {
     0: "configs[0]: 12-atom chain, 6-31G-shaped s/sp shells, 50 points/atom",
@@ -456,6 +457,20 @@ def amat_and_solver_sweep(pcm, torch, dev, flush, model, peak_tflops, with_solve
                     e1.record(stream); torch.cuda.synchronize()
                     tsol.append(e0.elapsed_time(e1))
                 rec[name] = {"iters": int(it), "ms": min(tsol), "ms_per_iter": min(tsol) / max(it, 1), "converged": bool(ok), "true_resid": rt}
+            if Ms == RBJ_SWEEP_M:   # PAPER.md:192-196 (Figure 8, S1, S2): the block size against CG steps, build and solve time
+                rec["rbj_block_sweep"] = []
+                for blk in RBJ_SWEEP_BLOCKS:
+                    torch.cuda.synchronize()
+                    e0.record(stream); pcm.pcm_rbj_build(c4, blk, seed=7, stream=stream); e1.record(stream); torch.cuda.synchronize()
+                    tbuild = e0.elapsed_time(e1)
+                    tsol, it, ok = [], 0, False
+                    for _ in range(2):
+                        flush.zero_()
+                        e0.record(stream)
+                        _, it, rr, rt, ok = pcm.pcm_cg_solve(c4, b, x, tol=CG_TOL, max_iter=5000, precond=2, stream=stream)
+                        e1.record(stream); torch.cuda.synchronize()
+                        tsol.append(e0.elapsed_time(e1))
+                    rec["rbj_block_sweep"].append({"block": blk, "iters": int(it), "solve_ms": min(tsol), "build_ms": tbuild, "converged": bool(ok)})
             if Ms < 20000:   # the same solve through the separate-launch path (pcm_options.cg_path = 1), for comparison
                 c1 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0),
                                    s4.xyz, s4.zeta, s4.switch, cg_path=1)
