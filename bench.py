@@ -579,9 +579,9 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     side = torch.cuda.Stream(device=dev, priority=-1)   # the RBJ build depends on the geometry only: it overlaps pcm_potential
 
-    # Up to 100k points the RBJ block selection is one CTA: queued on a side stream it hides behind pcm_potential.  Above, it is a
+    # Up to 150k points the RBJ block selection is one CTA: queued on a side stream it hides behind pcm_potential.  Above, it is a
     # cooperative kernel on every SM: overlapped it would only slow the potential down, so it is queued after it.
-    overlap = M <= 100_000
+    overlap = M <= 150_000     # up to there the RBJ selection is one CTA (pcm_solver.cu RBJ_LOCAL_MAX) and runs beside the potential
 
     def step():
         if overlap:

@@ -78,7 +78,7 @@ typedef struct pcm_options {
                               mbarrier, double-buffered) from a per-call packed (x, y, z, q) array instead of per-thread loads;
                               0 (default).  Same results bit for bit */
     int rbj_global_scan;   /* 1: pcm_rbj_build selects every block with the cooperative global row scan instead of the one-CTA
-                              neighbourhood search (same blocks; the default uses the scan only above 100 000 points or l > 256) */
+                              neighbourhood search (same blocks; the default uses the scan only above 150 000 points or l > 256) */
     int potential_pr;      /* bit L set: pcm_potential sweeps the products of total angular momentum L in the Fock layout (product
                               in registers, warp-shuffle reduction over the 32 products of a warp per point) instead of the
                               point-in-registers layout.  Same values up to the summation order.  Default 0 (measured: DESIGN.md) */
@@ -108,6 +108,9 @@ typedef struct pcm_info {
     int64_t amat_persistent;           /* 1: pcm_cg_solve / pcm_amatvec use the persistent-kernel path (pcm_options.cg_path) */
     int64_t components;                /* elements (mu, nu) of P / F in blocks of surviving shell pairs I <= J: what pcm_potential reads
                                           and pcm_fock writes (times two for the transposes of off-diagonal shell pairs) */
+    int64_t rbj_selection;             /* how the last pcm_rbj_build chose its blocks: 1 = one-CTA neighbourhood selection, 2 = global row
+                                          scan, 3 = global row scan after the neighbourhood selection reported "capacity" (an asynchronous
+                                          build shows 1 until the call that completes it has seen the report); same blocks in every case */
 } pcm_info;
 
 /* Fills *opt with the defaults listed above. */

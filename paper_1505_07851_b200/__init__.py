@@ -50,7 +50,7 @@ class pcm_info(C.Structure):
                 ("zeta_min", C.c_double), ("zeta_max", C.c_double),
                 ("rbj_block", C.c_int64), ("rbj_nblocks", C.c_int64), ("device_bytes", C.c_int64),
                 ("amat_near_patches", C.c_int64), ("amat_stored_bytes", C.c_int64), ("amat_far_stored_bytes", C.c_int64),
-                ("amat_persistent", C.c_int64), ("components", C.c_int64)]
+                ("amat_persistent", C.c_int64), ("components", C.c_int64), ("rbj_selection", C.c_int64)]
 
 
 class PcmError(RuntimeError):

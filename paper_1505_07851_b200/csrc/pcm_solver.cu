@@ -253,6 +253,7 @@ __global__ void __launch_bounds__(RBJ_THREADS) rbj_select_kernel(const double4 *
 // descending, caller index ascending).  Used for block sizes <= 256; err = 3 asks the host to fall back.
 // ---------------------------------------------------------------------------------------------
 constexpr int RBL_THREADS = 1024;
+constexpr int64_t RBJ_LOCAL_MAX = 150000;   // points up to which pcm_rbj_build uses this form
 constexpr int RBL_RAW = 3072;   // candidate capacity (raw)
 constexpr int RBL_CAP = 1024;   // candidates above the histogram cut that are ranked
 constexpr int RBL_GL = 1024;    // candidate groups kept in shared memory (more: the global list)
@@ -322,6 +323,11 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
         if (tid == 0) { asg[k] = 1; atomicSub(&gc[k >> 5], 1); }
         __syncthreads();
         if (take > 0) {
+            // this step's bracket of the radius: lo = a radius that was not enough, hi = one whose candidates overflowed the
+            // store (unassigned points are unevenly spread late in the selection: one growth step can take in a whole
+            // untouched region); between them the radius is bisected.  Uniform over the CTA.
+            double lo = 0.0, hi = 0.0;
+            int tries = 0;
             while (true) {
                 // ---- candidate groups: bounding box closer than rho and something unassigned in it
                 const double rho = S.rho, rho2 = rho * rho;
@@ -362,10 +368,18 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                 }
                 __syncthreads();
                 const int nraw = S.nraw;
-                if (nraw > RBL_RAW) { if (tid == 0) *err = 3; return; }
-                if (nraw < take) {   // not enough unassigned points within rho (all_in cannot be set: take <= unassigned)
+                if (nraw > RBL_RAW) {   // more candidates than the store holds: a smaller radius
+                    hi = rho;
+                    if (++tries > 64 || !(hi - lo > 1e-9 * hi)) { if (tid == 0) *err = 3; return; }
                     __syncthreads();
-                    if (tid == 0) { S.rho = rho * 1.6; err[1] += 1; }
+                    if (tid == 0) { S.rho = lo > 0.0 ? 0.5 * (lo + hi) : rho / 1.6; err[1] += 1; }
+                    __syncthreads();
+                    continue;
+                }
+                if (nraw < take) {   // not enough unassigned points within rho (all_in cannot be set: take <= unassigned)
+                    lo = rho;
+                    __syncthreads();
+                    if (tid == 0) { S.rho = hi > 0.0 ? 0.5 * (lo + hi) : rho * 1.6; err[1] += 1; }
                     __syncthreads();
                     continue;
                 }
@@ -400,7 +414,15 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                 }
                 __syncthreads();
                 const int n = S.ncut;
-                if (n > RBL_CAP || n < take) { if (tid == 0) *err = n < take ? 1 : 3; return; }
+                if (n < take) { if (tid == 0) *err = 1; return; }
+                if (n > RBL_CAP) {      // too many keys in the cut bucket to rank: a smaller radius, as above
+                    hi = rho;
+                    if (++tries > 64 || !(hi - lo > 1e-9 * hi)) { if (tid == 0) *err = 3; return; }
+                    __syncthreads();
+                    if (tid == 0) { S.rho = lo > 0.0 ? 0.5 * (lo + hi) : rho / 1.6; err[1] += 1; }
+                    __syncthreads();
+                    continue;
+                }
                 // ---- rank by (key descending, caller index ascending); tau = the take-th largest key
                 // one warp per candidate, the lanes stride over the others (n^2 / 1024 comparisons per thread)
                 for (int cand = tid >> 5; cand < n; cand += RBL_THREADS / 32) {
@@ -419,10 +441,15 @@ __global__ void __launch_bounds__(RBL_THREADS) rbj_select_local_kernel(const dou
                 if (tid == 0) {
                     const double tau = S.tau;
                     S.ok = S.all_in || tau * rho > 1.0;          // tau > 1/rho: nothing outside rho can reach the block
-                    S.rho = S.ok ? fmax(1.25 / tau, 1.0) : fmax(rho * 1.6, 1.0001 / tau);
+                    S.rho = S.ok ? fmax(1.25 / tau, 1.0) : hi > 0.0 ? 0.5 * (rho + hi) : fmax(rho * 1.6, 1.0001 / tau);
                 }
                 __syncthreads();
-                if (!S.ok) { if (tid == 0) err[1] += 1; continue; }
+                if (!S.ok) {
+                    lo = rho;
+                    if (++tries > 64 || (hi > 0.0 && !(hi - lo > 1e-9 * hi))) { if (tid == 0) *err = 3; return; }
+                    if (tid == 0) err[1] += 1;
+                    continue;
+                }
                 if (tid == 0) { err[2] += n; err[3] += nraw; }
                 if (rank < take) {
                     const int j = S.cidx[tid];
@@ -1109,11 +1136,10 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
     double t1 = 0, t2 = 0;
     if (verbose) { cudaStreamSynchronize(s); t1 = now(); }
     // block sizes up to 256: the single-CTA neighbourhood selection; it reports err = 3 (capacity) to fall back
-    bool local_done = false;
+    bool local_done = false, fell_back = force_global;
     // (measured: 0.8 vs 1.6 ms at M = 8 930, 6.1 vs 9.6 ms at 50k, 86 vs 78 ms at 200k, where scanning 6 250 group boxes per
-    // block with one CTA costs more than the two grid barriers of the global scan; at the 102 470 points of configs[3] the
-    // one-CTA form runs out of candidate capacity after 11 ms and the scan has to run anyway)
-    if (block <= 256 && M <= 100000 && !force_global && !ctx->opt.rbj_global_scan) {
+    // block with one CTA costs more than the two grid barriers of the global scan)
+    if (block <= 256 && M <= RBJ_LOCAL_MAX && !force_global && !ctx->opt.rbj_global_scan) {
         const int ng = (int)cdiv(M, 32);
         int *d_gcount = (int *)w.cand_idx, *d_glist = d_gcount + ng;   // scratch of the global path, 2 M ints
         const size_t base_smem = (sizeof(RblShared) + 15) / 16 * 16;
@@ -1138,11 +1164,13 @@ int rbj_build(pcm_ctx *ctx, int block, uint64_t seed, const int64_t *pivot_order
         }
         if (h_e == 0) local_done = true;
         else if (h_e == 3) {   // start over with the global row scan
+            fell_back = true;
             RBJ_TRY(cudaMemsetAsync(w.assigned, 0, (size_t)M, s));
             RBJ_TRY(cudaMemsetAsync(small, 0, 64, s));
         }
         }
     }
+    ctx->info.rbj_selection = local_done ? 1 : fell_back ? 3 : 2;
     // one cooperative launch: all CTAs must be co-resident for the grid barrier
     if (!local_done) {
         int per_sm = 0;

@@ -291,25 +291,58 @@ def test_store_far_rule_leaves_large_cavities_on_the_fly(pcm):
     pcm.pcm_destroy(c)
 
 
+def test_rbj_neighbourhood_radius_is_bisected_when_candidates_overflow(pcm, torch_cuda):
+    """A sparse shell of points around a dense ball of 6 000: when a pivot of the shell has used up its sparse neighbours, the next
+    growth step of its search radius takes in the whole ball -- more candidates than the one-CTA selection stores.  The radius is
+    then bisected between the last one that was too small and the one that overflowed; the selection stays with the one-CTA
+    form (rbj_selection = 1) and finds the blocks of the global row scan."""
+    rng = np.random.default_rng(5)
+    nb, ns = 6000, 1500
+    d = rng.normal(size=(nb, 3))
+    ball = d / np.linalg.norm(d, axis=1)[:, None] * 1.5 * rng.uniform(0, 1, (nb, 1)) ** (1 / 3)
+    d = rng.normal(size=(ns, 3))
+    shell = d / np.linalg.norm(d, axis=1)[:, None] * rng.uniform(6.0, 40.0, (ns, 1))
+    xyz = np.concatenate([shell, ball])
+    M = nb + ns
+    s = synth.Surface(xyz=xyz, zeta=rng.uniform(4.0, 6.0, M), switch=rng.uniform(0.2, 1.0, M), atom=np.zeros(M, np.int32))
+    po = np.arange(M, dtype=np.int64)               # the shell's points are the first pivots
+    c_loc, c_scan = points_ctx(pcm, s), points_ctx(pcm, s, rbj_global_scan=True)
+    pcm.pcm_rbj_build(c_loc, 64, pivot_order=po)
+    pcm.pcm_rbj_build(c_scan, 64, pivot_order=po)
+    assert pcm.pcm_get_info(c_loc).rbj_selection == 1 and pcm.pcm_get_info(c_scan).rbj_selection == 2
+    o1, b1, i1 = pcm.pcm_rbj_get(c_loc)
+    o2, b2, i2 = pcm.pcm_rbj_get(c_scan)
+    assert sorted(o1.tolist()) == list(range(M))
+    assert np.array_equal(o1, o2) and np.array_equal(b1, b2)
+    assert all(np.array_equal(a, b) for a, b in zip(i1, i2))
+    for c in (c_loc, c_scan):
+        pcm.pcm_destroy(c)
+
+
 def test_rbj_capacity_fallback_sync_and_async(pcm, orc, torch_cuda):
-    """5 000 points packed into a ball of radius 0.6 bohr: every unassigned point is a candidate of every pivot, which exceeds the
-    candidate capacity of the one-CTA neighbourhood selection -- it reports 'capacity' and the build repeats with the global row
-    scan.  Synchronous build, asynchronous build (completed by pcm_rbj_get) and a build forced onto the scan give the same
-    blocks; the blocks are valid against the oracle's A, and the preconditioned solve converges."""
+    """One point at the centre of a sphere that carries 4 999 others, the centre first in the pivot order: every radius of the
+    one-CTA neighbourhood selection holds either no candidate or 4 999 of them, more than its store takes, and bisecting the
+    radius cannot separate points that are equally far -- it reports 'capacity' and the build repeats with the global row
+    scan (pcm_info.rbj_selection = 3).  Synchronous build, asynchronous build (completed by pcm_rbj_get) and a build forced
+    onto the scan give the same blocks; the blocks are valid against the oracle's A, and the preconditioned solve converges."""
     torch = torch_cuda
     rng = np.random.default_rng(23)
     M = 5000
     d = rng.normal(size=(M, 3))
-    xyz = d / np.linalg.norm(d, axis=1)[:, None] * 0.6 * rng.uniform(0, 1, (M, 1)) ** (1 / 3)
+    xyz = d / np.linalg.norm(d, axis=1)[:, None] * 2.0
+    xyz[0] = 0.0
     s = synth.Surface(xyz=xyz, zeta=rng.uniform(4.0, 6.0, M), switch=rng.uniform(0.2, 1.0, M), atom=np.zeros(M, np.int32))
+    po = np.arange(M, dtype=np.int64)
     c_sync, c_async, c_scan = points_ctx(pcm, s), points_ctx(pcm, s), points_ctx(pcm, s, rbj_global_scan=True)
-    pcm.pcm_rbj_build(c_sync, 64, seed=3)
+    pcm.pcm_rbj_build(c_sync, 64, pivot_order=po)
     side = torch.cuda.Stream()
-    pcm.pcm_rbj_build_async(c_async, 64, seed=3, stream=side)
-    pcm.pcm_rbj_build(c_scan, 64, seed=3)
+    pcm.pcm_rbj_build_async(c_async, 64, pivot_order=po, stream=side)
+    pcm.pcm_rbj_build(c_scan, 64, pivot_order=po)
     o1, b1, i1 = pcm.pcm_rbj_get(c_sync)
     o2, b2, i2 = pcm.pcm_rbj_get(c_async)          # completes the pending build (and its fallback)
     o3, b3, i3 = pcm.pcm_rbj_get(c_scan)
+    assert [pcm.pcm_get_info(c).rbj_selection for c in (c_sync, c_async, c_scan)] == [3, 3, 2]
+    assert o1[0] == 0
     assert sorted(o1.tolist()) == list(range(M))
     assert np.array_equal(o1, o2) and np.array_equal(o1, o3) and np.array_equal(b1, b3)
     assert all(np.array_equal(a, b) and np.array_equal(a, c) for a, b, c in zip(i1, i2, i3))
