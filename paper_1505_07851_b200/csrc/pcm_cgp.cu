@@ -33,23 +33,36 @@ constexpr int CGP_WARPS = CGP_THREADS / 32;
 constexpr int CGP_R = 4;                          // row groups per warp
 constexpr int CGP_ROWS = CGP_R * 32;              // rows of a row block
 constexpr int CGP_C = 2;
+constexpr double CGP_FAR_AWAY = 1.0715086071862673e301;     // 2^1000: the r^2 of a row that is to contribute nothing
 enum { CGP_CTL_STOP = 0, CGP_CTL_ITERS = 1, CGP_CTL_BAR_COUNT = 3, CGP_CTL_BAR_GEN = 4, CGP_CTL_BAR_ERR = 5 };
+
+// What a warp needs to start its share of the sweep, in one 64-byte load (instead of three dependent ones through seg_start,
+// strip and the near-piece tables: after an L2 flush each of those is a trip to HBM with nothing to overlap it).
+struct alignas(16) CgpWarpInit {
+    int64_t hb, he;            // its half strips
+    int2 strip0, strip1;       // descriptors of its first two strips
+    int64_t ne, ne_end;        // list entries of its first near piece (piece = warp index)
+    int32_t slot0, ncg0;       // first row-sum slot; column group of entry ne
+    int32_t pad[2];
+};
+static_assert(sizeof(CgpWarpInit) == 64, "CgpWarpInit is one 64-byte record");
 
 struct CgpArgs {
     int M, ng, nrb, nwarp;
+    const CgpWarpInit *winit;
     const double4 *pt, *colloc, *org;
     const int2 *strip;
     const int64_t *seg_start;
     const int32_t *seg_slot0, *rb_slot_start;
     double *yslot, *colpart;
-    double *afar;              // stored far field: [half strip][16 columns][4 row groups][32 lanes] values of 1/r (0 where near), or nullptr
+    double *afar;              // stored far field: [half strip][16 columns][4 row groups][32 lanes] values of 1/r (~2^-500 where near), or nullptr
     // stored near patches (PatchMap of A): pieces of <= NEAR_PIECE patches of one row group
     const double *nblk;
     const int64_t *nstart, *npstart;
     const int32_t *nlist, *npiece_rg;
     int64_t npiece;
     double *near;
-    // matvec form: y[qidx ? qidx[k] : k] = (A q)_k, q read through qidx
+    // matvec form: y[qidx ? qidx[k] : k] = (A q)_k, q in sorted order
     const double *q;
     const int32_t *qidx;
     double *y;
@@ -128,22 +141,22 @@ __device__ __forceinline__ void cgp_cp_wait_all() { asm volatile("cp.async.wait_
 // Per-warp shared memory (doubles): two staging buffers {columns (-2 (b - o), |b - o|^2) [32] double4, origin double4,
 // A-values [32], B-values [32]} (the charge of column t is fma(beta, B_t, A_t): CG direction z + beta p_old, or the caller's q
 // with beta = 0), the charges [32], the column-sum transpose [16][33], one half of a stored near patch [16][32] with the
-// A / B values of its 32 columns.
+// A / B values of its 32 columns and the charges formed from them.
 constexpr int CGP_STG = 128 + 4 + 32 + 32;             // one staging buffer
 constexpr int CGP_OFF_Q = 2 * CGP_STG;                 // charges
 constexpr int CGP_OFF_SC = CGP_OFF_Q + 32;             // transpose
 constexpr int CGP_OFF_NB = CGP_OFF_SC + 16 * 33;       // near half patch
 constexpr int CGP_OFF_NA = CGP_OFF_NB + 16 * 32;       // near A / B values
-constexpr int CGP_WSMEM2 = CGP_OFF_NA + 64;
+constexpr int CGP_OFF_NQ = CGP_OFF_NA + 64;            // charges of the near patch's 32 columns
+constexpr int CGP_WSMEM2 = CGP_OFF_NQ + 32;
 
-// where the vector the sweep multiplies comes from: value_j = fma(beta, B[j], A[ia(j)])
+// where the vector the sweep multiplies comes from: value_j = fma(beta, B[j], A[j]), all in sorted order (a caller-order q is
+// gathered first, cgp_gather_kernel: an index load in front of every staged column would sit on the sweep's critical path)
 struct PSrc {
-    const double *A, *B;         // CG: z, p_old; matvec: q, nullptr
-    const int32_t *idx;          // matvec: sorted -> caller index of q (nullptr: identity)
+    const double *A, *B;         // CG: z, p_old; matvec: q (sorted), nullptr
     double beta;
-    __device__ __forceinline__ int ia(int j) const { return idx ? idx[j] : j; }
     __device__ __forceinline__ double operator()(int j) const {
-        const double av = __ldcg(A + ia(j));
+        const double av = __ldcg(A + j);
         return B ? fma(beta, __ldcg(B + j), av) : av;
     }
 };
@@ -157,10 +170,10 @@ template <int MODE>
 __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int gw, int lane, double *wsm) {
     constexpr int R = CGP_R, C = CGP_C;
     const int M = a.M;
-    double *s_q = wsm + CGP_OFF_Q, *sc = wsm + CGP_OFF_SC, *s_nb = wsm + CGP_OFF_NB, *s_na = wsm + CGP_OFF_NA;
+    double *s_q = wsm + CGP_OFF_Q, *sc = wsm + CGP_OFF_SC, *s_nb = wsm + CGP_OFF_NB, *s_na = wsm + CGP_OFF_NA, *s_nq = wsm + CGP_OFF_NQ;
     // ---- near pieces of this warp: piece gw, gw + nwarp, ...; state = (entry e, half) of the half patch in flight
     int64_t piece = gw, ne = 0, ne_end = 0;
-    int nhalf = 0;
+    int nhalf = 0, ncg = 0, ncg_next = 0;     // column group of patch ne, and of patch ne + 1 (loaded one half strip ahead)
     double ynear = 0.0;
     bool near_inflight = false;
     auto near_open = [&]() {          // bounds of the current piece (or none left)
@@ -170,6 +183,7 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
             ne_end = min(a.nstart[rg + 1], ne + NEAR_PIECE);
             nhalf = 0;
             ynear = 0.0;
+            ncg = a.nlist[ne];
         }
     };
     auto near_issue = [&]() {         // copy half `nhalf` of patch `ne` and the A / B values of its columns
@@ -177,19 +191,29 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
         const double *blk = a.nblk + (size_t)ne * 1024 + (size_t)nhalf * 512;
 #pragma unroll
         for (int k = 0; k < 8; ++k) cgp_cp16(s_nb + (k * 32 + lane) * 2, blk + (k * 32 + lane) * 2, 16);
-        const int j = a.nlist[ne] * 32 + lane;
-        cgp_cp8(s_na + lane, pv.A + (j < M ? pv.ia(j) : 0), j < M ? 8 : 0);
+        const int j = ncg * 32 + lane;
+        cgp_cp8(s_na + lane, pv.A + min(j, M - 1), j < M ? 8 : 0);
         cgp_cp8(s_na + 32 + lane, pv.B ? pv.B + min(j, M - 1) : pv.A, (pv.B && j < M) ? 8 : 0);
+        if (nhalf == 0 && ne + 1 < ne_end) ncg_next = a.nlist[ne + 1];      // used a half strip from now: no wait on this load
         near_inflight = true;
     };
     auto near_consume = [&]() {       // after cp_wait_all + __syncwarp: add the half patch, advance, store a finished piece
         if (!near_inflight) return;
-        const double qj = fma(pv.beta, s_na[32 + lane], s_na[lane]);
+        // the charges go through shared memory and come back as broadcast loads, two per instruction (a shuffle of a double
+        // by a run-time lane costs ~20 instructions here; this loop was 500 of them per half patch)
+        s_nq[lane] = fma(pv.beta, s_na[32 + lane], s_na[lane]);
+        __syncwarp();
         const double *col = s_nb + lane;
+        const double2 *qq = reinterpret_cast<const double2 *>(s_nq + nhalf * 16);
 #pragma unroll
-        for (int t = 0; t < 16; ++t) ynear = fma(__shfl_sync(0xffffffffu, qj, nhalf * 16 + t), col[t * 32], ynear);
+        for (int t = 0; t < 16; t += 2) {
+            const double2 q2 = qq[t >> 1];
+            ynear = fma(q2.x, col[t * 32], ynear);
+            ynear = fma(q2.y, col[(t + 1) * 32], ynear);
+        }
         if (++nhalf == 2) {
             nhalf = 0;
+            ncg = ncg_next;
             if (++ne == ne_end) {
                 a.near[piece * 32 + lane] = ynear;
                 piece += a.nwarp;
@@ -199,11 +223,18 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
         near_inflight = false;
         __syncwarp();                 // every lane has read its column before the next copy may overwrite the buffer
     };
-    near_open();
+    CgpWarpInit wi;
+    {
+        const int4 *src = reinterpret_cast<const int4 *>(a.winit + gw);
+        int4 *dst = reinterpret_cast<int4 *>(&wi);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) dst[k] = __ldg(src + k);
+    }
+    if (piece < a.npiece) { ne = wi.ne; ne_end = wi.ne_end; ncg = wi.ncg0; }
     near_issue();
     // ---- far half strips [hb, he)
-    const int64_t hb = a.seg_start[gw], he = a.seg_start[gw + 1];
-    int slot = a.seg_slot0[gw];
+    const int64_t hb = wi.hb, he = wi.he;
+    int slot = wi.slot0;
     int cur_rb = -1, buf = 0;
     double qa[R], y[R], ax[R], ay[R], az[R];
 #pragma unroll
@@ -215,17 +246,29 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
         cgp_cp16(sb + 4 * lane, src, j < M ? 16 : 0);
         cgp_cp16(sb + 4 * lane + 2, reinterpret_cast<const double *>(src) + 2, j < M ? 16 : 0);
         if (lane < 2) cgp_cp16(sb + 128 + 2 * lane, reinterpret_cast<const double *>(a.org + cg) + 2 * lane, 16);
-        cgp_cp8(sb + 132 + lane, pv.A + (j < M ? pv.ia(j) : 0), j < M ? 8 : 0);
+        cgp_cp8(sb + 132 + lane, pv.A + min(j, M - 1), j < M ? 8 : 0);
         cgp_cp8(sb + 164 + lane, pv.B ? pv.B + min(j, M - 1) : pv.A, (pv.B && j < M) ? 8 : 0);
     };
     // d_next: the strip whose columns are in flight into buffer nbuf; d_next2: the one after it (descriptor only)
     const int64_t last_s = (he - 1) >> 1;
     int2 d_next = make_int2(0, 0), d_next2 = make_int2(0, 0);
     int nbuf = 0;
+    auto load_rows = [&](int rb_) {      // charges and coordinates of the 4 x 32 rows of row block rb_
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int ii = (rb_ * R + r) * 32 + lane;
+            qa[r] = ii < M ? pv(ii) : 0.0;              // padding rows: zero charge, their sums are not used
+            const double4 p = a.pt[min(ii, M - 1)];
+            ax[r] = ii < M ? p.x : p.x + 3e8; ay[r] = p.y; az[r] = p.z;   // padding rows: far away
+            y[r] = 0.0;
+        }
+    };
     if (hb < he) {
-        d_next = a.strip[hb >> 1];
+        d_next = wi.strip0;
+        d_next2 = wi.strip1;
         stage_issue(d_next, 0);
-        if ((hb >> 1) + 1 <= last_s) d_next2 = a.strip[(hb >> 1) + 1];
+        cur_rb = d_next.x;        // the first row block's rows are loaded here, beside the copies, not after waiting for them
+        load_rows(cur_rb);
     }
     int64_t cur_s = -1;
     double alx[R], aly[R], alz[R], a2[R];
@@ -250,14 +293,7 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
                     ++slot;
                 }
                 cur_rb = rb;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const int ii = (rb * R + r) * 32 + lane;
-                    qa[r] = ii < M ? pv(ii) : 0.0;              // padding rows: zero charge, their sums are not used
-                    const double4 p = a.pt[min(ii, M - 1)];
-                    ax[r] = ii < M ? p.x : p.x + 3e8; ay[r] = p.y; az[r] = p.z;   // padding rows: far away
-                    y[r] = 0.0;
-                }
+                load_rows(rb);
             }
             sym = cg >= rb * R + R;
             const double *sb = wsm + buf * CGP_STG;
@@ -267,6 +303,10 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
             for (int r = 0; r < R; ++r) {
                 alx[r] = ax[r] - o.x; aly[r] = ay[r] - o.y; alz[r] = az[r] - o.z;
                 a2[r] = fma(alz[r], alz[r], fma(aly[r], aly[r], alx[r] * alx[r]));
+                // Row groups whose patch against this column group is near (stored, added by the near pieces) are moved out
+                // of reach instead of being selected away per evaluation: r^2 = 2^1000 whatever the column, 1/r ~ 2^-500, and
+                // a charge times that is absorbed without a trace by the first genuine term of any sum it enters.
+                if (!((m >> r) & 1u)) a2[r] = CGP_FAR_AWAY;
             }
             // prefetch the next strip of this segment into the other buffer, and the descriptor of the one after it
             if (sidx + 1 <= last_s) {
@@ -280,17 +320,17 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
         near_issue();
         const double4 *sp = reinterpret_cast<const double4 *>(wsm + buf * CGP_STG) + half * 16;
         const double *sq = s_q + half * 16;
-        // Strips with a near patch among the 4 row groups run the same blocked loop with the near rows' 1/r replaced by 0
-        // (selected, not multiplied: a near patch may hold r = 0): three rows of wasted arithmetic at worst, but no slow
-        // path whose cost the partition would have to know (near patches cluster at the start of a row block's strips).
-        const bool full = m == (1u << R) - 1u;
+        // Strips with a near patch among the 4 row groups run the same blocked loop (the near rows sit at r^2 = 2^1000, see
+        // above): three rows of wasted arithmetic at worst, but no slow path whose cost the partition would have to know
+        // (near patches cluster at the start of a row block's strips), and no select in the loop.
         double *ah = MODE ? a.afar + (size_t)h * (16 * R * 32) + lane : nullptr;
+        double *scp = sc + lane;
 #pragma unroll 1
-        for (int t = 0; t < 16; t += C) {
+        for (int t = 0; t < 16; t += C, sp += C, sq += C, scp += C * 33) {
             double4 b[C];
             double qb[C], r2[C][R], cc[C];
 #pragma unroll
-            for (int c = 0; c < C; ++c) { b[c] = sp[t + c]; qb[c] = sq[t + c]; }
+            for (int c = 0; c < C; ++c) { b[c] = sp[c]; qb[c] = sq[c]; }
             if (MODE == 2) {
 #pragma unroll
                 for (int c = 0; c < C; ++c)
@@ -312,13 +352,12 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
                         rs = r2[c][r];
                     } else {
                         rs = rsqrt_fast(r2[c][r]);
-                        if (!full && !((m >> r) & 1u)) rs = 0.0;
                         if (MODE == 1) ah[((t + c) * R + r) * 32] = rs;
                     }
                     y[r] = fma(qb[c], rs, y[r]);
                     cc[c] = fma(qa[r], rs, cc[c]);
                 }
-                if (sym) sc[(t + c) * 33 + lane] = cc[c];
+                if (sym) scp[c * 33] = cc[c];
             }
         }
         if (sym) {
@@ -507,11 +546,18 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
     while (!stop) {
         const double *pold = cur ? a.p1 : a.p0;
         double *pnew = cur ? a.p0 : a.p1;
-        PSrc pv{a.z, pold, nullptr, beta};
+        PSrc pv{a.z, pold, beta};
         cgp_stamp(a, iters, 0);
         unsigned long long t0 = 0;
         if (a.dbg && iters == 1 && tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+        unsigned long long w0 = 0;
+        if (a.dbg && iters == 1) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(w0));
         cgp_sweep<MODE>(a, pv, gw, lane, wsm);
+        if (a.dbg && iters == 1 && lane == 0) {      // this warp's own sweep time (calibrates the cost model of plan_sweep)
+            unsigned long long w1;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(w1));
+            a.dbg[CGP_DBG_ITERS * 8 + 1024 + gw] = w1 - w0;
+        }
         if (a.dbg && iters == 1) {
             __syncthreads();
             if (tid == 0) { unsigned long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); a.dbg[CGP_DBG_ITERS * 8 + blockIdx.x] = t1 - t0; }
@@ -561,13 +607,19 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
     }
 }
 
+// q in the caller's order -> sorted order
+__global__ void cgp_gather_kernel(const double *__restrict__ q, const int32_t *__restrict__ idx, double *__restrict__ qs, int M) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < M) qs[k] = q[idx[k]];
+}
+
 // y = A q with the same sweep and row sums: one launch, one grid barrier
 template <int MODE>
 __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_matvec_kernel(CgpArgs a) {
     extern __shared__ double dyn[];
     const unsigned G = gridDim.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    PSrc pv{a.q, nullptr, a.qidx, 0.0};
+    PSrc pv{a.q, nullptr, 0.0};
     if (a.phase != 2) cgp_sweep<MODE>(a, pv, blockIdx.x * CGP_WARPS + warp, lane, dyn + warp * CGP_WSMEM2);
     if (MODE == 1 || a.phase == 1) return;      // filling the store, or the sweep half of a two-launch product
     if (a.phase == 0) cgp_grid_sync(a.ctl, G);
@@ -689,7 +741,30 @@ int plan_sweep(pcm_ctx *ctx) {
         const double x = pt[j].x - o.x, y = pt[j].y - o.y, z = pt[j].z - o.z;
         colloc[j] = make_double4(-2.0 * x, -2.0 * y, -2.0 * z, std::fma(z, z, std::fma(y, y, x * x)));
     }
+    std::vector<CgpWarpInit> winit((size_t)sp.nwarp);
+    {
+        std::vector<int32_t> list_host((size_t)std::max<int64_t>(pm.nnear, 1), 0);
+        if (pm.nnear > 0) PCM_CUDA(ctx, cudaMemcpy(list_host.data(), pm.list, (size_t)pm.nnear * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        for (int w = 0; w < sp.nwarp; ++w) {
+            CgpWarpInit &wi = winit[(size_t)w];
+            wi = CgpWarpInit{};
+            wi.hb = seg_start[w]; wi.he = seg_start[w + 1];
+            wi.slot0 = seg_slot0[w];
+            if (wi.hb < wi.he) {
+                const int64_t s0 = wi.hb >> 1, last = (wi.he - 1) >> 1;
+                wi.strip0 = strip[(size_t)s0];
+                wi.strip1 = s0 + 1 <= last ? strip[(size_t)s0 + 1] : make_int2(0, 0);
+            }
+            if (w < pm.npiece) {
+                const int64_t rg = pm.piece_rg_host[(size_t)w];
+                wi.ne = pm.start_host[rg] + (w - pm.pstart_host[rg]) * NEAR_PIECE;
+                wi.ne_end = std::min(pm.start_host[rg + 1], wi.ne + NEAR_PIECE);
+                wi.ncg0 = list_host[(size_t)wi.ne];
+            }
+        }
+    }
     int rc;
+    if ((rc = upload2(ctx, &sp.winit, winit))) return rc;
     if ((rc = upload2(ctx, &sp.strip, strip))) return rc;
     if ((rc = upload2(ctx, &sp.seg_start, seg_start))) return rc;
     if ((rc = upload2(ctx, &sp.seg_slot0, seg_slot0))) return rc;
@@ -753,6 +828,7 @@ static CgpArgs cgp_args(pcm_ctx *ctx) {
     const PatchMap &pm = ctx->amat_map;
     CgpArgs a{};
     a.M = (int)ctx->M; a.ng = sp.ng; a.nrb = sp.nrb; a.nwarp = sp.nwarp;
+    a.winit = sp.winit;
     a.pt = ctx->pt; a.colloc = sp.colloc; a.org = sp.org;
     a.strip = sp.strip; a.seg_start = sp.seg_start; a.seg_slot0 = sp.seg_slot0; a.rb_slot_start = sp.rb_slot_start;
     a.yslot = sp.yslot; a.colpart = sp.colpart;
@@ -769,8 +845,11 @@ static CgpArgs cgp_args(pcm_ctx *ctx) {
 int cgp_matvec(pcm_ctx *ctx, const double *q, const int32_t *idx, double *y, cudaStream_t s) {
     CgpArgs a = cgp_args(ctx);
     a.q = q; a.qidx = idx; a.y = y;
-    void *args[] = {&a};
-    (void)args;
+    if (idx) {      // (pbuf is the solve's second direction vector: free between solves, calls on a context are stream-ordered)
+        cgp_gather_kernel<<<(unsigned)cdiv2(a.M, 256), 256, 0, s>>>(q, idx, ctx->cgp.pbuf, a.M);
+        a.q = ctx->cgp.pbuf;
+        ctx->launch_total += 1;
+    }
     // Two ordinary launches (sweep; row sums) instead of one cooperative launch with a grid barrier: a cooperative launch costs
     // ~20 us more between the events around it than its kernel runs (measured at M = 10k: 94 us against 72 us under ncu), which a
     // single A q does not win back; inside a solve the launch happens once, so pcm_cg_solve keeps the cooperative kernel.
@@ -800,21 +879,34 @@ int cgp_solve(pcm_ctx *ctx, double *r, double *z, double *p, double *Ap, double 
     PCM_CUDA(ctx, cudaMemsetAsync(p, 0, (size_t)ctx->M * 8, s));                // beta = 0 on the first iteration: p = z + 0 * 0
     const bool verbose = getenv("PCM_VERBOSE") != nullptr;
     if (verbose) {
-        PCM_CUDA(ctx, cudaMalloc(&a.dbg, (CGP_DBG_ITERS * 8 + 1024) * 8));
-        PCM_CUDA(ctx, cudaMemsetAsync(a.dbg, 0, (CGP_DBG_ITERS * 8 + 1024) * 8, s));
+        PCM_CUDA(ctx, cudaMalloc(&a.dbg, (CGP_DBG_ITERS * 8 + 1024 + (size_t)a.nwarp) * 8));
+        PCM_CUDA(ctx, cudaMemsetAsync(a.dbg, 0, (CGP_DBG_ITERS * 8 + 1024 + (size_t)a.nwarp) * 8, s));
     }
     void *args[] = {&a};
     const void *k = a.afar ? (const void *)cgp_solve_kernel<2> : (const void *)cgp_solve_kernel<0>;
     PCM_CUDA(ctx, cudaLaunchCooperativeKernel(k, dim3((unsigned)ctx->cgp.grid), dim3(CGP_THREADS), args, smem, s));
     ctx->launch_total += 1;
     if (verbose) {   // CTA 0's view of the phases: sweep, wait, row sums, wait, update, wait (microseconds)
-        unsigned long long h[CGP_DBG_ITERS * 8 + 1024];
-        PCM_CUDA(ctx, cudaMemcpyAsync(h, a.dbg, sizeof(h), cudaMemcpyDeviceToHost, s));
+        std::vector<unsigned long long> hv(CGP_DBG_ITERS * 8 + 1024 + (size_t)a.nwarp);
+        unsigned long long *h = hv.data();
+        PCM_CUDA(ctx, cudaMemcpyAsync(h, a.dbg, hv.size() * 8, cudaMemcpyDeviceToHost, s));
         PCM_CUDA(ctx, cudaStreamSynchronize(s));
         cudaFree(a.dbg);
         {
+            double sn = 0.0, sf = 0.0, mx = 0.0;
+            int64_t nn = 0, nf = 0;
+            for (int w = 0; w < a.nwarp; ++w) {
+                const double t = h[CGP_DBG_ITERS * 8 + 1024 + w] * 1e-3;
+                mx = std::max(mx, t);
+                if (w < a.npiece) { sn += t; ++nn; } else { sf += t; ++nf; }
+            }
+            fprintf(stderr, "[pcm] sweep time per warp (us): %lld warps with a near piece, mean %.1f; %lld without, mean %.1f; max %.1f\n", (long long)nn,
+                    nn ? sn / nn : 0.0, (long long)nf, nf ? sf / nf : 0.0, mx);
+        }
+        {
             std::vector<double> t;
             for (int c = 0; c < ctx->cgp.grid && c < 1024; ++c) t.push_back(h[CGP_DBG_ITERS * 8 + c] * 1e-3);
+            if (getenv("PCM_CTADUMP")) { for (size_t c = 0; c < t.size(); ++c) fprintf(stderr, "[cta] %zu %.2f\n", c, t[c]); }
             std::sort(t.begin(), t.end());
             if (!t.empty()) fprintf(stderr, "[pcm] sweep time per CTA (us): min %.1f p25 %.1f median %.1f p75 %.1f max %.1f\n", t.front(), t[t.size() / 4],
                                     t[t.size() / 2], t[3 * t.size() / 4], t.back());

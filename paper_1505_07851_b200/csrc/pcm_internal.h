@@ -74,6 +74,7 @@ struct SweepPlan {
     int grid = 0, nwarp = 0, ng = 0, nrb = 0, nslot = 0;
     int64_t nstrip = 0;
     size_t smem = 0;
+    struct CgpWarpInit *winit = nullptr;   // [nwarp] start-up record of every warp (pcm_cgp.cu)
     int2 *strip = nullptr;            // [nstrip] (row block, column group | far mask of the 4 row groups << 24)
     int64_t *seg_start = nullptr;     // [nwarp + 1] strips of every warp
     int32_t *seg_slot0 = nullptr;     // [nwarp + 1] first row-sum slot of every warp
