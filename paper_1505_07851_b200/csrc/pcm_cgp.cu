@@ -39,7 +39,7 @@ enum { CGP_CTL_STOP = 0, CGP_CTL_ITERS = 1, CGP_CTL_BAR_COUNT = 3, CGP_CTL_BAR_G
 // What a warp needs to start its share of the sweep, in one 64-byte load (instead of three dependent ones through seg_start,
 // strip and the near-piece tables: after an L2 flush each of those is a trip to HBM with nothing to overlap it).
 struct alignas(16) CgpWarpInit {
-    int64_t hb, he;            // its half strips
+    int64_t hb, he;            // its column pairs (pair h belongs to strip h >> 4)
     int2 strip0, strip1;       // descriptors of its first two strips
     int64_t ne, ne_end;        // list entries of its first near piece (piece = warp index)
     int32_t slot0, ncg0;       // first row-sum slot; column group of entry ne
@@ -232,8 +232,8 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
     }
     if (piece < a.npiece) { ne = wi.ne; ne_end = wi.ne_end; ncg = wi.ncg0; }
     near_issue();
-    // ---- far half strips [hb, he)
-    const int64_t hb = wi.hb, he = wi.he;
+    // ---- far column pairs [hb, he): pair h is columns 2 (h & 7), 2 (h & 7) + 1 of half (h >> 3) & 1 of strip h >> 4
+    const int hb = (int)wi.hb, he = (int)wi.he;
     int slot = wi.slot0;
     int cur_rb = -1, buf = 0;
     double qa[R], y[R], ax[R], ay[R], az[R];
@@ -250,7 +250,7 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
         cgp_cp8(sb + 164 + lane, pv.B ? pv.B + min(j, M - 1) : pv.A, (pv.B && j < M) ? 8 : 0);
     };
     // d_next: the strip whose columns are in flight into buffer nbuf; d_next2: the one after it (descriptor only)
-    const int64_t last_s = (he - 1) >> 1;
+    const int last_s = (he - 1) >> 4;
     int2 d_next = make_int2(0, 0), d_next2 = make_int2(0, 0);
     int nbuf = 0;
     auto load_rows = [&](int rb_) {      // charges and coordinates of the 4 x 32 rows of row block rb_
@@ -270,14 +270,17 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
         cur_rb = d_next.x;        // the first row block's rows are loaded here, beside the copies, not after waiting for them
         load_rows(cur_rb);
     }
-    int64_t cur_s = -1;
+    int cur_s = -1;
     double alx[R], aly[R], alz[R], a2[R];
     unsigned m = 0;
     bool sym = false;
     int rb = 0, cg = 0;
-    for (int64_t h = hb; h < he; ++h) {
-        const int64_t sidx = h >> 1;
-        const int half = (int)(h & 1);
+    for (int h = hb; h < he;) {
+        // one pass = the columns [tb, te) of one half strip: all 16 except at the two ends of the segment, which may lie
+        // anywhere (a column, with all 128 rows, still belongs to one warp, so the sums keep their fixed order)
+        const int sidx = h >> 4;
+        const int half = (h >> 3) & 1;
+        const int tb = 2 * (h & 7), te = min(16, tb + 2 * (he - h));
         cgp_cp_wait_all();
         __syncwarp();
         near_consume();
@@ -318,15 +321,15 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
             __syncwarp();
         }
         near_issue();
-        const double4 *sp = reinterpret_cast<const double4 *>(wsm + buf * CGP_STG) + half * 16;
-        const double *sq = s_q + half * 16;
+        const double4 *sp = reinterpret_cast<const double4 *>(wsm + buf * CGP_STG) + half * 16 + tb;
+        const double *sq = s_q + half * 16 + tb;
         // Strips with a near patch among the 4 row groups run the same blocked loop (the near rows sit at r^2 = 2^1000, see
         // above): three rows of wasted arithmetic at worst, but no slow path whose cost the partition would have to know
         // (near patches cluster at the start of a row block's strips), and no select in the loop.
-        double *ah = MODE ? a.afar + (size_t)h * (16 * R * 32) + lane : nullptr;
-        double *scp = sc + lane;
+        double *ah = MODE ? a.afar + (size_t)(h >> 3) * (16 * R * 32) + lane : nullptr;
+        double *scp = sc + lane + tb * 33;
 #pragma unroll 1
-        for (int t = 0; t < 16; t += C, sp += C, sq += C, scp += C * 33) {
+        for (int t = tb; t < te; t += C, sp += C, sq += C, scp += C * 33) {
             double4 b[C];
             double qb[C], r2[C][R], cc[C];
 #pragma unroll
@@ -369,8 +372,9 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
             for (int k = 1; k < 16; ++k) t += col[k];
             const double o2 = __shfl_xor_sync(0xffffffffu, t, 16);
             const int j = cg * 32 + half * 16 + lane;
-            if (lane < 16 && j < M) a.colpart[(size_t)rb * M + j] = t + o2;
+            if (lane >= tb && lane < te && j < M) a.colpart[(size_t)rb * M + j] = t + o2;
         }
+        h += (te - tb) >> 1;
     }
     if (cur_rb >= 0) {
 #pragma unroll
@@ -691,7 +695,8 @@ int plan_sweep(pcm_ctx *ctx) {
             cost.push_back((float)CGP_R);      // a strip costs its 4 patches whatever the mask (the near rows are computed and discarded)
         }
     // near pieces go round-robin to the warps (piece q to warp q mod nwarp), before the far segment; their cost shortens it
-    const double near_cost = 0.3;    // a stored near patch against a far patch, in warp time (0.6 and 1.0 measured no different)
+    const double near_cost = 0.5;    // a stored near patch against a far patch, in warp time (PCM_VERBOSE prints the mean sweep
+                                     // time of warps with / without a near piece: 0.3 left the near CTAs 1.8 us behind at M = 10k)
     std::vector<double> wnear((size_t)sp.nwarp, 0.0);
     for (int64_t q = 0; q < pm.npiece; ++q) {
         const int64_t rg = pm.piece_rg_host[q];
@@ -702,19 +707,22 @@ int plan_sweep(pcm_ctx *ctx) {
     for (float c : cost) total += c;
     for (double c : wnear) total += c;
     const double target = total / sp.nwarp;
-    // segments in HALF strips (16 columns of the 4 row groups, cost CGP_R / 2): half strip h belongs to strip h >> 1
-    const int64_t nhalf = 2 * (int64_t)strip.size();
+    // Segments in column PAIRS (2 columns against the 4 row groups, cost CGP_R / 16; pair h belongs to strip h >> 4): what one
+    // pass of the sweep's inner loop does, so every warp gets its share to within one pass.  (Half strips as the unit left
+    // warps with 10 or 11 of them at M = 10k, and the CTAs with the 11s finished 3 us after the others.)
+    const int64_t nhalf = 2 * (int64_t)strip.size(), npair = 16 * (int64_t)strip.size();
     std::vector<int64_t> seg_start((size_t)sp.nwarp + 1, 0);
     {
         int64_t h = 0;
-        double done_far = 0.0, boundary = 0.0;
-        const double hc = 0.5 * CGP_R;
+        double boundary = 0.0;
+        const double pc = CGP_R / 16.0;
         for (int w = 0; w < sp.nwarp; ++w) {
             seg_start[w] = h;
             boundary += target - wnear[w];
-            while (h < nhalf && (w == sp.nwarp - 1 || done_far + 0.5 * hc <= boundary)) { done_far += hc; ++h; }
+            const int64_t to = w == sp.nwarp - 1 ? npair : std::min<int64_t>(npair, (int64_t)std::llround(boundary / pc));
+            h = std::max(h, to);
         }
-        seg_start[sp.nwarp] = nhalf;
+        seg_start[sp.nwarp] = npair;
     }
     // row-sum slots: one per (segment, row block) run, numbered in order (the slots of a row block are consecutive)
     std::vector<int32_t> seg_slot0((size_t)sp.nwarp + 1, 0), rb_slot_start((size_t)nrb + 1, 0);
@@ -724,8 +732,9 @@ int plan_sweep(pcm_ctx *ctx) {
         for (int w = 0; w < sp.nwarp; ++w) {
             seg_slot0[w] = nslot;
             int last = -1;
-            for (int64_t h = seg_start[w]; h < seg_start[w + 1]; ++h)
-                if (strip[h >> 1].x != last) { last = strip[h >> 1].x; ++nslot; ++cnt[last]; }
+            if (seg_start[w] < seg_start[w + 1])
+                for (int64_t si = seg_start[w] >> 4; si <= (seg_start[w + 1] - 1) >> 4; ++si)
+                    if (strip[(size_t)si].x != last) { last = strip[(size_t)si].x; ++nslot; ++cnt[last]; }
         }
         seg_slot0[sp.nwarp] = nslot;
         for (int64_t rb = 0; rb < nrb; ++rb) rb_slot_start[rb + 1] = rb_slot_start[rb] + cnt[rb];
@@ -751,7 +760,7 @@ int plan_sweep(pcm_ctx *ctx) {
             wi.hb = seg_start[w]; wi.he = seg_start[w + 1];
             wi.slot0 = seg_slot0[w];
             if (wi.hb < wi.he) {
-                const int64_t s0 = wi.hb >> 1, last = (wi.he - 1) >> 1;
+                const int64_t s0 = wi.hb >> 4, last = (wi.he - 1) >> 4;
                 wi.strip0 = strip[(size_t)s0];
                 wi.strip1 = s0 + 1 <= last ? strip[(size_t)s0 + 1] : make_int2(0, 0);
             }
@@ -808,7 +817,7 @@ int plan_sweep(pcm_ctx *ctx) {
     if (getenv("PCM_VERBOSE")) {
         double mx = 0.0;
         for (int w = 0; w < sp.nwarp; ++w) {
-            const double c = wnear[w] + 0.5 * CGP_R * (double)(seg_start[w + 1] - seg_start[w]);
+            const double c = wnear[w] + CGP_R / 16.0 * (double)(seg_start[w + 1] - seg_start[w]);
             mx = std::max(mx, c);
         }
         int64_t partial = 0, pfar = 0, ffar = 0;

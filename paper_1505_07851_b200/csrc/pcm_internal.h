@@ -76,7 +76,7 @@ struct SweepPlan {
     size_t smem = 0;
     struct CgpWarpInit *winit = nullptr;   // [nwarp] start-up record of every warp (pcm_cgp.cu)
     int2 *strip = nullptr;            // [nstrip] (row block, column group | far mask of the 4 row groups << 24)
-    int64_t *seg_start = nullptr;     // [nwarp + 1] strips of every warp
+    int64_t *seg_start = nullptr;     // [nwarp + 1] column pairs of every warp (pair h belongs to strip h >> 4)
     int32_t *seg_slot0 = nullptr;     // [nwarp + 1] first row-sum slot of every warp
     int32_t *rb_slot_start = nullptr; // [nrb + 1] slots of every row block (consecutive)
     double4 *colloc = nullptr;        // [M] (-2 (b - o), |b - o|^2), o = first point of the column's group
