@@ -363,7 +363,30 @@ int pcm_fp64_peak(pcm_ctx *ctx, int reps, double *tflops);
  */
 int pcm_schwarz_bound(int la, double alpha, const double *A, int lb, double beta, const double *B, double *out);
 
-/* Text of the last error on this context (ctx == NULL: of the last failed pcm_setup on this thread). */
+/*
+ * pcm_amatvec_static -- y = A q (Eq. 2, 3, 8; A_ij = erf(zeta'_ij r_ij)/r_ij,
+ * zeta'_ij = zeta_i zeta_j/sqrt(zeta_i^2 + zeta_j^2), A_ii = zeta_i sqrt(2/pi)/S_i) WITHOUT a context and without
+ * allocating anything: no cudaMalloc, cudaFree or allocating library routine on this path, so it may be called under
+ * CUDA graph capture, from serving loops and from harnesses that forbid allocation.  Its only scratch (16 partial sums
+ * per row, added in a fixed order) is a static __device__ array of 16 x PCM_STATIC_MAX_POINTS doubles = 2 MiB that every
+ * GPU loading the library holds until the process exits.
+ *   npoint: 0 ... PCM_STATIC_MAX_POINTS; more is refused with PCM_ERR_ARG (use pcm_setup + pcm_amatvec, which is also
+ *   several times faster: this variant sweeps the full square with erf, no symmetry, no stored near field).
+ *   pt_xyz_dev [3 npoint] (x, y, z per point), pt_zeta_dev, pt_switch_dev, q_dev [npoint]: DEVICE, read;
+ *   y_dev [npoint]: DEVICE, overwritten; all in the caller's point order; the caller keeps ownership.
+ *   stream: cudaStream_t; asynchronous (two launches).  Coincident points give the limit 2 zeta'/sqrt(pi).
+ * The scratch array is shared by all calls on a device and keeps the last call's contents; a call writes every slot it
+ * reads, so nothing needs clearing, but CALLS THAT OVERLAP ON ONE GPU (two streams, two threads) RACE on it: keep them
+ * stream-ordered.  pcm_amatvec_static_init resolves the array's device address for the CURRENT device (once per device;
+ * the first use also loads the module): call it at set-up, outside any capture; pcm_amatvec_static does it itself on
+ * a device it has not seen.  Errors: PCM_ERR_ARG, PCM_ERR_CUDA (text: pcm_last_error(NULL)).
+ */
+#define PCM_STATIC_MAX_POINTS 16384
+int pcm_amatvec_static_init(void);
+int pcm_amatvec_static(int64_t npoint, const double *pt_xyz_dev, const double *pt_zeta_dev, const double *pt_switch_dev,
+                       const double *q_dev, double *y_dev, void *stream);
+
+/* Text of the last error on this context (ctx == NULL: of the last failed context-free call on this thread). */
 const char *pcm_last_error(pcm_ctx *ctx);
 
 /* Frees device and host state.  NULL is allowed. */

@@ -33,7 +33,9 @@ EXPORTS = (
     "pcm_cg_threshold", "pcm_gradient", "pcm_last_cg_matvec_ms", "pcm_rbj_build_async", "pcm_switching", "pcm_set_cavity", "pcm_surface_gradient",
     "pcm_schwarz_bound", "pcm_last_error", "pcm_destroy",
     "pcm_build_cavity", "pcm_cavity_size", "pcm_cavity_get", "pcm_cavity_device", "pcm_cavity_destroy", "pcm_setup_cavity",
+    "pcm_amatvec_static_init", "pcm_amatvec_static",
 )
+PCM_STATIC_MAX_POINTS = 16384
 
 
 class pcm_options(C.Structure):
@@ -273,6 +275,24 @@ def pcm_amatvec(ctx: Context, q, y=None, stream=None):
     if y is None:
         y = torch.empty(ctx.M, dtype=torch.float64, device=q.device)
     _check(lib().pcm_amatvec(ctx.handle, _dev(q, ctx.M, ctx), _dev(y, ctx.M, ctx), _stream(stream)), ctx.handle)
+    return y
+
+
+def pcm_amatvec_static_init() -> None:
+    """Resolves the static scratch array on the current device (set-up; once per device, outside any graph capture)."""
+    _check(lib().pcm_amatvec_static_init())
+
+
+def pcm_amatvec_static(pt_xyz, pt_zeta, pt_switch, q, y=None, stream=None):
+    """y = A q without a context and without any allocation inside the library (include/pcm.h).  All arguments are CUDA
+    float64 tensors in the caller's point order: pt_xyz [M, 3], pt_zeta, pt_switch, q [M], M <= PCM_STATIC_MAX_POINTS.
+    Pass y to keep the call free of allocations on the Python side too."""
+    import torch
+    M = int(q.numel())
+    if y is None:
+        y = torch.empty(M, dtype=torch.float64, device=q.device)
+    _check(lib().pcm_amatvec_static(C.c_int64(M), _dev(pt_xyz, 3 * M), _dev(pt_zeta, M), _dev(pt_switch, M), _dev(q, M), _dev(y, M),
+                                    _stream(stream)))
     return y
 
 

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpcm_b200.so")
-SOURCES = ["pcm_setup.cu", "pcm_kernels.cu", "pcm_solver.cu", "pcm_cgp.cu", "pcm_surface.cu", "pcm_cavity.cu", "pcm_api.cu"]
+SOURCES = ["pcm_setup.cu", "pcm_kernels.cu", "pcm_solver.cu", "pcm_cgp.cu", "pcm_surface.cu", "pcm_cavity.cu", "pcm_static.cu", "pcm_api.cu"]
 HEADERS = ["pcm_internal.h", "pcm_device.cuh", "pcm_gradient.inl"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
