@@ -611,8 +611,15 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
     }
 }
 
+// The three launches of a single A q (gather, sweep, row sums) form a chain of programmatic dependent launches: a kernel lets
+// its successor be scheduled at once and the successor waits for it (completion and visibility) before it touches memory, so
+// the launch latencies overlap the kernel before.  Without the launch attribute both instructions do nothing.
+__device__ __forceinline__ void cgp_pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void cgp_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // q in the caller's order -> sorted order
 __global__ void cgp_gather_kernel(const double *__restrict__ q, const int32_t *__restrict__ idx, double *__restrict__ qs, int M) {
+    cgp_pdl_launch_dependents();
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k < M) qs[k] = q[idx[k]];
 }
@@ -624,6 +631,8 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_matvec_kernel(CgpArgs a) {
     const unsigned G = gridDim.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     PSrc pv{a.q, nullptr, 0.0};
+    cgp_pdl_launch_dependents();
+    cgp_pdl_wait();
     if (a.phase != 2) cgp_sweep<MODE>(a, pv, blockIdx.x * CGP_WARPS + warp, lane, dyn + warp * CGP_WSMEM2);
     if (MODE == 1 || a.phase == 1) return;      // filling the store, or the sweep half of a two-launch product
     if (a.phase == 0) cgp_grid_sync(a.ctl, G);
@@ -862,12 +871,23 @@ int cgp_matvec(pcm_ctx *ctx, const double *q, const int32_t *idx, double *y, cud
     // Two ordinary launches (sweep; row sums) instead of one cooperative launch with a grid barrier: a cooperative launch costs
     // ~20 us more between the events around it than its kernel runs (measured at M = 10k: 94 us against 72 us under ncu), which a
     // single A q does not win back; inside a solve the launch happens once, so pcm_cg_solve keeps the cooperative kernel.
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3(CGP_THREADS);
+    cfg.stream = s;
+    cfg.attrs = at;
     a.phase = 1;
-    if (a.afar) cgp_matvec_kernel<2><<<(unsigned)ctx->cgp.grid, CGP_THREADS, ctx->cgp.smem, s>>>(a);
-    else cgp_matvec_kernel<0><<<(unsigned)ctx->cgp.grid, CGP_THREADS, ctx->cgp.smem, s>>>(a);
+    cfg.gridDim = dim3((unsigned)ctx->cgp.grid);
+    cfg.dynamicSmemBytes = ctx->cgp.smem;
+    cfg.numAttrs = idx ? 1 : 0;          // chained to the gather kernel, if there is one
+    PCM_CUDA(ctx, cudaLaunchKernelEx(&cfg, a.afar ? cgp_matvec_kernel<2> : cgp_matvec_kernel<0>, a));
     a.phase = 2;
-    const unsigned rgrid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(cdiv2(a.ng, CGP_TEAMS), 4 * (int64_t)ctx->cgp.grid));
-    cgp_matvec_kernel<0><<<rgrid, CGP_THREADS, CGP_WARPS * 32 * 8, s>>>(a);
+    cfg.gridDim = dim3((unsigned)std::max<int64_t>(1, std::min<int64_t>(cdiv2(a.ng, CGP_TEAMS), 4 * (int64_t)ctx->cgp.grid)));
+    cfg.dynamicSmemBytes = CGP_WARPS * 32 * 8;
+    cfg.numAttrs = 1;
+    PCM_CUDA(ctx, cudaLaunchKernelEx(&cfg, cgp_matvec_kernel<0>, a));
     PCM_CUDA(ctx, cudaGetLastError());
     ctx->launch_total += 2;
     return PCM_OK;

@@ -305,6 +305,33 @@ def test_amatvec_coincident_and_mixed_exponents(pcm, orc, torch_cuda):
     np.testing.assert_array_equal(pcm.pcm_amatvec(ctx2, dev(torch_cuda, q)).cpu().numpy(), y)
 
 
+def test_amatvec_chained_launches_back_to_back(pcm, torch_cuda):
+    """Below 20 000 points pcm_amatvec is three launches chained as programmatic dependent launches (gather of q into sorted
+    order, the one-launch sweep, the row sums: each may be scheduled while the one before it still runs and waits for it before
+    it touches memory).  60 back-to-back calls with alternating q and y poisoned in between: every result bit-identical to the
+    one of a call with the device idle before and after it."""
+    torch = torch_cuda
+    z0, zi = np.zeros(0), np.zeros(0, np.int32)
+    for M in (300, 4100):
+        s, qa, qb = synth.make_solver_points(M, seed=1021)
+        ctx = pcm.pcm_setup(zi, np.zeros((0, 3)), zi, z0, z0, s.xyz, s.zeta, s.switch)
+        qs = [dev(torch, qa), dev(torch, qb)]
+        ref = []
+        for q in qs:
+            torch.cuda.synchronize()
+            ref.append(pcm.pcm_amatvec(ctx, q).clone())
+            torch.cuda.synchronize()
+        ys = [torch.empty(M, dtype=torch.float64, device="cuda") for _ in range(60)]
+        for y in ys:
+            y.fill_(float("nan"))
+        for it, y in enumerate(ys):          # no synchronisation inside the loop
+            pcm.pcm_amatvec(ctx, qs[it & 1], y)
+        torch.cuda.synchronize()
+        for it, y in enumerate(ys):
+            assert torch.equal(y, ref[it & 1]), (M, it)
+        pcm.pcm_destroy(ctx)
+
+
 def test_fock_tma_tiles_and_serial_classes_give_the_same_bits(pcm, orc, torch_cuda):
     """pcm_options.tma_tiles (point tiles brought in by cp.async.bulk + mbarrier from a packed (x, y, z, q) array) and
     pcm_options.serial_classes (class kernels as ordinary launches instead of a chain of dependent launches) change how the work is moved and
