@@ -44,6 +44,7 @@ UNIT = "prim-pair*point/s"
 CONFIG_INDEX = 3
 RBJ_BLOCK = 64
 CG_TOL = 1e-8
+PERSIST_MAX = 26_000   # points below which the library runs A q / PCG through the persistent sweep (pcm_internal.h AMAT_PERSIST_MAX)
 SWEEP_M = (2_500, 10_000, 50_000, 100_000, 200_000)
 STORED_M = (2_500, 5_000, 10_000, 50_000)   # stored-A variant against the on-the-fly sweep
 SOLVER_M = (2_500, 10_000, 50_000, 200_000)   # configs[4]: full pcm_cg_solve, RBJ-64 against Jacobi
@@ -69,7 +70,7 @@ HAND_WORK = {
 
 def work_of(model: dict, op: str, L: int = 0, M: int = 0, amat_key: str | None = None) -> dict:
     """{instr, flop, traffic_per_unit, source} of one unit of kernel `op` (integral class L, or the A q sweep at M points)."""
-    key = f"{op}_L{L}" if op in ("potential", "fock") else (amat_key or ("amatvec_R4" if M >= 20000 else "amatvec_cgp"))
+    key = f"{op}_L{L}" if op in ("potential", "fock") else (amat_key or ("amatvec_R4" if M >= PERSIST_MAX else "amatvec_cgp"))
     rec = model.get(key)
     if rec is None and key == "amatvec_cgp":       # an older capture: the separate-launch small-M kernel
         key = "amatvec_R2"
@@ -471,7 +472,7 @@ def amat_and_solver_sweep(pcm, torch, dev, flush, model, peak_tflops, with_solve
                         e1.record(stream); torch.cuda.synchronize()
                         tsol.append(e0.elapsed_time(e1))
                     rec["rbj_block_sweep"].append({"block": blk, "iters": int(it), "solve_ms": min(tsol), "build_ms": tbuild, "converged": bool(ok)})
-            if Ms < 20000:   # the same solve through the separate-launch path (pcm_options.cg_path = 1), for comparison
+            if Ms < PERSIST_MAX:   # the same solve through the separate-launch path (pcm_options.cg_path = 1), for comparison
                 c1 = pcm.pcm_setup(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0, np.int32), np.zeros(0), np.zeros(0),
                                    s4.xyz, s4.zeta, s4.switch, cg_path=1)
                 pcm.pcm_rbj_build(c1, RBJ_BLOCK, seed=7, stream=stream)

@@ -61,7 +61,7 @@ typedef struct pcm_options {
                               evaluated once at pcm_setup and kept on the device (8 KB per 32 x 32 patch, up to 16 GB; beyond
                               that, or with 0, they are re-evaluated in every pcm_amatvec).  Same values either way. */
     int cg_path;           /* pcm_cg_solve / pcm_amatvec: 0 (default) = one persistent cooperative kernel per solve and one launch per
-                              A q below 20 000 points, separate kernel launches above; 1 = always separate launches (the
+                              A q below 26 000 points, separate kernel launches above; 1 = always separate launches (the
                               reference path); 2 = the persistent kernel at any size its buffers allow; 3 = separate launches with
                               every CG vector operation in a kernel of its own (no fused update kernel: the bit-exactness
                               reference of path 1).  Same recurrences; paths 0/2 and 1/3 add the partial sums of A q in different
@@ -201,7 +201,7 @@ int pcm_rbj_get(pcm_ctx *ctx, int64_t *order_host, int64_t *bstart_host, double 
  * tol is the absolute Euclidean norm of the recurrence residual (the paper's delta).
  * iters (HOST, may be NULL): matrix-vector products after the initial residual.
  * resid (HOST, may be NULL): resid[0] = final recurrence ||r||, resid[1] = true ||b - A x|| recomputed at exit.
- * Synchronous.  Below 20 000 points the iterations run inside one persistent kernel and the host reads the outcome once;
+ * Synchronous.  Below 26 000 points the iterations run inside one persistent kernel and the host reads the outcome once;
  * above, iterations are queued eight at a time between read-backs of the device-side convergence flag.  Returns PCM_OK,
  * PCM_NOT_CONVERGED, or PCM_ERR_NUMERIC when the residual is not finite (non-finite b, p.Ap = 0).
  * SURVEY.md 8(b) proposed `block` and `seed` as arguments of this call: they are arguments of pcm_rbj_build[_async], because

@@ -1,5 +1,5 @@
 // pcm_cgp.cu -- the whole preconditioned CG solve as ONE persistent cooperative kernel, and the
-// warp-granular symmetric A q sweep it is built on, for cavities below AMAT_R4_MIN points (where an iteration is tens of
+// warp-granular symmetric A q sweep it is built on, for cavities below AMAT_PERSIST_MAX points (where an iteration is tens of
 // microseconds and launches, tails and partial-sum round trips cost as much as the arithmetic).
 //
 // Work partition (plan_sweep, fixed at pcm_setup).  Rows are cut into blocks of 4 row groups (128 points); a "strip" is
@@ -720,6 +720,7 @@ int plan_sweep(pcm_ctx *ctx) {
     // pass of the sweep's inner loop does, so every warp gets its share to within one pass.  (Half strips as the unit left
     // warps with 10 or 11 of them at M = 10k, and the CTAs with the 11s finished 3 us after the others.)
     const int64_t nhalf = 2 * (int64_t)strip.size(), npair = 16 * (int64_t)strip.size();
+    if (npair >= (int64_t)1 << 30) return PCM_OK;      // the sweep indexes pairs with 32-bit integers: the classic path takes over
     std::vector<int64_t> seg_start((size_t)sp.nwarp + 1, 0);
     {
         int64_t h = 0;

@@ -68,7 +68,7 @@ constexpr int NEAR_PIECE = 4;
 
 // Warp-granular partition of the symmetric A q sweep and the buffers of the persistent PCG kernel (pcm_cgp.cu); built by
 // plan_sweep at pcm_setup for cavities below AMAT_PERSIST_MAX points whose near patches are stored.
-constexpr int64_t AMAT_PERSIST_MAX = 20000;
+constexpr int64_t AMAT_PERSIST_MAX = 26000;     // measured crossover with the R = 4 kernel: one A q 24k points, a PCG iteration 28 - 30k
 struct SweepPlan {
     bool ready = false;
     int grid = 0, nwarp = 0, ng = 0, nrb = 0, nslot = 0;

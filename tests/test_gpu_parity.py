@@ -306,7 +306,7 @@ def test_amatvec_coincident_and_mixed_exponents(pcm, orc, torch_cuda):
 
 
 def test_amatvec_chained_launches_back_to_back(pcm, torch_cuda):
-    """Below 20 000 points pcm_amatvec is three launches chained as programmatic dependent launches (gather of q into sorted
+    """Below 26 000 points pcm_amatvec is three launches chained as programmatic dependent launches (gather of q into sorted
     order, the one-launch sweep, the row sums: each may be scheduled while the one before it still runs and waits for it before
     it touches memory).  60 back-to-back calls with alternating q and y poisoned in between: every result bit-identical to the
     one of a call with the device idle before and after it."""
