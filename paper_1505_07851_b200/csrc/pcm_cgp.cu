@@ -236,9 +236,9 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
     const int hb = (int)wi.hb, he = (int)wi.he;
     int slot = wi.slot0;
     int cur_rb = -1, buf = 0;
-    double qa[R], y[R], ax[R], ay[R], az[R];
+    double qa[R], y[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) { qa[r] = y[r] = ax[r] = ay[r] = az[r] = 0.0; }
+    for (int r = 0; r < R; ++r) { qa[r] = y[r] = 0.0; }
     auto stage_issue = [&](int2 st, int b) {     // columns of strip st into staging buffer b
         double *sb = wsm + b * CGP_STG;
         const int cg = st.y & 0xffffff, j = cg * 32 + lane;
@@ -253,13 +253,13 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
     const int last_s = (he - 1) >> 4;
     int2 d_next = make_int2(0, 0), d_next2 = make_int2(0, 0);
     int nbuf = 0;
-    auto load_rows = [&](int rb_) {      // charges and coordinates of the 4 x 32 rows of row block rb_
+    // The rows' coordinates are NOT kept in registers across strips: they are read again (4 x 32 bytes per lane, L1 hits)
+    // whenever a strip starts and turned into the strip's local coordinates at once -- 24 registers less in the inner loop.
+    auto load_rows = [&](int rb_) {      // charges of the 4 x 32 rows of row block rb_
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int ii = (rb_ * R + r) * 32 + lane;
             qa[r] = ii < M ? pv(ii) : 0.0;              // padding rows: zero charge, their sums are not used
-            const double4 p = a.pt[min(ii, M - 1)];
-            ax[r] = ii < M ? p.x : p.x + 3e8; ay[r] = p.y; az[r] = p.z;   // padding rows: far away
             y[r] = 0.0;
         }
     };
@@ -304,7 +304,9 @@ __device__ __forceinline__ void cgp_sweep(const CgpArgs &a, const PSrc &pv, int 
             const double4 o = *reinterpret_cast<const double4 *>(sb + 128);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                alx[r] = ax[r] - o.x; aly[r] = ay[r] - o.y; alz[r] = az[r] - o.z;
+                const int ii = (rb * R + r) * 32 + lane;
+                const double4 p = a.pt[min(ii, M - 1)];
+                alx[r] = (ii < M ? p.x : p.x + 3e8) - o.x; aly[r] = p.y - o.y; alz[r] = p.z - o.z;   // padding rows: far away
                 a2[r] = fma(alz[r], alz[r], fma(aly[r], aly[r], alx[r] * alx[r]));
                 // Row groups whose patch against this column group is near (stored, added by the near pieces) are moved out
                 // of reach instead of being selected away per evaluation: r^2 = 2^1000 whatever the column, 1/r ~ 2^-500, and
