@@ -360,7 +360,7 @@ static int grad_launch_near(pcm_ctx *ctx, const double *q, cudaStream_t s) {
     }
     if (c.fock_map.npiece > 0) {
         const PatchMap &pm = c.fock_map;
-        fock_near_kernel<L + 1><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+        fock_near_kernel<L + 1><<<(unsigned)pm.npiece, TPB, 0, s>>>(
             c.prodA, c.prodB, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
             c.near_gfock, boysL1);
         PCM_LAUNCH_CHECK(ctx);

@@ -667,7 +667,13 @@ __global__ void __launch_bounds__(TPB) fock_tma_kernel(const double4 *__restrict
     }
 }
 
-// near patches of the Fock sweep: one warp per piece; lane = product.  Writes near[piece][h][lane].
+// near patches of the Fock sweep: one CTA per piece (<= NEAR_PIECE listed point groups of one product group); lane = product;
+// warp w takes the points [8 w, 8 w + 8) of every listed group, so a piece is four chains of <= 32 evaluations instead of one
+// of <= 128 (the kernel is latency-bound: at 300 atoms its grid was one wave of warps that each ran 128 evaluations in series,
+// 17 - 47 % of the warp slots occupied).  The four partial sums are added in warp order.  Writes near[piece][h][lane].
+constexpr int NEAR_WARPS = TPB / 32;                 // warps that share a piece
+constexpr int NEAR_PER = SUB / NEAR_WARPS;           // listed entries of a patch per warp
+static_assert(NEAR_PIECE * NEAR_PER <= SUB, "a warp stages its share of a piece in one pass, one record per lane");
 template <int L>
 __global__ void __launch_bounds__(TPB) fock_near_kernel(const double4 *__restrict__ prodA, const double2 *__restrict__ prodB,
                                                         int64_t npad, const double4 *__restrict__ pt, const double *__restrict__ q,
@@ -676,11 +682,11 @@ __global__ void __launch_bounds__(TPB) fock_near_kernel(const double4 *__restric
                                                         const int32_t *__restrict__ piece_rg, int64_t npiece,
                                                         double *__restrict__ near, const double *__restrict__ boysL) {
     constexpr int NH = nherm(L);
-    __shared__ double4 s_pt[TPB / 32][SUB];
-    __shared__ double s_iz[TPB / 32][SUB];
+    __shared__ double4 s_pt[NEAR_WARPS][SUB];
+    __shared__ double s_iz[NEAR_WARPS][SUB];
+    __shared__ double s_sum[NEAR_WARPS - 1][NH * SUB];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
-    if (piece >= npiece) return;
+    const int64_t piece = blockIdx.x;
     const int64_t rg = piece_rg[piece];
     const int64_t ip = rg * SUB + lane;  // < npad (npad is a multiple of 32)
     const double4 A = prodA[ip];
@@ -690,9 +696,10 @@ __global__ void __launch_bounds__(TPB) fock_near_kernel(const double4 *__restric
 #pragma unroll
     for (int h = 0; h < NH; ++h) sink.acc[h] = 0.0;
     const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
-    for (int64_t e = ebeg; e < eend; ++e) {
-        const int k = list[e] * SUB + lane;
-        __syncwarp();
+    const int np = (int)(eend - ebeg);
+    {   // lane -> point (lane & 7) of this warp's share of listed group lane >> 3
+        const int pe = lane / NEAR_PER;
+        const int k = pe < np ? list[ebeg + pe] * SUB + warp * NEAR_PER + (lane % NEAR_PER) : M;
         if (k < M) {
             const double4 c = pt[k];
             s_pt[warp][lane] = make_double4(c.x, c.y, c.z, q[qidx ? qidx[k] : k]);
@@ -701,31 +708,44 @@ __global__ void __launch_bounds__(TPB) fock_near_kernel(const double4 *__restric
             s_pt[warp][lane] = make_double4(-3e8, -3e8, -3e8, 0.0);
             s_iz[warp][lane] = 1.0;
         }
-        __syncwarp();
+    }
+    __syncwarp();
+    const int nev = np * NEAR_PER;
 #pragma unroll 1
-        for (int t = 0; t < SUB; t += 2) {
-            const double4 c0 = s_pt[warp][t], c1 = s_pt[warp][t + 1];
-            const double x0 = A.x - c0.x, y0 = A.y - c0.y, z0 = A.z - c0.z;
-            const double x1 = A.x - c1.x, y1 = A.y - c1.y, z1 = A.z - c1.z;
-            const double r20 = fma(z0, z0, fma(y0, y0, x0 * x0));
-            const double r21 = fma(z1, z1, fma(y1, y1, x1 * x1));
-            double g0[L + 1], g1[L + 1];
-            if (min(hi32(r20), hi32(r21)) > thr_hi) {
-                seeds_far<L>(r20, g0);
-                seeds_far<L>(r21, g1);
-            } else {
-                seeds_general<L>(r20, B.x, B.y, s_iz[warp][t], boysL, g0);
-                seeds_general<L>(r21, B.x, B.y, s_iz[warp][t + 1], boysL, g1);
-            }
+    for (int t = 0; t < nev; t += 2) {
+        const double4 c0 = s_pt[warp][t], c1 = s_pt[warp][t + 1];
+        const double x0 = A.x - c0.x, y0 = A.y - c0.y, z0 = A.z - c0.z;
+        const double x1 = A.x - c1.x, y1 = A.y - c1.y, z1 = A.z - c1.z;
+        const double r20 = fma(z0, z0, fma(y0, y0, x0 * x0));
+        const double r21 = fma(z1, z1, fma(y1, y1, x1 * x1));
+        double g0[L + 1], g1[L + 1];
+        if (min(hi32(r20), hi32(r21)) > thr_hi) {
+            seeds_far<L>(r20, g0);
+            seeds_far<L>(r21, g1);
+        } else {
+            seeds_general<L>(r20, B.x, B.y, s_iz[warp][t], boysL, g0);
+            seeds_general<L>(r21, B.x, B.y, s_iz[warp][t + 1], boysL, g1);
+        }
 #pragma unroll
-            for (int n2 = 0; n2 <= L; ++n2) { g0[n2] *= c0.w; g1[n2] *= c1.w; }
-            hermite_R<L>(x0, y0, z0, g0, sink);
-            hermite_R<L>(x1, y1, z1, g1, sink);
+        for (int n2 = 0; n2 <= L; ++n2) { g0[n2] *= c0.w; g1[n2] *= c1.w; }
+        hermite_R<L>(x0, y0, z0, g0, sink);
+        hermite_R<L>(x1, y1, z1, g1, sink);
+    }
+    if (warp > 0) {
+#pragma unroll
+        for (int h = 0; h < NH; ++h) s_sum[warp - 1][h * SUB + lane] = sink.acc[h];
+    }
+    __syncthreads();
+    if (warp == 0) {
+        double *out = near + (size_t)piece * NH * SUB + lane;
+#pragma unroll
+        for (int h = 0; h < NH; ++h) {
+            double v = sink.acc[h];
+#pragma unroll
+            for (int w = 0; w < NEAR_WARPS - 1; ++w) v += s_sum[w][h * SUB + lane];
+            out[h * SUB] = v;
         }
     }
-    double *out = near + (size_t)piece * NH * SUB + lane;
-#pragma unroll
-    for (int h = 0; h < NH; ++h) out[h * SUB] = sink.acc[h];
 }
 
 // herm[0][h][i] = sum_c herm[c][h][i] + sum of the near pieces of product i; plane = nh * npad.  As reduce_slots_kernel:
@@ -1060,8 +1080,9 @@ __global__ void __launch_bounds__(TPB) potential_pr_kernel(const double4 *__rest
     }
 }
 
-// near patches of the potential sweep: one warp per piece; lane = point; the 32 products of a listed group are
-// staged in the warp's own shared memory.  Writes near[piece][lane].
+// near patches of the potential sweep: one CTA per piece; lane = point; warp w takes the products [8 w, 8 w + 8) of every listed
+// product group (see fock_near_kernel) and stages their records -- one per lane, the whole piece in one pass -- in its own
+// shared memory.  The four partial sums are added in warp order.  Writes near[piece][lane].
 template <int L>
 __global__ void __launch_bounds__(TPB) potential_near_kernel(const double4 *__restrict__ prodA, const double2 *__restrict__ prodB,
                                                              const double *__restrict__ herm, int64_t npad,
@@ -1072,45 +1093,51 @@ __global__ void __launch_bounds__(TPB) potential_near_kernel(const double4 *__re
                                                              const double *__restrict__ boysL) {
     constexpr int NH = nherm(L);
     constexpr int REC = pot_rec_near<L>();
-    __shared__ __align__(16) double s_rec[TPB / 32][SUB * REC];
+    __shared__ __align__(16) double s_rec[NEAR_WARPS][SUB * REC];
+    __shared__ double s_sum[NEAR_WARPS][SUB];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t piece = (int64_t)blockIdx.x * (TPB / 32) + warp;
-    if (piece >= npiece) return;
+    const int64_t piece = blockIdx.x;
     const int64_t rg = piece_rg[piece];
     const int k = (int)rg * SUB + lane;
     const double4 c = pt[min(k, M - 1)];
     double v = 0.0;
     const int64_t ebeg = start[rg] + (piece - pstart[rg]) * NEAR_PIECE, eend = min(start[rg + 1], ebeg + NEAR_PIECE);
+    const int np = (int)(eend - ebeg);
     double *mine = s_rec[warp];
-    for (int64_t e = ebeg; e < eend; ++e) {
-        const int64_t i0 = (int64_t)list[e] * SUB;
-        __syncwarp();
-        {
-            const double4 a = prodA[i0 + lane];
-            const double2 b = prodB[i0 + lane];
-            double *r = mine + lane * REC;
-            r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = a.w;
-            r[4 + NH] = b.x; r[5 + NH] = b.y;
+    if (lane / NEAR_PER < np) {     // lane -> product (lane & 7) of this warp's share of listed group lane >> 3
+        const int64_t i = (int64_t)list[ebeg + lane / NEAR_PER] * SUB + warp * NEAR_PER + (lane % NEAR_PER);
+        const double4 a = prodA[i];
+        const double2 b = prodB[i];
+        double *r = mine + lane * REC;
+        r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = a.w;
+        r[4 + NH] = b.x; r[5 + NH] = b.y;
 #pragma unroll
-            for (int h = 0; h < NH; ++h) r[4 + h] = herm[(size_t)h * npad + i0 + lane];
-        }
-        __syncwarp();
-#pragma unroll 1
-        for (int t = 0; t < SUB; ++t) {
-            const double *rec = mine + t * REC;
-            const double2 h01 = *reinterpret_cast<const double2 *>(rec);
-            const double2 h23 = *reinterpret_cast<const double2 *>(rec + 2);
-            const double x = h01.x - c.x, y = h01.y - c.y, z = h23.x - c.z;
-            const double r2 = fma(z, z, fma(y, y, x * x));
-            double g[L + 1];
-            if (hi32(r2) > hi32(h23.y)) seeds_far<L>(r2, g);
-            else seeds_general<L>(r2, rec[4 + NH], rec[5 + NH], c.w, boysL, g);
-            PotSink<L> sink{rec + 4, v};
-            hermite_R<L>(x, y, z, g, sink);
-            v = sink.v;
-        }
+        for (int h = 0; h < NH; ++h) r[4 + h] = herm[(size_t)h * npad + i];
     }
-    near[piece * SUB + lane] = v;
+    __syncwarp();
+    const int nev = np * NEAR_PER;
+#pragma unroll 1
+    for (int t = 0; t < nev; ++t) {
+        const double *rec = mine + t * REC;
+        const double2 h01 = *reinterpret_cast<const double2 *>(rec);
+        const double2 h23 = *reinterpret_cast<const double2 *>(rec + 2);
+        const double x = h01.x - c.x, y = h01.y - c.y, z = h23.x - c.z;
+        const double r2 = fma(z, z, fma(y, y, x * x));
+        double g[L + 1];
+        if (hi32(r2) > hi32(h23.y)) seeds_far<L>(r2, g);
+        else seeds_general<L>(r2, rec[4 + NH], rec[5 + NH], c.w, boysL, g);
+        PotSink<L> sink{rec + 4, v};
+        hermite_R<L>(x, y, z, g, sink);
+        v = sink.v;
+    }
+    s_sum[warp][lane] = v;
+    __syncthreads();
+    if (warp == 0) {
+        double t = s_sum[0][lane];
+#pragma unroll
+        for (int w = 1; w < NEAR_WARPS; ++w) t += s_sum[w][lane];
+        near[piece * SUB + lane] = t;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1438,7 +1465,7 @@ static int launch_fock_near(pcm_ctx *ctx, const double *q, cudaStream_t s) {
     ClassData &c = ctx->cls[L];
     const PatchMap &pm = c.fock_map;
     if (c.n == 0 || pm.npiece == 0) return PCM_OK;
-    fock_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+    fock_near_kernel<L><<<(unsigned)pm.npiece, TPB, 0, s>>>(
         c.prodA, c.prodB, c.npad, ctx->pt, q, ctx->s2c, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
         c.near_fock, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
     PCM_LAUNCH_CHECK(ctx);
@@ -1564,7 +1591,7 @@ static int launch_potential_near(pcm_ctx *ctx, cudaStream_t s) {
     ClassData &c = ctx->cls[L];
     const PatchMap &pm = c.pot_map;
     if (c.n == 0 || pm.npiece == 0) return PCM_OK;
-    potential_near_kernel<L><<<(unsigned)ceil_div(pm.npiece, TPB / 32), TPB, 0, s>>>(
+    potential_near_kernel<L><<<(unsigned)pm.npiece, TPB, 0, s>>>(
         c.prodA, c.prodB, c.herm, c.npad, ctx->pt, (int)ctx->M, pm.start, pm.list, pm.pstart, pm.piece_rg, pm.npiece,
         c.near_pot, ctx->boys + (size_t)L * BOYS_ROWS * BOYS_STRIDE);
     PCM_LAUNCH_CHECK(ctx);
