@@ -12,6 +12,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
                   const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
                   const double *pt_zeta, const double *pt_switch);
 const char *setup_error_text();
+void setup_stage(const char *name);
 void pivot_order(uint64_t seed, int64_t M, int64_t *perm);
 int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter, int precond, int use_x0, int *iters,
              double *resid, cudaStream_t s);
@@ -125,6 +126,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
 
     // scratch sized from the fixed work partition
     const int64_t M = ctx->M;
+    setup_stage("gradient tables");
     if ((rc = plan_all(ctx))) return fail(rc);
     for (int L = 0; L <= MAXL; ++L) {
         ClassData &c = ctx->cls[L];
@@ -137,8 +139,12 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     ctx->ypart_slots = ctx->plan_amat.chunks;
     if (ctx->opt.tma_tiles && (rc = dev_alloc_t(ctx, &ctx->ptq, (size_t)std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->near_amat, (size_t)ctx->amat_map.npiece * 32))) return fail(rc);
+    setup_stage("work partition, scratch");
     if ((rc = fill_amat_blocks(ctx))) return fail(rc);
+    if (getenv("PCM_VERBOSE")) cudaDeviceSynchronize();
+    setup_stage("stored near patches of A");
     if ((rc = plan_sweep(ctx))) return fail(rc);
+    setup_stage("persistent sweep plan");
     if ((rc = dev_alloc_t(ctx, &ctx->vpart, (size_t)std::max<int64_t>(ctx->vpart_slots, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->ypart, (size_t)ctx->ypart_slots * std::max<int64_t>(M, 1)))) return fail(rc);
     if ((rc = dev_alloc_t(ctx, &ctx->colpart, (size_t)std::max<int64_t>(ctx->plan_amat.xb, 1) * std::max<int64_t>(M, 1)))) return fail(rc);
@@ -149,6 +155,7 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->cg_scal_host, 64 * sizeof(double));
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { ctx->err = std::string("pcm_setup: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
+    setup_stage("solver scratch");
     ctx->info.device_bytes = ctx->device_bytes;
     ctx->info.amat_near_patches = ctx->amat_map.nnear;
     ctx->info.amat_stored_bytes = ctx->amat_blocks ? ctx->amat_map.nnear * 32 * 32 * 8 : 0;

@@ -1,12 +1,12 @@
 // pcm_setup.cu -- host side of step a1: shell-pair enumeration, Eq. 15 screening,
 // Hermite Gaussian product merging, class sort, SoA packing and upload.  Also the Boys tables.
 #include <algorithm>
+#include <chrono>
 #include <array>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
-#include <unordered_map>
 
 #include "pcm_internal.h"
 
@@ -198,14 +198,6 @@ static inline uint64_t hilbert_key(uint64_t x, uint64_t y, uint64_t z) {
     return (spread21(X[0]) << 2) | (spread21(X[1]) << 1) | spread21(X[2]);
 }
 
-struct KeyHash {
-    size_t operator()(const std::array<uint64_t, 4> &k) const {
-        uint64_t h = 0x9E3779B97F4A7C15ULL;
-        for (uint64_t v : k) { h ^= v + 0x9E3779B97F4A7C15ULL + (h << 6) + (h >> 2); h *= 0xBF58476D1CE4E5B9ULL; }
-        return (size_t)h;
-    }
-};
-
 struct HostMember {
     int32_t sp;       // shell pair (final index)
     int32_t prod;     // product (temporary index, remapped after the sort)
@@ -293,10 +285,21 @@ static int class_of(int la, int lb) {
     return tab[lo][hi];
 }
 
+// PCM_VERBOSE: wall time of the stages of pcm_setup
+void setup_stage(const char *name) {
+    static const bool verbose = getenv("PCM_VERBOSE") != nullptr;
+    static std::chrono::steady_clock::time_point last;
+    if (!verbose) return;
+    const auto now = std::chrono::steady_clock::now();
+    if (name) fprintf(stderr, "[pcm] setup: %-40s %8.1f ms\n", name, std::chrono::duration<double, std::milli>(now - last).count());
+    last = now;
+}
+
 int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *shell_xyz, const int *shell_nprim,
                   const double *prim_exp, const double *prim_coef, int64_t npoint, const double *pt_xyz,
                   const double *pt_zeta, const double *pt_switch) {
     const pcm_options &opt = ctx->opt;
+    setup_stage(nullptr);
     // ------------------------------------------------------------------ points (Hilbert order, boxes of 32)
     ctx->M = npoint;
     GroupBoxes ptboxes;  // radius^2 entry 0: the product groups carry the far-field radius of a (product, point) pair
@@ -314,6 +317,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         const double pspan = npoint ? std::max({phi[0] - plo[0], phi[1] - plo[1], phi[2] - plo[2], 1e-9}) : 1.0;
         const double pcell = std::max(pspan / 2097151.0, 0.25);
         std::vector<uint64_t> key((size_t)npoint);
+#pragma omp parallel for schedule(static)
         for (int64_t k = 0; k < npoint; ++k)
             key[k] = hilbert_key((uint64_t)((pt_xyz[3 * k] - plo[0]) / pcell), (uint64_t)((pt_xyz[3 * k + 1] - plo[1]) / pcell),
                                  (uint64_t)((pt_xyz[3 * k + 2] - plo[2]) / pcell));
@@ -352,6 +356,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         for (int64_t g = 0; g < ng; ++g) amat_boxes.b[(size_t)g * 7 + 6] = TFAR_AMAT * 2.0 / (zmin * zmin);
         if ((rc = build_patch_map(ctx, amat_boxes, amat_boxes, ctx->amat_map, npoint < 4 * AMAT_PERSIST_MAX))) return rc;
     }
+    setup_stage("points, A q patch map");
     {
         std::vector<double> tab;
         build_boys_tables(tab);
@@ -359,6 +364,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         if (rc) return rc;
     }
 
+    setup_stage("Boys tables");
     // ------------------------------------------------------------------ shells
     std::vector<int64_t> poff(nshell + 1, 0), boff(nshell + 1, 0);
     std::vector<double> amin(nshell), cmax(nshell);
@@ -411,6 +417,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
             if (!hp.prims.empty()) per_row[I].push_back(std::move(hp));
         }
     }
+    setup_stage("shell pairs, Eq. 15 screening");
     std::vector<HostPair> pairs;
     for (auto &row : per_row) for (auto &hp : row) pairs.push_back(std::move(hp));
     per_row.clear();
@@ -423,6 +430,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
     info.prim_pairs_unscreened = unscreened;
     info.zeta_min = ctx->zeta_min; info.zeta_max = ctx->zeta_max;
 
+    setup_stage("pair list by class");
     // ------------------------------------------------------------------ members, products, G matrices
     std::vector<HostMember> members;
     std::vector<double> G, dG, m_ap;
@@ -432,9 +440,28 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
     std::vector<int32_t> c_sp, c_ab;
     struct HostProd { double p, x, y, z; int L; };
     std::vector<HostProd> prods;
-    std::unordered_map<std::array<uint64_t, 4>, int32_t, KeyHash> pmap;
     auto bits = [](double d) { uint64_t u; std::memcpy(&u, &d, 8); return u; };
 
+    // pass 1 (serial, light): offsets of every shell pair's members and G blocks, component list, counts
+    std::vector<int64_t> sp_goff(pairs.size() + 1, 0);
+    for (size_t sp = 0; sp < pairs.size(); ++sp) {
+        const HostPair &hp = pairs[sp];
+        const int I = hp.I, J = hp.J, la = shell_l[I], lb = shell_l[J], nh = nherm(la + lb);
+        const int na = la == 2 ? (opt.d_pure ? 5 : 6) : NCART[la], nb = lb == 2 ? (opt.d_pure ? 5 : 6) : NCART[lb];
+        sp_i0[sp] = (int32_t)boff[I]; sp_j0[sp] = (int32_t)boff[J];
+        sp_dims[sp] = na | (nb << 8) | ((I == J ? 1 : 0) << 16);
+        for (int ab = 0; ab < na * nb; ++ab) { c_sp.push_back((int32_t)sp); c_ab.push_back(ab); }
+        info.shell_pairs[hp.cls] += 1;
+        info.prim_pairs[hp.cls] += (int64_t)hp.prims.size();
+        sp_mstart[sp + 1] = sp_mstart[sp] + (int64_t)hp.prims.size();
+        sp_goff[sp + 1] = sp_goff[sp] + (int64_t)hp.prims.size() * na * nb * nh;
+    }
+    members.resize((size_t)sp_mstart[pairs.size()]);
+    G.assign((size_t)sp_goff[pairs.size()], 0.0);
+    if (want_grad) { dG.assign(3 * G.size(), 0.0); m_ap.resize(members.size()); }
+    std::vector<HostProd> mprod(members.size());       // the Gaussian product of every member, before merging
+    // pass 2 (all host threads): the G (and dG) block of every member -- independent of one another
+#pragma omp parallel for schedule(dynamic, 256)
     for (size_t sp = 0; sp < pairs.size(); ++sp) {
         const HostPair &hp = pairs[sp];
         const int I = hp.I, J = hp.J, la = shell_l[I], lb = shell_l[J], L = la + lb, nh = nherm(L);
@@ -443,43 +470,22 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         int na, nb;
         component_matrix(la, opt.d_pure, Ta, na);
         component_matrix(lb, opt.d_pure, Tb, nb);
-        sp_i0[sp] = (int32_t)boff[I]; sp_j0[sp] = (int32_t)boff[J];
-        sp_dims[sp] = na | (nb << 8) | ((I == J ? 1 : 0) << 16);
-        for (int ab = 0; ab < na * nb; ++ab) { c_sp.push_back((int32_t)sp); c_ab.push_back(ab); }
-        info.shell_pairs[hp.cls] += 1;
-        info.prim_pairs[hp.cls] += (int64_t)hp.prims.size();
-        sp_mstart[sp] = (int64_t)members.size();
-        for (auto ij : hp.prims) {
+        for (size_t k = 0; k < hp.prims.size(); ++k) {
+            const auto ij = hp.prims[k];
             const double a = prim_exp[poff[I] + ij.first], b = prim_exp[poff[J] + ij.second];
             const double cc = prim_coef[poff[I] + ij.first] * prim_coef[poff[J] + ij.second] * ((I == J && ij.first != ij.second) ? 2.0 : 1.0);
             const double p = a + b;
             const double Px = (a * A[0] + b * B[0]) / p, Py = (a * A[1] + b * B[1]) / p, Pz = (a * A[2] + b * B[2]) / p;
-            int32_t prod;
-            if (opt.merge_products) {
-                std::array<uint64_t, 4> key = {bits(p), bits(Px), bits(Py), bits(Pz)};
-                auto it = pmap.find(key);
-                if (it == pmap.end()) {
-                    prod = (int32_t)prods.size();
-                    pmap.emplace(key, prod);
-                    prods.push_back({p, Px, Py, Pz, L});
-                } else {
-                    prod = it->second;
-                    prods[prod].L = std::max(prods[prod].L, L);
-                }
-            } else {
-                prod = (int32_t)prods.size();
-                prods.push_back({p, Px, Py, Pz, L});
-            }
-            HostMember m;
-            m.sp = (int32_t)sp; m.prod = prod; m.L = (int8_t)L; m.goff = (int64_t)G.size();
-            members.push_back(m);
+            const size_t mi = (size_t)sp_mstart[sp] + k;
+            mprod[mi] = {p, Px, Py, Pz, L};
+            HostMember &m = members[mi];
+            m.sp = (int32_t)sp; m.prod = -1; m.L = (int8_t)L; m.goff = sp_goff[sp] + (int64_t)k * na * nb * nh;
             // G[ab][h] = cc (pi/p)^{3/2} sum_cart Ta[a][ca] Tb[b][cb] Ex Ey Ez   (K_AB is inside E^{00}_0)
             E1D Ex, Ey, Ez;
             hermite_E(a, b, A[0], B[0], la, lb, Ex);
             hermite_E(a, b, A[1], B[1], la, lb, Ey);
             hermite_E(a, b, A[2], B[2], la, lb, Ez);
             const double pref = cc * std::pow(M_PI / p, 1.5);
-            G.resize(G.size() + (size_t)na * nb * nh, 0.0);
             double *g = G.data() + m.goff;
             E1D Dx, Dy, Dz;
             double *dg = nullptr;
@@ -487,9 +493,8 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
                 hermite_dE(a, b, A[0], B[0], la, lb, Ex, Dx);
                 hermite_dE(a, b, A[1], B[1], la, lb, Ey, Dy);
                 hermite_dE(a, b, A[2], B[2], la, lb, Ez, Dz);
-                dG.resize(3 * G.size(), 0.0);
                 dg = dG.data() + 3 * m.goff;
-                m_ap.push_back(a / p);
+                m_ap[mi] = a / p;
             }
             for (int ca = 0; ca < NCART[la]; ++ca)
                 for (int cb = 0; cb < NCART[lb]; ++cb) {
@@ -519,11 +524,49 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
                 }
         }
     }
+    setup_stage("G matrices of the members");
+    // pass 3 (serial, in member order: the product numbering is that of the first member that carries it): members with
+    // bit-identical (p, P) share one product
+    // (an open-addressing table of product indices keyed by the four bit patterns: one allocation, linear probing)
+    size_t cap = 16;
+    while (cap < 2 * members.size() + 1) cap <<= 1;
+    std::vector<int32_t> table(opt.merge_products ? cap : 0, -1);
+    for (size_t mi = 0; mi < members.size(); ++mi) {
+        const HostProd &q = mprod[mi];
+        int32_t prod = -1;
+        if (opt.merge_products) {
+            const uint64_t kp = bits(q.p), kx = bits(q.x), ky = bits(q.y), kz = bits(q.z);
+            uint64_t hsh = kp * 0x9E3779B97F4A7C15ull;
+            hsh = (hsh ^ (hsh >> 29) ^ kx) * 0xBF58476D1CE4E5B9ull;
+            hsh = (hsh ^ (hsh >> 31) ^ ky) * 0x94D049BB133111EBull;
+            hsh = (hsh ^ (hsh >> 30) ^ kz) * 0x9E3779B97F4A7C15ull;
+            size_t slot = (size_t)(hsh >> 17) & (cap - 1);
+            for (;; slot = (slot + 1) & (cap - 1)) {
+                const int32_t cand = table[slot];
+                if (cand < 0) break;
+                const HostProd &r = prods[cand];
+                if (bits(r.p) == kp && bits(r.x) == kx && bits(r.y) == ky && bits(r.z) == kz) { prod = cand; break; }
+            }
+            if (prod < 0) {
+                prod = (int32_t)prods.size();
+                table[slot] = prod;
+                prods.push_back(q);
+            } else {
+                prods[prod].L = std::max(prods[prod].L, q.L);
+            }
+        } else {
+            prod = (int32_t)prods.size();
+            prods.push_back(q);
+        }
+        members[mi].prod = prod;
+    }
+    mprod.clear(); mprod.shrink_to_fit();
     sp_mstart[pairs.size()] = (int64_t)members.size();
     ctx->nmember = (int64_t)members.size();
     ctx->ncomp = (int64_t)c_sp.size();
     for (int c = 0; c < PCM_NCLASS; ++c) info.prim_pairs_total += info.prim_pairs[c];
 
+    setup_stage("members, products, G matrices");
     // ------------------------------------------------------------------ sort products by (L, reach, Hilbert(P), p)
     // "reach" = binary order of magnitude of 1/p + 1/zeta_min^2, which the far-field radius^2 is proportional to:
     // tight products (far from every surface point) and diffuse ones end up in different groups of 32, so that the
@@ -541,23 +584,29 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
     const double izmin2 = 1.0 / (ctx->zeta_min * ctx->zeta_min);
     std::vector<uint64_t> mort(np);
     std::vector<int> reach(np);
+#pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < np; ++i) {
         mort[i] = hilbert_key((uint64_t)((prods[i].x - lo[0]) / cell), (uint64_t)((prods[i].y - lo[1]) / cell),
                               (uint64_t)((prods[i].z - lo[2]) / cell));
         reach[i] = std::min(std::max(std::ilogb(1.0 / prods[i].p + izmin2), -6), 4);
     }
     std::vector<int32_t> order(np);
-    for (int64_t i = 0; i < np; ++i) order[i] = (int32_t)i;
-    std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
-        if (prods[x].L != prods[y].L) return prods[x].L < prods[y].L;
-        if (reach[x] != reach[y]) return reach[x] < reach[y];
-        if (mort[x] != mort[y]) return mort[x] < mort[y];
-        if (prods[x].p != prods[y].p) return prods[x].p > prods[y].p;
-        return x < y;
-    });
+    {   // the keys travel with the index: the comparisons stay in one array instead of chasing three
+        struct SortKey { uint64_t mort; double p; int32_t cls_reach, idx; };
+        std::vector<SortKey> sk((size_t)np);
+        for (int64_t i = 0; i < np; ++i) sk[i] = {mort[i], prods[i].p, (prods[i].L << 8) | (reach[i] + 16), (int32_t)i};
+        std::sort(sk.begin(), sk.end(), [](const SortKey &x, const SortKey &y) {
+            if (x.cls_reach != y.cls_reach) return x.cls_reach < y.cls_reach;
+            if (x.mort != y.mort) return x.mort < y.mort;
+            if (x.p != y.p) return x.p > y.p;
+            return x.idx < y.idx;
+        });
+        for (int64_t i = 0; i < np; ++i) order[i] = sk[i].idx;
+    }
     std::vector<int32_t> newidx(np);
     for (int64_t i = 0; i < np; ++i) newidx[order[i]] = (int32_t)i;
 
+    setup_stage("product sort");
     // per class SoA
     int64_t first = 0;
     for (int L = 0; L <= MAXL; ++L) {
@@ -595,6 +644,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
     info.prim_pair_points = (double)info.prim_pairs_total * (double)npoint;
     info.product_points = (double)np * (double)npoint;
 
+    setup_stage("class arrays, patch maps");
     // members: remap products, CSR product -> members
     std::vector<int32_t> m_prod(members.size()), m_cls(members.size()), m_sp(members.size());
     std::vector<int64_t> m_goff(members.size());
@@ -641,6 +691,7 @@ int build_context(pcm_ctx *ctx, int nshell, const int *shell_l, const double *sh
         if ((rc = upload(ctx, &ctx->comp_nu, ctx->comp_nu_host))) return rc;
         if ((rc = upload(ctx, &ctx->comp_diag, ctx->comp_diag_host))) return rc;
     }
+    setup_stage("member tables, uploads");
     ctx->nshell = nshell;
     if (want_grad) {
         std::vector<int32_t> shI(pairs.size()), shJ(pairs.size());
