@@ -756,6 +756,7 @@ __global__ void __launch_bounds__(256) reduce_herm_kernel(double *__restrict__ h
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t k = (int64_t)blockIdx.x * 32 + lane;   // npad is a multiple of 32: the 32 elements share h and the row group
     double s = 0.0;
+    pdl_launch_dependents();
     if (k < plane) {
         for (int c = w; c < chunks; c += 8) s += herm[(size_t)c * plane + k];
         const int64_t h = k / npad, i = k - h * npad, rg = i / SUB;
@@ -769,6 +770,7 @@ __global__ void __launch_bounds__(256) reduce_herm_kernel(double *__restrict__ h
         for (int q = 0; q < 8; ++q) t += s_tmp[q * 32 + lane];
         herm[k] = t;
     }
+    pdl_wait_predecessor();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1158,6 +1160,7 @@ __global__ void density_to_hermite_kernel(int64_t n, int64_t first, int64_t npad
                                           const double *__restrict__ G, const int32_t *__restrict__ sp_i0,
                                           const int32_t *__restrict__ sp_j0, const int32_t *__restrict__ sp_dims,
                                           const double *__restrict__ P, int64_t ldp, double *__restrict__ herm) {
+    pdl_launch_dependents();
     constexpr int NH = nherm(L);
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= npad) return;
@@ -1187,6 +1190,7 @@ __global__ void density_to_hermite_kernel(int64_t n, int64_t first, int64_t npad
     }
 #pragma unroll
     for (int h = 0; h < NH; ++h) herm[(size_t)h * npad + i] = D[h];
+    pdl_wait_predecessor();
 }
 
 // The same transform with one warp per product (used for L >= 2, where a product has several members of up to 25
@@ -1202,7 +1206,8 @@ __global__ void __launch_bounds__(128) density_to_hermite_warp_kernel(int64_t n,
     constexpr int NH = nherm(L);
     const int lane = threadIdx.x & 31;
     const int64_t i = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
-    if (i >= npad) return;
+    pdl_launch_dependents();
+    if (i >= npad) { pdl_wait_predecessor(); return; }
     double D[NH];
 #pragma unroll
     for (int h = 0; h < NH; ++h) D[h] = 0.0;
@@ -1234,6 +1239,7 @@ __global__ void __launch_bounds__(128) density_to_hermite_warp_kernel(int64_t n,
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
         if (lane == 0) herm[(size_t)h * npad + i] = v;
     }
+    pdl_wait_predecessor();
 }
 
 // F_ab (+)= sum_members sum_h G[ab][h] H_h(product of the member).  Thread = one component (a,b) of one shell pair;
@@ -1445,6 +1451,21 @@ int launch_amatvec_sorted(pcm_ctx *ctx, const double *q, double *y, cudaStream_t
 
 // One class kernel; chained: with the programmatic-serialization attribute, i.e. it may start while the last wave of the launch
 // before it on s is still running (see pdl_launch_dependents above; both kernels must be class kernels of the same call).
+constexpr int64_t PDL_DENSITY_MAX = 16384;    // products up to which the density transforms of a call are chained
+template <class... KArgs, class... Args>
+static cudaError_t launch_class_b(void (*kernel)(KArgs...), dim3 grid, int block, cudaStream_t s, bool chained, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = chained ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
 template <class... KArgs, class... Args>
 static cudaError_t launch_class(void (*kernel)(KArgs...), dim3 grid, cudaStream_t s, bool chained, Args... args) {
     cudaLaunchConfig_t cfg = {};
@@ -1493,13 +1514,13 @@ static int launch_fock_class(pcm_ctx *ctx, const double *q, cudaStream_t s, bool
 }
 
 template <int L>
-static int reduce_fock_class(pcm_ctx *ctx, cudaStream_t s) {
+static int reduce_fock_class(pcm_ctx *ctx, cudaStream_t s, bool chained = false) {
     ClassData &c = ctx->cls[L];
     const int64_t chunks = ctx->plan_fock[L].chunks;
     if (c.n == 0) return PCM_OK;
     const int64_t plane = (int64_t)nherm(L) * c.npad;
-    reduce_herm_kernel<<<(unsigned)ceil_div(plane, 32), 256, 0, s>>>(c.herm, plane, (int)chunks, c.npad, nherm(L), c.near_fock,
-                                                                      c.fock_map.pstart);
+    PCM_CUDA(ctx, launch_class_b(reduce_herm_kernel, dim3((unsigned)ceil_div(plane, 32)), 256, s, chained, c.herm, plane, (int)chunks, c.npad,
+                                 nherm(L), (const double *)c.near_fock, (const int64_t *)c.fock_map.pstart));
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
@@ -1553,11 +1574,18 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
     if (!accumulate && ctx->nbf > 0)
         PCM_CUDA(ctx, cudaMemset2DAsync(F, (size_t)ldf * 8, 0, (size_t)ctx->nbf * 8, (size_t)ctx->nbf, s));
     if (ctx->M > 0 && ctx->ncomp > 0) {
-        if ((rc = reduce_fock_class<0>(ctx, s))) return rc;
-        if ((rc = reduce_fock_class<1>(ctx, s))) return rc;
-        if ((rc = reduce_fock_class<2>(ctx, s))) return rc;
-        if ((rc = reduce_fock_class<3>(ctx, s))) return rc;
-        if ((rc = reduce_fock_class<4>(ctx, s))) return rc;
+        // the per-class reductions are independent of one another: a chain of programmatic dependent launches (each starts
+        // as soon as the one before it is resident and waits for it before it exits), the pair transform after them an ordinary one
+        bool ch = false;
+        if ((rc = reduce_fock_class<0>(ctx, s, ch))) return rc;
+        ch = ch || ctx->cls[0].n > 0;
+        if ((rc = reduce_fock_class<1>(ctx, s, ch))) return rc;
+        ch = ch || ctx->cls[1].n > 0;
+        if ((rc = reduce_fock_class<2>(ctx, s, ch))) return rc;
+        ch = ch || ctx->cls[2].n > 0;
+        if ((rc = reduce_fock_class<3>(ctx, s, ch))) return rc;
+        ch = ch || ctx->cls[3].n > 0;
+        if ((rc = reduce_fock_class<4>(ctx, s, ch))) return rc;
         ClassPtrs cp;
         for (int L = 0; L <= MAXL; ++L) { cp.herm[L] = ctx->cls[L].herm; cp.npad[L] = ctx->cls[L].npad; cp.first[L] = ctx->cls[L].first; }
         hermite_to_fock_kernel<<<(unsigned)ceil_div(ctx->ncomp, 128), 128, 0, s>>>(
@@ -1570,17 +1598,19 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
 }
 
 template <int L>
-static int launch_density_class(pcm_ctx *ctx, const double *P, int64_t ldp, cudaStream_t s) {
+static int launch_density_class(pcm_ctx *ctx, const double *P, int64_t ldp, cudaStream_t s, bool chained = false) {
     ClassData &c = ctx->cls[L];
     if (c.n == 0) return PCM_OK;
     if (L >= 2)
-        density_to_hermite_warp_kernel<L><<<(unsigned)(c.npad / 4), 128, 0, s>>>(
-            c.n, c.first, c.npad, ctx->pm_start, ctx->pm_list, ctx->m_sp, ctx->m_cls, ctx->m_goff, ctx->G, ctx->sp_i0,
-            ctx->sp_j0, ctx->sp_dims, P, ldp, c.herm);
+        PCM_CUDA(ctx, launch_class_b(density_to_hermite_warp_kernel<L>, dim3((unsigned)(c.npad / 4)), 128, s, chained, c.n, c.first, c.npad,
+                                     (const int64_t *)ctx->pm_start, (const int32_t *)ctx->pm_list, (const int32_t *)ctx->m_sp,
+                                     (const int32_t *)ctx->m_cls, (const int64_t *)ctx->m_goff, (const double *)ctx->G,
+                                     (const int32_t *)ctx->sp_i0, (const int32_t *)ctx->sp_j0, (const int32_t *)ctx->sp_dims, P, ldp, c.herm));
     else
-        density_to_hermite_kernel<L><<<(unsigned)(c.npad / 128), 128, 0, s>>>(
-            c.n, c.first, c.npad, ctx->pm_start, ctx->pm_list, ctx->m_sp, ctx->m_cls, ctx->m_goff, ctx->G, ctx->sp_i0,
-            ctx->sp_j0, ctx->sp_dims, P, ldp, c.herm);
+        PCM_CUDA(ctx, launch_class_b(density_to_hermite_kernel<L>, dim3((unsigned)(c.npad / 128)), 128, s, chained, c.n, c.first, c.npad,
+                                     (const int64_t *)ctx->pm_start, (const int32_t *)ctx->pm_list, (const int32_t *)ctx->m_sp,
+                                     (const int32_t *)ctx->m_cls, (const int64_t *)ctx->m_goff, (const double *)ctx->G,
+                                     (const int32_t *)ctx->sp_i0, (const int32_t *)ctx->sp_j0, (const int32_t *)ctx->sp_dims, P, ldp, c.herm));
     PCM_LAUNCH_CHECK(ctx);
     { ctx->launches[ctx->cur_op]++; ctx->launch_total++; }
     return PCM_OK;
@@ -1634,11 +1664,21 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
     int rc;
     if (ctx->M == 0) return PCM_OK;
     if ((rc = mark(ctx, 0, s))) return rc;
-    if ((rc = launch_density_class<0>(ctx, P, ldp, s))) return rc;
-    if ((rc = launch_density_class<1>(ctx, P, ldp, s))) return rc;
-    if ((rc = launch_density_class<2>(ctx, P, ldp, s))) return rc;
-    if ((rc = launch_density_class<3>(ctx, P, ldp, s))) return rc;
-    if ((rc = launch_density_class<4>(ctx, P, ldp, s))) return rc;
+    {   // The per-class transforms are independent of one another.  For small solutes, where a call is a string of launch
+        // latencies, they form a chain of programmatic dependent launches (configs[0]: pcm_potential 96 -> 79 us); at 300 atoms
+        // the chain measured 3 - 6 % slower for the whole call than three ordinary launches, so it stops at PDL_DENSITY_MAX products.
+        const bool chain = ctx->nprod <= PDL_DENSITY_MAX;
+        bool ch = false;
+        if ((rc = launch_density_class<0>(ctx, P, ldp, s, ch))) return rc;
+        ch = chain && (ch || ctx->cls[0].n > 0);
+        if ((rc = launch_density_class<1>(ctx, P, ldp, s, ch))) return rc;
+        ch = chain && (ch || ctx->cls[1].n > 0);
+        if ((rc = launch_density_class<2>(ctx, P, ldp, s, ch))) return rc;
+        ch = chain && (ch || ctx->cls[2].n > 0);
+        if ((rc = launch_density_class<3>(ctx, P, ldp, s, ch))) return rc;
+        ch = chain && (ch || ctx->cls[3].n > 0);
+        if ((rc = launch_density_class<4>(ctx, P, ldp, s, ch))) return rc;
+    }
     if ((rc = mark(ctx, 1, s))) return rc;
     // near kernels of all classes on the near stream (they need the Hermite densities), concurrently with the main kernels on s
     PCM_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
