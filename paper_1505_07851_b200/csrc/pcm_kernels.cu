@@ -1576,15 +1576,16 @@ int launch_fock(pcm_ctx *ctx, const double *q, double *F, int64_t ldf, int accum
     if (ctx->M > 0 && ctx->ncomp > 0) {
         // the per-class reductions are independent of one another: a chain of programmatic dependent launches (each starts
         // as soon as the one before it is resident and waits for it before it exits), the pair transform after them an ordinary one
+        const bool chain = !ctx->opt.serial_classes;      // serial_classes: ordinary launches throughout (the reference of the tests)
         bool ch = false;
         if ((rc = reduce_fock_class<0>(ctx, s, ch))) return rc;
-        ch = ch || ctx->cls[0].n > 0;
+        ch = chain && (ch || ctx->cls[0].n > 0);
         if ((rc = reduce_fock_class<1>(ctx, s, ch))) return rc;
-        ch = ch || ctx->cls[1].n > 0;
+        ch = chain && (ch || ctx->cls[1].n > 0);
         if ((rc = reduce_fock_class<2>(ctx, s, ch))) return rc;
-        ch = ch || ctx->cls[2].n > 0;
+        ch = chain && (ch || ctx->cls[2].n > 0);
         if ((rc = reduce_fock_class<3>(ctx, s, ch))) return rc;
-        ch = ch || ctx->cls[3].n > 0;
+        ch = chain && (ch || ctx->cls[3].n > 0);
         if ((rc = reduce_fock_class<4>(ctx, s, ch))) return rc;
         ClassPtrs cp;
         for (int L = 0; L <= MAXL; ++L) { cp.herm[L] = ctx->cls[L].herm; cp.npad[L] = ctx->cls[L].npad; cp.first[L] = ctx->cls[L].first; }
@@ -1667,7 +1668,7 @@ int launch_potential(pcm_ctx *ctx, const double *P, int64_t ldp, double *v, cuda
     {   // The per-class transforms are independent of one another.  For small solutes, where a call is a string of launch
         // latencies, they form a chain of programmatic dependent launches (configs[0]: pcm_potential 96 -> 79 us); at 300 atoms
         // the chain measured 3 - 6 % slower for the whole call than three ordinary launches, so it stops at PDL_DENSITY_MAX products.
-        const bool chain = ctx->nprod <= PDL_DENSITY_MAX;
+        const bool chain = ctx->nprod <= PDL_DENSITY_MAX && !ctx->opt.serial_classes;
         bool ch = false;
         if ((rc = launch_density_class<0>(ctx, P, ldp, s, ch))) return rc;
         ch = chain && (ch || ctx->cls[0].n > 0);

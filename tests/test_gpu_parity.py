@@ -354,19 +354,22 @@ def test_fock_tma_tiles_and_serial_classes_give_the_same_bits(pcm, orc, torch_cu
         pcm.pcm_destroy(ref)
 
 
-def test_chained_class_launches_are_ordered_before_the_reduction(pcm, torch_cuda):
+@pytest.mark.parametrize("n_atoms", [160, 24])
+def test_chained_class_launches_are_ordered_before_the_reduction(pcm, torch_cuda, n_atoms):
     """The default path launches the class kernels of a call as a chain of programmatic dependent launches (each may start
     while the one before it is still in its last wave).  Completion must stay in launch order so that the reduction after the
     chain sees every partial sum: all five classes, several waves per kernel, 40 back-to-back calls, every result bit-identical
-    to the one of ordinary launches (serial_classes)."""
+    to the one of ordinary launches (serial_classes).  The per-class Hermite reductions of pcm_fock are chained the same way,
+    and so are the density transforms of pcm_potential for small solutes (24 atoms: below the 16 384-product limit)."""
     torch = torch_cuda
-    w = synth.make_workload(3, n_atoms=160, n_pts=110, seed=99)
+    w = synth.make_workload(3, n_atoms=n_atoms, n_pts=110, seed=99)
     qd, Pd = dev(torch, w.q), dev(torch, w.P)
     ser = pcm.setup_from_workload(w.basis, w.surface, serial_classes=True)
     F0, v0 = pcm.pcm_fock(ser, qd).clone(), pcm.pcm_potential(ser, Pd).clone()
     pcm.pcm_destroy(ser)
     ctx = pcm.setup_from_workload(w.basis, w.surface)
     assert all(n > 0 for n in pcm.pcm_get_info(ctx).products)
+    assert (sum(pcm.pcm_get_info(ctx).products) <= 16384) == (n_atoms == 24)
     F, v = torch.empty_like(F0), torch.empty_like(v0)
     for it in range(40):
         F.fill_(float("nan")); v.fill_(float("nan"))
