@@ -391,9 +391,12 @@ def small_config_extras(pcm, torch, w, ctx, P, q, flush):
     out["rbj_solve_us"], out["rbj_solve_us_median"] = timed(lambda: its.append(pcm.pcm_cg_solve(ctx, y, x, tol=CG_TOL, max_iter=2000, precond=2, stream=stream)[1]), reps=5)
     out["rbj_solve_iters"] = int(its[-1])
     v = torch.empty(ctx.M, dtype=torch.float64, device=dev)
+    # ordinary launches (the library's per-kernel timing is on here, which also keeps it from replaying its own graph)
     out["potential_us_plain"], _ = timed(lambda: pcm.pcm_potential(ctx, P, v, stream=stream))
-    try:   # the ~20 launches of one pcm_potential call replayed from a CUDA graph
+    try:   # the ~10 launches of one pcm_potential call replayed from a CUDA graph: the library's own (pcm_options.graph_calls,
+           # on by default at this size), then one the caller captures
         pcm.pcm_set_timing(ctx, False)
+        out["potential_us_library_graph"], _ = timed(lambda: pcm.pcm_potential(ctx, P, v, stream=stream))
         side = torch.cuda.Stream(device=dev)
         side.wait_stream(stream)
         g = torch.cuda.CUDAGraph()

@@ -82,6 +82,13 @@ typedef struct pcm_options {
     int potential_pr;      /* bit L set: pcm_potential sweeps the products of total angular momentum L in the Fock layout (product
                               in registers, warp-shuffle reduction over the 32 products of a warp per point) instead of the
                               point-in-registers layout.  Same values up to the summation order.  Default 0 (measured: DESIGN.md) */
+    int graph_calls;       /* pcm_potential / pcm_fock replayed from a CUDA graph: the ~10 launches of a call are captured once
+                              (on an internal stream) and the instantiated graph is launched into the caller's stream for as
+                              long as the call's pointer arguments, leading dimension and flags stay the same (they are the key;
+                              any change re-captures).  0 (default) = for small solutes only, where a call is a string of launch
+                              latencies (products x points < 5e7); 1 = always; -1 = never.  Not used while pcm_set_timing is on
+                              or while the caller's stream is itself being captured (the launches then go into that capture).
+                              Same kernels, same results bit for bit */
 } pcm_options;
 
 typedef struct pcm_info {

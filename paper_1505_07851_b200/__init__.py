@@ -40,7 +40,7 @@ PCM_STATIC_MAX_POINTS = 16384
 
 class pcm_options(C.Structure):
     _fields_ = [("screen_eps", C.c_double), ("d_pure", C.c_int), ("device", C.c_int), ("merge_products", C.c_int),
-                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("store_far", C.c_int), ("serial_classes", C.c_int), ("tma_tiles", C.c_int), ("rbj_global_scan", C.c_int), ("potential_pr", C.c_int)]
+                ("gradient", C.c_int), ("store_near", C.c_int), ("cg_path", C.c_int), ("store_far", C.c_int), ("serial_classes", C.c_int), ("tma_tiles", C.c_int), ("rbj_global_scan", C.c_int), ("potential_pr", C.c_int), ("graph_calls", C.c_int)]
 
 
 class pcm_info(C.Structure):
@@ -201,7 +201,7 @@ def pcm_options_default() -> pcm_options:
 def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_zeta, pt_switch=None, *,
               screen_eps: float = 1e-12, d_pure: bool = True, device: int = -1, merge_products: bool = True,
               gradient: bool = False, store_near: bool = True, cg_path: int = 0, store_far: int = 0, tma_tiles: bool = False,
-              serial_classes: bool = False, rbj_global_scan: bool = False, potential_pr: int = 0) -> Context:
+              serial_classes: bool = False, rbj_global_scan: bool = False, potential_pr: int = 0, graph_calls: int = 0) -> Context:
     """Host numpy arrays in, context out (include/pcm.h: pcm_setup)."""
     import torch
     if not torch.cuda.is_available():
@@ -234,6 +234,7 @@ def pcm_setup(shell_l, shell_xyz, shell_nprim, prim_exp, prim_coef, pt_xyz, pt_z
     opt.serial_classes = 1 if serial_classes else 0
     opt.rbj_global_scan = 1 if rbj_global_scan else 0
     opt.potential_pr = int(potential_pr)
+    opt.graph_calls = int(graph_calls)
     h = C.c_void_p()
     rc = lib().pcm_setup(C.byref(h), len(sl), _hp(sl), _hp(sx), _hp(sn), _hp(pe), _hp(pc), len(pz), _hp(px), _hp(pz),
                          _hp(ps), C.byref(opt))

@@ -20,6 +20,50 @@ int cg_solve(pcm_ctx *ctx, const double *b, double *x, double tol, int max_iter,
 
 using namespace pcm;
 
+// One call replayed from its CUDA graph when pcm_options.graph_calls allows: captured on ctx->graph_stream the first time and
+// whenever the key (p0, p1, ld, flag) changes, launched into the caller's stream s.  Falls back to plain launches on s when
+// graphs are off, per-kernel timing is on, s is itself being captured, or anything about the capture fails.
+template <class F>
+static int graphed_call(pcm_ctx *ctx, CallGraph &cg, const void *p0, const void *p1, int64_t ld, int flag, int op, cudaStream_t s, F &&launch) {
+    if (!ctx->graph_ok || ctx->timing) return launch(s);
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &st) != cudaSuccess || st != cudaStreamCaptureStatusNone) {
+        (void)cudaGetLastError();
+        return launch(s);
+    }
+    if (cg.exec && cg.p0 == p0 && cg.p1 == p1 && cg.ld == ld && cg.flag == flag) {
+        PCM_CUDA(ctx, cudaGraphLaunch(cg.exec, s));
+        ctx->launches[op] = cg.nlaunch;
+        ctx->launch_total += cg.nlaunch;
+        return PCM_OK;
+    }
+    if (cg.exec) { cudaGraphExecDestroy(cg.exec); cg.exec = nullptr; }
+    cudaStream_t cs = ctx->graph_stream;
+    if (cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        (void)cudaGetLastError();
+        ctx->graph_ok = false;
+        return launch(s);
+    }
+    const int64_t before = ctx->launch_total;
+    const int rc = launch(cs);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(cs, &g);
+    if (rc == PCM_OK && e == cudaSuccess && g) e = cudaGraphInstantiate(&cg.exec, g, 0);
+    if (g) cudaGraphDestroy(g);
+    if (rc != PCM_OK) return rc;
+    if (e != cudaSuccess || !cg.exec) {       // no graph on this system: plain launches from now on
+        (void)cudaGetLastError();
+        cg.exec = nullptr;
+        ctx->graph_ok = false;
+        ctx->launch_total = before;
+        return launch(s);
+    }
+    cg.p0 = p0; cg.p1 = p1; cg.ld = ld; cg.flag = flag;
+    cg.nlaunch = (int)(ctx->launch_total - before);
+    PCM_CUDA(ctx, cudaGraphLaunch(cg.exec, s));
+    return PCM_OK;
+}
+
 extern "C" {
 
 void pcm_options_default(pcm_options *opt) {
@@ -44,6 +88,9 @@ static void free_ctx(pcm_ctx *ctx) {
     if (ctx->io_b) cudaFree(ctx->io_b);
     for (auto &e : ctx->ev) if (e) cudaEventDestroy(e);
     for (auto &e : ctx->cg_ev) if (e) cudaEventDestroy(e);
+    if (ctx->graph_pot.exec) cudaGraphExecDestroy(ctx->graph_pot.exec);
+    if (ctx->graph_fock.exec) cudaGraphExecDestroy(ctx->graph_fock.exec);
+    if (ctx->graph_stream) cudaStreamDestroy(ctx->graph_stream);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->near_stream) cudaStreamDestroy(ctx->near_stream);
     if (ctx->ev_rbj) { if (ctx->rbj_pending) cudaEventSynchronize(ctx->ev_rbj); cudaEventDestroy(ctx->ev_rbj); }
@@ -156,6 +203,12 @@ int pcm_setup(pcm_ctx **out, int nshell, const int *shell_l, const double *shell
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { ctx->err = std::string("pcm_setup: ") + cudaGetErrorString(e); return fail(PCM_ERR_CUDA); }
     setup_stage("solver scratch");
+    // small solutes: a call is a string of launch latencies -> replay it from a CUDA graph (pcm_options.graph_calls)
+    ctx->graph_ok = ctx->opt.graph_calls > 0 || (ctx->opt.graph_calls == 0 && ctx->info.product_points < 5e7);
+    if (ctx->graph_ok && cudaStreamCreateWithFlags(&ctx->graph_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        (void)cudaGetLastError();
+        ctx->graph_ok = false;
+    }
     ctx->info.device_bytes = ctx->device_bytes;
     ctx->info.amat_near_patches = ctx->amat_map.nnear;
     ctx->info.amat_stored_bytes = ctx->amat_blocks ? ctx->amat_map.nnear * 32 * 32 * 8 : 0;
@@ -174,7 +227,8 @@ int pcm_potential(pcm_ctx *ctx, const double *P_dev, int64_t ldp, double *v_dev,
     if (ctx->M == 0) return PCM_OK;
     if (!v_dev || (ctx->nbf > 0 && (!P_dev || ldp < ctx->nbf))) return set_error(ctx, PCM_ERR_ARG, "pcm_potential: bad argument");
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
-    return launch_potential(ctx, P_dev, ldp, v_dev, (cudaStream_t)stream);
+    return graphed_call(ctx, ctx->graph_pot, P_dev, v_dev, ldp, 0, 0, (cudaStream_t)stream,
+                        [&](cudaStream_t s) { return launch_potential(ctx, P_dev, ldp, v_dev, s); });
 }
 
 int pcm_fock(pcm_ctx *ctx, const double *q_dev, double *F_dev, int64_t ldf, int accumulate, void *stream) {
@@ -182,7 +236,8 @@ int pcm_fock(pcm_ctx *ctx, const double *q_dev, double *F_dev, int64_t ldf, int 
     if (ctx->nbf == 0) return PCM_OK;
     if (!F_dev || ldf < ctx->nbf || (ctx->M > 0 && !q_dev)) return set_error(ctx, PCM_ERR_ARG, "pcm_fock: bad argument");
     PCM_CUDA(ctx, cudaSetDevice(ctx->device));
-    return launch_fock(ctx, q_dev, F_dev, ldf, accumulate, (cudaStream_t)stream);
+    return graphed_call(ctx, ctx->graph_fock, q_dev, F_dev, ldf, accumulate ? 1 : 0, 1, (cudaStream_t)stream,
+                        [&](cudaStream_t s) { return launch_fock(ctx, q_dev, F_dev, ldf, accumulate, s); });
 }
 
 int pcm_amatvec(pcm_ctx *ctx, const double *q_dev, double *y_dev, void *stream) {

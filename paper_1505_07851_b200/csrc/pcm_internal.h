@@ -114,8 +114,21 @@ struct Plan {             // work partition of one hot kernel launch: grid = (xb
 
 }  // namespace pcm
 
+// One pcm_potential / pcm_fock call as an instantiated CUDA graph (pcm_options.graph_calls); the key is what the captured
+// kernels were given: two pointers, a leading dimension, a flag.
+struct CallGraph {
+    cudaGraphExec_t exec = nullptr;
+    const void *p0 = nullptr, *p1 = nullptr;
+    int64_t ld = 0;
+    int flag = 0;
+    int nlaunch = 0;
+};
+
 struct pcm_ctx {
     int device = 0;
+    CallGraph graph_pot, graph_fock;
+    cudaStream_t graph_stream = nullptr;     // the calls are captured here and replayed into the caller's stream
+    bool graph_ok = false;
     int sm_count = 148;
     pcm_options opt{};
     pcm_info info{};

@@ -433,3 +433,54 @@ def test_potential_product_in_registers_layout(pcm, orc, torch_cuda):
     assert np.all(np.abs(v - v0) <= 1e-12 * np.abs(v0) + 1e-14)
     pcm.pcm_destroy(c)
     pcm.pcm_destroy(c0)
+
+
+def test_graph_replayed_calls_equal_plain_launches(pcm, torch_cuda):
+    """pcm_options.graph_calls: pcm_potential / pcm_fock of a small solute are captured once and replayed from a CUDA graph.
+    Same kernels, so every result must equal the plain launches' bit for bit -- on replays, after a change of buffers (new key:
+    re-capture), with accumulate toggled, on the default and on a side stream, with the option forced on for a larger
+    solute, and when the caller captures the call into a graph of its own."""
+    torch = torch_cuda
+    for n_atoms, kw in ((None, {}), (60, {"graph_calls": 1})):
+        w = synth.make_workload(0) if n_atoms is None else synth.make_workload(1, n_atoms=n_atoms)
+        qd, Pd = dev(torch, w.q), dev(torch, w.P)
+        plain = pcm.setup_from_workload(w.basis, w.surface, graph_calls=-1)
+        v0, F0 = pcm.pcm_potential(plain, Pd).clone(), pcm.pcm_fock(plain, qd).clone()
+        pcm.pcm_destroy(plain)
+        ctx = pcm.setup_from_workload(w.basis, w.surface, **kw)
+        v, F = torch.empty_like(v0), torch.empty_like(F0)
+        for it in range(6):                           # first call captures, the others replay
+            v.fill_(float("nan")); F.fill_(float("nan"))
+            pcm.pcm_potential(ctx, Pd, v)
+            pcm.pcm_fock(ctx, qd, F)
+            assert torch.equal(v, v0) and torch.equal(F, F0), (n_atoms, it)
+        pcm.pcm_fock(ctx, qd, F, accumulate=True)      # another flag: another graph
+        assert torch.equal(F, F0 + F0)
+        pcm.pcm_fock(ctx, qd, F, accumulate=True)
+        assert torch.equal(F, (F0 + F0) + F0)
+        P2, q2 = (2.0 * Pd).contiguous(), (-0.5 * qd).contiguous()   # other buffers: another key
+        v2, F2 = torch.empty_like(v0), torch.empty_like(F0)
+        pcm.pcm_potential(ctx, P2, v2)
+        pcm.pcm_fock(ctx, q2, F2)
+        assert torch.equal(v2, 2.0 * v0) and torch.equal(F2, -0.5 * F0)
+        pcm.pcm_potential(ctx, Pd, v)                  # and back
+        assert torch.equal(v, v0)
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            for it in range(3):
+                v.fill_(float("nan")); F.fill_(float("nan"))
+                pcm.pcm_potential(ctx, Pd, v, stream=side)
+                pcm.pcm_fock(ctx, qd, F, stream=side)
+        side.synchronize()
+        assert torch.equal(v, v0) and torch.equal(F, F0)
+        g = torch.cuda.CUDAGraph()                     # the caller's own capture: the launches go into it
+        v.fill_(float("nan"))
+        with torch.cuda.graph(g, stream=side):
+            pcm.pcm_potential(ctx, Pd, v, stream=torch.cuda.current_stream())
+        g.replay(); g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(v, v0)
+        pcm.pcm_potential(ctx, Pd, v2)                 # the library's own graph still works after it
+        assert torch.equal(v2, v0)
+        pcm.pcm_destroy(ctx)
