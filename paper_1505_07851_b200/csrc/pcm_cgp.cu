@@ -129,6 +129,35 @@ __device__ __forceinline__ double cgp_ordered_sum(const double *partial, int n, 
     for (int i = threadIdx.x; i < n; i += CGP_THREADS) s += __ldcg(partial + i);
     return cgp_block_sum(s, s_w, s_bc);
 }
+// two sums at once: the same additions in the same order as two calls of the functions above, one round of barriers instead
+// of two (s_w: 2 x CGP_WARPS doubles, s_bc: 2)
+__device__ __forceinline__ void cgp_block_sum2(double &a, double &b, double *s_w, double *s_bc) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o);
+        b += __shfl_down_sync(0xffffffffu, b, o);
+    }
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) { s_w[threadIdx.x >> 5] = a; s_w[CGP_WARPS + (threadIdx.x >> 5)] = b; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double ta = threadIdx.x < CGP_WARPS ? s_w[threadIdx.x] : 0.0, tb = threadIdx.x < CGP_WARPS ? s_w[CGP_WARPS + threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = CGP_WARPS / 2; o > 0; o >>= 1) {
+            ta += __shfl_down_sync(0xffffffffu, ta, o);
+            tb += __shfl_down_sync(0xffffffffu, tb, o);
+        }
+        if (threadIdx.x == 0) { s_bc[0] = ta; s_bc[1] = tb; }
+    }
+    __syncthreads();
+    a = s_bc[0];
+    b = s_bc[1];
+}
+__device__ __forceinline__ void cgp_ordered_sum2(const double *pa, const double *pb, int n, double &a, double &b, double *s_w, double *s_bc) {
+    a = 0.0; b = 0.0;
+    for (int i = threadIdx.x; i < n; i += CGP_THREADS) { a += __ldcg(pa + i); b += __ldcg(pb + i); }
+    cgp_block_sum2(a, b, s_w, s_bc);
+}
 
 // cp.async (LDGSTS): global -> shared without registers; src_bytes < size zero-fills the rest (padding columns)
 __device__ __forceinline__ void cgp_cp16(void *dst, const void *src, int src_bytes) {
@@ -507,8 +536,26 @@ __device__ __forceinline__ void cgp_update(const CgpArgs &a, const double *p, do
                 }
                 team_sync();
             }
-            rr = team_sum(rr);
-            rz = team_sum(rz);
+            {   // both sums in one round of team barriers (the additions and their order are those of team_sum)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    rr += __shfl_down_sync(0xffffffffu, rr, o);
+                    rz += __shfl_down_sync(0xffffffffu, rz, o);
+                }
+                team_sync();
+                if ((tt & 31) == 0) { s_part[tt >> 5] = rr; s_part[TT / 32 + (tt >> 5)] = rz; }
+                team_sync();
+                if (tt < 32) {
+                    rr = tt < TT / 32 ? s_part[tt] : 0.0;
+                    rz = tt < TT / 32 ? s_part[TT / 32 + tt] : 0.0;
+#pragma unroll
+                    for (int o = TT / 64; o > 0; o >>= 1) {
+                        rr += __shfl_down_sync(0xffffffffu, rr, o);
+                        rz += __shfl_down_sync(0xffffffffu, rz, o);
+                    }
+                }
+                team_sync();
+            }
             if (tt == 0) { a.part2[b] = rr; a.part2[a.nblocks + b] = rz; }
         }
         __syncthreads();
@@ -526,8 +573,7 @@ __device__ __forceinline__ void cgp_update(const CgpArgs &a, const double *p, do
             rr = fma(ri, ri, rr);
             rz = fma(ri, zi, rz);
         }
-        rr = cgp_block_sum(rr, s_w, s_bc);
-        rz = cgp_block_sum(rz, s_w, s_bc);
+        cgp_block_sum2(rr, rz, s_w, s_bc);
         if (tid == 0) { a.part2[blockIdx.x] = rr; a.part2[G + blockIdx.x] = rz; }
     }
 }
@@ -535,18 +581,19 @@ __device__ __forceinline__ void cgp_update(const CgpArgs &a, const double *p, do
 template <int MODE>
 __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
     extern __shared__ double dyn[];
-    __shared__ double s_w[CGP_WARPS];
-    __shared__ double s_bc;
+    __shared__ double s_w[2 * CGP_WARPS];
+    __shared__ double s_bc2[2];
+    double &s_bc = s_bc2[0];
     const unsigned G = gridDim.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int gw = blockIdx.x * CGP_WARPS + warp;
     const int nU = a.precond == 2 ? a.nblocks : (int)G;
     double *wsm = dyn + warp * CGP_WSMEM2;
     // z = C r, r.r, r.z of the initial residual
-    cgp_update(a, nullptr, 0.0, true, dyn, s_w, &s_bc);
+    cgp_update(a, nullptr, 0.0, true, dyn, s_w, s_bc2);
     cgp_grid_sync(a.ctl, G);
-    double srr = cgp_ordered_sum(a.part2, nU, s_w, &s_bc);
-    double rz_old = cgp_ordered_sum(a.part2 + nU, nU, s_w, &s_bc);
+    double srr, rz_old;
+    cgp_ordered_sum2(a.part2, a.part2 + nU, nU, srr, rz_old, s_w, s_bc2);
     double beta = 0.0, pAp = 0.0;
     int iters = 0, cur = 0;
     bool stop = !(sqrt(srr) > a.tol) || a.max_iter <= 0;
@@ -595,12 +642,12 @@ __global__ void __launch_bounds__(CGP_THREADS, 1) cgp_solve_kernel(CgpArgs a) {
         cgp_stamp(a, iters, 4);
         pAp = cgp_ordered_sum(a.part1, a.ng, s_w, &s_bc);
         const double alpha = rz_old / pAp;
-        cgp_update(a, pnew, alpha, false, dyn, s_w, &s_bc);
+        cgp_update(a, pnew, alpha, false, dyn, s_w, s_bc2);
         cgp_stamp(a, iters, 5);
         cgp_grid_sync(a.ctl, G);
         cgp_stamp(a, iters, 6);
-        srr = cgp_ordered_sum(a.part2, nU, s_w, &s_bc);
-        const double srz = cgp_ordered_sum(a.part2 + nU, nU, s_w, &s_bc);
+        double srz;
+        cgp_ordered_sum2(a.part2, a.part2 + nU, nU, srr, srz, s_w, s_bc2);
         beta = srz / rz_old;
         rz_old = srz;
         ++iters;
