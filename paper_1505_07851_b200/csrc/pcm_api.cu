@@ -88,6 +88,7 @@ static void free_ctx(pcm_ctx *ctx) {
     if (ctx->io_b) cudaFree(ctx->io_b);
     for (auto &e : ctx->ev) if (e) cudaEventDestroy(e);
     for (auto &e : ctx->cg_ev) if (e) cudaEventDestroy(e);
+    if (ctx->graph_pot.exec || ctx->graph_fock.exec) cudaDeviceSynchronize();     // a replay may still be running
     if (ctx->graph_pot.exec) cudaGraphExecDestroy(ctx->graph_pot.exec);
     if (ctx->graph_fock.exec) cudaGraphExecDestroy(ctx->graph_fock.exec);
     if (ctx->graph_stream) cudaStreamDestroy(ctx->graph_stream);
