@@ -434,10 +434,17 @@ def amat_and_solver_sweep(pcm, torch, dev, flush, model, peak_tflops, with_solve
             pcm.pcm_amatvec(c4, qd, yd)
             ts.append(sum(pcm.pcm_last_kernel_ms(c4, pcm.OP_AMATVEC)[:2]))
         ms = min(ts)
+        tw = []          # the same call with whatever the previous one left in L2 (the condition inside a PCG solve); reported, not the headline
+        for _ in range(5):
+            pcm.pcm_amatvec(c4, qd, yd)
+            tw.append(sum(pcm.pcm_last_kernel_ms(c4, pcm.OP_AMATVEC)[:2]))
+        ms_warm = min(tw)
         wk = work_of(model, "amatvec", M=Ms)
         pairs = 0.5 * float(Ms) * Ms
         tf = pairs * wk["flop"] / (ms * 1e-3) * 1e-12
-        sweep.append({"M": Ms, "ms": ms, "ms_median": statistics.median(ts), "entries_per_s": float(Ms) * Ms / (ms * 1e-3),
+        sweep.append({"M": Ms, "ms": ms, "ms_median": statistics.median(ts), "ms_warm_l2": ms_warm,
+                      "frac_of_fp64_peak_warm_l2": pairs * wk["flop"] / (ms_warm * 1e-3) * 1e-12 / peak_tflops,
+                      "entries_per_s": float(Ms) * Ms / (ms * 1e-3),
                       "pair_evaluations_per_s": pairs / (ms * 1e-3), "tflops": tf, "frac_of_fp64_peak": tf / peak_tflops,
                       "fp64_pipe_frac": pairs * wk["instr"] * 2.0 / (ms * 1e-3) * 1e-12 / peak_tflops, "work_model": wk["key"], "work_source": wk["source"],
                       "stored_near_bytes": int(i4.amat_stored_bytes),
